@@ -1,0 +1,335 @@
+"""fp64 CPU oracle for the GMMNLSE / MPA hot path  --  TEST INFRASTRUCTURE ONLY.
+
+This file is the plain, slow, obviously-correct statement of what the CUDA path
+in ``paper_1708_05324_b200/csrc`` computes.  It is written from the paper
+(Wright et al., arXiv 1708.05324; citations are ``PAPER.md:<line>``) and shares
+no code with the CUDA path.  Only ``tests/``, ``__graft_entry__.smoke()`` and
+``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may import it; the
+product path never does.
+
+Everything is complex128 / float64 numpy.  There is no blocking, packing or
+symmetry exploitation: the nonlinear term is the ordered P^2-pair sum of Eq. 1.
+
+Conventions (S1; fixed by Eq. 1 <-> Eq. 12 consistency,
+PAPER.md:53 vs PAPER.md:209: ``(1 + i/w0 d_t)  <->  (1 + w/w0)`` i.e.
+``d_t <-> -i w``):
+
+    to-frequency   At_k = sum_n A_n exp(+2 pi i k n / N)          (un-normalised)
+    to-time        A_n  = (1/N) sum_k At_k exp(-2 pi i k n / N)
+    w_k = 2 pi k' / (N dt),  k' = k for k < N/2 else k - N
+    D_w^(p) = i [ dbeta0 + dbeta1 w + sum_{k>=2} beta_k w^k / k! ]
+
+Parity pins for every function live in ``tests/test_oracle_*.py`` (closed
+forms, brute force, invariants, convergence orders).  Nothing here is
+"parity unpinned".  (The step-index LP-mode S *values* produced by the input
+generator are unpinned, but S is an input to both sides -- see DESIGN.md.)
+"""
+from __future__ import annotations
+
+import math
+import numpy as np
+
+__all__ = [
+    "dft_direct", "fft_radix2", "to_freq", "to_time", "omega_grid",
+    "dispersion_operator", "raman_transfer", "pair_products",
+    "raman_convolve_direct", "raman_convolve", "nonlinear_term",
+    "nonlinear_term_literal", "nonlinear_op", "nonlinear_op_freq",
+    "rk4ip_step", "rk4ip_propagate", "mpa_large_step", "mpa_propagate",
+    "energy", "photon_number", "conserved_quantity",
+]
+
+
+# --------------------------------------------------------------------------- O1
+def dft_direct(x: np.ndarray, sign: int) -> np.ndarray:
+    """O(N^2) DFT along the last axis: X_k = sum_n x_n exp(sign 2 pi i k n / N).
+
+    Used only to check :func:`fft_radix2` on tiny N (and for tiny-N pins).
+    """
+    x = np.asarray(x, dtype=np.complex128)
+    N = x.shape[-1]
+    n = np.arange(N)
+    W = np.exp(sign * 2j * np.pi * np.outer(n, n) / N)     # W[k, n]
+    return x @ W.T
+
+
+def fft_radix2(x: np.ndarray, sign: int) -> np.ndarray:
+    """Recursive radix-2 decimation-in-time FFT along the last axis (N = 2^q).
+
+    X_k = sum_n x_n exp(sign 2 pi i k n / N); un-normalised for both signs.
+    Textbook Cooley-Tukey: X_k = E_k + w^k O_k, X_{k+N/2} = E_k - w^k O_k.
+    """
+    x = np.asarray(x, dtype=np.complex128)
+    N = x.shape[-1]
+    if N == 1:
+        return x.copy()
+    if N & (N - 1):
+        raise ValueError("N must be a power of two")
+    even = fft_radix2(x[..., 0::2], sign)
+    odd = fft_radix2(x[..., 1::2], sign)
+    w = np.exp(sign * 2j * np.pi * np.arange(N // 2) / N)
+    t = w * odd
+    return np.concatenate([even + t, even - t], axis=-1)
+
+
+def to_freq(A: np.ndarray) -> np.ndarray:
+    """At_k = sum_n A_n exp(+2 pi i k n/N)  (the paper's F{.}, reading S1)."""
+    return fft_radix2(A, +1)
+
+
+def to_time(At: np.ndarray) -> np.ndarray:
+    """A_n = (1/N) sum_k At_k exp(-2 pi i k n/N)."""
+    return fft_radix2(At, -1) / At.shape[-1]
+
+
+def omega_grid(N: int, dt: float) -> np.ndarray:
+    """Angular-frequency offset of bin k; Nyquist bin is -N/2 (reading S9)."""
+    k = np.arange(N)
+    kp = np.where(k < N // 2, k, k - N)
+    return 2.0 * np.pi * kp / (N * dt)
+
+
+# ------------------------------------------------------------------ linear part
+def dispersion_operator(beta: np.ndarray, omega: np.ndarray) -> np.ndarray:
+    """D_w^(p) = i[dbeta0 + dbeta1 w + sum_{k>=2} beta_k w^k / k!].
+
+    ``beta[p][k]`` = beta_k^(p) in s^k/m (k=0: dbeta0 [1/m], k=1: dbeta1 [s/m]).
+    Follows from Eq. 1's first three terms with d_t -> -i w:
+    -dbeta1 d_t -> +i dbeta1 w;  i^{m+1} beta_m/m! d_t^m -> i beta_m w^m / m!.
+    """
+    beta = np.atleast_2d(np.asarray(beta, dtype=np.float64))
+    P, nb = beta.shape
+    D = np.zeros((P, omega.shape[0]), dtype=np.float64)
+    for k in range(nb):
+        D += beta[:, k:k + 1] * omega[None, :] ** k / math.factorial(k)
+    return 1j * D
+
+
+# ---------------------------------------------------------------- nonlinear part
+def raman_transfer(h_R: np.ndarray, dt: float) -> np.ndarray:
+    """ht_R(w_k) = dt * F{h_R}_k  with h_R sampled at t_j = j dt (reading S6/S7)."""
+    return dt * to_freq(np.asarray(h_R, dtype=np.float64))
+
+
+def pair_products(A: np.ndarray) -> np.ndarray:
+    """T_mn(t) = A_m(t) A_n*(t) for all P^2 ordered pairs (Eq. 1)."""
+    return A[:, None, :] * np.conj(A[None, :, :])
+
+
+def raman_convolve_direct(T: np.ndarray, h_R: np.ndarray, dt: float) -> np.ndarray:
+    """R[i] = dt sum_j h_R[j] T[(i-j) mod N]  -- the literal circular sum (S7).
+
+    Discretisation of  int_0^inf h_R(tau) T(t - tau) dtau  (Eq. 1) on the
+    periodic grid.  O(N^2): tiny N only.
+    """
+    N = T.shape[-1]
+    R = np.zeros_like(T, dtype=np.complex128)
+    for i in range(N):
+        for j in range(N):
+            R[..., i] += h_R[j] * T[..., (i - j) % N]
+    return dt * R
+
+
+def raman_convolve(T: np.ndarray, h_R: np.ndarray, dt: float) -> np.ndarray:
+    """Same circular convolution through O1 (convolution theorem)."""
+    return to_time(raman_transfer(h_R, dt) * to_freq(T))
+
+
+def nonlinear_term(A, S, f_R=0.0, h_R=None, dt=1.0, direct_conv=False):
+    """N_p(t) = sum_{lmn} S_plmn A_l [(1-fR) A_m A_n* + fR (h_R (*) A_m A_n*)].
+
+    Eq. 1 bracket with S^K = S^R = S (Eq. 2; reading
+    S8).  Staged exactly as the definition reads: all P^2 ordered pair streams
+    T_mn, their Raman convolution, the blend, the sum over (m,n) (a matmul
+    step), the sum over l.  No symmetry of S is used.
+    """
+    A = np.asarray(A, dtype=np.complex128)
+    S = np.asarray(S, dtype=np.float64)
+    P, N = A.shape
+    T = pair_products(A)                                  # [m][n][t]
+    if f_R != 0.0:
+        R = (raman_convolve_direct if direct_conv else raman_convolve)(T, h_R, dt)
+        B = (1.0 - f_R) * T + f_R * R
+    else:
+        B = T
+    U = S.reshape(P * P, P * P) @ B.reshape(P * P, N)     # U[(p l)][t]
+    U = U.reshape(P, P, N)
+    return np.einsum("plt,lt->pt", U, A)
+
+
+def nonlinear_term_literal(A, S, f_R=0.0, h_R=None, dt=1.0):
+    """The same sum as four nested Python loops + the literal convolution.
+
+    Brute-force cross-check of :func:`nonlinear_term` for P <= 4, N <= 32.
+    """
+    A = np.asarray(A, dtype=np.complex128)
+    P, N = A.shape
+    out = np.zeros((P, N), dtype=np.complex128)
+    for p in range(P):
+        for l in range(P):
+            for m in range(P):
+                for n in range(P):
+                    s = S[p, l, m, n]
+                    if s == 0.0:
+                        continue
+                    T = A[m] * np.conj(A[n])
+                    term = (1.0 - f_R) * T
+                    if f_R != 0.0:
+                        R = np.zeros(N, dtype=np.complex128)
+                        for i in range(N):
+                            acc = 0.0
+                            for j in range(N):
+                                acc += h_R[j] * T[(i - j) % N]
+                            R[i] = dt * acc
+                        term = term + f_R * R
+                    out[p] += s * A[l] * term
+    return out
+
+
+def _shock_factor(omega, omega0, shock):
+    return (1.0 + omega / omega0) if shock else np.ones_like(omega)
+
+
+def nonlinear_op_freq(At, S, kappa, omega, omega0, f_R, h_R, dt, shock=True):
+    """N^(At) = i kappa (1 + w/w0) F{ N_p[F^-1 At] }  (Eq. 12 prefactor)."""
+    A = to_time(At)
+    Nt = nonlinear_term(A, S, f_R, h_R, dt)
+    return 1j * kappa * _shock_factor(omega, omega0, shock) * to_freq(Nt)
+
+
+def nonlinear_op(A, S, kappa, omega0, f_R, h_R, dt, shock=True):
+    """dA_p(t) = i kappa (1 + i/w0 d_t) N_p[A](t): last term of Eq. 1, time in/out."""
+    A = np.asarray(A, dtype=np.complex128)
+    omega = omega_grid(A.shape[-1], dt)
+    return to_time(nonlinear_op_freq(to_freq(A), S, kappa, omega, omega0, f_R, h_R, dt, shock))
+
+
+# ------------------------------------------------------------------- O3: RK4IP
+def rk4ip_step(At, h, D, nl):
+    """One RK4IP step (textbook interaction-picture RK4; named by north_star).
+
+    ``nl(At)`` is the frequency-domain nonlinear operator; E = exp(D h / 2).
+    """
+    E = np.exp(D * (h / 2.0))
+    AI = E * At
+    k1 = E * (h * nl(At))
+    k2 = h * nl(AI + k1 / 2.0)
+    k3 = h * nl(AI + k2 / 2.0)
+    k4 = h * nl(E * (AI + k3))
+    return E * (AI + k1 / 6.0 + k2 / 3.0 + k3 / 3.0) + k4 / 6.0
+
+
+def rk4ip_propagate(A0, L, dz, beta, S, kappa, omega0, f_R, h_R, dt, shock=True, n_steps=None):
+    """Propagate A0[p][t] over L with fixed step dz using RK4IP; returns A(L)[p][t]."""
+    A0 = np.asarray(A0, dtype=np.complex128)
+    N = A0.shape[-1]
+    omega = omega_grid(N, dt)
+    D = dispersion_operator(beta, omega)
+    if n_steps is None:
+        n_steps = int(round(L / dz))
+    nl = lambda X: nonlinear_op_freq(X, S, kappa, omega, omega0, f_R, h_R, dt, shock)
+    At = to_freq(A0)
+    for _ in range(n_steps):
+        At = rk4ip_step(At, dz, D, nl)
+    return to_time(At)
+
+
+# --------------------------------------------------------------------- O4: MPA
+def mpa_large_step(psi0, M, dz, D, nl_time, K, tol=1e-6, max_iter=None, fixed_iter=0,
+                   history=None):
+    """One MPA large step z0 -> z0 + M dz  (Eqs. 11-12).
+
+    psi0[p][w] = At(z0).  Planes j = 0..M (reading S10).  ``nl_time(A_t)`` returns
+    N_p[A](t); ``K[w] = i kappa (1 + w/w0)``.  Returns (At(z0 + M dz), n_iter,
+    last_err, converged).
+
+      first iterate      psi_j = psi_0
+      each iteration     A_j = psi_j exp(D j dz)            (Eq. 11)
+                         G_j = K exp(-D j dz) F{N[A_j]}     (Eq. 12 integrand)
+                         psi_j <- psi_0 + dz [G_0/2 + G_1 + .. + G_{j-1} + G_j/2]
+                                                            (trapezoid)
+      stop when err = max_j ||psi_j^new - psi_j|| / ||psi_j^new|| < tol   (S12)
+    """
+    P, N = psi0.shape
+    if max_iter is None:
+        max_iter = 2 * M + 4
+    psi = np.broadcast_to(psi0, (M + 1, P, N)).copy()
+    G = np.zeros((M + 1, P, N), dtype=np.complex128)
+    G[0] = K * to_freq(nl_time(to_time(psi0)))             # depends on psi_0 only (S10)
+    n_iter, err, converged = 0, np.inf, False
+    while True:
+        for j in range(1, M + 1):
+            Aj = to_time(psi[j] * np.exp(D * (j * dz)))
+            G[j] = K * np.exp(-D * (j * dz)) * to_freq(nl_time(Aj))
+        new = np.empty_like(psi)
+        new[0] = psi0
+        for j in range(1, M + 1):
+            acc = 0.5 * G[0] + 0.5 * G[j]
+            for i in range(1, j):
+                acc = acc + G[i]
+            new[j] = psi0 + dz * acc
+        err = 0.0
+        for j in range(1, M + 1):
+            num = np.sqrt(np.sum(np.abs(new[j] - psi[j]) ** 2))
+            den = np.sqrt(np.sum(np.abs(new[j]) ** 2))
+            err = max(err, num / den if den > 0 else 0.0)
+        psi = new
+        n_iter += 1
+        if history is not None:
+            history.append(psi.copy())
+        if fixed_iter > 0:
+            if n_iter >= fixed_iter:
+                converged = True
+                break
+        elif err < tol:
+            converged = True
+            break
+        elif n_iter >= max_iter:
+            break
+    return psi[M] * np.exp(D * (M * dz)), n_iter, err, converged
+
+
+def mpa_propagate(A0, L, dz, M, beta, S, kappa, omega0, f_R, h_R, dt, shock=True,
+                  tol=1e-6, max_iter=None, fixed_iter=0, stats=None, history=None):
+    """Propagate with MPA; the last large step uses M' = (L/dz) mod M planes."""
+    A0 = np.asarray(A0, dtype=np.complex128)
+    N = A0.shape[-1]
+    omega = omega_grid(N, dt)
+    D = dispersion_operator(beta, omega)
+    K = 1j * kappa * _shock_factor(omega, omega0, shock)
+    nl_time = lambda A: nonlinear_term(A, S, f_R, h_R, dt)
+    n_small = int(round(L / dz))
+    psi0 = to_freq(A0)
+    done = 0
+    tot_it, n_large, n_noconv, last_err = 0, 0, 0, 0.0
+    while done < n_small:
+        Mc = min(M, n_small - done)
+        hist = [] if history is not None else None
+        psi0, it, last_err, conv = mpa_large_step(psi0, Mc, dz, D, nl_time, K, tol,
+                                                   max_iter, fixed_iter, hist)
+        if history is not None:
+            history.append(hist)
+        tot_it += it
+        n_large += 1
+        n_noconv += 0 if conv else 1
+        done += Mc
+    if stats is not None:
+        stats.update(large_steps=n_large, iterations=tot_it, last_err=last_err,
+                     not_converged=n_noconv)
+    return to_time(psi0)
+
+
+# ------------------------------------------------------------------ invariants
+def energy(A, dt):
+    """sum_p sum_n |A_p(t_n)|^2 dt  [J]  -- conserved with shock off (S15)."""
+    return float(np.sum(np.abs(A) ** 2) * dt)
+
+
+def photon_number(A, dt, omega0):
+    """sum_p sum_k |At_p,k|^2 / (1 + w_k/w0)  -- conserved with shock on (S15)."""
+    At = to_freq(np.asarray(A, dtype=np.complex128))
+    w = omega_grid(A.shape[-1], dt)
+    return float(np.sum(np.abs(At) ** 2 / (1.0 + w / omega0)))
+
+
+def conserved_quantity(A, dt, omega0, shock):
+    return photon_number(A, dt, omega0) if shock else energy(A, dt)

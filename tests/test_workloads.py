@@ -1,0 +1,87 @@
+"""Pins for the synthetic-input generators (S tensor, modes, pulses).  CPU only."""
+import itertools
+import math
+
+import numpy as np
+import pytest
+
+from paper_1708_05324_b200 import workloads as W
+
+
+def test_constants():
+    assert abs(W.OMEGA0 - 1.828788e15) / 1.828788e15 < 1e-6
+    assert abs(W.N2 * W.OMEGA0 / W.C_LIGHT - 1.40304e-13) / 1.40304e-13 < 1e-5
+    assert abs(W.grin_spot_size() - 6.4017e-6) < 1e-10
+
+
+def test_grin_S_closed_forms_and_symmetry():
+    # Eq. 2 for Hermite-Gaussian modes: S_1111 = 1/(pi w^2), S_2222 = 3/4 S_1111, S_1122 = 1/2 S_1111
+    F, dA, groups = W.grin_modes(2)
+    S = W.coupling_tensor(F, dA)
+    w = W.grin_spot_size()
+    s0 = 1.0 / (math.pi * w * w)
+    assert abs(S[0, 0, 0, 0] / s0 - 1) < 1e-12
+    assert abs(1 / S[0, 0, 0, 0] - 128.75e-12) < 0.01e-12            # A_eff = 1/S_pppp
+    assert abs(S[1, 1, 1, 1] / (0.75 * s0) - 1) < 1e-12
+    assert abs(S[0, 0, 1, 1] / (0.5 * s0) - 1) < 1e-12
+    # all 24 index permutations equal (real scalar F_p)
+    P = S.shape[0]
+    for perm in itertools.permutations(range(4)):
+        assert np.array_equal(S, np.transpose(S, perm)) or np.allclose(S, np.transpose(S, perm), rtol=1e-13, atol=1e-3)
+    # Gram matrix of pair fields: PSD
+    ev = np.linalg.eigvalsh(S.reshape(P * P, P * P))
+    assert ev.min() > -1e-6 * ev.max()
+    # parity selection rule: odd total order in x or y integrates to zero
+    assert abs(S[0, 0, 0, 1]) < 1e-6 * s0
+    assert list(groups) == [0, 1, 1, 2, 2, 2]
+
+
+def test_coupling_tensor_vs_direct_quadrature():
+    rng = np.random.default_rng(0)
+    F = rng.standard_normal((3, 8, 8))
+    S = W.coupling_tensor(F, 0.5)
+    f = F.reshape(3, -1)
+    nrm = np.sqrt((f * f).sum(1) * 0.5)
+    for p, l, m, n in itertools.product(range(3), repeat=4):
+        want = (f[p] * f[l] * f[m] * f[n]).sum() * 0.5 / (nrm[p] * nrm[l] * nrm[m] * nrm[n])
+        assert abs(S[p, l, m, n] - want) < 1e-12 * abs(want) + 1e-15
+
+
+def test_step_index_modes():
+    k0 = 2 * math.pi / W.LAMBDA0
+    V = k0 * 25e-6 * 0.22
+    assert abs(V - 33.55) < 0.01
+    table = W.lp_mode_table(V)
+    # ordering: LP01, LP11, LP21, LP02 (mode 6 counting orientations), ...
+    assert [(l, m) for l, m, _ in table[:4]] == [(0, 1), (1, 1), (2, 1), (0, 2)]
+    from scipy.special import jv, kv
+    for l, m, u in table[:12]:
+        w = math.sqrt(V * V - u * u)
+        lhs = u * jv(l - 1, u) / jv(l, u)
+        rhs = -w * kv(l - 1, w) / kv(l, w)
+        assert abs(lhs - rhs) < 1e-8 * abs(rhs)
+    F, dA, betas, labels = W.step_index_modes(8)
+    assert labels[:6] == ["LP01", "LP11a", "LP11b", "LP21a", "LP21b", "LP02"]
+    f = F.reshape(8, -1)
+    G = f @ f.T * dA
+    d = np.sqrt(np.diag(G))
+    G = G / d[:, None] / d[None, :]
+    assert np.max(abs(G - np.eye(8))) < 2e-3        # orthogonal on the grid (quadrature of a kinked field)
+    assert np.all(np.diff(betas) <= 1e-9)
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3])
+def test_configs_shapes_and_seeding(idx):
+    a = W.make_config(idx, N=512)
+    b = W.make_config(idx, N=512)
+    assert np.array_equal(a.A0, b.A0) and np.array_equal(a.beta, b.beta)
+    assert a.A0.shape == (a.P, 512) and a.S.shape == (a.P,) * 4
+    if idx > 1:
+        assert abs(np.max(np.sum(abs(a.A0) ** 2, axis=0)) / a.meta["p_peak"] - 1) < 0.05
+        assert a.beta[0, 1] == 0.0 and np.all(a.beta[:, 0] <= 0)
+        assert math.pi / a.dt < a.omega0                       # shock factor stays positive
+        # intensity FWHM of the launch (S18)
+        I = np.sum(abs(W.make_config(idx, N=4096).A0) ** 2, axis=0)
+        t = (np.arange(4096) - 2048) * a.dt
+        above = t[I >= 0.5 * I.max()]
+        assert abs((above[-1] - above[0]) / a.meta["fwhm"] - 1) < 0.05
