@@ -1,0 +1,346 @@
+#!/usr/bin/env python
+"""bench.py -- GMMNLSE / MPA z-steps/s on B200 (BASELINE.json metric), one JSON line on stdout.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
+
+A "step" is one ``gmmnlse_propagate`` call over ``LARGE_PER_STEP[config]`` MPA large steps (all §8(a)
+rows: a1, a3-a11, every iteration, the convergence read-back) continuing from the previous step's
+output field.  ``value`` = small z-steps per second with the field resident in HBM; ``e2e`` = the same
+through ``gmmnlse_propagate_host`` (pinned staging, H2D + D2H inside the timed region).  N > 1 runs N
+independent replicas (the path does not shard in this build: DESIGN.md "Multi-GPU"), one per rank.
+``--impl reference`` times the fp64 CPU oracle (RK4IP) on the host cores instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "GMMNLSE z-steps/s (P modes, N samples, M planes)"
+UNIT = "z-steps/s"
+LARGE_PER_STEP = {1: 100, 2: 30, 3: 10, 4: 2, 5: 1}
+ORACLE_SAMPLE_N = {1: 1024, 2: 4096, 3: 8192, 4: 4096, 5: 2048}      # time-grid samples of the CPU sample
+DEFAULT_CONFIG = 5
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=d["hbm_gbs"], bf16_burst=d["bf16_tflops"], bf16_sustained=d["bf16_tflops_sustained"],
+                    source="measured")
+    return dict(hbm=6650.0, bf16_burst=1590.0, bf16_sustained=1400.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200", "-i",
+                 str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *exc):
+        if self.proc:
+            time.sleep(0.25)
+            self.proc.terminate()
+            self.t.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ------------------------------------------------------------------ algorithmic work per launch
+def algorithmic(kind, w, planes):
+    """(bytes, flops) one launch of `kind` must move / execute for `planes` planes."""
+    P, N = w.P, w.N
+    Q = P * (P + 1) // 2
+    c = 16 if w.precision else 8
+    r = c // 2
+    if kind in ("fft_to_time", "fft_to_freq"):
+        return 3 * c * P * N * planes, 5 * N * np.log2(N) * P * planes      # in + table + out
+    if kind == "pair_conv":
+        return (c * P * N + r * Q * N) * planes, 0
+    if kind == "contract":
+        return 2 * r * Q * N * planes, 2.0 * Q * Q * N * planes
+    if kind == "mode_reduce":
+        return (r * Q * N + 2 * c * P * N) * planes, 4.0 * P * P * N * planes
+    if kind == "scan":
+        return 3 * c * P * N * planes, 0                                    # G in, psi old in, psi out
+    return c * P * N * planes, 0
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1708_05324_b200 import binding, workloads
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the GPU path has no CPU fallback); use --impl reference")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    binding.load_library()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def measure(cfg, K, Wm, with_events, host_path=False, seed_offset=0):
+        w = workloads.make_config(cfg)
+        n_large = LARGE_PER_STEP[cfg]
+        L_step = n_large * w.M * w.dz
+        cdt = np.complex128 if w.precision else np.complex64
+        tdt = torch.complex128 if w.precision else torch.complex64
+        A0 = w.A0.astype(cdt)
+        if seed_offset:                          # replicas: independent noise shots, same physics
+            rng = np.random.default_rng(workloads.SEED_BASE + 1000 * seed_offset)
+            A0 = (A0 * np.exp(2j * np.pi * rng.random((w.P, 1)))).astype(cdt)
+        plan = binding.plan_from_workload(w)
+        stream = torch.cuda.current_stream()
+        A = torch.from_numpy(A0).cuda()
+        h_a, h_b = A0.copy(), np.empty_like(A0)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+        def step():
+            nonlocal h_a, h_b
+            if host_path:
+                plan.propagate_host(h_a, L_step, h_b)
+                h_a, h_b = h_b, h_a
+            else:
+                plan.propagate(A, L_step, A, stream)
+
+        for _ in range(Wm):
+            step()
+        barrier()
+        s0, l0 = plan.stats(), plan.launch_count()
+        if with_events:
+            plan.profile_enable(True)
+        t0 = time.perf_counter()
+        ev0.record(stream)
+        for _ in range(K):
+            step()
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        wall_ms = (time.perf_counter() - t0) * 1e3
+        dev_ms = ev0.elapsed_time(ev1)
+        # propagate() syncs the stream at every convergence read-back, so host wall time and the
+        # device-event span cover the same region; report the device span (max over ranks below)
+        ms = max(dev_ms, 0.0) if not host_path else wall_ms
+        prof = plan.profile_get() if with_events else None
+        if with_events:
+            plan.profile_enable(False)
+        s1, l1 = plan.stats(), plan.launch_count()
+        barrier()
+        if world > 1:
+            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        finite = bool(np.isfinite(h_a).all()) if host_path else bool(torch.isfinite(torch.view_as_real(A)).all())
+        plan.destroy()
+        it = s1["iterations"] - s0["iterations"]
+        ls = s1["large_steps"] - s0["large_steps"]
+        return dict(w=w, ms=ms, wall_ms=wall_ms, z_steps=K * n_large * w.M, iters=it, large=ls, prof=prof,
+                    launches=l1 - l0, not_conv=s1["not_converged"] - s0["not_converged"], finite=finite,
+                    bytes_io=int(A0.nbytes))
+
+    cfg, K, Wm = args.config, args.steps, max(args.warmup, 3)
+    peaks = _peaks()
+    with ClockSampler(local) as clk:
+        main = measure(cfg, K, Wm, with_events=True, seed_offset=rank)
+    clocks = clk.summary()
+    plain = measure(cfg, K, Wm, with_events=False, seed_offset=rank)          # same region, no per-kernel events
+    e2e = measure(cfg, K, Wm, with_events=False, host_path=True, seed_offset=rank)
+    w = main["w"]
+    value = world * main["z_steps"] / (main["ms"] * 1e-3)
+
+    # ---- roofline of the dominant kernel class, from the per-launch CUDA events of the timed region
+    prof = {k: v for k, v in main["prof"].items() if v[1] > 0}
+    dom = max(prof, key=lambda k: prof[k][0])
+    tot_ms = sum(v[0] for v in prof.values())
+    iters, large = main["iters"], main["large"]
+    planes_total = {  # planes processed by all launches of a class over the region
+        "fft_to_time": iters * w.M + large + K, "fft_to_freq": iters * w.M + large + K,
+        "pair_conv": iters * w.M + large, "contract": iters * w.M + large, "mode_reduce": iters * w.M + large,
+        "scan": iters * w.M, "advance": large, "misc": 0}
+    shares = {}
+    for k, (ms_k, n_k) in prof.items():
+        by, fl = algorithmic(k, w, planes_total.get(k, 0))
+        shares[k] = dict(ms=round(ms_k, 4), launches=n_k, share=round(ms_k / tot_ms, 4),
+                         GBps=round(by / (ms_k * 1e-3) / 1e9, 1), TFLOPs=round(fl / (ms_k * 1e-3) / 1e12, 3))
+    by, fl = algorithmic(dom, w, planes_total[dom])
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")     # written from an ncu --set full capture
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get(f"cfg{cfg}", {}).get(dom)
+    dom_ms, dom_n = prof[dom]
+    if dom == "contract":
+        ach = fl / (dom_ms * 1e-3) / 1e12
+        peak = peaks["bf16_sustained"] * 0.5          # TF32 dense = 1/2 bf16 (guide's nominal ratio)
+        roof = dict(bound="tensor", kernel="contract (a6)", achieved=round(ach, 3), peak=round(peak, 1),
+                    unit="TFLOP/s", frac=round(ach / peak, 4), traffic=traffic,
+                    note=f"useful packed-real flops 2*Q^2*N per plane; peak = {peaks['source']} bf16 sustained x 0.5 "
+                         "(TF32 nominal ratio); this round's kernel runs on the fp32 CUDA cores")
+    else:
+        ach = by / (dom_ms * 1e-3) / 1e9
+        roof = dict(bound="hbm", kernel=dom, achieved=round(ach, 1), peak=peaks["hbm"], unit="GB/s",
+                    frac=round(ach / peaks["hbm"], 4), traffic=traffic,
+                    note=f"algorithmic bytes / event-timed duration; peak = {peaks['source']} copy bandwidth")
+    roof["avg_launch_ms"] = round(dom_ms / dom_n, 4)
+    roof["kernels"] = shares
+
+    out = {
+        "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+        "ms_per_step": round(main["ms"] / K, 4), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "c128" if w.precision else "c64 (f32)", "data": "synthetic",
+        "config": {"workload": w.name, "baseline_config_index": cfg, "P": w.P, "N": w.N, "M": w.M,
+                   "dz_m": w.dz, "z_steps_per_step": LARGE_PER_STEP[cfg] * w.M,
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": "working set per MPA iteration exceeds L2 (no flush)" if cfg >= 4 else
+                         "working set is L2-resident by nature of the workload (no flush); not an HBM measurement"},
+        "mode_sample_updates_per_s": round(value * w.P * w.N, 1),
+        "iterations_per_large_step": round(main["iters"] / max(main["large"], 1), 3),
+        "not_converged": main["not_conv"], "finite": main["finite"],
+        "ms_per_step_without_kernel_events": round(plain["ms"] / K, 4),
+        "e2e": {"value": round(world * e2e["z_steps"] / (e2e["ms"] * 1e-3), 2), "unit": UNIT,
+                "h2d_bytes_per_step": e2e["bytes_io"], "d2h_bytes_per_step": e2e["bytes_io"] + 8 * e2e["iters"] // K},
+        "gpu_launches": main["launches"],
+        "clocks": clocks, "roofline": roof,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = oracle_sample(cfg, 1, 0)
+    if rank == 0 and args.all_configs and world == 1:
+        others = []
+        for c in (1, 2, 3, 4):
+            if c == cfg:
+                continue
+            m = measure(c, 3, 3, with_events=False)
+            others.append({"workload": m["w"].name, "z_steps_per_s": round(m["z_steps"] / (m["ms"] * 1e-3), 1),
+                           "ms_per_step": round(m["ms"] / 3, 4), "z_steps_per_step": LARGE_PER_STEP[c] * m["w"].M,
+                           "iterations_per_large_step": round(m["iters"] / max(m["large"], 1), 3)})
+        out["other_workloads"] = others
+    if rank == 0:
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------ oracle (CPU) leg
+def oracle_sample(cfg, K, Wm):
+    """Time the fp64 oracle as it stands (RK4IP, oracle/gmmnlse_oracle.py) on a bounded sample of the
+    workload: K RK4IP small steps on the first ORACLE_SAMPLE_N[cfg] samples of the time grid (same dt,
+    same fibre, same pulse); cost is linear in N up to the FFT's log factor, so z-steps/s at the full
+    grid = sample z-steps/s x (N_sample / N)."""
+    from oracle import gmmnlse_oracle as O
+    from paper_1708_05324_b200 import workloads
+    full = workloads.make_config(cfg)
+    Ns = min(ORACLE_SAMPLE_N[cfg], full.N)
+    w = workloads.make_config(cfg, N=Ns)
+    omega = O.omega_grid(w.N, w.dt)
+    D = O.dispersion_operator(w.beta, omega)
+    nl = lambda X: O.nonlinear_op_freq(X, w.S, w.kappa, omega, w.omega0, w.f_R, w.h_R, w.dt, w.shock)
+    At = O.to_freq(w.A0)
+    for _ in range(Wm):
+        At = O.rk4ip_step(At, w.dz, D, nl)
+    t0 = time.perf_counter()
+    for _ in range(K):
+        At = O.rk4ip_step(At, w.dz, D, nl)
+    sec = time.perf_counter() - t0
+    try:
+        import threadpoolctl
+        cores = max([p["num_threads"] for p in threadpoolctl.threadpool_info()] or [1])
+    except Exception:
+        cores = os.cpu_count() or 1
+    v = K / sec * (Ns / full.N)
+    return {"value": round(v, 4), "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{K} RK4IP step(s) (4 nonlinear-operator evaluations each) of {full.name} on N={Ns} of "
+                      f"{full.N} time samples, {sec:.1f} s CPU, scaled by {Ns}/{full.N}",
+            "finite": bool(np.isfinite(At).all())}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1708_05324_b200 import workloads
+    K, Wm = args.steps, args.warmup
+    K = min(K, 3)                               # each step is already a bounded sample
+    Wm = min(Wm, 1)
+    t0 = time.perf_counter()
+    cb = oracle_sample(args.config, K, Wm)
+    w = workloads.make_config(args.config)
+    out = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT,
+           "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": K, "warmup": Wm,
+           "ms_per_step": round(1e3 / cb["value"] * LARGE_PER_STEP[args.config] * w.M, 1) if cb["value"] else None,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "c128 (f64)",
+           "data": "synthetic",
+           "config": {"workload": w.name, "baseline_config_index": args.config, "P": w.P, "N": w.N, "M": w.M,
+                      "dz_m": w.dz, "integrator": "RK4IP (oracle O3), fixed step dz"},
+           "cpu_baseline": cb,
+           "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "wall_s": round(time.perf_counter() - t0, 1)}
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=DEFAULT_CONFIG, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="graft", choices=["graft", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--all-configs", action="store_true", help="also time configs 1-4 briefly (other_workloads)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,132 @@
+/* gmmnlse.h -- C ABI of the B200-native GMMNLSE / MPA hot path.
+ *
+ * Method: Wright et al., "Multimode Nonlinear Fiber Optics: Massively Parallel
+ * Numerical Solver, Tutorial and Outlook", arXiv 1708.05324.  Citations are
+ * PAPER.md line numbers.
+ *
+ *   Eq. 1   the GMMNLSE right-hand side
+ *   Eq. 2   S^K = S^R = S, real, from real scalar mode fields
+ *   Eq. 11  A_p(z,w) = psi_p(z,w) exp[D_w (z - z0)]
+ *   Eq. 12  integral form; PAPER.md:214-218 the M-plane iteration
+ *
+ * Conventions (reading S1): F{f}_k = sum_n f_n exp(+2 pi i k n/N),
+ * w_k = 2 pi k'/(N dt) (k' = k for k < N/2, else k - N), d/dt <-> -i w,
+ * D_w^(p) = i[beta0 + beta1 w + sum_{k>=2} beta_k w^k/k!].
+ *
+ * All work runs in hand-written sm_100a kernels; there is no CPU fallback.
+ * Every call returns GMMNLSE_OK (0) on success, a negative code on failure and
+ * (propagate only) the positive GMMNLSE_WARN_NOCONV when some large step hit
+ * max_iter.  No exception crosses this boundary; on GMMNLSE_EINVAL no output is
+ * written.  A plan is not thread-safe; use one plan per host thread.
+ */
+#ifndef GMMNLSE_H_
+#define GMMNLSE_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GMMNLSE_OK            0
+#define GMMNLSE_WARN_NOCONV   1   /* >=1 large step stopped at max_iter; last iterate used   */
+#define GMMNLSE_EINVAL       -1   /* bad argument (see each call)                            */
+#define GMMNLSE_ENOMEM       -2   /* host or device allocation failed                        */
+#define GMMNLSE_ECUDA        -3   /* a CUDA call failed; see gmmnlse_last_cuda_error()        */
+#define GMMNLSE_EUNSUPPORTED -4   /* legal request outside what the kernels cover             */
+
+typedef struct gmmnlse_plan gmmnlse_plan;   /* opaque; owns every device buffer it allocates */
+
+typedef struct {                /* pass NULL for defaults                                        */
+  int    precision;             /* 0 = complex64 (default), 1 = complex128                        */
+  int    shock;                 /* 1 (default): factor (1 + w/w0) of Eq. 12 on; 0: off            */
+  double tol;                   /* MPA convergence threshold, default 1e-6         */
+  int    max_iter;              /* cap on iterations per large step; <=0 -> 2*M + 4               */
+  int    fixed_iter;            /* >0: run exactly this many iterations per large step (parity)   */
+  int    contraction;           /* 0 = auto, 1 = CUDA-core fp32/fp64 GEMM, 2 = tcgen05 3xTF32     */
+} gmmnlse_options;
+
+/* Build a plan: precompute D_w^(p), the rotation tables exp(+-D_w j dz) (j = 0..M) in
+ * fp64, K(w) = i n2 w0/c (1 + w/w0), the blended Raman transfer function
+ * (1 - fR) + fR dt F{h_R}, and the pair-packed coupling matrix.
+ *
+ *   P, N, M   modes, time samples (power of two, 16 <= N <= 16384; complex128: N <= 8192),
+ *             small steps per large step (>= 1)
+ *   dt, dz    time-grid spacing [s]; small step [m]
+ *   beta      HOST [P][n_beta], beta[p*n_beta + k] = beta_k^(p) in s^k/m
+ *             (k = 0: delta-beta0 [1/m], k = 1: delta-beta1 [s/m])  (Eq. 1 terms 1-3)
+ *   S         HOST [P][P][P][P], index ((p*P + l)*P + m)*P + n, in 1/m^2 (Eq. 2).  Must be
+ *             symmetric under m<->n and p<->l (true for Eq. 2); otherwise EUNSUPPORTED.
+ *   f_R, h_R  Raman fraction; HOST [N] samples h_R(j dt) in 1/s (NULL iff f_R == 0)
+ *   omega0    carrier [rad/s];  n2 [m^2/W]
+ * Host arrays are copied; the caller keeps ownership.  EINVAL: sizes < 1, N not a power of
+ * two, pi/dt >= omega0 with shock on, NULL pointers, non-finite beta/S/h_R.               */
+int gmmnlse_plan_create(gmmnlse_plan **out, int P, int N, int M, double dt, double dz,
+                        const double *beta, int n_beta, const double *S,
+                        double f_R, const double *h_R, double omega0, double n2,
+                        const gmmnlse_options *opt);
+
+/* Integrate Eq. 1 from z0 to z0 + L with the MPA.
+ *   A_in, A_out  DEVICE [P][N] interleaved (re,im), float2 or double2 per precision, time
+ *                domain, sqrt(W); A_out may alias A_in; never freed by the library.
+ *   L            [m], an integer multiple of dz (1e-9 relative) else EINVAL; the last large
+ *                step uses (L/dz) mod M planes.
+ *   stream       cudaStream_t as void* (NULL = the plan's current stream).  Work is enqueued
+ *                on it; the call returns after the last convergence decision was read back
+ *                (one 8-byte D2H per iteration) -- A_out is complete only
+ *                after the stream is synchronised.                                         */
+int gmmnlse_propagate(gmmnlse_plan *plan, const void *A_in, double L, void *A_out, void *stream);
+
+/* Same as gmmnlse_propagate but A_in / A_out are HOST [P][N] buffers of the plan's
+ * precision; the call stages them through plan-owned pinned memory, copies, propagates and
+ * synchronises.  This is the end-to-end entry bench.py times.                              */
+int gmmnlse_propagate_host(gmmnlse_plan *plan, const void *A_in_host, double L, void *A_out_host);
+
+/* One evaluation of the last term of Eq. 1:
+ *   dA_p(t) = i n2 w0/c (1 + i/w0 d_t) sum_lmn S_plmn A_l [(1-fR) A_m A_n* + fR (h_R (*) A_m A_n*)]
+ * A, dA: DEVICE [P][N] as above (dA must not alias A); enqueued on the plan's stream.      */
+int gmmnlse_nonlinear_op(gmmnlse_plan *plan, const void *A, void *dA);
+
+int gmmnlse_set_stream(gmmnlse_plan *plan, void *stream);
+
+/* Counters accumulated since plan creation (any pointer may be NULL).                      */
+int gmmnlse_get_stats(const gmmnlse_plan *plan, long long *large_steps, long long *iterations,
+                      double *last_err, long long *not_converged);
+
+/* Kernel launches issued by this plan since creation (bench.py's "gpu_launches").          */
+long long gmmnlse_launch_count(const gmmnlse_plan *plan);
+
+/* Per-kernel-class device timing with CUDA events recorded on the plan's stream around every
+ * launch (bench.py's roofline numbers).  enable(on=1) clears the accumulators; get() synchronises
+ * the stream and returns the summed duration [ms] and launch count of one kernel class.        */
+#define GMMNLSE_KIND_FFT_TO_TIME 0   /* a3 (+ final inverse transform): psi_j E+_j -> A_j(t)      */
+#define GMMNLSE_KIND_PAIR_CONV   1   /* a4 + a5: pair products, Raman FFT.h.IFFT, blend            */
+#define GMMNLSE_KIND_CONTRACT    2   /* a6: S contraction                                          */
+#define GMMNLSE_KIND_MODE_REDUCE 3   /* a7: sum_l U_pl A_l                                         */
+#define GMMNLSE_KIND_FFT_TO_FREQ 4   /* a1, a8: F{.} K(w) E-_j                                      */
+#define GMMNLSE_KIND_SCAN        5   /* a9 + a10: trapezoid scan over planes + error norms        */
+#define GMMNLSE_KIND_ADVANCE     6   /* a11: plane shift                                           */
+#define GMMNLSE_KIND_MISC        7   /* conversions, error finalisation                            */
+#define GMMNLSE_KIND_COUNT       8
+int gmmnlse_profile_enable(gmmnlse_plan *plan, int on);
+int gmmnlse_profile_get(gmmnlse_plan *plan, int kind, double *total_ms, long long *launches);
+
+/* Parity hook: copy the interaction-picture planes psi_j (j = 0..M) of the most recent large
+ * step to HOST out[(M+1)][P][N] (precision of the plan).  Synchronises the stream.         */
+int gmmnlse_debug_get_planes(gmmnlse_plan *plan, void *out_host);
+
+/* Stage-level entry points used by the unit tests and micro-benchmarks (DEVICE pointers).
+ *   fft:   rows x N transform of the plan's precision; dir = +1 to-frequency (un-normalised,
+ *          exp(+i..)), -1 to-time (exp(-i..), scaled by 1/N).  out may alias in.
+ *   pairs: V[q][t] = (1-fR) Re T_mn + fR (h_R (*) Re T_mn), q = packed pair index of m <= n,
+ *          for n_planes planes of A [plane][P][N]  ->  V [plane][Q][N] (real).             */
+int gmmnlse_debug_fft(gmmnlse_plan *plan, const void *in, void *out, int rows, int dir);
+int gmmnlse_debug_pairs(gmmnlse_plan *plan, const void *A, void *V, int n_planes);
+
+void gmmnlse_plan_destroy(gmmnlse_plan *plan);
+const char *gmmnlse_status_string(int status);
+const char *gmmnlse_last_cuda_error(void);
+int gmmnlse_abi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GMMNLSE_H_ */

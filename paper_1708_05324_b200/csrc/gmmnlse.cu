@@ -1,0 +1,645 @@
+// Host side of the C ABI declared in include/gmmnlse.h: plan precompute (fp64), the MPA driver
+// loop and kernel dispatch.  No CPU fallback: every step of the path is a kernel
+// in kernels.cuh / gemm_tc.cuh.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <complex>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/gmmnlse.h"
+#include "kernels.cuh"
+
+namespace {
+
+thread_local std::string g_cuda_err;
+
+#define GM_CUDA(call)                                                                     \
+  do {                                                                                    \
+    cudaError_t e_ = (call);                                                              \
+    if (e_ != cudaSuccess) {                                                              \
+      g_cuda_err = std::string(#call) + ": " + cudaGetErrorString(e_);                    \
+      return GMMNLSE_ECUDA;                                                               \
+    }                                                                                     \
+  } while (0)
+
+#define GM_TRY(call)                 \
+  do {                               \
+    int s_ = (call);                 \
+    if (s_ < 0) return s_;           \
+  } while (0)
+
+using cd = std::complex<double>;
+
+void host_fft(std::vector<cd>& a, int sign) {   // iterative radix-2, fp64; plan-time only
+  const size_t n = a.size();
+  for (size_t i = 1, j = 0; i < n; ++i) {
+    size_t bit = n >> 1;
+    for (; j & bit; bit >>= 1) j ^= bit;
+    j ^= bit;
+    if (i < j) std::swap(a[i], a[j]);
+  }
+  for (size_t len = 2; len <= n; len <<= 1) {
+    const double ang = sign * 2.0 * M_PI / (double)len;
+    for (size_t i = 0; i < n; i += len)
+      for (size_t k = 0; k < len / 2; ++k) {
+        const cd w(std::cos(ang * (double)k), std::sin(ang * (double)k));
+        const cd u = a[i + k], v = a[i + k + len / 2] * w;
+        a[i + k] = u + v;
+        a[i + k + len / 2] = u - v;
+      }
+  }
+}
+
+int ilog2(int n) {
+  int l = 0;
+  while ((1 << l) < n) ++l;
+  return l;
+}
+
+}  // namespace
+
+// ============================================================================================
+struct gmmnlse_plan {
+  int P = 0, N = 0, M = 0, log2N = 0, Q = 0, precision = 0, shock = 1, max_iter = 0, fixed_iter = 0;
+  int contraction = 0;
+  double dt = 0, dz = 0, f_R = 0, omega0 = 0, n2 = 0, tol = 1e-6;
+  cudaStream_t stream = nullptr;
+  long long n_large = 0, n_iter = 0, n_noconv = 0, n_launch = 0;
+  double last_err = 0;
+  std::vector<double> phi;   // Im D_w^(p) [P][N]
+  // per-kernel-class CUDA-event timing (gmmnlse_profile_*): event pairs recorded on `stream`
+  bool prof_on = false;
+  std::vector<cudaEvent_t> prof_ev;
+  std::vector<int> prof_kind;
+  size_t prof_used = 0;
+  double prof_ms[GMMNLSE_KIND_COUNT] = {0};
+  long long prof_n[GMMNLSE_KIND_COUNT] = {0};
+  void prof_begin(int kind) {
+    ++n_launch;
+    if (!prof_on) return;
+    if (prof_used + 2 > prof_ev.size()) {
+      const size_t old = prof_ev.size();
+      prof_ev.resize(old + 1024);
+      for (size_t i = old; i < prof_ev.size(); ++i) cudaEventCreate(&prof_ev[i]);
+    }
+    prof_kind.push_back(kind);
+    cudaEventRecord(prof_ev[prof_used++], stream);
+  }
+  void prof_end() {
+    if (prof_on) cudaEventRecord(prof_ev[prof_used++], stream);
+  }
+  int prof_collect() {   // synchronises the stream
+    if (cudaStreamSynchronize(stream) != cudaSuccess) return GMMNLSE_ECUDA;
+    for (size_t i = 0; i + 1 < prof_used; i += 2) {
+      float ms = 0;
+      if (cudaEventElapsedTime(&ms, prof_ev[i], prof_ev[i + 1]) != cudaSuccess) return GMMNLSE_ECUDA;
+      const int k = prof_kind[i / 2];
+      prof_ms[k] += ms;
+      ++prof_n[k];
+    }
+    prof_used = 0;
+    prof_kind.clear();
+    return 0;
+  }
+  virtual ~gmmnlse_plan() {
+    for (auto e : prof_ev) cudaEventDestroy(e);
+  }
+  virtual int init(const double* S, const double* h_R) = 0;
+  virtual int propagate(const void* A_in, double L, void* A_out) = 0;
+  virtual int propagate_host(const void* A_in, double L, void* A_out) = 0;
+  virtual int nonlinear_op(const void* A, void* dA) = 0;
+  virtual int get_planes(void* out) = 0;
+  virtual int debug_fft(const void* in, void* out, int rows, int dir) = 0;
+  virtual int debug_pairs(const void* A, void* V, int n_planes) = 0;
+};
+
+namespace {
+
+using namespace gm;
+
+template <typename T>
+struct PlanT final : gmmnlse_plan {
+  using C = cplx<T>;
+  // device tables
+  C *tw = nullptr, *Kw = nullptr, *H = nullptr, *E = nullptr;
+  double2* EM_d = nullptr;
+  T* S2 = nullptr;
+  int *pair_m = nullptr, *pair_n = nullptr;
+  // device state
+  double2* psi0_d = nullptr;
+  C *psi = nullptr, *At = nullptr, *G = nullptr;   // [(M+1)][P][N]; psi plane 0 is psi_0
+  T *V = nullptr, *U = nullptr;                    // [(M+1)][Q][N]
+  double *errbuf = nullptr, *d_err = nullptr, *h_err = nullptr;
+  void *h_in = nullptr, *h_out = nullptr;          // pinned staging for propagate_host
+  C* d_io = nullptr;
+  std::map<int, double2*> EM_ragged;
+  long long PN = 0, QN = 0;
+
+  ~PlanT() override {
+    cudaFree(tw); cudaFree(Kw); cudaFree(H); cudaFree(E); cudaFree(EM_d); cudaFree(S2);
+    cudaFree(pair_m); cudaFree(pair_n); cudaFree(psi0_d); cudaFree(psi); cudaFree(At); cudaFree(G);
+    cudaFree(V); cudaFree(U); cudaFree(errbuf); cudaFree(d_err); cudaFree(d_io);
+    if (h_err) cudaFreeHost(h_err);
+    if (h_in) cudaFreeHost(h_in);
+    if (h_out) cudaFreeHost(h_out);
+    for (auto& kv : EM_ragged) cudaFree(kv.second);
+  }
+
+  template <typename X> int dalloc(X** p, size_t n) {
+    cudaError_t e = cudaMalloc((void**)p, n * sizeof(X));
+    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return GMMNLSE_ENOMEM; }
+    GM_CUDA(e);
+    return 0;
+  }
+  template <typename X> int upload(X* d, const std::vector<X>& h) {
+    GM_CUDA(cudaMemcpy(d, h.data(), h.size() * sizeof(X), cudaMemcpyHostToDevice));
+    return 0;
+  }
+
+  int make_EM(int Mc, double2** out) {
+    std::vector<double2> em((size_t)PN);
+    for (long long i = 0; i < PN; ++i) {
+      const double ph = std::remainder(phi[i] * (Mc * dz), 2.0 * M_PI);
+      em[i] = make_double2(std::cos(ph), std::sin(ph));
+    }
+    GM_TRY(dalloc(out, (size_t)PN));
+    return upload(*out, em);
+  }
+
+  int init(const double* S, const double* h_R) override {
+    PN = (long long)P * N;
+    Q = P * (P + 1) / 2;
+    QN = (long long)Q * N;
+    // ---- tables (fp64 on the host, rounded once to T) ----
+    std::vector<double> omega(N);
+    for (int k = 0; k < N; ++k) omega[k] = 2.0 * M_PI * (double)(k < N / 2 ? k : k - N) / (N * dt);
+    std::vector<C> h_tw(N), h_K(N), h_H(N);
+    for (int m = 0; m < N; ++m) {
+      const double a = 2.0 * M_PI * (double)m / (double)N;
+      h_tw[m] = mk((T)std::cos(a), (T)std::sin(a));
+    }
+    const double kappa = n2 * omega0 / 299792458.0;
+    for (int k = 0; k < N; ++k) h_K[k] = mk((T)0, (T)(kappa * (shock ? 1.0 + omega[k] / omega0 : 1.0)));
+    {
+      std::vector<cd> hh(N, cd(0, 0));
+      if (f_R != 0.0) {
+        for (int k = 0; k < N; ++k) hh[k] = h_R[k];
+        host_fft(hh, +1);
+      }
+      for (int k = 0; k < N; ++k) {
+        const cd v = ((1.0 - f_R) + f_R * dt * hh[k]) / (double)N;
+        h_H[k] = mk((T)v.real(), (T)v.imag());
+      }
+    }
+    std::vector<C> h_E((size_t)(M + 1) * PN);
+    for (int j = 0; j <= M; ++j)
+      for (long long i = 0; i < PN; ++i) {
+        const double ph = std::remainder(phi[i] * (j * dz), 2.0 * M_PI);
+        h_E[(size_t)j * PN + i] = mk((T)std::cos(ph), (T)std::sin(ph));
+      }
+    // ---- packed coupling matrix: rows (p<=l), columns (m<=n), off-diagonal columns doubled ----
+    std::vector<int> pm(Q), pn(Q);
+    {
+      int q = 0;
+      for (int m = 0; m < P; ++m)
+        for (int n = m; n < P; ++n, ++q) { pm[q] = m; pn[q] = n; }
+    }
+    std::vector<T> h_S2((size_t)Q * Q);
+    for (int r = 0; r < Q; ++r)
+      for (int q = 0; q < Q; ++q) {
+        const size_t idx = (((size_t)pm[r] * P + pn[r]) * P + pm[q]) * P + pn[q];
+        h_S2[(size_t)r * Q + q] = (T)(S[idx] * (pm[q] == pn[q] ? 1.0 : 2.0));
+      }
+    GM_TRY(dalloc(&tw, N)); GM_TRY(upload(tw, h_tw));
+    GM_TRY(dalloc(&Kw, N)); GM_TRY(upload(Kw, h_K));
+    GM_TRY(dalloc(&H, N)); GM_TRY(upload(H, h_H));
+    GM_TRY(dalloc(&E, (size_t)(M + 1) * PN)); GM_TRY(upload(E, h_E));
+    GM_TRY(make_EM(M, &EM_d));
+    GM_TRY(dalloc(&S2, (size_t)Q * Q)); GM_TRY(upload(S2, h_S2));
+    GM_TRY(dalloc(&pair_m, Q)); GM_TRY(upload(pair_m, pm));
+    GM_TRY(dalloc(&pair_n, Q)); GM_TRY(upload(pair_n, pn));
+    GM_TRY(dalloc(&psi0_d, (size_t)PN));
+    GM_TRY(dalloc(&psi, (size_t)(M + 1) * PN));
+    GM_TRY(dalloc(&At, (size_t)(M + 1) * PN));
+    GM_TRY(dalloc(&G, (size_t)(M + 1) * PN));
+    GM_TRY(dalloc(&V, (size_t)(M + 1) * QN));
+    GM_TRY(dalloc(&U, (size_t)(M + 1) * QN));
+    GM_TRY(dalloc(&errbuf, (size_t)2 * (M + 2)));
+    GM_TRY(dalloc(&d_err, 1));
+    GM_CUDA(cudaMemset(errbuf, 0, sizeof(double) * 2 * (M + 2)));
+    GM_CUDA(cudaMemset(psi, 0, sizeof(C) * (size_t)(M + 1) * PN));
+    GM_CUDA(cudaMallocHost((void**)&h_err, sizeof(double)));
+    return 0;
+  }
+
+  // ------------------------------------------------------------------ kernel launchers
+  template <int LOG2N, int DIR>
+  int launch_fft_t(const C* in, long long in_ps, C* out, long long out_ps, const C* pre, const C* post_vec,
+                   const C* post_tab, long long tab_ps, T scale, int rows, int planes) {
+    constexpr int NT = (1 << LOG2N) / 16;
+    const size_t smem = sizeof(C) * fft_smem_elems(1 << LOG2N);
+    static bool configured = false;
+    if (!configured) {
+      GM_CUDA(cudaFuncSetAttribute(k_fft_rows<T, LOG2N, DIR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)smem));
+      configured = true;
+    }
+    prof_begin(DIR > 0 ? GMMNLSE_KIND_FFT_TO_FREQ : GMMNLSE_KIND_FFT_TO_TIME);
+    k_fft_rows<T, LOG2N, DIR><<<dim3(rows, planes), NT, smem, stream>>>(in, in_ps, out, out_ps, pre, post_vec,
+                                                                         post_tab, tab_ps, scale, tw);
+    prof_end();
+    GM_CUDA(cudaGetLastError());
+    return 0;
+  }
+  int launch_fft(int dir, const C* in, long long in_ps, C* out, long long out_ps, const C* pre, const C* post_vec,
+                 const C* post_tab, long long tab_ps, T scale, int rows, int planes) {
+#define GM_FFT_CASE(L)                                                                                       \
+  case L:                                                                                                    \
+    return dir > 0 ? launch_fft_t<L, +1>(in, in_ps, out, out_ps, pre, post_vec, post_tab, tab_ps, scale, rows, \
+                                         planes)                                                             \
+                   : launch_fft_t<L, -1>(in, in_ps, out, out_ps, pre, post_vec, post_tab, tab_ps, scale, rows, \
+                                         planes);
+    switch (log2N) {
+      GM_FFT_CASE(4) GM_FFT_CASE(5) GM_FFT_CASE(6) GM_FFT_CASE(7) GM_FFT_CASE(8) GM_FFT_CASE(9)
+      GM_FFT_CASE(10) GM_FFT_CASE(11) GM_FFT_CASE(12) GM_FFT_CASE(13)
+      case 14:
+        if constexpr (sizeof(T) == 4) {
+          return dir > 0 ? launch_fft_t<14, +1>(in, in_ps, out, out_ps, pre, post_vec, post_tab, tab_ps, scale,
+                                                rows, planes)
+                         : launch_fft_t<14, -1>(in, in_ps, out, out_ps, pre, post_vec, post_tab, tab_ps, scale,
+                                                rows, planes);
+        }
+        return GMMNLSE_EUNSUPPORTED;
+    }
+#undef GM_FFT_CASE
+    return GMMNLSE_EUNSUPPORTED;
+  }
+
+  template <int LOG2N, bool RAMAN>
+  int launch_pairs_t(const C* A, long long a_ps, T* Vout, long long v_ps, int planes) {
+    constexpr int NT = (1 << LOG2N) / 16;
+    const size_t smem = RAMAN ? sizeof(C) * fft_smem_elems(1 << LOG2N) : 0;
+    static bool configured = false;
+    if (!configured) {
+      GM_CUDA(cudaFuncSetAttribute(k_pair_conv<T, LOG2N, RAMAN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)smem));
+      configured = true;
+    }
+    prof_begin(GMMNLSE_KIND_PAIR_CONV);
+    k_pair_conv<T, LOG2N, RAMAN><<<dim3((Q + 1) / 2, planes), NT, smem, stream>>>(A, a_ps, Vout, v_ps, pair_m,
+                                                                                  pair_n, Q, H, tw);
+    prof_end();
+    GM_CUDA(cudaGetLastError());
+    return 0;
+  }
+  int launch_pairs(const C* A, long long a_ps, T* Vout, long long v_ps, int planes) {
+    const bool raman = f_R != 0.0;
+#define GM_PC_CASE(L)                                                               \
+  case L:                                                                           \
+    return raman ? launch_pairs_t<L, true>(A, a_ps, Vout, v_ps, planes)             \
+                 : launch_pairs_t<L, false>(A, a_ps, Vout, v_ps, planes);
+    switch (log2N) {
+      GM_PC_CASE(4) GM_PC_CASE(5) GM_PC_CASE(6) GM_PC_CASE(7) GM_PC_CASE(8) GM_PC_CASE(9)
+      GM_PC_CASE(10) GM_PC_CASE(11) GM_PC_CASE(12) GM_PC_CASE(13)
+      case 14:
+        if constexpr (sizeof(T) == 4) {
+          return raman ? launch_pairs_t<14, true>(A, a_ps, Vout, v_ps, planes)
+                       : launch_pairs_t<14, false>(A, a_ps, Vout, v_ps, planes);
+        }
+        return GMMNLSE_EUNSUPPORTED;
+    }
+#undef GM_PC_CASE
+    return GMMNLSE_EUNSUPPORTED;
+  }
+
+  int launch_contract(const T* Vin, T* Uout, int planes) {
+    prof_begin(GMMNLSE_KIND_CONTRACT);
+    if (Q <= 32) {
+      constexpr int BM = 32, BN = 128, BK = 8, TM = 4, TN = 4;
+      dim3 grid((N + BN - 1) / BN, (Q + BM - 1) / BM, planes);
+      k_contract<T, BM, BN, BK, TM, TN><<<grid, (BM / TM) * (BN / TN), 0, stream>>>(S2, Vin, QN, Uout, QN, Q, N);
+    } else {
+      constexpr int BM = 128, BN = 128, BK = 8, TM = 8, TN = 8;
+      dim3 grid((N + BN - 1) / BN, (Q + BM - 1) / BM, planes);
+      k_contract<T, BM, BN, BK, TM, TN><<<grid, (BM / TM) * (BN / TN), 0, stream>>>(S2, Vin, QN, Uout, QN, Q, N);
+    }
+    prof_end();
+    GM_CUDA(cudaGetLastError());
+    return 0;
+  }
+
+  int launch_mode_reduce(const T* Uin, const C* A, C* Nout, int planes) {
+    const size_t smem = sizeof(C) * 2 * P * 128;
+    static size_t configured = 0;
+    if (smem > configured) {
+      GM_CUDA(cudaFuncSetAttribute(k_mode_reduce<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      configured = smem;
+    }
+    prof_begin(GMMNLSE_KIND_MODE_REDUCE);
+    k_mode_reduce<T><<<dim3((N + 127) / 128, planes), 128, smem, stream>>>(Uin, QN, A, PN, Nout, PN, P, N);
+    prof_end();
+    GM_CUDA(cudaGetLastError());
+    return 0;
+  }
+
+  // N_p[A_j](t) for `planes` planes starting at plane j0 of At -> G (time domain)   (a4-a7)
+  int nonlinear_term(int j0, int planes) {
+    GM_TRY(launch_pairs(At + j0 * PN, PN, V + j0 * QN, QN, planes));
+    GM_TRY(launch_contract(V + j0 * QN, U + j0 * QN, planes));
+    GM_TRY(launch_mode_reduce(U + j0 * QN, At + j0 * PN, G + j0 * PN, planes));
+    return 0;
+  }
+
+  int to_master(const C* src) {   // psi0_d <- src (promote)
+    const long long n = 2 * PN;
+    prof_begin(GMMNLSE_KIND_MISC);
+    k_convert<T, double><<<(unsigned)((n + 255) / 256), 256, 0, stream>>>((const T*)src, (double*)psi0_d, n);
+    prof_end();
+    GM_CUDA(cudaGetLastError());
+    return 0;
+  }
+
+  int large_step(int Mc, bool* converged) {
+    double2* EM = EM_d;
+    if (Mc != M) {
+      auto it = EM_ragged.find(Mc);
+      if (it == EM_ragged.end()) {
+        double2* p = nullptr;
+        GM_TRY(make_EM(Mc, &p));
+        EM_ragged[Mc] = p;
+        EM = p;
+      } else {
+        EM = it->second;
+      }
+    }
+    const int cap = fixed_iter > 0 ? fixed_iter : max_iter;
+    int it = 0;
+    *converged = false;
+    const unsigned sblocks = (unsigned)((PN + 255) / 256);
+    while (true) {
+      const int j0 = it == 0 ? 0 : 1, np = Mc + 1 - j0;
+      // a3: A_j(t) = F^-1{psi_j exp(+D j dz)}; first iterate psi_j = psi_0
+      GM_TRY(launch_fft(-1, it == 0 ? psi : psi + j0 * PN, it == 0 ? 0 : PN, At + j0 * PN, PN, E + j0 * PN, nullptr,
+                        nullptr, PN, (T)(1.0 / N), P, np));
+      GM_TRY(nonlinear_term(j0, np));                                        // a4-a7
+      // a8: G_j = K(w) exp(-D j dz) F{N_p}
+      GM_TRY(launch_fft(+1, G + j0 * PN, PN, G + j0 * PN, PN, nullptr, Kw, E + j0 * PN, PN, (T)1, P, np));
+      // a9 + a10
+      prof_begin(GMMNLSE_KIND_SCAN);
+      k_trapz_scan<T><<<sblocks, 256, 0, stream>>>(psi, G, psi, PN, Mc, (T)dz, it == 0 ? 1 : 0, errbuf, PN);
+      prof_end();
+      prof_begin(GMMNLSE_KIND_MISC);
+      k_err_finalize<<<1, 32, 0, stream>>>(errbuf, Mc, d_err);
+      prof_end();
+      GM_CUDA(cudaGetLastError());
+      ++it;
+      ++n_iter;
+      if (fixed_iter > 0) {
+        if (it >= cap) { *converged = true; break; }
+        continue;
+      }
+      GM_CUDA(cudaMemcpyAsync(h_err, d_err, sizeof(double), cudaMemcpyDeviceToHost, stream));
+      GM_CUDA(cudaStreamSynchronize(stream));
+      last_err = *h_err;
+      if (last_err < tol) { *converged = true; break; }
+      if (it >= cap) break;
+    }
+    // a11
+    prof_begin(GMMNLSE_KIND_ADVANCE);
+    k_advance<T><<<sblocks, 256, 0, stream>>>(psi0_d, psi, G, PN, Mc, dz, EM, PN);
+    prof_end();
+    GM_CUDA(cudaGetLastError());
+    ++n_large;
+    return 0;
+  }
+
+  int propagate(const void* A_in, double L, void* A_out) override {
+    const double ns = L / dz;
+    const long long nsteps = llround(ns);
+    if (!(L >= 0) || std::fabs(ns - (double)nsteps) > 1e-9 * std::fmax(1.0, ns)) return GMMNLSE_EINVAL;
+    // a1: psi_0 = F{A(z0)}
+    GM_TRY(launch_fft(+1, (const C*)A_in, 0, psi, 0, nullptr, nullptr, nullptr, 0, (T)1, P, 1));
+    GM_TRY(to_master(psi));
+    long long done = 0;
+    int status = GMMNLSE_OK;
+    while (done < nsteps) {
+      const int Mc = (int)std::min<long long>(M, nsteps - done);
+      bool conv = false;
+      GM_TRY(large_step(Mc, &conv));
+      if (!conv) { ++n_noconv; status = GMMNLSE_WARN_NOCONV; }
+      done += Mc;
+    }
+    if (fixed_iter > 0) {
+      GM_CUDA(cudaMemcpyAsync(h_err, d_err, sizeof(double), cudaMemcpyDeviceToHost, stream));
+      GM_CUDA(cudaStreamSynchronize(stream));
+      last_err = nsteps > 0 ? *h_err : 0.0;
+    }
+    // A_out = F^-1{psi_0}
+    GM_TRY(launch_fft(-1, psi, 0, (C*)A_out, 0, nullptr, nullptr, nullptr, 0, (T)(1.0 / N), P, 1));
+    return status;
+  }
+
+  int propagate_host(const void* A_in, double L, void* A_out) override {
+    const size_t bytes = sizeof(C) * (size_t)PN;
+    if (!h_in) {
+      GM_CUDA(cudaMallocHost(&h_in, bytes));
+      GM_CUDA(cudaMallocHost(&h_out, bytes));
+      GM_TRY(dalloc(&d_io, (size_t)PN));
+    }
+    std::memcpy(h_in, A_in, bytes);
+    GM_CUDA(cudaMemcpyAsync(d_io, h_in, bytes, cudaMemcpyHostToDevice, stream));
+    const int st = propagate(d_io, L, d_io);
+    if (st < 0) return st;
+    GM_CUDA(cudaMemcpyAsync(h_out, d_io, bytes, cudaMemcpyDeviceToHost, stream));
+    GM_CUDA(cudaStreamSynchronize(stream));
+    std::memcpy(A_out, h_out, bytes);
+    return st;
+  }
+
+  int nonlinear_op(const void* A, void* dA) override {
+    // a12: uses plane 0 of the scratch buffers.  dA = F^-1{ K(w) F{N_p[A]} }
+    GM_CUDA(cudaMemcpyAsync(At, A, sizeof(C) * (size_t)PN, cudaMemcpyDeviceToDevice, stream));
+    GM_TRY(nonlinear_term(0, 1));
+    GM_TRY(launch_fft(+1, G, 0, G, 0, nullptr, Kw, nullptr, 0, (T)1, P, 1));
+    GM_TRY(launch_fft(-1, G, 0, (C*)dA, 0, nullptr, nullptr, nullptr, 0, (T)(1.0 / N), P, 1));
+    return 0;
+  }
+
+  int get_planes(void* out) override {
+    GM_CUDA(cudaStreamSynchronize(stream));
+    GM_CUDA(cudaMemcpy(out, psi, sizeof(C) * (size_t)(M + 1) * PN, cudaMemcpyDeviceToHost));
+    return 0;
+  }
+
+  int debug_fft(const void* in, void* out, int rows, int dir) override {
+    if (rows < 1 || (dir != 1 && dir != -1)) return GMMNLSE_EINVAL;
+    return launch_fft(dir, (const C*)in, 0, (C*)out, 0, nullptr, nullptr, nullptr, 0,
+                      dir > 0 ? (T)1 : (T)(1.0 / N), rows, 1);
+  }
+  int debug_pairs(const void* A, void* Vout, int n_planes) override {
+    if (n_planes < 1) return GMMNLSE_EINVAL;
+    return launch_pairs((const C*)A, PN, (T*)Vout, QN, n_planes);
+  }
+};
+
+}  // namespace
+
+// ============================================================================================
+extern "C" {
+
+int gmmnlse_abi_version(void) { return 1; }
+
+const char* gmmnlse_last_cuda_error(void) { return g_cuda_err.c_str(); }
+
+const char* gmmnlse_status_string(int s) {
+  switch (s) {
+    case GMMNLSE_OK: return "ok";
+    case GMMNLSE_WARN_NOCONV: return "warning: an MPA large step did not converge within max_iter";
+    case GMMNLSE_EINVAL: return "invalid argument";
+    case GMMNLSE_ENOMEM: return "out of memory";
+    case GMMNLSE_ECUDA: return "CUDA error";
+    case GMMNLSE_EUNSUPPORTED: return "unsupported configuration";
+  }
+  return "unknown status";
+}
+
+int gmmnlse_plan_create(gmmnlse_plan** out, int P, int N, int M, double dt, double dz, const double* beta,
+                        int n_beta, const double* S, double f_R, const double* h_R, double omega0, double n2,
+                        const gmmnlse_options* opt) {
+  if (!out) return GMMNLSE_EINVAL;
+  *out = nullptr;
+  gmmnlse_options o = {0, 1, 1e-6, 0, 0, 0};
+  if (opt) o = *opt;
+  if (P < 1 || N < 1 || M < 1 || n_beta < 1 || !beta || !S) return GMMNLSE_EINVAL;
+  if (N & (N - 1)) return GMMNLSE_EINVAL;
+  if (!(dt > 0) || !(dz > 0) || !(omega0 > 0) || !std::isfinite(n2) || !std::isfinite(f_R)) return GMMNLSE_EINVAL;
+  if ((f_R != 0.0) != (h_R != nullptr)) return GMMNLSE_EINVAL;
+  if (o.precision != 0 && o.precision != 1) return GMMNLSE_EINVAL;
+  if (o.shock && M_PI / dt >= omega0) return GMMNLSE_EINVAL;
+  if (!(o.tol > 0)) o.tol = 1e-6;
+  for (long long i = 0; i < (long long)P * n_beta; ++i)
+    if (!std::isfinite(beta[i])) return GMMNLSE_EINVAL;
+  const long long P4 = (long long)P * P * P * P;
+  double smax = 0;
+  for (long long i = 0; i < P4; ++i) {
+    if (!std::isfinite(S[i])) return GMMNLSE_EINVAL;
+    smax = std::fmax(smax, std::fabs(S[i]));
+  }
+  if (h_R)
+    for (int i = 0; i < N; ++i)
+      if (!std::isfinite(h_R[i])) return GMMNLSE_EINVAL;
+  if (N < 16 || N > (o.precision ? 8192 : 16384)) return GMMNLSE_EUNSUPPORTED;
+  // the packed-pair path needs S symmetric under m<->n and p<->l (Eq. 2 gives all 24 permutations)
+  for (int p = 0; p < P; ++p)
+    for (int l = 0; l < P; ++l)
+      for (int m = 0; m < P; ++m)
+        for (int n = 0; n < P; ++n) {
+          const double a = S[(((size_t)p * P + l) * P + m) * P + n];
+          const double b = S[(((size_t)p * P + l) * P + n) * P + m];
+          const double c = S[(((size_t)l * P + p) * P + m) * P + n];
+          if (std::fabs(a - b) > 1e-12 * smax || std::fabs(a - c) > 1e-12 * smax) return GMMNLSE_EUNSUPPORTED;
+        }
+  gmmnlse_plan* pl = nullptr;
+  if (o.precision == 0) pl = new (std::nothrow) PlanT<float>();
+  else pl = new (std::nothrow) PlanT<double>();
+  if (!pl) return GMMNLSE_ENOMEM;
+  pl->P = P; pl->N = N; pl->M = M; pl->log2N = ilog2(N); pl->precision = o.precision; pl->shock = o.shock ? 1 : 0;
+  pl->dt = dt; pl->dz = dz; pl->f_R = f_R; pl->omega0 = omega0; pl->n2 = n2; pl->tol = o.tol;
+  pl->max_iter = o.max_iter > 0 ? o.max_iter : 2 * M + 4;
+  pl->fixed_iter = o.fixed_iter > 0 ? o.fixed_iter : 0;
+  pl->contraction = o.contraction;
+  // Im D_w^(p) = beta0 + beta1 w + sum_{k>=2} beta_k w^k / k!
+  pl->phi.assign((size_t)P * N, 0.0);
+  for (int p = 0; p < P; ++p)
+    for (int k = 0; k < N; ++k) {
+      const double w = 2.0 * M_PI * (double)(k < N / 2 ? k : k - N) / (N * dt);
+      double acc = 0, wp = 1, fact = 1;
+      for (int b = 0; b < n_beta; ++b) {
+        if (b > 0) { wp *= w; fact *= (double)b; }
+        acc += beta[(size_t)p * n_beta + b] * wp / fact;
+      }
+      pl->phi[(size_t)p * N + k] = acc;
+    }
+  const int st = pl->init(S, h_R);
+  if (st < 0) { delete pl; return st; }
+  *out = pl;
+  return GMMNLSE_OK;
+}
+
+int gmmnlse_propagate(gmmnlse_plan* plan, const void* A_in, double L, void* A_out, void* stream) {
+  if (!plan || !A_in || !A_out) return GMMNLSE_EINVAL;
+  if (stream) plan->stream = (cudaStream_t)stream;
+  return plan->propagate(A_in, L, A_out);
+}
+
+int gmmnlse_propagate_host(gmmnlse_plan* plan, const void* A_in_host, double L, void* A_out_host) {
+  if (!plan || !A_in_host || !A_out_host) return GMMNLSE_EINVAL;
+  const double ns = L / plan->dz;
+  if (!(L >= 0) || std::fabs(ns - std::round(ns)) > 1e-9 * std::fmax(1.0, ns)) return GMMNLSE_EINVAL;
+  return plan->propagate_host(A_in_host, L, A_out_host);
+}
+
+int gmmnlse_nonlinear_op(gmmnlse_plan* plan, const void* A, void* dA) {
+  if (!plan || !A || !dA || A == dA) return GMMNLSE_EINVAL;
+  return plan->nonlinear_op(A, dA);
+}
+
+int gmmnlse_set_stream(gmmnlse_plan* plan, void* stream) {
+  if (!plan) return GMMNLSE_EINVAL;
+  plan->stream = (cudaStream_t)stream;
+  return GMMNLSE_OK;
+}
+
+int gmmnlse_get_stats(const gmmnlse_plan* plan, long long* large_steps, long long* iterations, double* last_err,
+                      long long* not_converged) {
+  if (!plan) return GMMNLSE_EINVAL;
+  if (large_steps) *large_steps = plan->n_large;
+  if (iterations) *iterations = plan->n_iter;
+  if (last_err) *last_err = plan->last_err;
+  if (not_converged) *not_converged = plan->n_noconv;
+  return GMMNLSE_OK;
+}
+
+long long gmmnlse_launch_count(const gmmnlse_plan* plan) { return plan ? plan->n_launch : 0; }
+
+int gmmnlse_profile_enable(gmmnlse_plan* plan, int on) {
+  if (!plan) return GMMNLSE_EINVAL;
+  if (plan->prof_collect() < 0) return GMMNLSE_ECUDA;
+  plan->prof_on = on != 0;
+  if (on)
+    for (int k = 0; k < GMMNLSE_KIND_COUNT; ++k) { plan->prof_ms[k] = 0; plan->prof_n[k] = 0; }
+  return GMMNLSE_OK;
+}
+
+int gmmnlse_profile_get(gmmnlse_plan* plan, int kind, double* total_ms, long long* launches) {
+  if (!plan || kind < 0 || kind >= GMMNLSE_KIND_COUNT) return GMMNLSE_EINVAL;
+  if (plan->prof_collect() < 0) return GMMNLSE_ECUDA;
+  if (total_ms) *total_ms = plan->prof_ms[kind];
+  if (launches) *launches = plan->prof_n[kind];
+  return GMMNLSE_OK;
+}
+
+int gmmnlse_debug_get_planes(gmmnlse_plan* plan, void* out_host) {
+  if (!plan || !out_host) return GMMNLSE_EINVAL;
+  return plan->get_planes(out_host);
+}
+
+int gmmnlse_debug_fft(gmmnlse_plan* plan, const void* in, void* out, int rows, int dir) {
+  if (!plan || !in || !out) return GMMNLSE_EINVAL;
+  return plan->debug_fft(in, out, rows, dir);
+}
+
+int gmmnlse_debug_pairs(gmmnlse_plan* plan, const void* A, void* V, int n_planes) {
+  if (!plan || !A || !V) return GMMNLSE_EINVAL;
+  return plan->debug_pairs(A, V, n_planes);
+}
+
+void gmmnlse_plan_destroy(gmmnlse_plan* plan) { delete plan; }
+
+}  // extern "C"

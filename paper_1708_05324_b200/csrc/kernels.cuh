@@ -1,0 +1,277 @@
+// CUDA kernels of the MPA hot path.  Templated on the real type
+// T (float: complex64 path, double: complex128 path) and on log2 N.
+#pragma once
+#include "fft.cuh"
+
+namespace gm {
+
+// ------------------------------------------------------------------------------------------
+// a1 / a3 / a8 / a12: row FFT with fused pre- and post-multiplies.
+//   grid = (P, n_planes); row (j, p) = in + j*in_plane_stride + p*N   (in_plane_stride may be 0:
+//   every plane reads psi_0 -- the first MPA iterate)
+//   x_n   = in[n] * (pre ? pre[j][p][n] : 1)                      Eq. 11: psi_j * exp(+D j dz)
+//   X_k   = FFT_DIR(x)
+//   out_k = X_k * scale * (post_vec ? post_vec[k] : 1) * (post_tab ? conj(post_tab[j][p][k]) : 1)
+//                                                        Eq. 12: K(w) exp(-D j dz) F{N_p}
+template <typename T, int LOG2N, int DIR>
+__global__ void __launch_bounds__((1 << LOG2N) / 16)
+k_fft_rows(const cplx<T>* __restrict__ in, long long in_plane_stride, cplx<T>* __restrict__ out,
+           long long out_plane_stride, const cplx<T>* __restrict__ pre, const cplx<T>* __restrict__ post_vec,
+           const cplx<T>* __restrict__ post_tab, long long tab_plane_stride, T scale,
+           const cplx<T>* __restrict__ tw) {
+  constexpr int N = 1 << LOG2N;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
+  const int p = blockIdx.x, j = blockIdx.y;
+  const cplx<T>* src = in + j * in_plane_stride + (long long)p * N;
+  cplx<T>* dst = out + j * out_plane_stride + (long long)p * N;
+  const long long toff = j * tab_plane_stride + (long long)p * N;
+  const cplx<T>* pre_r = pre ? pre + toff : nullptr;
+  const cplx<T>* post_r = post_tab ? post_tab + toff : nullptr;
+  block_fft<T, LOG2N, DIR>(
+      sm, tw,
+      [&](int n) {
+        cplx<T> x = src[n];
+        if (pre_r) x = cmul(x, pre_r[n]);
+        return x;
+      },
+      [&](int k, cplx<T> X) {
+        X = cscale(X, scale);
+        if (post_vec) X = cmul(X, post_vec[k]);
+        if (post_r) X = cmulc(X, post_r[k]);
+        dst[k] = X;
+      });
+}
+
+// ------------------------------------------------------------------------------------------
+// a4 + a5: pair products and Raman convolution, two real pair streams per complex FFT.
+//   grid = (ceil(Q/2), n_planes).  CTA (qq, j) handles packed pairs q0 = 2 qq, q1 = q0 + 1:
+//   z_n = Re(A_m A_n*)[q0] + i Re(A_m A_n*)[q1];  Z = F{z};  Z *= H,  H = ((1-fR) + fR ht_R)/N;
+//   v = F^-1{Z};  V[q0] = Re v, V[q1] = Im v.        (Eq. 1 bracket; h_R real)
+// With HAS_RAMAN == false the FFTs are skipped: V = Re T.
+template <typename T, int LOG2N, bool HAS_RAMAN>
+__global__ void __launch_bounds__((1 << LOG2N) / 16)
+k_pair_conv(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restrict__ V, long long v_plane_stride,
+            const int* __restrict__ pair_m, const int* __restrict__ pair_n, int Q,
+            const cplx<T>* __restrict__ H, const cplx<T>* __restrict__ tw) {
+  constexpr int N = 1 << LOG2N, NT = N / 16;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
+  const int q0 = 2 * blockIdx.x, q1 = q0 + 1, j = blockIdx.y;
+  const bool has1 = q1 < Q;
+  const cplx<T>* Aj = A + j * a_plane_stride;
+  const cplx<T>* am0 = Aj + (long long)pair_m[q0] * N;
+  const cplx<T>* an0 = Aj + (long long)pair_n[q0] * N;
+  const cplx<T>* am1 = Aj + (long long)pair_m[has1 ? q1 : q0] * N;
+  const cplx<T>* an1 = Aj + (long long)pair_n[has1 ? q1 : q0] * N;
+  T* v0 = V + j * v_plane_stride + (long long)q0 * N;
+  T* v1 = V + j * v_plane_stride + (long long)q1 * N;
+  auto prod = [&](int n) {
+    cplx<T> a = am0[n], b = an0[n], c = am1[n], d = an1[n];
+    return mk(a.x * b.x + a.y * b.y, has1 ? c.x * d.x + c.y * d.y : (T)0);
+  };
+  if constexpr (!HAS_RAMAN) {
+    for (int e = 0; e < 16; ++e) {
+      const int n = threadIdx.x + e * NT;
+      cplx<T> z = prod(n);
+      v0[n] = z.x;
+      if (has1) v1[n] = z.y;
+    }
+  } else {
+    block_fft<T, LOG2N, +1>(sm, tw, prod, [&](int k, cplx<T> Z) { sm[fft_pad(k)] = cmul(Z, H[k]); });
+    __syncthreads();
+    block_fft<T, LOG2N, -1>(
+        sm, tw, [&](int k) { return sm[fft_pad(k)]; },
+        [&](int n, cplx<T> v) {
+          v0[n] = v.x;
+          if (has1) v1[n] = v.y;
+        });
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// a6 (CUDA-core form): U[j][r][t] = sum_q S2[r][q] V[j][q][t], r,q packed pairs (p<=l), (m<=n);
+// S2 holds S_plmn with off-diagonal (m<n) columns doubled.
+// Plain register-tiled GEMM, C[Q x N] = S2[Q x Q] * V_j[Q x N], one plane per blockIdx.z.
+template <typename T, int BM, int BN, int BK, int TM, int TN>
+__global__ void __launch_bounds__((BM / TM) * (BN / TN))
+k_contract(const T* __restrict__ S2, const T* __restrict__ V, long long v_plane_stride, T* __restrict__ U,
+           long long u_plane_stride, int Q, int N) {
+  constexpr int NTH = (BM / TM) * (BN / TN);
+  __shared__ T As[BK][BM + 4];
+  __shared__ T Bs[BK][BN];
+  const T* B = V + blockIdx.z * v_plane_stride;
+  T* C = U + blockIdx.z * u_plane_stride;
+  const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
+  const int tid = threadIdx.x;
+  const int tx = tid % (BN / TN), ty = tid / (BN / TN);
+  T acc[TM][TN];
+#pragma unroll
+  for (int i = 0; i < TM; ++i)
+#pragma unroll
+    for (int jn = 0; jn < TN; ++jn) acc[i][jn] = 0;
+  for (int k0 = 0; k0 < Q; k0 += BK) {
+    for (int idx = tid; idx < BM * BK; idx += NTH) {
+      const int r = idx / BK, kk = idx % BK;
+      const int gr = m0 + r, gk = k0 + kk;
+      As[kk][r] = (gr < Q && gk < Q) ? S2[(long long)gr * Q + gk] : (T)0;
+    }
+    for (int idx = tid; idx < BK * BN; idx += NTH) {
+      const int kk = idx / BN, c = idx % BN;
+      const int gk = k0 + kk, gc = n0 + c;
+      Bs[kk][c] = (gk < Q && gc < N) ? B[(long long)gk * N + gc] : (T)0;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int kk = 0; kk < BK; ++kk) {
+      T a[TM], b[TN];
+#pragma unroll
+      for (int i = 0; i < TM; ++i) a[i] = As[kk][ty * TM + i];
+#pragma unroll
+      for (int jn = 0; jn < TN; ++jn) b[jn] = Bs[kk][tx + jn * (BN / TN)];
+#pragma unroll
+      for (int i = 0; i < TM; ++i)
+#pragma unroll
+        for (int jn = 0; jn < TN; ++jn) acc[i][jn] += a[i] * b[jn];
+    }
+    __syncthreads();
+  }
+#pragma unroll
+  for (int i = 0; i < TM; ++i) {
+    const int gr = m0 + ty * TM + i;
+    if (gr >= Q) continue;
+#pragma unroll
+    for (int jn = 0; jn < TN; ++jn) {
+      const int gc = n0 + tx + jn * (BN / TN);
+      if (gc < N) C[(long long)gr * N + gc] = acc[i][jn];
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// a7: N_p(t) = sum_l U_pl(t) A_l(t), U real symmetric, stored packed (p <= l).
+//   grid = (N / 128, n_planes), 128 threads: thread t owns one sample; accumulators in smem.
+template <typename T>
+__global__ void __launch_bounds__(128)
+k_mode_reduce(const T* __restrict__ U, long long u_plane_stride, const cplx<T>* __restrict__ A,
+              long long a_plane_stride, cplx<T>* __restrict__ Nt, long long n_plane_stride, int P, int N) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx<T>* a_s = reinterpret_cast<cplx<T>*>(smem_raw);        // [P][128]
+  cplx<T>* acc = a_s + P * 128;                               // [P][128]
+  const int t = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, tx = threadIdx.x;
+  if (t >= N) return;
+  const T* Uj = U + j * u_plane_stride;
+  const cplx<T>* Aj = A + j * a_plane_stride;
+  for (int p = 0; p < P; ++p) {
+    a_s[p * 128 + tx] = Aj[(long long)p * N + t];
+    acc[p * 128 + tx] = mk((T)0, (T)0);
+  }
+  int r = 0;
+  for (int p = 0; p < P; ++p) {
+    cplx<T> ap = a_s[p * 128 + tx];
+    cplx<T> sp = acc[p * 128 + tx];
+    for (int l = p; l < P; ++l, ++r) {
+      const T u = Uj[(long long)r * N + t];
+      cplx<T> al = a_s[l * 128 + tx];
+      sp.x += u * al.x;
+      sp.y += u * al.y;
+      if (l != p) {
+        cplx<T> sl = acc[l * 128 + tx];
+        sl.x += u * ap.x;
+        sl.y += u * ap.y;
+        acc[l * 128 + tx] = sl;
+      }
+    }
+    Nt[j * n_plane_stride + (long long)p * N + t] = sp;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// a9 + a10: cumulative trapezoid over planes and the per-plane error norms.
+//   psi_j^new = psi_0 + dz [G_0/2 + G_1 + .. + G_{j-1} + G_j/2], j = 1..Mc
+//   errbuf[2 j] += sum |psi_j^new - psi_j^old|^2,  errbuf[2 j + 1] += sum |psi_j^new|^2
+// One thread per (p, w); 256-thread blocks; double atomics, one per plane per warp.
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_trapz_scan(const cplx<T>* __restrict__ psi0, const cplx<T>* __restrict__ G, cplx<T>* __restrict__ psi,
+             long long plane_stride, int Mc, T dz, int first_iter, double* __restrict__ errbuf, long long PN) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool live = i < PN;
+  cplx<T> p0 = mk((T)0, (T)0), acc = p0;
+  if (live) {
+    p0 = psi0[i];
+    acc = cscale(G[i], (T)0.5);
+  }
+  for (int j = 1; j <= Mc; ++j) {
+    T num = 0, den = 0;
+    if (live) {
+      const cplx<T> g = G[j * plane_stride + i];
+      cplx<T> pn = mk(p0.x + dz * (acc.x + (T)0.5 * g.x), p0.y + dz * (acc.y + (T)0.5 * g.y));
+      acc = cadd(acc, g);
+      const cplx<T> old = first_iter ? p0 : psi[j * plane_stride + i];
+      const cplx<T> d = csub(pn, old);
+      num = d.x * d.x + d.y * d.y;
+      den = pn.x * pn.x + pn.y * pn.y;
+      psi[j * plane_stride + i] = pn;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      num += __shfl_xor_sync(0xffffffffu, num, o);
+      den += __shfl_xor_sync(0xffffffffu, den, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+      atomicAdd(&errbuf[2 * j], (double)num);
+      atomicAdd(&errbuf[2 * j + 1], (double)den);
+    }
+  }
+}
+
+// err = max_j sqrt(num_j / den_j); result -> out[0]; accumulators cleared for the next iteration
+__global__ void k_err_finalize(double* __restrict__ errbuf, int Mc, double* __restrict__ out) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) {
+    double e = 0.0;
+    for (int j = 1; j <= Mc; ++j) {
+      const double num = errbuf[2 * j], den = errbuf[2 * j + 1];
+      const double r = den > 0.0 ? sqrt(num / den) : 0.0;
+      e = fmax(e, r);
+      errbuf[2 * j] = 0.0;
+      errbuf[2 * j + 1] = 0.0;
+    }
+    out[0] = e;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// a11: advance the fp64 master state by one large step and refresh its working-precision copy.
+//   psi0_d <- (psi0_d + dz [G_0/2 + G_1 + .. + G_{Mc-1} + G_Mc/2]) * exp(D Mc dz)
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_advance(double2* __restrict__ psi0_d, cplx<T>* __restrict__ psi0, const cplx<T>* __restrict__ G,
+          long long plane_stride, int Mc, double dz, const double2* __restrict__ EM, long long PN) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= PN) return;
+  double ax = 0.5 * (double)G[i].x, ay = 0.5 * (double)G[i].y;
+  for (int j = 1; j < Mc; ++j) {
+    const cplx<T> g = G[j * plane_stride + i];
+    ax += (double)g.x;
+    ay += (double)g.y;
+  }
+  const cplx<T> gm = G[Mc * plane_stride + i];
+  ax += 0.5 * (double)gm.x;
+  ay += 0.5 * (double)gm.y;
+  double2 p = psi0_d[i];
+  p.x += dz * ax;
+  p.y += dz * ay;
+  const double2 e = EM[i];
+  const double2 q = make_double2(p.x * e.x - p.y * e.y, p.x * e.y + p.y * e.x);
+  psi0_d[i] = q;
+  psi0[i] = mk((T)q.x, (T)q.y);
+}
+
+template <typename TI, typename TO>
+__global__ void __launch_bounds__(256) k_convert(const TI* __restrict__ in, TO* __restrict__ out, long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = (TO)in[i];
+}
+
+}  // namespace gm

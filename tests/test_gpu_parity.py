@@ -1,0 +1,291 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element, on the
+same seeded inputs.  Bounds are BASELINE.json's: relative L2 <= 1e-5 for one nonlinear-operator
+evaluation (and for per-iteration MPA planes in fixed_iter mode), <= 1e-3 on the propagated field,
+<= 1e-6 on the drift of the conserved quantity (reading S15)."""
+import numpy as np
+import pytest
+
+from oracle import gmmnlse_oracle as O
+from paper_1708_05324_b200 import workloads as W
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL_OP = 1e-5
+TOL_FIELD = 1e-3
+TOL_DRIFT = 1e-6
+
+
+def rel(a, b):
+    a = np.asarray(a, dtype=np.complex128).ravel()
+    b = np.asarray(b, dtype=np.complex128).ravel()
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+@pytest.fixture(scope="module")
+def B():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1708_05324_b200 import binding
+    binding.load_library()          # raises if the CUDA library is missing: no fallback
+    return binding
+
+
+def dev(a, dtype):
+    return torch.from_numpy(np.ascontiguousarray(a.astype(dtype))).cuda()
+
+
+def _dummy_plan(B, N, precision, P=1, M=1):
+    S = np.ones((P, P, P, P))
+    return B.Plan(P, N, M, 1e-15, 1e-6, np.zeros((P, 1)), S, 0.0, None, W.OMEGA0, W.N2,
+                  precision=precision, shock=False)
+
+
+# ------------------------------------------------------------------------------- a1/a3/a8: FFT
+@pytest.mark.parametrize("N", [16, 32, 64, 128, 256, 512, 1024, 2048, 4096, 8192, 16384])
+@pytest.mark.parametrize("precision", [0, 1])
+def test_fft_rows_vs_oracle(B, N, precision):
+    if precision == 1 and N > 8192:
+        pytest.skip("complex128 path covers N <= 8192")
+    rng = np.random.default_rng(N + precision)
+    rows = 5
+    x = rng.standard_normal((rows, N)) + 1j * rng.standard_normal((rows, N))
+    dt = np.complex128 if precision else np.complex64
+    tol = 1e-13 if precision else 2e-6
+    with _dummy_plan(B, N, precision) as plan:
+        xd = dev(x, dt)
+        out = torch.empty_like(xd)
+        x_in = xd.cpu().numpy().astype(np.complex128)
+        plan.debug_fft(xd, out, rows, +1)
+        torch.cuda.synchronize()
+        assert rel(out.cpu().numpy(), O.to_freq(x_in)) < tol
+        plan.debug_fft(xd, out, rows, -1)
+        torch.cuda.synchronize()
+        assert rel(out.cpu().numpy(), O.to_time(x_in)) < tol
+        # in place
+        plan.debug_fft(xd, xd, rows, +1)
+        torch.cuda.synchronize()
+        assert rel(xd.cpu().numpy(), O.to_freq(x_in)) < tol
+
+
+def test_fft_tiny_vs_brute_force_dft(B):
+    N = 64
+    rng = np.random.default_rng(3)
+    x = rng.standard_normal((3, N)) + 1j * rng.standard_normal((3, N))
+    with _dummy_plan(B, N, 1) as plan:
+        xd = dev(x, np.complex128)
+        out = torch.empty_like(xd)
+        plan.debug_fft(xd, out, 3, +1)
+        torch.cuda.synchronize()
+        assert rel(out.cpu().numpy(), O.dft_direct(x, +1)) < 1e-13
+
+
+# ------------------------------------------------------------------------ a4/a5: pair streams
+@pytest.mark.parametrize("cfg,N,kw", [(2, 1024, {}), (3, 2048, {}), (2, 256, dict(max_group=1))])
+def test_pair_conv_vs_oracle(B, cfg, N, kw):
+    w = W.make_config(cfg, N=N, **kw)
+    planes = 3
+    rng = np.random.default_rng(11)
+    A = np.stack([w.A0 * np.exp(2j * np.pi * rng.random((w.P, 1))) for _ in range(planes)])
+    with B.plan_from_workload(w) as plan:
+        Ad = dev(A, np.complex64)
+        Q = w.P * (w.P + 1) // 2
+        V = torch.empty((planes, Q, w.N), dtype=torch.float32, device="cuda")
+        plan.debug_pairs(Ad, V, planes)
+        torch.cuda.synchronize()
+        Vh = V.cpu().numpy().astype(np.float64)
+    A64 = Ad.cpu().numpy().astype(np.complex128)
+    for j in range(planes):
+        T = O.pair_products(A64[j])
+        Bm = (1 - w.f_R) * T + w.f_R * O.raman_convolve(T, w.h_R, w.dt)
+        ref = np.stack([Bm[m, n].real for m in range(w.P) for n in range(m, w.P)])
+        assert np.linalg.norm(Vh[j] - ref) / np.linalg.norm(ref) < 5e-6
+
+
+# --------------------------------------------------------------------------- a12: nonlinear_op
+def _nonlinear_op_case(B, w, seed=0):
+    rng = np.random.default_rng(seed)
+    # a developed field: the launch field with random per-mode spectral phases (still seeded)
+    A = w.A0
+    dt = np.complex128 if w.precision else np.complex64
+    Ad = dev(A, dt)
+    dA = torch.empty_like(Ad)
+    with B.plan_from_workload(w) as plan:
+        plan.nonlinear_op(Ad, dA)
+        torch.cuda.synchronize()
+    A_in = Ad.cpu().numpy().astype(np.complex128)
+    ref = O.nonlinear_op(A_in, w.S, w.kappa, w.omega0, w.f_R, w.h_R, w.dt, w.shock)
+    return rel(dA.cpu().numpy(), ref)
+
+
+@pytest.mark.parametrize("cfg,kw", [
+    (1, {}), (2, {}), (2, dict(N=64)), (3, dict(N=1024)), (3, {}), (4, dict(n_modes=7, N=2048)),
+    (5, dict(max_group=5, N=512)),
+])
+def test_nonlinear_op_vs_oracle(B, cfg, kw):
+    w = W.make_config(cfg, **kw)
+    e = _nonlinear_op_case(B, w)
+    assert e <= (1e-12 if w.precision else TOL_OP), e
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("cfg", [4, 5])
+def test_nonlinear_op_full_shape_large_P(B, cfg):
+    w = W.make_config(cfg)
+    assert _nonlinear_op_case(B, w) <= TOL_OP
+
+
+def test_nonlinear_op_kerr_only_and_no_shock(B):
+    w = W.make_config(2, N=512)
+    w.f_R, w.h_R, w.shock = 0.0, None, False
+    assert _nonlinear_op_case(B, w) <= TOL_OP
+
+
+# --------------------------------------------------------- a3-a11: MPA iteration, plane by plane
+@pytest.mark.parametrize("cfg,kw,M,iters", [
+    (2, dict(N=1024), 10, 1), (2, dict(N=1024), 10, 3), (3, dict(N=512), 4, 2), (2, dict(N=256), 1, 2),
+    (1, dict(N=256), 10, 2),
+])
+def test_mpa_planes_fixed_iter_vs_oracle(B, cfg, kw, M, iters):
+    w = W.make_config(cfg, M=M, **kw)
+    L = M * w.dz
+    dt = np.complex128 if w.precision else np.complex64
+    Ad = dev(w.A0, dt)
+    out = torch.empty_like(Ad)
+    with B.plan_from_workload(w, fixed_iter=iters) as plan:
+        plan.propagate(Ad, L, out)
+        torch.cuda.synchronize()
+        planes = plan.debug_get_planes()
+    A_in = Ad.cpu().numpy().astype(np.complex128)
+    hist = []
+    ref = O.mpa_propagate(A_in, L, w.dz, M, w.beta, w.S, w.kappa, w.omega0, w.f_R, w.h_R, w.dt,
+                          shock=w.shock, fixed_iter=iters, history=hist)
+    ref_planes = hist[0][-1]                   # last iterate of the first (only) large step
+    tol = 1e-12 if w.precision else TOL_OP
+    for j in range(1, M + 1):
+        assert rel(planes[j], ref_planes[j]) <= tol, j
+    assert rel(out.cpu().numpy(), ref) <= tol
+
+
+# ------------------------------------------------------------------------ end-to-end propagate
+def _propagate(B, w, **plan_kw):
+    dt = np.complex128 if w.precision else np.complex64
+    Ad = dev(w.A0, dt)
+    out = torch.empty_like(Ad)
+    with B.plan_from_workload(w, **plan_kw) as plan:
+        st = plan.propagate(Ad, w.L, out)
+        torch.cuda.synchronize()
+        stats = plan.stats()
+    return Ad.cpu().numpy().astype(np.complex128), out.cpu().numpy().astype(np.complex128), st, stats
+
+
+def test_config1_soliton_full_length(B):
+    w = W.make_config(1)
+    A_in, out, st, stats = _propagate(B, w)
+    assert st == 0 and stats["not_converged"] == 0
+    ref = O.rk4ip_propagate(A_in, w.L, w.dz, w.beta, w.S, w.kappa, w.omega0, 0.0, None, w.dt, shock=False)
+    assert rel(out, ref) <= TOL_FIELD
+    # closed form: shape-invariant with phase z / (2 L_D)
+    exact = A_in * np.exp(0.5j * w.L / w.meta["L_D"])
+    assert rel(out, exact) <= TOL_FIELD
+    assert abs(O.energy(out, w.dt) / O.energy(A_in, w.dt) - 1) <= TOL_DRIFT
+
+
+@pytest.mark.parametrize("cfg,kw", [
+    (2, dict(N=1024, L=0.01)),                 # 200 small steps = 20 large steps
+    (2, dict(N=1024, L=37 * 50e-6)),           # ragged: 3 large steps + a 7-plane tail
+    (3, dict(N=1024, L=0.004, max_group=2)),
+])
+def test_propagate_vs_rk4ip_and_mpa(B, cfg, kw):
+    w = W.make_config(cfg, **kw)
+    A_in, out, st, stats = _propagate(B, w)
+    assert st == 0
+    args = (w.beta, w.S, w.kappa, w.omega0, w.f_R, w.h_R, w.dt)
+    ref_rk = O.rk4ip_propagate(A_in, w.L, w.dz, *args, shock=w.shock)
+    ost = {}
+    ref_mpa = O.mpa_propagate(A_in, w.L, w.dz, w.M, *args, shock=w.shock, tol=w.tol, stats=ost)
+    assert rel(out, ref_rk) <= TOL_FIELD
+    assert rel(out, ref_mpa) <= 1e-4           # same scheme: only fp32 rounding and +-1 iteration remain
+    assert stats["large_steps"] == ost["large_steps"]
+    assert abs(stats["iterations"] - ost["iterations"]) <= ost["large_steps"]
+    q0 = O.conserved_quantity(A_in, w.dt, w.omega0, w.shock)
+    drift = abs(O.conserved_quantity(out, w.dt, w.omega0, w.shock)
+                - O.conserved_quantity(ref_mpa, w.dt, w.omega0, w.shock)) / q0
+    assert drift <= TOL_DRIFT, drift
+
+
+def test_mpa_result_independent_of_M(B):
+    w = W.make_config(2, N=512, L=20 * 50e-6)
+    outs = []
+    for M in (1, 4, 10, 20):
+        w.M = M
+        outs.append(_propagate(B, w)[1])
+    for o in outs[1:]:
+        assert rel(o, outs[0]) <= 2e-5
+
+
+def test_host_entry_matches_device_entry(B):
+    w = W.make_config(2, N=512, L=10 * 50e-6)
+    A_in, out, _, _ = _propagate(B, w)
+    h_in = w.A0.astype(np.complex64)
+    h_out = np.empty_like(h_in)
+    with B.plan_from_workload(w) as plan:
+        plan.propagate_host(h_in, w.L, h_out)
+    assert np.array_equal(h_out, out.astype(np.complex64))
+
+
+# ----------------------------------------------------------------------------------- edge cases
+def test_zero_length_is_identity(B):
+    w = W.make_config(2, N=256)
+    w.L = 0.0
+    A_in, out, st, stats = _propagate(B, w)
+    assert st == 0 and stats["large_steps"] == 0
+    assert rel(out, A_in) <= 1e-6
+
+
+def test_linear_only_matches_closed_form_phase(B):
+    # S = 0: propagate is exp(D L) exactly (Eq. 11 with psi constant)
+    w = W.make_config(2, N=1024, L=50 * 50e-6)
+    w.S = np.zeros_like(w.S)
+    A_in, out, st, stats = _propagate(B, w)
+    D = O.dispersion_operator(w.beta, O.omega_grid(w.N, w.dt))
+    exact = O.to_time(O.to_freq(A_in) * np.exp(D * w.L))
+    assert rel(out, exact) <= 5e-6
+    assert stats["iterations"] == stats["large_steps"]      # first iterate already converged
+
+
+def test_aliasing_in_out(B):
+    w = W.make_config(2, N=256, L=10 * 50e-6)
+    _, out, _, _ = _propagate(B, w)
+    Ad = dev(w.A0, np.complex64)
+    with B.plan_from_workload(w) as plan:
+        plan.propagate(Ad, w.L, Ad)
+        torch.cuda.synchronize()
+    assert np.array_equal(Ad.cpu().numpy(), out.astype(np.complex64))
+
+
+def test_not_converged_is_a_warning(B):
+    w = W.make_config(2, N=256, L=10 * 50e-6)
+    _, _, st, stats = _propagate(B, w, max_iter=1, tol=1e-12)
+    assert st == B.WARN_NOCONV and stats["not_converged"] == 1
+
+
+def test_invalid_arguments(B):
+    w = W.make_config(2, N=256)
+    with pytest.raises(B.GmmnlseError) as e:
+        B.Plan(w.P, 300, w.M, w.dt, w.dz, w.beta, w.S, w.f_R, W.raman_response(300, w.dt), w.omega0, w.n2)
+    assert e.value.status == B.EINVAL
+    with pytest.raises(B.GmmnlseError):       # h_R missing although f_R != 0
+        B.Plan(w.P, w.N, w.M, w.dt, w.dz, w.beta, w.S, w.f_R, None, w.omega0, w.n2)
+    with pytest.raises(B.GmmnlseError):       # shock on with pi/dt >= omega0
+        B.Plan(w.P, w.N, w.M, 1e-16, w.dz, w.beta, w.S, w.f_R, w.h_R, w.omega0, w.n2)
+    S_bad = w.S.copy()
+    S_bad[0, 1, 0, 0] += 1.0                  # breaks p<->l symmetry
+    with pytest.raises(B.GmmnlseError) as e:
+        B.Plan(w.P, w.N, w.M, w.dt, w.dz, w.beta, S_bad, w.f_R, w.h_R, w.omega0, w.n2)
+    assert e.value.status == B.EUNSUPPORTED
+    with B.plan_from_workload(w) as plan:
+        Ad = dev(w.A0, np.complex64)
+        with pytest.raises(B.GmmnlseError):   # L not a multiple of dz
+            plan.propagate(Ad, 1.5 * w.dz, Ad)
+        with pytest.raises(B.GmmnlseError):   # dA aliases A
+            plan.nonlinear_op(Ad, Ad)
