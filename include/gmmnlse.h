@@ -41,7 +41,10 @@ typedef struct {                /* pass NULL for defaults                       
   double tol;                   /* MPA convergence threshold, default 1e-6         */
   int    max_iter;              /* cap on iterations per large step; <=0 -> 2*M + 4               */
   int    fixed_iter;            /* >0: run exactly this many iterations per large step (parity)   */
-  int    contraction;           /* 0 = auto, 1 = CUDA-core fp32/fp64 GEMM, 2 = tcgen05 3xTF32     */
+  int    contraction;           /* a6 kernel: 0 = auto (3 when Q = P(P+1)/2 >= 64, complex64, N % 128 == 0; else 1),
+                                   1 = CUDA-core fp32/fp64 GEMM, 2 = tcgen05 3xTF32 on CTA pairs
+                                   (cta_group::2), 3 = tcgen05 3xTF32 single CTA.  2-3 need complex64 and
+                                   N % 128 == 0 (else EUNSUPPORTED)                                */
 } gmmnlse_options;
 
 /* Build a plan: precompute D_w^(p), the rotation tables exp(+-D_w j dz) (j = 0..M) in
@@ -120,6 +123,17 @@ int gmmnlse_debug_get_planes(gmmnlse_plan *plan, void *out_host);
  *          for n_planes planes of A [plane][P][N]  ->  V [plane][Q][N] (real).             */
 int gmmnlse_debug_fft(gmmnlse_plan *plan, const void *in, void *out, int rows, int dir);
 int gmmnlse_debug_pairs(gmmnlse_plan *plan, const void *A, void *V, int n_planes);
+/*   contract: U[plane][r][t] = sum_q S2[r][q] V[plane][q][t] over packed pairs r = (p<=l), q = (m<=n),
+ *          S2 = S_plmn with the m<n columns doubled (Eq. 1's sum over m,n); V, U DEVICE
+ *          [n_planes][Q][N] real of the plan's precision, U must not alias V.
+ *   contraction_kind: which a6 kernel the plan selected: 1 CUDA cores, 2 tcgen05 single CTA,
+ *          3 tcgen05 CTA pairs.                                                              */
+int gmmnlse_debug_contract(gmmnlse_plan *plan, const void *V, void *U, int n_planes);
+int gmmnlse_contraction_kind(const gmmnlse_plan *plan);
+/*   set_tc_chunk: k-blocks (32 packed pairs each) a tensor-memory accumulator holds before the epilogue
+ *          drains it into fp32 registers (default 2); bounds the bias of the tensor core's truncating
+ *          accumulate.  k >= 1.                          */
+int gmmnlse_debug_set_tc_chunk(gmmnlse_plan *plan, int k);
 
 void gmmnlse_plan_destroy(gmmnlse_plan *plan);
 const char *gmmnlse_status_string(int status);

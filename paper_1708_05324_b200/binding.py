@@ -50,6 +50,9 @@ SIGNATURES = {
     "gmmnlse_debug_get_planes": (C.c_int, [C.c_void_p, C.c_void_p]),
     "gmmnlse_debug_fft": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int]),
     "gmmnlse_debug_pairs": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
+    "gmmnlse_debug_contract": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
+    "gmmnlse_contraction_kind": (C.c_int, [C.c_void_p]),
+    "gmmnlse_debug_set_tc_chunk": (C.c_int, [C.c_void_p, C.c_int]),
     "gmmnlse_plan_destroy": (None, [C.c_void_p]),
     "gmmnlse_status_string": (C.c_char_p, [C.c_int]),
     "gmmnlse_last_cuda_error": (C.c_char_p, []),
@@ -168,6 +171,16 @@ class Plan:
 
     def debug_pairs(self, A, V, n_planes: int) -> None:
         _check(self._lib, self._lib.gmmnlse_debug_pairs(self._h, _ptr(A), _ptr(V), n_planes))
+
+    def debug_contract(self, V, U, n_planes: int) -> None:
+        _check(self._lib, self._lib.gmmnlse_debug_contract(self._h, _ptr(V), _ptr(U), n_planes))
+
+    def contraction_kind(self) -> int:
+        """1 = CUDA cores, 2 = tcgen05 single CTA, 3 = tcgen05 CTA pairs."""
+        return int(self._lib.gmmnlse_contraction_kind(self._h))
+
+    def debug_set_tc_chunk(self, k: int) -> None:
+        _check(self._lib, self._lib.gmmnlse_debug_set_tc_chunk(self._h, int(k)))
 
     def destroy(self) -> None:
         if self._h:

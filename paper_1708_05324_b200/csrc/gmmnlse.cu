@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "../../include/gmmnlse.h"
+#include "gemm_tc.cuh"
 #include "kernels.cuh"
 
 namespace {
@@ -54,6 +55,46 @@ void host_fft(std::vector<cd>& a, int sign) {   // iterative radix-2, fp64; plan
         a[i + k + len / 2] = u - v;
       }
   }
+}
+
+// fp32 value rounded to TF32 (10 explicit mantissa bits), round to nearest even; finite inputs only
+float round_tf32(double x) {
+  float f = (float)x;
+  uint32_t u;
+  std::memcpy(&u, &f, 4);
+  u += 0xFFFu + ((u >> 13) & 1u);
+  u &= 0xFFFFE000u;
+  std::memcpy(&f, &u, 4);
+  return f;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// fp32 tensor map, 128-byte swizzle span (16- or 32-byte atoms); dims/box innermost first; strides in bytes for dims 1..rank-1
+int encode_tmap_f32(CUtensorMap* out, void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides,
+                    const cuuint32_t* box, CUtensorMapSwizzle swz) {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* ptr = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &q);
+    if (e != cudaSuccess || q != cudaDriverEntryPointSuccess || !ptr) {
+      g_cuda_err = "cudaGetDriverEntryPoint(cuTensorMapEncodeTiled) failed";
+      return GMMNLSE_ECUDA;
+    }
+    fn = (EncodeTiledFn)ptr;
+  }
+  const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+  CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, (cuuint32_t)rank, base, dims, strides, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, swz, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    g_cuda_err = "cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)r);
+    return GMMNLSE_ECUDA;
+  }
+  return 0;
 }
 
 int ilog2(int n) {
@@ -117,6 +158,9 @@ struct gmmnlse_plan {
   virtual int get_planes(void* out) = 0;
   virtual int debug_fft(const void* in, void* out, int rows, int dir) = 0;
   virtual int debug_pairs(const void* A, void* V, int n_planes) = 0;
+  virtual int debug_contract(const void* V, void* U, int n_planes) = 0;
+  virtual int contraction_kind() const = 0;
+  virtual int set_tc_chunk(int k) = 0;
 };
 
 namespace {
@@ -140,11 +184,16 @@ struct PlanT final : gmmnlse_plan {
   C* d_io = nullptr;
   std::map<int, double2*> EM_ragged;
   long long PN = 0, QN = 0;
+  // tcgen05 contraction (complex64 path only): TF32 hi/lo split of S2, zero-padded to [R_pad][Q_pad]
+  float *S2hi = nullptr, *S2lo = nullptr;
+  CUtensorMap tmV, tmShi, tmSlo;
+  int tc_cg = 0, tc_NT = 0, tc_nrt = 0, tc_KB = 0, tc_stages = 0, tc_kchunk = 2, n_sm = 0;
 
   ~PlanT() override {
     cudaFree(tw); cudaFree(Kw); cudaFree(H); cudaFree(E); cudaFree(EM_d); cudaFree(S2);
     cudaFree(pair_m); cudaFree(pair_n); cudaFree(psi0_d); cudaFree(psi); cudaFree(At); cudaFree(G);
     cudaFree(V); cudaFree(U); cudaFree(errbuf); cudaFree(d_err); cudaFree(d_io);
+    cudaFree(S2hi); cudaFree(S2lo);
     if (h_err) cudaFreeHost(h_err);
     if (h_in) cudaFreeHost(h_in);
     if (h_out) cudaFreeHost(h_out);
@@ -211,10 +260,12 @@ struct PlanT final : gmmnlse_plan {
         for (int n = m; n < P; ++n, ++q) { pm[q] = m; pn[q] = n; }
     }
     std::vector<T> h_S2((size_t)Q * Q);
+    std::vector<double> h_S2d((size_t)Q * Q);
     for (int r = 0; r < Q; ++r)
       for (int q = 0; q < Q; ++q) {
         const size_t idx = (((size_t)pm[r] * P + pn[r]) * P + pm[q]) * P + pn[q];
-        h_S2[(size_t)r * Q + q] = (T)(S[idx] * (pm[q] == pn[q] ? 1.0 : 2.0));
+        h_S2d[(size_t)r * Q + q] = S[idx] * (pm[q] == pn[q] ? 1.0 : 2.0);
+        h_S2[(size_t)r * Q + q] = (T)h_S2d[(size_t)r * Q + q];
       }
     GM_TRY(dalloc(&tw, N)); GM_TRY(upload(tw, h_tw));
     GM_TRY(dalloc(&Kw, N)); GM_TRY(upload(Kw, h_K));
@@ -235,7 +286,104 @@ struct PlanT final : gmmnlse_plan {
     GM_CUDA(cudaMemset(errbuf, 0, sizeof(double) * 2 * (M + 2)));
     GM_CUDA(cudaMemset(psi, 0, sizeof(C) * (size_t)(M + 1) * PN));
     GM_CUDA(cudaMallocHost((void**)&h_err, sizeof(double)));
+    GM_TRY(init_tc(h_S2d));
     return 0;
+  }
+
+  // ------------------------------------------------------------------ tcgen05 contraction setup
+  // contraction option: 0 auto (tensor cores when Q >= 64), 1 CUDA cores, 2 tcgen05 cta_group::2,
+  // 3 tcgen05 cta_group::1.
+  int make_v_tmap(CUtensorMap* tm, const T* base, int planes) {
+    const cuuint64_t dims[3] = {(cuuint64_t)N, (cuuint64_t)Q, (cuuint64_t)planes};
+    const cuuint64_t strides[2] = {(cuuint64_t)N * 4, (cuuint64_t)QN * 4};
+    const cuuint32_t box[3] = {32, tc::BK, 1};
+    // t-contiguous operand: 32-byte swizzle atoms (the only MN-major layout kind::tf32 accepts)
+    return encode_tmap_f32(tm, (void*)base, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B);
+  }
+  int init_tc(const std::vector<double>& h_S2) {
+    if constexpr (sizeof(T) != 4) {
+      if (contraction >= 2) return GMMNLSE_EUNSUPPORTED;
+      return 0;
+    } else {
+      const bool want = contraction >= 2 || (contraction == 0 && Q >= 64);
+      if (!want) return 0;
+      // auto picks the single-CTA form: measured 1.76 ms against 1.86 ms for CTA pairs at config 5
+      int cg = contraction == 2 ? 2 : 1;
+      if (N % (tc::TM * cg) != 0) {
+        if (N % tc::TM == 0) cg = 1;
+        else if (contraction >= 2) return GMMNLSE_EUNSUPPORTED;
+        else return 0;
+      }
+      int dev = 0;
+      GM_CUDA(cudaGetDevice(&dev));
+      GM_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+      tc_nrt = (Q + 207) / 208;                                  // NT <= 208: 3 epilogue slices of <= 72
+      tc_NT = (((Q + tc_nrt - 1) / tc_nrt) + 15) / 16 * 16;
+      tc_KB = (Q + tc::BK - 1) / tc::BK;
+      const int Rp = tc_nrt * tc_NT, Qp = tc_KB * tc::BK;
+      int smax = 0;
+      GM_CUDA(cudaDeviceGetAttribute(&smax, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+      tc_stages = tc::MAX_STAGES;
+      while (tc_stages > 1 && tc::smem_bytes(tc_NT, cg, tc_stages) > (size_t)smax) --tc_stages;
+      if (tc::smem_bytes(tc_NT, cg, tc_stages) > (size_t)smax) return GMMNLSE_EUNSUPPORTED;
+      std::vector<float> hi((size_t)Rp * Qp, 0.f), lo((size_t)Rp * Qp, 0.f);
+      for (int r = 0; r < Q; ++r)
+        for (int q = 0; q < Q; ++q) {
+          const double s = h_S2[(size_t)r * Q + q];
+          const float h = round_tf32(s);
+          hi[(size_t)r * Qp + q] = h;
+          lo[(size_t)r * Qp + q] = round_tf32(s - (double)h);
+        }
+      GM_TRY(dalloc(&S2hi, hi.size())); GM_TRY(upload(S2hi, hi));
+      GM_TRY(dalloc(&S2lo, lo.size())); GM_TRY(upload(S2lo, lo));
+      const cuuint64_t dims[2] = {(cuuint64_t)Qp, (cuuint64_t)Rp};
+      const cuuint64_t strides[1] = {(cuuint64_t)Qp * 4};
+      const cuuint32_t box[2] = {tc::BK, (cuuint32_t)(tc_NT / cg)};
+      GM_TRY(encode_tmap_f32(&tmShi, S2hi, 2, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B));
+      GM_TRY(encode_tmap_f32(&tmSlo, S2lo, 2, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B));
+      GM_TRY(make_v_tmap(&tmV, V, M + 1));
+      const int smem = (int)tc::smem_bytes(tc_NT, cg, tc_stages);
+      if (cg == 2)
+        GM_CUDA(cudaFuncSetAttribute(tc::k_contract_tc<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+      else
+        GM_CUDA(cudaFuncSetAttribute(tc::k_contract_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+      tc_cg = cg;
+      return 0;
+    }
+  }
+
+  int launch_contract_tc(const CUtensorMap& vmap, int plane0, T* Uout, int planes) {
+    if constexpr (sizeof(T) != 4) {
+      return GMMNLSE_EUNSUPPORTED;
+    } else {
+      tc::Params prm;
+      prm.U = Uout;
+      prm.u_plane_stride = QN;
+      prm.Q = Q; prm.N = N; prm.NT = tc_NT; prm.KB = tc_KB; prm.n_rt = tc_nrt;
+      prm.t_tiles = N / (tc::TM * tc_cg);
+      prm.total_tiles = planes * prm.t_tiles * tc_nrt;
+      prm.plane0 = plane0; prm.stages = tc_stages; prm.kchunk = tc_kchunk;
+      const int pairs = std::min(n_sm / tc_cg, prm.total_tiles);
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)(pairs * tc_cg));
+      cfg.blockDim = dim3(tc::NTHREADS);
+      cfg.dynamicSmemBytes = tc::smem_bytes(tc_NT, tc_cg, tc_stages);
+      cfg.stream = stream;
+      cudaLaunchAttribute attr[1];
+      attr[0].id = cudaLaunchAttributeClusterDimension;
+      attr[0].val.clusterDim.x = (unsigned)tc_cg;
+      attr[0].val.clusterDim.y = 1;
+      attr[0].val.clusterDim.z = 1;
+      cfg.attrs = attr;
+      cfg.numAttrs = 1;
+      prof_begin(GMMNLSE_KIND_CONTRACT);
+      cudaError_t e;
+      if (tc_cg == 2) e = cudaLaunchKernelEx(&cfg, tc::k_contract_tc<2>, vmap, tmShi, tmSlo, prm);
+      else e = cudaLaunchKernelEx(&cfg, tc::k_contract_tc<1>, vmap, tmShi, tmSlo, prm);
+      prof_end();
+      GM_CUDA(e);
+      return 0;
+    }
   }
 
   // ------------------------------------------------------------------ kernel launchers
@@ -319,6 +467,13 @@ struct PlanT final : gmmnlse_plan {
   }
 
   int launch_contract(const T* Vin, T* Uout, int planes) {
+    if (tc_cg) {
+      if (Vin >= V && Vin < V + (size_t)(M + 1) * QN)              // the plan's own buffer
+        return launch_contract_tc(tmV, (int)((Vin - V) / QN), Uout, planes);
+      CUtensorMap tmp;
+      GM_TRY(make_v_tmap(&tmp, Vin, planes));
+      return launch_contract_tc(tmp, 0, Uout, planes);
+    }
     prof_begin(GMMNLSE_KIND_CONTRACT);
     if (Q <= 32) {
       constexpr int BM = 32, BN = 128, BK = 8, TM = 4, TN = 4;
@@ -335,14 +490,15 @@ struct PlanT final : gmmnlse_plan {
   }
 
   int launch_mode_reduce(const T* Uin, const C* A, C* Nout, int planes) {
-    const size_t smem = sizeof(C) * 2 * P * 128;
+    const size_t smem = sizeof(C) * P * 128;
     static size_t configured = 0;
     if (smem > configured) {
       GM_CUDA(cudaFuncSetAttribute(k_mode_reduce<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       configured = smem;
     }
+    const int G = P >= 12 ? 4 : (P >= 4 ? 2 : 1);              // mode groups per CTA
     prof_begin(GMMNLSE_KIND_MODE_REDUCE);
-    k_mode_reduce<T><<<dim3((N + 127) / 128, planes), 128, smem, stream>>>(Uin, QN, A, PN, Nout, PN, P, N);
+    k_mode_reduce<T><<<dim3((N + 127) / 128, planes), 128 * G, smem, stream>>>(Uin, QN, A, PN, Nout, PN, P, N);
     prof_end();
     GM_CUDA(cudaGetLastError());
     return 0;
@@ -392,7 +548,8 @@ struct PlanT final : gmmnlse_plan {
       GM_TRY(launch_fft(+1, G + j0 * PN, PN, G + j0 * PN, PN, nullptr, Kw, E + j0 * PN, PN, (T)1, P, np));
       // a9 + a10
       prof_begin(GMMNLSE_KIND_SCAN);
-      k_trapz_scan<T><<<sblocks, 256, 0, stream>>>(psi, G, psi, PN, Mc, (T)dz, it == 0 ? 1 : 0, errbuf, PN);
+      k_trapz_scan<T><<<sblocks, 256, sizeof(double) * 2 * (Mc + 1), stream>>>(psi, G, psi, PN, Mc, (T)dz,
+                                                                               it == 0 ? 1 : 0, errbuf, PN);
       prof_end();
       prof_begin(GMMNLSE_KIND_MISC);
       k_err_finalize<<<1, 32, 0, stream>>>(errbuf, Mc, d_err);
@@ -485,6 +642,16 @@ struct PlanT final : gmmnlse_plan {
   int debug_pairs(const void* A, void* Vout, int n_planes) override {
     if (n_planes < 1) return GMMNLSE_EINVAL;
     return launch_pairs((const C*)A, PN, (T*)Vout, QN, n_planes);
+  }
+  int contraction_kind() const override { return tc_cg ? 1 + tc_cg : 1; }
+  int set_tc_chunk(int k) override {
+    if (k < 1) return GMMNLSE_EINVAL;
+    tc_kchunk = k;
+    return 0;
+  }
+  int debug_contract(const void* Vin, void* Uout, int n_planes) override {
+    if (n_planes < 1) return GMMNLSE_EINVAL;
+    return launch_contract((const T*)Vin, (T*)Uout, n_planes);
   }
 };
 
@@ -639,6 +806,15 @@ int gmmnlse_debug_pairs(gmmnlse_plan* plan, const void* A, void* V, int n_planes
   if (!plan || !A || !V) return GMMNLSE_EINVAL;
   return plan->debug_pairs(A, V, n_planes);
 }
+
+int gmmnlse_debug_contract(gmmnlse_plan* plan, const void* V, void* U, int n_planes) {
+  if (!plan || !V || !U || V == U) return GMMNLSE_EINVAL;
+  return plan->debug_contract(V, U, n_planes);
+}
+
+int gmmnlse_contraction_kind(const gmmnlse_plan* plan) { return plan ? plan->contraction_kind() : 0; }
+
+int gmmnlse_debug_set_tc_chunk(gmmnlse_plan* plan, int k) { return plan ? plan->set_tc_chunk(k) : GMMNLSE_EINVAL; }
 
 void gmmnlse_plan_destroy(gmmnlse_plan* plan) { delete plan; }
 

@@ -149,40 +149,48 @@ k_contract(const T* __restrict__ S2, const T* __restrict__ V, long long v_plane_
 }
 
 // ------------------------------------------------------------------------------------------
-// a7: N_p(t) = sum_l U_pl(t) A_l(t), U real symmetric, stored packed (p <= l).
-//   grid = (N / 128, n_planes), 128 threads: thread t owns one sample; accumulators in smem.
+// a7: N_p(t) = sum_l U_pl(t) A_l(t), U real symmetric, stored packed: row r(p,l) = p P - p(p-1)/2 + (l-p)
+// for p <= l.  grid = (N / 128, n_planes); blockDim = 128 * G: thread (tx, g) owns sample t = 128 bx + tx
+// and modes p = g, g + G, ...; the A tile [P][128] is staged in shared memory, the accumulator of one
+// (p, t) lives in registers, so the U loads of a row are independent and pipeline freely.  Each U value
+// is read twice (once as U_pl, once as U_lp) by threads of the same CTA: the second read hits L1/L2.
 template <typename T>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(512)
 k_mode_reduce(const T* __restrict__ U, long long u_plane_stride, const cplx<T>* __restrict__ A,
               long long a_plane_stride, cplx<T>* __restrict__ Nt, long long n_plane_stride, int P, int N) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* a_s = reinterpret_cast<cplx<T>*>(smem_raw);        // [P][128]
-  cplx<T>* acc = a_s + P * 128;                               // [P][128]
-  const int t = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, tx = threadIdx.x;
-  if (t >= N) return;
-  const T* Uj = U + j * u_plane_stride;
-  const cplx<T>* Aj = A + j * a_plane_stride;
-  for (int p = 0; p < P; ++p) {
-    a_s[p * 128 + tx] = Aj[(long long)p * N + t];
-    acc[p * 128 + tx] = mk((T)0, (T)0);
+  const int tx = threadIdx.x & 127, g = threadIdx.x >> 7, G = blockDim.x >> 7, j = blockIdx.y;
+  const int t0 = blockIdx.x * 128;
+  const cplx<T>* Aj = A + j * a_plane_stride + t0;
+  for (int i = threadIdx.x; i < P * 128; i += blockDim.x) {
+    const int x = i & 127;
+    a_s[i] = t0 + x < N ? Aj[(long long)(i >> 7) * N + x] : mk((T)0, (T)0);
   }
-  int r = 0;
-  for (int p = 0; p < P; ++p) {
-    cplx<T> ap = a_s[p * 128 + tx];
-    cplx<T> sp = acc[p * 128 + tx];
-    for (int l = p; l < P; ++l, ++r) {
-      const T u = Uj[(long long)r * N + t];
-      cplx<T> al = a_s[l * 128 + tx];
-      sp.x += u * al.x;
-      sp.y += u * al.y;
-      if (l != p) {
-        cplx<T> sl = acc[l * 128 + tx];
-        sl.x += u * ap.x;
-        sl.y += u * ap.y;
-        acc[l * 128 + tx] = sl;
-      }
+  __syncthreads();
+  const int t = t0 + tx;
+  if (t >= N) return;
+  const T* Ut = U + j * u_plane_stride + t;
+  const cplx<T>* at = a_s + tx;
+  for (int p = g; p < P; p += G) {
+    T sx = 0, sy = 0;
+    long long r = p;                                  // r(0, p)
+#pragma unroll 8
+    for (int l = 0; l < p; ++l) {                     // column part: U_lp, l < p
+      const T u = Ut[r * N];
+      const cplx<T> a = at[l * 128];
+      sx += u * a.x;
+      sy += u * a.y;
+      r += P - l - 1;                                 // r(l+1, p) - r(l, p)
     }
-    Nt[j * n_plane_stride + (long long)p * N + t] = sp;
+#pragma unroll 8
+    for (int l = p; l < P; ++l, ++r) {                // row part: U_pl, l >= p; r == r(p, p) here
+      const T u = Ut[r * N];
+      const cplx<T> a = at[l * 128];
+      sx += u * a.x;
+      sy += u * a.y;
+    }
+    Nt[j * n_plane_stride + (long long)p * N + t] = mk(sx, sy);
   }
 }
 
@@ -190,40 +198,54 @@ k_mode_reduce(const T* __restrict__ U, long long u_plane_stride, const cplx<T>* 
 // a9 + a10: cumulative trapezoid over planes and the per-plane error norms.
 //   psi_j^new = psi_0 + dz [G_0/2 + G_1 + .. + G_{j-1} + G_j/2], j = 1..Mc
 //   errbuf[2 j] += sum |psi_j^new - psi_j^old|^2,  errbuf[2 j + 1] += sum |psi_j^new|^2
-// One thread per (p, w); 256-thread blocks; double atomics, one per plane per warp.
+// One thread per (p, w); 256-thread blocks.  Planes are walked four at a time so that the eight loads
+// of a batch are in flight together; norms are reduced warp -> shared memory (fp64) -> one global
+// atomic per plane per block (a global atomic per warp serialised on 2 Mc addresses: 0.36 ms at config 5).
+// Dynamic shared memory: 2 (Mc + 1) doubles.
 template <typename T>
 __global__ void __launch_bounds__(256)
 k_trapz_scan(const cplx<T>* __restrict__ psi0, const cplx<T>* __restrict__ G, cplx<T>* __restrict__ psi,
              long long plane_stride, int Mc, T dz, int first_iter, double* __restrict__ errbuf, long long PN) {
+  extern __shared__ double s_err[];
+  for (int i = threadIdx.x; i < 2 * (Mc + 1); i += blockDim.x) s_err[i] = 0.0;
+  __syncthreads();
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const bool live = i < PN;
-  cplx<T> p0 = mk((T)0, (T)0), acc = p0;
-  if (live) {
-    p0 = psi0[i];
-    acc = cscale(G[i], (T)0.5);
-  }
-  for (int j = 1; j <= Mc; ++j) {
-    T num = 0, den = 0;
-    if (live) {
-      const cplx<T> g = G[j * plane_stride + i];
-      cplx<T> pn = mk(p0.x + dz * (acc.x + (T)0.5 * g.x), p0.y + dz * (acc.y + (T)0.5 * g.y));
-      acc = cadd(acc, g);
-      const cplx<T> old = first_iter ? p0 : psi[j * plane_stride + i];
-      const cplx<T> d = csub(pn, old);
-      num = d.x * d.x + d.y * d.y;
-      den = pn.x * pn.x + pn.y * pn.y;
-      psi[j * plane_stride + i] = pn;
+  const long long ii = live ? i : 0;                 // dead threads read a valid address, write nothing
+  const cplx<T> p0 = psi0[ii];
+  cplx<T> acc = cscale(G[ii], (T)0.5);
+  constexpr int B = 4;
+  for (int j0 = 1; j0 <= Mc; j0 += B) {
+    cplx<T> g[B], old[B];
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+      const int j = min(j0 + b, Mc);
+      g[b] = G[j * plane_stride + ii];
+      old[b] = first_iter ? p0 : psi[j * plane_stride + ii];
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      num += __shfl_xor_sync(0xffffffffu, num, o);
-      den += __shfl_xor_sync(0xffffffffu, den, o);
-    }
-    if ((threadIdx.x & 31) == 0) {
-      atomicAdd(&errbuf[2 * j], (double)num);
-      atomicAdd(&errbuf[2 * j + 1], (double)den);
+    for (int b = 0; b < B; ++b) {
+      const int j = j0 + b;
+      if (j > Mc) break;
+      const cplx<T> pn = mk(p0.x + dz * (acc.x + (T)0.5 * g[b].x), p0.y + dz * (acc.y + (T)0.5 * g[b].y));
+      acc = cadd(acc, g[b]);
+      const cplx<T> d = csub(pn, old[b]);
+      T num = live ? d.x * d.x + d.y * d.y : (T)0;
+      T den = live ? pn.x * pn.x + pn.y * pn.y : (T)0;
+      if (live) psi[j * plane_stride + i] = pn;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        num += __shfl_xor_sync(0xffffffffu, num, o);
+        den += __shfl_xor_sync(0xffffffffu, den, o);
+      }
+      if ((threadIdx.x & 31) == 0) {
+        atomicAdd(&s_err[2 * j], (double)num);
+        atomicAdd(&s_err[2 * j + 1], (double)den);
+      }
     }
   }
+  __syncthreads();
+  for (int k = 2 + threadIdx.x; k < 2 * (Mc + 1); k += blockDim.x) atomicAdd(&errbuf[k], s_err[k]);
 }
 
 // err = max_j sqrt(num_j / den_j); result -> out[0]; accumulators cleared for the next iteration

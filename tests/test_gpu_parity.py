@@ -289,3 +289,62 @@ def test_invalid_arguments(B):
             plan.propagate(Ad, 1.5 * w.dz, Ad)
         with pytest.raises(B.GmmnlseError):   # dA aliases A
             plan.nonlinear_op(Ad, Ad)
+
+
+# ------------------------------------------------------------------------ a6: S contraction
+def _packed_S2(S):
+    """[Q][Q] packed coupling matrix of Eq. 1's sum over (m, n): rows (p <= l), columns (m <= n), the
+    m < n columns doubled because V_nm = V_mn for real S."""
+    P = S.shape[0]
+    iu = np.triu_indices(P)
+    Q = iu[0].size
+    S2 = S.reshape(P * P, P, P)[:, iu[0], iu[1]] * np.where(iu[0] == iu[1], 1.0, 2.0)[None, :]
+    return S2.reshape(P, P, Q)[iu[0], iu[1], :]
+
+
+@pytest.mark.parametrize("cfg,N,kw,kind", [
+    (3, 1024, {}, 1), (3, 1024, {}, 3), (3, 1024, {}, 2),          # Q = 120: one r-tile of 128, K = 4 blocks
+    (4, 512, {}, 3), (4, 512, {}, 2),                              # Q = 210: two r-tiles of 112
+    (5, 256, {}, 3), (5, 256, {}, 2), (5, 256, {}, 1),             # Q = 1035: five r-tiles of 208, ragged K
+    (3, 128, dict(max_group=3), 3),                                # Q = 55 < 64: tensor path forced, N = 128
+])
+def test_contraction_vs_fp64_matmul(B, cfg, N, kw, kind):
+    w = W.make_config(cfg, N=N, **kw)
+    Q = w.P * (w.P + 1) // 2
+    planes = 3
+    rng = np.random.default_rng(cfg * 100 + kind)
+    # pair streams with the dynamic range of |A|^2 products: peak to 1e-6 of peak along t
+    V = (rng.standard_normal((planes, Q, N)) * np.exp(rng.uniform(-7, 7, (planes, 1, N)))).astype(np.float32)
+    with B.plan_from_workload(w, contraction=kind) as plan:
+        assert plan.contraction_kind() == {1: 1, 2: 3, 3: 2}[kind]
+        Vd = torch.from_numpy(V).cuda()
+        U = torch.full((planes, Q, N), float("nan"), dtype=torch.float32, device="cuda")
+        plan.debug_contract(Vd, U, planes)
+        torch.cuda.synchronize()
+        Uh = U.cpu().numpy().astype(np.float64)
+    # the definition, written out with the oracle-side tensor: U_pl = sum_mn S_plmn V_mn, V symmetric
+    P = w.P
+    iu = np.triu_indices(P)
+    Vfull = np.zeros((planes, P, P, N))
+    Vfull[:, iu[0], iu[1], :] = V
+    Vfull[:, iu[1], iu[0], :] = V
+    ref_full = np.einsum("ab,jbt->jat", w.S.reshape(P * P, P * P), Vfull.reshape(planes, P * P, N))
+    ref = ref_full.reshape(planes, P, P, N)[:, iu[0], iu[1], :]
+    assert np.isfinite(Uh).all()
+    assert np.linalg.norm(Uh - ref) / np.linalg.norm(ref) <= 1e-6
+    # column-wise (per time sample and plane): no sample may be off by more than a few fp32 ulps of its scale
+    col = np.linalg.norm(Uh - ref, axis=1) / np.linalg.norm(ref, axis=1)
+    assert col.max() <= 3e-6, col.max()
+
+
+def test_contraction_auto_selects_tensor_cores_for_large_P(B):
+    w = W.make_config(3, N=1024)
+    with B.plan_from_workload(w) as plan:
+        assert plan.contraction_kind() == 2
+    w = W.make_config(2, N=1024)
+    with B.plan_from_workload(w) as plan:
+        assert plan.contraction_kind() == 1
+    w = W.make_config(1)
+    with pytest.raises(B.GmmnlseError) as e:           # complex128 has no tensor-core path
+        B.plan_from_workload(w, contraction=3)
+    assert e.value.status == B.EUNSUPPORTED
