@@ -130,8 +130,8 @@ int gmmnlse_debug_pairs(gmmnlse_plan *plan, const void *A, void *V, int n_planes
  *          3 tcgen05 CTA pairs.                                                              */
 int gmmnlse_debug_contract(gmmnlse_plan *plan, const void *V, void *U, int n_planes);
 int gmmnlse_contraction_kind(const gmmnlse_plan *plan);
-/*   set_tc_chunk: k-blocks (32 packed pairs each) a tensor-memory accumulator holds before the epilogue
- *          drains it into fp32 registers (default 2); bounds the bias of the tensor core's truncating
+/*   set_tc_chunk: k-blocks (16 packed pairs each) a tensor-memory accumulator holds before the epilogue
+ *          drains it into fp32 registers (default 4); bounds the bias of the tensor core's truncating
  *          accumulate.  k >= 1.                          */
 int gmmnlse_debug_set_tc_chunk(gmmnlse_plan *plan, int k);
 

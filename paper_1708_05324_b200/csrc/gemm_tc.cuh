@@ -8,7 +8,9 @@
 //     (one column r at a time, 32 lanes = 32 consecutive t) are coalesced into U[r][t].
 //   * N = r: NT packed pair rows per tile, NT = 16-multiple <= 256 chosen so that n_rt*NT >= Q with
 //     < 2 % padding (Q = 1035 -> 5 x 208).
-//   * K = q: 32 per k-block (one 128-byte swizzle row of fp32), 4 MMAs of K = 8 per product.
+//   * K = q: BK = 16 per k-block (a 64-byte swizzle row of S2), 2 MMAs of K = 8 per product; the small
+//     k-block lets 5 stages (43 KB each) fit in shared memory: with BK = 32 only 2 fit and the MMA pipe
+//     starved on TMA latency (measured 1.58 ms against a 1.06 ms MMA-only floor at config 5).
 //   A is "MN-major" (t contiguous in V[q][t]) in the 32-byte-atom 128-byte swizzle, the one MN-major
 //   layout kind::tf32 accepts; B is K-major (q contiguous in S2[r][q]) in the plain 128-byte swizzle.
 //
@@ -36,13 +38,15 @@
 namespace gm {
 namespace tc {
 
-constexpr int BK = 32;                                  // q per k-block
+constexpr int BK = 16;                                  // q per k-block (16: 5 smem stages fit; 32: only 2)
+constexpr int B_LAYOUT = BK == 32 ? 2 : 4;              // smem descriptor layout type of B: SWIZZLE_128B / SWIZZLE_64B
+constexpr int B_SBO = 8 * BK * 4;                       // bytes between 8-row groups of B
 constexpr int TM = 128;                                 // t per CTA
 constexpr int NUM_EPI_WARPS = 12;                       // 3 per TMEM lane group
 constexpr int NTHREADS = 32 * (6 + NUM_EPI_WARPS);      // 576
 constexpr int EPI_COLS = 72;                            // max columns one epilogue warp accumulates
 constexpr int A_BYTES = TM * BK * 4;                    // 16 KiB: one A tile (raw or lo)
-constexpr int MAX_STAGES = 4;
+constexpr int MAX_STAGES = 8;
 constexpr int TMEM_COLS = 512;
 constexpr int ACC_COLS = 256;                           // column stride between the two accumulators
 
@@ -50,6 +54,8 @@ struct Params {
   float* U;                    // [plane][Q][N]
   long long u_plane_stride;    // elements
   int Q, N, NT, KB, n_rt, t_tiles, total_tiles, plane0, stages, kchunk;
+  int probe;                   // timing probes only (results wrong): 1 skip V_lo conversion, 2 skip TMA after the first
+                               // fill, 4 skip the U stores
 };
 
 __host__ __device__ inline int b_bytes(int NT, int CG) { return (NT / CG) * BK * 4; }
@@ -67,10 +73,10 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
   const uint32_t raw_addr = smem_u32(smem_raw);
   const uint32_t base = (raw_addr + 1023u) & ~1023u;     // 1024-byte aligned: swizzle atoms
   unsigned char* sm = smem_raw + (base - raw_addr);
-  // barrier block (first 1 KiB): full[4] empty[4] conv[4] tmem_full[2] tmem_empty[2] tmem_slot
-  const uint32_t bar_full = base, bar_empty = base + 32, bar_conv = base + 64, bar_tfull = base + 96,
-                 bar_tempty = base + 112, slot_addr = base + 128;
-  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(sm + 128);
+  // barrier block (first 1 KiB): full[8] empty[8] conv[8] tmem_full[2] tmem_empty[2] tmem_slot
+  const uint32_t bar_full = base, bar_empty = base + 64, bar_conv = base + 128, bar_tfull = base + 192,
+                 bar_tempty = base + 208, slot_addr = base + 224;
+  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(sm + 224);
   const uint32_t tiles_addr = base + 1024;
   unsigned char* tiles_ptr = sm + 1024;
 
@@ -114,7 +120,6 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
-      const uint32_t tx = (uint32_t)(A_BYTES + 2 * nb);
       for (int tile = pair; tile < p.total_tiles; tile += npairs) {
         const int pl = tile / tiles_per_plane, rem = tile - pl * tiles_per_plane;
         const int tt = rem / p.n_rt, rt = rem - tt * p.n_rt;
@@ -124,12 +129,22 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
           mbar_wait(bar_empty + 8 * stage, phase ^ 1u, 1);
           const uint32_t fb = bar_full + 8 * stage;
           const uint32_t sa = tiles_addr + stage * sbytes;
-          mbar_arrive_expect_tx(fb, tx);
+          const bool warm = tile != pair || kb >= stages;
+          const bool skipA = warm && (p.probe & (2 | 8)), skipB = warm && (p.probe & (2 | 16));
+          if (skipA && skipB) {
+            mbar_arrive(fb);
+          } else {
+            mbar_arrive_expect_tx(fb, (skipA ? 0u : (uint32_t)A_BYTES) + (skipB ? 0u : (uint32_t)(2 * nb)));
+            if (!skipA) {
 #pragma unroll
-          for (int i = 0; i < TM / 32; ++i)                       // 4 boxes of 32 t x 32 q
-            tma_load_3d(sa + i * (BK * 128), &tmV, fb, t0 + 32 * i, kb * BK, p.plane0 + pl);
-          tma_load_2d(sa + 2 * A_BYTES, &tmShi, fb, kb * BK, r0);
-          tma_load_2d(sa + 2 * A_BYTES + nb, &tmSlo, fb, kb * BK, r0);
+              for (int i = 0; i < TM / 32; ++i)                   // 4 boxes of 32 t x BK q
+                tma_load_3d(sa + i * (BK * 128), &tmV, fb, t0 + 32 * i, kb * BK, p.plane0 + pl);
+            }
+            if (!skipB) {
+              tma_load_2d(sa + 2 * A_BYTES, &tmShi, fb, kb * BK, r0);
+              tma_load_2d(sa + 2 * A_BYTES + nb, &tmSlo, fb, kb * BK, r0);
+            }
+          }
           if (++stage == stages) { stage = 0; phase ^= 1u; }
         }
       }
@@ -156,9 +171,10 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
           // (128 B) per q, 4-q groups 512 B apart (SBO), 32-t groups BK*128 B apart (LBO)
           const uint64_t a_raw = make_smem_desc(sa, BK * 128, 512, 1);
           const uint64_t a_lo = make_smem_desc(sa + A_BYTES, BK * 128, 512, 1);
-          // B: K-major, 8-row groups 1024 B apart (SBO); LBO unused for swizzled K-major
-          const uint64_t b_hi = make_smem_desc(sa + 2 * A_BYTES, 16, 1024, 2);
-          const uint64_t b_lo = make_smem_desc(sa + 2 * A_BYTES + nb, 16, 1024, 2);
+          // B: K-major rows of BK q (64 B: SWIZZLE_64B), 8-row groups B_SBO apart; LBO unused when swizzled
+          const uint64_t b_hi = make_smem_desc(sa + 2 * A_BYTES, 16, B_SBO, B_LAYOUT);
+          const uint64_t b_lo = make_smem_desc(sa + 2 * A_BYTES + nb, 16, B_SBO, B_LAYOUT);
+          if (!(p.probe & 32))
 #pragma unroll
           for (int kk = 0; kk < BK / 8; ++kk) {
             const uint64_t da = (uint64_t)(kk * (1024 >> 4));      // next 8 q of A: +1024 B
@@ -187,6 +203,7 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
         mbar_wait(bar_full + 8 * stage, phase, 4);
         float4* raw = reinterpret_cast<float4*>(tiles_ptr + (size_t)stage * sbytes);
         float4* lo = reinterpret_cast<float4*>(tiles_ptr + (size_t)stage * sbytes + A_BYTES);
+        if (!(p.probe & 1))
 #pragma unroll
         for (int j = 0; j < A_BYTES / 16 / 128; ++j) {
           const int idx = tid_c + 128 * j;
@@ -261,7 +278,7 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
 #pragma unroll
       for (int c = 0; c < EPI_COLS; ++c) {
         const int r = rbase + c;
-        if (c < ncols && r < p.Q) Uout[(long long)r * p.N] = accr[c];
+        if (c < ncols && r < p.Q && !(p.probe & 4)) Uout[(long long)r * p.N] = accr[c];
       }
     }
   }

@@ -187,7 +187,7 @@ struct PlanT final : gmmnlse_plan {
   // tcgen05 contraction (complex64 path only): TF32 hi/lo split of S2, zero-padded to [R_pad][Q_pad]
   float *S2hi = nullptr, *S2lo = nullptr;
   CUtensorMap tmV, tmShi, tmSlo;
-  int tc_cg = 0, tc_NT = 0, tc_nrt = 0, tc_KB = 0, tc_stages = 0, tc_kchunk = 2, n_sm = 0;
+  int tc_cg = 0, tc_NT = 0, tc_nrt = 0, tc_KB = 0, tc_stages = 0, tc_kchunk = 4, tc_probe = 0, tc_stage_cap = 0, n_sm = 0;
 
   ~PlanT() override {
     cudaFree(tw); cudaFree(Kw); cudaFree(H); cudaFree(E); cudaFree(EM_d); cudaFree(S2);
@@ -339,8 +339,9 @@ struct PlanT final : gmmnlse_plan {
       const cuuint64_t dims[2] = {(cuuint64_t)Qp, (cuuint64_t)Rp};
       const cuuint64_t strides[1] = {(cuuint64_t)Qp * 4};
       const cuuint32_t box[2] = {tc::BK, (cuuint32_t)(tc_NT / cg)};
-      GM_TRY(encode_tmap_f32(&tmShi, S2hi, 2, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B));
-      GM_TRY(encode_tmap_f32(&tmSlo, S2lo, 2, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B));
+      const CUtensorMapSwizzle bsw = tc::BK == 32 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B;
+      GM_TRY(encode_tmap_f32(&tmShi, S2hi, 2, dims, strides, box, bsw));
+      GM_TRY(encode_tmap_f32(&tmSlo, S2lo, 2, dims, strides, box, bsw));
       GM_TRY(make_v_tmap(&tmV, V, M + 1));
       const int smem = (int)tc::smem_bytes(tc_NT, cg, tc_stages);
       if (cg == 2)
@@ -363,6 +364,8 @@ struct PlanT final : gmmnlse_plan {
       prm.t_tiles = N / (tc::TM * tc_cg);
       prm.total_tiles = planes * prm.t_tiles * tc_nrt;
       prm.plane0 = plane0; prm.stages = tc_stages; prm.kchunk = tc_kchunk;
+      prm.probe = tc_probe;
+      if (tc_stage_cap > 0 && tc_stage_cap < prm.stages) prm.stages = tc_stage_cap;
       const int pairs = std::min(n_sm / tc_cg, prm.total_tiles);
       cudaLaunchConfig_t cfg = {};
       cfg.gridDim = dim3((unsigned)(pairs * tc_cg));
@@ -645,8 +648,10 @@ struct PlanT final : gmmnlse_plan {
   }
   int contraction_kind() const override { return tc_cg ? 1 + tc_cg : 1; }
   int set_tc_chunk(int k) override {
-    if (k < 1) return GMMNLSE_EINVAL;
-    tc_kchunk = k;
+    if ((k & 0xFF) < 1) return GMMNLSE_EINVAL;
+    tc_kchunk = k & 0xFF;
+    tc_probe = (k >> 8) & 0xFF;          // timing probes (gemm_tc.cuh Params::probe); results are wrong when set
+    tc_stage_cap = (k >> 16) & 0xFF;     // cap on smem stages (0 = as many as fit)
     return 0;
   }
   int debug_contract(const void* Vin, void* Uout, int n_planes) override {
