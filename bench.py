@@ -249,6 +249,11 @@ def run_gpu(args):
                     note=f"useful flops 2*Q^2*N per plane; peak = {peaks['source']} bf16 sustained x 0.5 (TF32 nominal "
                          "ratio); executed = 3x useful (three TF32 MMAs per product); cuBLAS TF32 8192^3 on the same "
                          "box: 756 burst / 658 sustained TFLOP/s (profiles/r01c_summary.md)")
+    else:
+        ach = by / (dom_ms * 1e-3) / 1e9
+        roof = dict(bound="hbm", kernel=dom, achieved=round(ach, 1), peak=peaks["hbm"], unit="GB/s",
+                    frac=round(ach / peaks["hbm"], 4), traffic=traffic,
+                    note=f"algorithmic bytes / event-timed duration; peak = {peaks['source']} copy bandwidth")
     roof["avg_launch_ms"] = round(dom_ms / dom_n, 4)
     roof["kernels"] = shares
 
@@ -286,6 +291,62 @@ def run_gpu(args):
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------ M-sweep (Fig. 3 shape)
+def run_sweep(args):
+    """the paper's one performance experiment (Fig. 3) has a serial
+    integrator on the GPU against the MPA for several M on a 10-mode GRIN fibre with z_nl/dz ~ 200.  The
+    figure's bars are not available; this prints the same comparison for this implementation: the serial
+    RK4IP (gmmnlse_propagate_rk4ip) and the MPA at each M, same fibre, pulse, dz and length."""
+    import torch
+    from paper_1708_05324_b200 import binding, workloads
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --sweep-M: no CUDA device")
+    binding.load_library()
+    w = workloads.make_config(3, max_group=3)                     # 10-mode GRIN, 200 kW, 300 fs, N = 8192
+    gamma = w.kappa * w.S[0, 0, 0, 0]
+    z_nl = 1.0 / (gamma * w.meta.get("p_peak", 200e3))
+    w.dz = z_nl / 200.0
+    n_small = 400
+    L = n_small * w.dz
+    A = torch.from_numpy(w.A0.astype(np.complex64)).cuda()
+    stream = torch.cuda.current_stream()
+
+    def timed(fn, reps=3):
+        fn(); torch.cuda.synchronize()
+        best = 1e30
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); fn(); e1.record(stream); torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        return best
+
+    out_rk = torch.empty_like(A)
+    with binding.plan_from_workload(w, M=1) as plan:
+        ms = timed(lambda: plan.propagate_rk4ip(A, L, out_rk, stream))
+    ref = out_rk.cpu().numpy().astype(np.complex128)
+    res = {"sweep": "fig3-like", "workload": "10-mode GRIN (config-3 fibre, groups 0-3), N=8192, 200 kW 300 fs, "
+                                             "Kerr+Raman+shock", "P": w.P, "N": w.N, "dz_m": w.dz,
+           "z_nl_over_dz": 200.0, "small_steps": n_small, "unit": UNIT,
+           "serial_rk4ip": {"z_steps_per_s": round(n_small / (ms * 1e-3), 1), "ms": round(ms, 3),
+                            "nonlinear_evals_per_step": 4}, "mpa": []}
+    for M in (1, 2, 4, 5, 10, 20, 40):
+        out = torch.empty_like(A)
+        with binding.plan_from_workload(w, M=M) as plan:
+            ms = timed(lambda: plan.propagate(A, L, out, stream))
+            s0 = plan.stats()
+            plan.propagate(A, L, out, stream); torch.cuda.synchronize()
+            s1 = plan.stats()
+        o = out.cpu().numpy().astype(np.complex128)
+        res["mpa"].append({"M": M, "z_steps_per_s": round(n_small / (ms * 1e-3), 1), "ms": round(ms, 3),
+                           "iterations_per_large_step": round((s1["iterations"] - s0["iterations"])
+                                                              / max(s1["large_steps"] - s0["large_steps"], 1), 2),
+                           "rel_l2_vs_serial": float(np.linalg.norm(o - ref) / np.linalg.norm(ref))})
+    best = max(res["mpa"], key=lambda r: r["z_steps_per_s"])
+    res["best_M"] = best["M"]
+    res["mpa_over_serial"] = round(best["z_steps_per_s"] / res["serial_rk4ip"]["z_steps_per_s"], 2)
+    print(json.dumps(res))
 
 
 # ------------------------------------------------------------------------------ oracle (CPU) leg
@@ -354,8 +415,11 @@ def main():
     ap.add_argument("--impl", default="graft", choices=["graft", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--all-configs", action="store_true", help="also time configs 1-4 briefly (other_workloads)")
+    ap.add_argument("--sweep-M", action="store_true", help="serial RK4IP vs MPA(M) on a 10-mode GRIN (Fig. 3 shape)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.sweep_M:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_gpu(args)

@@ -83,6 +83,12 @@ int gmmnlse_propagate(gmmnlse_plan *plan, const void *A_in, double L, void *A_ou
  * synchronises.  This is the end-to-end entry bench.py times.                              */
 int gmmnlse_propagate_host(gmmnlse_plan *plan, const void *A_in_host, double L, void *A_out_host);
 
+/* Serial comparison integrator (the role of the split-step code the paper times the
+ * MPA against): fixed-step fourth-order Runge-Kutta in the interaction picture
+ * (RK4IP) with step dz, four nonlinear-operator evaluations per step through the same a3-a8 kernels, one
+ * plane per launch.  Arguments, layout and errors as gmmnlse_propagate; fully asynchronous (no read-back).  */
+int gmmnlse_propagate_rk4ip(gmmnlse_plan *plan, const void *A_in, double L, void *A_out, void *stream);
+
 /* One evaluation of the last term of Eq. 1:
  *   dA_p(t) = i n2 w0/c (1 + i/w0 d_t) sum_lmn S_plmn A_l [(1-fR) A_m A_n* + fR (h_R (*) A_m A_n*)]
  * A, dA: DEVICE [P][N] as above (dA must not alias A); enqueued on the plan's stream.      */

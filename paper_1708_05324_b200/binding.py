@@ -41,6 +41,7 @@ SIGNATURES = {
                                       C.POINTER(Options)]),
     "gmmnlse_propagate": (C.c_int, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]),
     "gmmnlse_propagate_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]),
+    "gmmnlse_propagate_rk4ip": (C.c_int, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]),
     "gmmnlse_nonlinear_op": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "gmmnlse_set_stream": (C.c_int, [C.c_void_p, C.c_void_p]),
     "gmmnlse_get_stats": (C.c_int, [C.c_void_p, _LLP, _LLP, _DP, _LLP]),
@@ -132,6 +133,11 @@ class Plan:
             if a.dtype != self.np_dtype or not a.flags.c_contiguous or a.size != self.P * self.N:
                 raise GmmnlseError(EINVAL, "host buffers must be C-contiguous [P][N] of the plan's precision")
         return _check(self._lib, self._lib.gmmnlse_propagate_host(self._h, _ptr(A_in), float(L), _ptr(A_out)))
+
+    def propagate_rk4ip(self, A_in, L, A_out, stream=None) -> int:
+        """gmmnlse_propagate_rk4ip: the serial RK4IP integrator (step dz) on the same kernels."""
+        return _check(self._lib, self._lib.gmmnlse_propagate_rk4ip(self._h, _ptr(A_in), float(L), _ptr(A_out),
+                                                                   _stream_ptr(stream)))
 
     def nonlinear_op(self, A, dA) -> int:
         return _check(self._lib, self._lib.gmmnlse_nonlinear_op(self._h, _ptr(A), _ptr(dA)))

@@ -100,6 +100,51 @@ template <typename T, int DIR> struct Dft<T, 16, DIR> {
   }
 };
 
+// DFT16 of a[r] w^r (the twiddled butterfly of a radix-16 Stockham pass), given w1 = w and w4 = w^4.
+// With r = 4 r1 + r2, k = k1 + 4 k2:
+//   X[k1 + 4 k2] = sum_r2 W4^(r2 k2) [ w^r2 W16^(r2 k1) sum_r1 W4^(r1 k1) (w^4)^r1 a[4 r1 + r2] ],
+// so only six twiddle values are ever needed (w^4, w^8, w^12, then w, w^2, w^3), three at a time: the
+// register peak stays ~20 below the form that first builds w^1..w^15.
+template <typename T, int DIR>
+__device__ __forceinline__ void dft16_twiddled(cplx<T>* a, cplx<T> w1, cplx<T> w4) {
+  {
+    const cplx<T> w8 = cmul(w4, w4);
+#pragma unroll
+    for (int r2 = 0; r2 < 4; ++r2) {
+      a[4 + r2] = cmul(a[4 + r2], w4);
+      a[8 + r2] = cmul(a[8 + r2], w8);
+    }
+    const cplx<T> w12 = cmul(w8, w4);
+#pragma unroll
+    for (int r2 = 0; r2 < 4; ++r2) a[12 + r2] = cmul(a[12 + r2], w12);
+  }
+  dft4<T, DIR>(a[0], a[4], a[8], a[12]);           // r2 = 0: b[0][k1] at a[4 k1]
+  dft4<T, DIR>(a[1], a[5], a[9], a[13]);
+  dft4<T, DIR>(a[2], a[6], a[10], a[14]);
+  dft4<T, DIR>(a[3], a[7], a[11], a[15]);
+  {
+    const cplx<T> w2 = cmul(w1, w1);
+#pragma unroll
+    for (int k1 = 0; k1 < 4; ++k1) {
+      a[4 * k1 + 1] = cmul(a[4 * k1 + 1], w1);
+      a[4 * k1 + 2] = cmul(a[4 * k1 + 2], w2);
+    }
+    const cplx<T> w3 = cmul(w2, w1);
+#pragma unroll
+    for (int k1 = 0; k1 < 4; ++k1) a[4 * k1 + 3] = cmul(a[4 * k1 + 3], w3);
+  }
+  a[5] = mul_w16<T, DIR, 1>(a[5]);  a[6] = mul_w16<T, DIR, 2>(a[6]);   a[7] = mul_w16<T, DIR, 3>(a[7]);
+  a[9] = mul_w16<T, DIR, 2>(a[9]);  a[10] = mul_w16<T, DIR, 4>(a[10]); a[11] = mul_w16<T, DIR, 6>(a[11]);
+  a[13] = mul_w16<T, DIR, 3>(a[13]); a[14] = mul_w16<T, DIR, 6>(a[14]); a[15] = mul_w16<T, DIR, 9>(a[15]);
+  dft4<T, DIR>(a[0], a[1], a[2], a[3]);            // k1 = 0 -> X[0],X[4],X[8],X[12]
+  dft4<T, DIR>(a[4], a[5], a[6], a[7]);
+  dft4<T, DIR>(a[8], a[9], a[10], a[11]);
+  dft4<T, DIR>(a[12], a[13], a[14], a[15]);
+  cplx<T> t;                                       // a[4 k1 + k2] = X[k1 + 4 k2] -> natural order
+  t = a[1]; a[1] = a[4]; a[4] = t;   t = a[2]; a[2] = a[8]; a[8] = t;   t = a[3]; a[3] = a[12]; a[12] = t;
+  t = a[6]; a[6] = a[9]; a[9] = t;   t = a[7]; a[7] = a[13]; a[13] = t; t = a[11]; a[11] = a[14]; a[14] = t;
+}
+
 __host__ __device__ constexpr int fft_hibit(int r) { int b = 1; while (b * 2 <= r) b *= 2; return b; }
 __device__ __forceinline__ int fft_pad(int a) { return a + (a >> 4); }
 __host__ __device__ constexpr int fft_smem_elems(int N) { return N + (N >> 4); }
@@ -114,7 +159,16 @@ __device__ __forceinline__ void fft_pass(cplx<T> (&v)[16], const cplx<T>* __rest
     cplx<T> a[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) a[r] = v[i + r * NB];
-    if constexpr (LOGNS > 0) {
+    if constexpr (LOGNS > 0 && LOGR == 4) {
+      const int k = (tid + i * NT) & (NS - 1);
+      constexpr int SH = LOG2N - LOGNS - LOGR;     // table index of w^1 is k << SH
+      cplx<T> w1 = tw[k << SH], w4 = tw[(4 * k) << SH];
+      if (DIR < 0) { w1.y = -w1.y; w4.y = -w4.y; }
+      dft16_twiddled<T, DIR>(a, w1, w4);
+#pragma unroll
+      for (int r = 0; r < R; ++r) v[i + r * NB] = a[r];
+      continue;
+    } else if constexpr (LOGNS > 0) {
       const int k = (tid + i * NT) & (NS - 1);
       constexpr int SH = LOG2N - LOGNS - LOGR;     // table index of w^1 is k << SH
       cplx<T> w[R];

@@ -154,6 +154,7 @@ struct gmmnlse_plan {
   virtual int init(const double* S, const double* h_R) = 0;
   virtual int propagate(const void* A_in, double L, void* A_out) = 0;
   virtual int propagate_host(const void* A_in, double L, void* A_out) = 0;
+  virtual int propagate_rk4ip(const void* A_in, double L, void* A_out) = 0;
   virtual int nonlinear_op(const void* A, void* dA) = 0;
   virtual int get_planes(void* out) = 0;
   virtual int debug_fft(const void* in, void* out, int rows, int dir) = 0;
@@ -184,6 +185,9 @@ struct PlanT final : gmmnlse_plan {
   C* d_io = nullptr;
   std::map<int, double2*> EM_ragged;
   long long PN = 0, QN = 0;
+  // serial RK4IP comparison integrator (allocated on first use)
+  C *rk_X = nullptr, *rk_AI = nullptr, *rk_K1 = nullptr, *rk_K2 = nullptr, *rk_K3 = nullptr;
+  double2* EH_d = nullptr;
   // tcgen05 contraction (complex64 path only): TF32 hi/lo split of S2, zero-padded to [R_pad][Q_pad]
   float *S2hi = nullptr, *S2lo = nullptr;
   CUtensorMap tmV, tmShi, tmSlo;
@@ -194,6 +198,7 @@ struct PlanT final : gmmnlse_plan {
     cudaFree(pair_m); cudaFree(pair_n); cudaFree(psi0_d); cudaFree(psi); cudaFree(At); cudaFree(G);
     cudaFree(V); cudaFree(U); cudaFree(errbuf); cudaFree(d_err); cudaFree(d_io);
     cudaFree(S2hi); cudaFree(S2lo);
+    cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
     if (h_err) cudaFreeHost(h_err);
     if (h_in) cudaFreeHost(h_in);
     if (h_out) cudaFreeHost(h_out);
@@ -622,6 +627,46 @@ struct PlanT final : gmmnlse_plan {
     return st;
   }
 
+  // Nh(X) = K F{N[F^-1 X]} for one [P][N] field in the frequency domain -> G plane 0      (a3-a8, one plane)
+  int nonlinear_freq(const C* Xf) {
+    GM_TRY(launch_fft(-1, Xf, 0, At, 0, nullptr, nullptr, nullptr, 0, (T)(1.0 / N), P, 1));
+    GM_TRY(nonlinear_term(0, 1));
+    GM_TRY(launch_fft(+1, G, 0, G, 0, nullptr, Kw, nullptr, 0, (T)1, P, 1));
+    return 0;
+  }
+
+  int propagate_rk4ip(const void* A_in, double L, void* A_out) override {
+    const double ns = L / dz;
+    const long long nsteps = llround(ns);
+    if (!(L >= 0) || std::fabs(ns - (double)nsteps) > 1e-9 * std::fmax(1.0, ns)) return GMMNLSE_EINVAL;
+    if (!rk_X) {
+      GM_TRY(dalloc(&rk_X, (size_t)PN)); GM_TRY(dalloc(&rk_AI, (size_t)PN)); GM_TRY(dalloc(&rk_K1, (size_t)PN));
+      GM_TRY(dalloc(&rk_K2, (size_t)PN)); GM_TRY(dalloc(&rk_K3, (size_t)PN));
+      std::vector<double2> eh((size_t)PN);
+      for (long long i = 0; i < PN; ++i) {
+        const double ph = std::remainder(phi[i] * (0.5 * dz), 2.0 * M_PI);
+        eh[i] = make_double2(std::cos(ph), std::sin(ph));
+      }
+      GM_TRY(dalloc(&EH_d, (size_t)PN));
+      GM_TRY(upload(EH_d, eh));
+    }
+    GM_TRY(launch_fft(+1, (const C*)A_in, 0, psi, 0, nullptr, nullptr, nullptr, 0, (T)1, P, 1));
+    GM_TRY(to_master(psi));
+    const unsigned blocks = (unsigned)((PN + 255) / 256);
+    for (long long s = 0; s < nsteps; ++s) {
+      for (int stage = 1; stage <= 4; ++stage) {
+        GM_TRY(nonlinear_freq(stage == 1 ? psi : rk_X));
+        prof_begin(GMMNLSE_KIND_ADVANCE);
+        k_rk4_stage<T><<<blocks, 256, 0, stream>>>(stage, psi0_d, psi, EH_d, G, rk_AI, rk_K1, rk_K2, rk_K3, rk_X, dz,
+                                                    PN);
+        prof_end();
+        GM_CUDA(cudaGetLastError());
+      }
+    }
+    GM_TRY(launch_fft(-1, psi, 0, (C*)A_out, 0, nullptr, nullptr, nullptr, 0, (T)(1.0 / N), P, 1));
+    return GMMNLSE_OK;
+  }
+
   int nonlinear_op(const void* A, void* dA) override {
     // a12: uses plane 0 of the scratch buffers.  dA = F^-1{ K(w) F{N_p[A]} }
     GM_CUDA(cudaMemcpyAsync(At, A, sizeof(C) * (size_t)PN, cudaMemcpyDeviceToDevice, stream));
@@ -755,6 +800,12 @@ int gmmnlse_propagate_host(gmmnlse_plan* plan, const void* A_in_host, double L, 
   const double ns = L / plan->dz;
   if (!(L >= 0) || std::fabs(ns - std::round(ns)) > 1e-9 * std::fmax(1.0, ns)) return GMMNLSE_EINVAL;
   return plan->propagate_host(A_in_host, L, A_out_host);
+}
+
+int gmmnlse_propagate_rk4ip(gmmnlse_plan* plan, const void* A_in, double L, void* A_out, void* stream) {
+  if (!plan || !A_in || !A_out) return GMMNLSE_EINVAL;
+  if (stream) plan->stream = (cudaStream_t)stream;
+  return plan->propagate_rk4ip(A_in, L, A_out);
 }
 
 int gmmnlse_nonlinear_op(gmmnlse_plan* plan, const void* A, void* dA) {

@@ -59,32 +59,43 @@ k_pair_conv(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restri
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
   const int q0 = 2 * blockIdx.x, q1 = q0 + 1, j = blockIdx.y;
   const bool has1 = q1 < Q;
-  const cplx<T>* Aj = A + j * a_plane_stride;
-  const cplx<T>* am0 = Aj + (long long)pair_m[q0] * N;
-  const cplx<T>* an0 = Aj + (long long)pair_n[q0] * N;
-  const cplx<T>* am1 = Aj + (long long)pair_m[has1 ? q1 : q0] * N;
-  const cplx<T>* an1 = Aj + (long long)pair_n[has1 ? q1 : q0] * N;
-  T* v0 = V + j * v_plane_stride + (long long)q0 * N;
-  T* v1 = V + j * v_plane_stride + (long long)q1 * N;
-  auto prod = [&](int n) {
-    cplx<T> a = am0[n], b = an0[n], c = am1[n], d = an1[n];
-    return mk(a.x * b.x + a.y * b.y, has1 ? c.x * d.x + c.y * d.y : (T)0);
-  };
-  if constexpr (!HAS_RAMAN) {
+  {
+    // phase 1: z_n = Re(A_m A_n*)[q0] + i Re(A_m A_n*)[q1], formed straight from the four field rows.  Kept
+    // apart from the FFT so that its pointers and in-flight loads do not add to the FFT's register peak
+    // (N = 16384 runs 1024 threads, i.e. 64 registers per thread).
+    const cplx<T>* Aj = A + j * a_plane_stride;
+    const cplx<T>* am0 = Aj + (long long)pair_m[q0] * N;
+    const cplx<T>* an0 = Aj + (long long)pair_n[q0] * N;
+    const cplx<T>* am1 = Aj + (long long)pair_m[has1 ? q1 : q0] * N;
+    const cplx<T>* an1 = Aj + (long long)pair_n[has1 ? q1 : q0] * N;
+    T* v0 = V + j * v_plane_stride + (long long)q0 * N;
+    T* v1 = V + j * v_plane_stride + (long long)q1 * N;
+#pragma unroll 4
     for (int e = 0; e < 16; ++e) {
       const int n = threadIdx.x + e * NT;
-      cplx<T> z = prod(n);
-      v0[n] = z.x;
-      if (has1) v1[n] = z.y;
+      const cplx<T> a = am0[n], b = an0[n], c = am1[n], d = an1[n];
+      const cplx<T> z = mk(a.x * b.x + a.y * b.y, has1 ? c.x * d.x + c.y * d.y : (T)0);
+      if constexpr (HAS_RAMAN) {
+        sm[fft_pad(n)] = z;
+      } else {
+        v0[n] = z.x;
+        if (has1) v1[n] = z.y;
+      }
     }
-  } else {
-    block_fft<T, LOG2N, +1>(sm, tw, prod, [&](int k, cplx<T> Z) { sm[fft_pad(k)] = cmul(Z, H[k]); });
+  }
+  if constexpr (HAS_RAMAN) {
     __syncthreads();
+    // phase 2: Z = F{z} . H   (H = ((1-fR) + fR ht_R)/N), in place in shared memory
+    block_fft<T, LOG2N, +1>(sm, tw, [&](int n) { return sm[fft_pad(n)]; },
+                            [&](int k, cplx<T> Z) { sm[fft_pad(k)] = cmul(Z, H[k]); });
+    __syncthreads();
+    // phase 3: v = F^-1{Z};  V[q0] = Re v, V[q1] = Im v
+    T* v0 = V + j * v_plane_stride + (long long)q0 * N;
     block_fft<T, LOG2N, -1>(
         sm, tw, [&](int k) { return sm[fft_pad(k)]; },
         [&](int n, cplx<T> v) {
           v0[n] = v.x;
-          if (has1) v1[n] = v.y;
+          if (has1) v0[N + n] = v.y;
         });
   }
 }
@@ -288,6 +299,49 @@ k_advance(double2* __restrict__ psi0_d, cplx<T>* __restrict__ psi0, const cplx<T
   const double2 q = make_double2(p.x * e.x - p.y * e.y, p.x * e.y + p.y * e.x);
   psi0_d[i] = q;
   psi0[i] = mk((T)q.x, (T)q.y);
+}
+
+// ------------------------------------------------------------------------------------------
+// Serial comparison integrator: the elementwise stages of one RK4IP step in the
+// frequency domain.  With E = exp(D h/2), Nh(X) = K F{N[F^-1 X]} (the same a4-a8 kernels, one plane):
+//   stage 1: AI = E At;  K1 = h E G;  X = AI + K1/2          (G = Nh(At))
+//   stage 2: K2 = h G;  X = AI + K2/2                        (G = Nh(X))
+//   stage 3: K3 = h G;  X = E (AI + K3)
+//   stage 4: At <- E (AI + K1/6 + K2/3 + K3/3) + h G/6       (fp64 master copy + working copy)
+// The interaction-picture form replaces the split-step scheme the paper compares against.
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_rk4_stage(int stage, double2* __restrict__ At_d, cplx<T>* __restrict__ At, const double2* __restrict__ EH,
+            const cplx<T>* __restrict__ G, cplx<T>* __restrict__ AI, cplx<T>* __restrict__ K1,
+            cplx<T>* __restrict__ K2, cplx<T>* __restrict__ K3, cplx<T>* __restrict__ X, double h, long long PN) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= PN) return;
+  const double2 e = EH[i];
+  const double gx = (double)G[i].x * h, gy = (double)G[i].y * h;
+  if (stage == 1) {
+    const double2 a = At_d[i];
+    const double aix = a.x * e.x - a.y * e.y, aiy = a.x * e.y + a.y * e.x;
+    const double k1x = gx * e.x - gy * e.y, k1y = gx * e.y + gy * e.x;
+    AI[i] = mk((T)aix, (T)aiy);
+    K1[i] = mk((T)k1x, (T)k1y);
+    X[i] = mk((T)(aix + 0.5 * k1x), (T)(aiy + 0.5 * k1y));
+  } else if (stage == 2) {
+    K2[i] = mk((T)gx, (T)gy);
+    X[i] = mk((T)((double)AI[i].x + 0.5 * gx), (T)((double)AI[i].y + 0.5 * gy));
+  } else if (stage == 3) {
+    K3[i] = mk((T)gx, (T)gy);
+    const double sx = (double)AI[i].x + gx, sy = (double)AI[i].y + gy;
+    X[i] = mk((T)(sx * e.x - sy * e.y), (T)(sx * e.y + sy * e.x));
+  } else {
+    // AI is recomputed from the fp64 master so that the state never passes through working precision
+    const double2 a = At_d[i];
+    const double aix = a.x * e.x - a.y * e.y, aiy = a.x * e.y + a.y * e.x;
+    const double sx = aix + (double)K1[i].x / 6.0 + ((double)K2[i].x + (double)K3[i].x) / 3.0;
+    const double sy = aiy + (double)K1[i].y / 6.0 + ((double)K2[i].y + (double)K3[i].y) / 3.0;
+    const double2 r = make_double2(sx * e.x - sy * e.y + gx / 6.0, sx * e.y + sy * e.x + gy / 6.0);
+    At_d[i] = r;
+    At[i] = mk((T)r.x, (T)r.y);
+  }
 }
 
 template <typename TI, typename TO>

@@ -348,3 +348,103 @@ def test_contraction_auto_selects_tensor_cores_for_large_P(B):
     with pytest.raises(B.GmmnlseError) as e:           # complex128 has no tensor-core path
         B.plan_from_workload(w, contraction=3)
     assert e.value.status == B.EUNSUPPORTED
+
+
+# --------------------------------------------- BASELINE.json full sizes, bench.py's launch configuration
+@pytest.mark.slow
+def test_config5_full_shape_one_large_step_planes_vs_oracle(B):
+    """P = 45, N = 8192, M = 20 (the shape bench.py times; tcgen05 contraction, 20-plane launches): every
+    plane of the second MPA iterate against the plain oracle MPA (O4), element by element."""
+    w = W.make_config(5)
+    L = w.M * w.dz
+    Ad = dev(w.A0, np.complex64)
+    out = torch.empty_like(Ad)
+    with B.plan_from_workload(w, fixed_iter=2) as plan:
+        assert plan.contraction_kind() == 2
+        plan.propagate(Ad, L, out)
+        torch.cuda.synchronize()
+        planes = plan.debug_get_planes()
+    A_in = Ad.cpu().numpy().astype(np.complex128)
+    hist = []
+    ref = O.mpa_propagate(A_in, L, w.dz, w.M, w.beta, w.S, w.kappa, w.omega0, w.f_R, w.h_R, w.dt,
+                          shock=w.shock, fixed_iter=2, history=hist)
+    ref_planes = hist[0][-1]
+    psi0 = O.to_freq(A_in)             # (the library's plane 0 already holds the advanced field after the call)
+    for j in range(1, w.M + 1):
+        assert rel(planes[j], ref_planes[j]) <= TOL_OP, j
+    # the nonlinear increment itself, psi_M - psi_0 (a few 1e-1 of psi at this power), not just psi_M
+    inc = rel(ref_planes[w.M] - psi0, psi0)
+    assert inc >= 1e-2, inc
+    assert rel(planes[w.M] - psi0, ref_planes[w.M] - psi0) <= 3 * TOL_OP / inc
+    assert rel(out.cpu().numpy(), ref) <= TOL_OP
+
+
+@pytest.mark.parametrize("cfg", [4, 5])
+def test_full_shape_properties_invariant_M_independence_order(B, cfg):
+    """Properties that hold at any size (no oracle run is affordable at these shapes over many steps):
+    the conserved quantity of reading S15, independence of the converged result from M, and second-order
+    convergence in dz of the MPA's implicit trapezoid rule."""
+    w = W.make_config(cfg)
+    n_large = 3
+    w.L = n_large * w.M * w.dz
+    A_in, out, st, stats = _propagate(B, w)
+    assert st == 0 and stats["not_converged"] == 0 and stats["large_steps"] == n_large
+    q0 = O.conserved_quantity(A_in, w.dt, w.omega0, w.shock)
+    q1 = O.conserved_quantity(out, w.dt, w.omega0, w.shock)
+    assert abs(q1 / q0 - 1.0) <= 2e-6, q1 / q0 - 1.0
+    # M-independence: half as many planes per large step, same dz, same length
+    M0 = w.M
+    w.M = M0 // 2
+    out_half = _propagate(B, w)[1]
+    assert rel(out_half, out) <= 2e-5
+    # order in dz: e(dz) / e(dz/2) ~ 4 against the dz/4 run
+    w.M = M0
+    outs = [out]
+    for k in (2, 4):
+        w2 = W.make_config(cfg)
+        w2.dz = w.dz / k
+        w2.L = w.L
+        outs.append(_propagate(B, w2)[1])
+    e1, e2 = rel(outs[0], outs[2]), rel(outs[1], outs[2])
+    assert e1 <= 1e-3
+    assert 2.5 <= e1 / e2 <= 8.0 or e1 < 5e-6, (e1, e2)
+
+
+# --------------------------------------------------- NEXT-1: serial RK4IP integrator on the same kernels
+@pytest.mark.parametrize("cfg,kw,tol,tol_mpa", [
+    (2, dict(N=1024, L=40 * 50e-6), 2e-5, TOL_FIELD),
+    # tcgen05 contraction, one plane per launch.  Config 3's dz = 100 um is 2.2 rad of inter-group beating per
+    # step (4 x 5517 /m), so the second-order MPA and the fourth-order RK4IP differ by 1-2e-3 there whatever
+    # the length (oracle MPA vs oracle RK4IP do too; DESIGN.md section 8): bound 5e-3 for the cross-check.
+    (3, dict(N=1024, L=20 * 100e-6), 2e-5, 5e-3),
+    (1, dict(N=256, L=50 * 2.5e-3), 1e-10, TOL_FIELD),          # complex128
+])
+def test_rk4ip_gpu_vs_oracle_rk4ip(B, cfg, kw, tol, tol_mpa):
+    w = W.make_config(cfg, **kw)
+    dt = np.complex128 if w.precision else np.complex64
+    Ad = dev(w.A0, dt)
+    out = torch.empty_like(Ad)
+    with B.plan_from_workload(w) as plan:
+        st = plan.propagate_rk4ip(Ad, w.L, out)
+        torch.cuda.synchronize()
+        out_mpa = torch.empty_like(Ad)
+        plan.propagate(Ad, w.L, out_mpa)
+        torch.cuda.synchronize()
+    assert st == 0
+    A_in = Ad.cpu().numpy().astype(np.complex128)
+    ref = O.rk4ip_propagate(A_in, w.L, w.dz, w.beta, w.S, w.kappa, w.omega0, w.f_R, w.h_R, w.dt, shock=w.shock)
+    assert rel(out.cpu().numpy(), ref) <= tol
+    # the two GPU integrators agree to the MPA's O(dz^2) truncation
+    assert rel(out_mpa.cpu().numpy(), out.cpu().numpy()) <= tol_mpa
+
+
+def test_rk4ip_gpu_zero_length_and_bad_length(B):
+    w = W.make_config(2, N=256)
+    Ad = dev(w.A0, np.complex64)
+    out = torch.empty_like(Ad)
+    with B.plan_from_workload(w) as plan:
+        plan.propagate_rk4ip(Ad, 0.0, out)
+        torch.cuda.synchronize()
+        assert rel(out.cpu().numpy(), Ad.cpu().numpy()) <= 1e-6
+        with pytest.raises(B.GmmnlseError):
+            plan.propagate_rk4ip(Ad, 0.5 * w.dz, out)
