@@ -45,6 +45,11 @@ typedef struct {                /* pass NULL for defaults                       
                                    1 = CUDA-core fp32/fp64 GEMM, 2 = tcgen05 3xTF32 on CTA pairs
                                    (cta_group::2), 3 = tcgen05 3xTF32 single CTA.  2-3 need complex64 and
                                    N % 128 == 0 (else EUNSUPPORTED)                                */
+  int    raman;                 /* a5 kernel: 0 = auto, 1 = FFT . h~_R . IFFT on the pair streams (any h_R),
+                                   2 = one-pole recurrence along t, exact when the samples are a damped
+                                   oscillation h_R[j] = Im(c zeta^j) (the tau1/tau2 form); auto picks 2 when
+                                   all N samples fit that form to 1e-10 of the peak, else 1; 2 on a response
+                                   that does not fit is EUNSUPPORTED                                */
 } gmmnlse_options;
 
 /* Build a plan: precompute D_w^(p), the rotation tables exp(+-D_w j dz) (j = 0..M) in
@@ -136,6 +141,8 @@ int gmmnlse_debug_pairs(gmmnlse_plan *plan, const void *A, void *V, int n_planes
  *          3 tcgen05 CTA pairs.                                                              */
 int gmmnlse_debug_contract(gmmnlse_plan *plan, const void *V, void *U, int n_planes);
 int gmmnlse_contraction_kind(const gmmnlse_plan *plan);
+/*   raman_kind: which a5 kernel the plan selected: 0 none (f_R = 0), 1 FFT, 2 recursive.          */
+int gmmnlse_raman_kind(const gmmnlse_plan *plan);
 /*   set_tc_chunk: k-blocks (16 packed pairs each) a tensor-memory accumulator holds before the epilogue
  *          drains it into fp32 registers (default 4); bounds the bias of the tensor core's truncating
  *          accumulate.  k >= 1.                          */

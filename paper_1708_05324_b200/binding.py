@@ -27,7 +27,7 @@ class GmmnlseError(RuntimeError):
 
 class Options(C.Structure):
     _fields_ = [("precision", C.c_int), ("shock", C.c_int), ("tol", C.c_double), ("max_iter", C.c_int),
-                ("fixed_iter", C.c_int), ("contraction", C.c_int)]
+                ("fixed_iter", C.c_int), ("contraction", C.c_int), ("raman", C.c_int)]
 
 
 _LIB = None
@@ -53,6 +53,7 @@ SIGNATURES = {
     "gmmnlse_debug_pairs": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
     "gmmnlse_debug_contract": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
     "gmmnlse_contraction_kind": (C.c_int, [C.c_void_p]),
+    "gmmnlse_raman_kind": (C.c_int, [C.c_void_p]),
     "gmmnlse_debug_set_tc_chunk": (C.c_int, [C.c_void_p, C.c_int]),
     "gmmnlse_plan_destroy": (None, [C.c_void_p]),
     "gmmnlse_status_string": (C.c_char_p, [C.c_int]),
@@ -103,7 +104,7 @@ class Plan:
     """Owner of one ``gmmnlse_plan``; methods mirror the C calls one to one."""
 
     def __init__(self, P, N, M, dt, dz, beta, S, f_R, h_R, omega0, n2, *, precision=0, shock=True,
-                 tol=1e-6, max_iter=0, fixed_iter=0, contraction=0):
+                 tol=1e-6, max_iter=0, fixed_iter=0, contraction=0, raman=0):
         self._lib = load_library()
         self._h = C.c_void_p()
         beta = np.ascontiguousarray(beta, dtype=np.float64).reshape(P, -1)
@@ -113,7 +114,7 @@ class Plan:
         hR = None if h_R is None else np.ascontiguousarray(h_R, dtype=np.float64)
         if hR is not None and hR.size != N:
             raise GmmnlseError(EINVAL, "h_R must hold N samples")
-        opt = Options(int(precision), int(bool(shock)), float(tol), int(max_iter), int(fixed_iter), int(contraction))
+        opt = Options(int(precision), int(bool(shock)), float(tol), int(max_iter), int(fixed_iter), int(contraction), int(raman))
         st = self._lib.gmmnlse_plan_create(
             C.byref(self._h), P, N, M, dt, dz, beta.ctypes.data_as(_DP), beta.shape[1], S.ctypes.data_as(_DP),
             f_R, None if hR is None else hR.ctypes.data_as(_DP), omega0, n2, C.byref(opt))
@@ -184,6 +185,10 @@ class Plan:
     def contraction_kind(self) -> int:
         """1 = CUDA cores, 2 = tcgen05 single CTA, 3 = tcgen05 CTA pairs."""
         return int(self._lib.gmmnlse_contraction_kind(self._h))
+
+    def raman_kind(self) -> int:
+        """0 = no Raman term, 1 = FFT convolution, 2 = recursive (damped-oscillator) form."""
+        return int(self._lib.gmmnlse_raman_kind(self._h))
 
     def debug_set_tc_chunk(self, k: int) -> None:
         _check(self._lib, self._lib.gmmnlse_debug_set_tc_chunk(self._h, int(k)))

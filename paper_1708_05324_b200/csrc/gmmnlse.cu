@@ -108,7 +108,7 @@ int ilog2(int n) {
 // ============================================================================================
 struct gmmnlse_plan {
   int P = 0, N = 0, M = 0, log2N = 0, Q = 0, precision = 0, shock = 1, max_iter = 0, fixed_iter = 0;
-  int contraction = 0;
+  int contraction = 0, raman = 0;
   double dt = 0, dz = 0, f_R = 0, omega0 = 0, n2 = 0, tol = 1e-6;
   cudaStream_t stream = nullptr;
   long long n_large = 0, n_iter = 0, n_noconv = 0, n_launch = 0;
@@ -162,6 +162,7 @@ struct gmmnlse_plan {
   virtual int debug_contract(const void* V, void* U, int n_planes) = 0;
   virtual int contraction_kind() const = 0;
   virtual int set_tc_chunk(int k) = 0;
+  virtual int raman_kind() const = 0;
 };
 
 namespace {
@@ -185,6 +186,10 @@ struct PlanT final : gmmnlse_plan {
   C* d_io = nullptr;
   std::map<int, double2*> EM_ragged;
   long long PN = 0, QN = 0;
+  // recursive Raman path (k_pair_iir): h_R[j] = Im(c zeta^j) detected from the samples
+  bool iir = false;
+  C iir_zeta, iir_cs, *iir_zp = nullptr;
+  T iir_omf = 0;
   // serial RK4IP comparison integrator (allocated on first use)
   C *rk_X = nullptr, *rk_AI = nullptr, *rk_K1 = nullptr, *rk_K2 = nullptr, *rk_K3 = nullptr;
   double2* EH_d = nullptr;
@@ -198,7 +203,7 @@ struct PlanT final : gmmnlse_plan {
     cudaFree(pair_m); cudaFree(pair_n); cudaFree(psi0_d); cudaFree(psi); cudaFree(At); cudaFree(G);
     cudaFree(V); cudaFree(U); cudaFree(errbuf); cudaFree(d_err); cudaFree(d_io);
     cudaFree(S2hi); cudaFree(S2lo);
-    cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
+    cudaFree(iir_zp); cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
     if (h_err) cudaFreeHost(h_err);
     if (h_in) cudaFreeHost(h_in);
     if (h_out) cudaFreeHost(h_out);
@@ -251,6 +256,7 @@ struct PlanT final : gmmnlse_plan {
         h_H[k] = mk((T)v.real(), (T)v.imag());
       }
     }
+    GM_TRY(fit_raman(h_R));
     std::vector<C> h_E((size_t)(M + 1) * PN);
     for (int j = 0; j <= M; ++j)
       for (long long i = 0; i < PN; ++i) {
@@ -293,6 +299,87 @@ struct PlanT final : gmmnlse_plan {
     GM_CUDA(cudaMallocHost((void**)&h_err, sizeof(double)));
     GM_TRY(init_tc(h_S2d));
     return 0;
+  }
+
+  // ------------------------------------------------------------------ recursive Raman detection
+  // Is h_R[j] = Im(c zeta^j) (a damped oscillation sampled at j dt)?  Fit the two-term recurrence
+  // h[j+2] = a1 h[j+1] + a2 h[j] on the leading samples, take zeta from x^2 = a1 x + a2, c from h[0], h[1],
+  // and accept only if every one of the N samples is reproduced to 1e-10 of the peak and zeta^N < 1e-14.
+  // options.raman: 0 auto, 1 force the FFT path, 2 require the recursive path (EUNSUPPORTED if it does not fit).
+  int fit_raman(const double* h) {
+    iir = false;
+    if (f_R == 0.0 || raman == 1 || N < 32) return raman == 2 && f_R != 0.0 ? GMMNLSE_EUNSUPPORTED : 0;
+    const int nfit = std::min(N - 2, 96);
+    long double s11 = 0, s12 = 0, s22 = 0, b1 = 0, b2 = 0, hmax = 0;
+    for (int jn = 0; jn < N; ++jn) hmax = std::max(hmax, (long double)std::fabs(h[jn]));
+    for (int jn = 0; jn < nfit; ++jn) {
+      const long double u = h[jn + 1], v = h[jn], y = h[jn + 2];
+      s11 += u * u; s12 += u * v; s22 += v * v; b1 += u * y; b2 += v * y;
+    }
+    const long double det = s11 * s22 - s12 * s12;
+    bool ok = hmax > 0 && std::fabs((double)det) > 1e-24 * (double)(s11 * s22);
+    double a1 = 0, a2 = 0;
+    if (ok) {
+      a1 = (double)((b1 * s22 - b2 * s12) / det);
+      a2 = (double)((s11 * b2 - s12 * b1) / det);
+      ok = a1 * a1 + 4.0 * a2 < 0.0;                        // complex pole pair
+    }
+    cd zeta, c;
+    if (ok) {
+      zeta = cd(0.5 * a1, std::sqrt(-a2 - 0.25 * a1 * a1));
+      c = cd((h[1] - h[0] * zeta.real()) / zeta.imag(), h[0]);
+      const double lnm = std::log(std::abs(zeta)), arg = std::arg(zeta);
+      ok = lnm < 0.0 && lnm * N < std::log(1e-14);
+      for (int jn = 0; ok && jn < N; ++jn) {
+        const cd zj = std::exp(lnm * jn) * cd(std::cos(arg * jn), std::sin(arg * jn));
+        if (std::fabs(h[jn] - (c * zj).imag()) > 1e-10 * (double)hmax) ok = false;
+      }
+    }
+    if (!ok) return raman == 2 ? GMMNLSE_EUNSUPPORTED : 0;
+    const int NT = N / 16;
+    std::vector<C> zp((size_t)NT + 33);
+    const double lnm = std::log(std::abs(zeta)), arg = std::arg(zeta);
+    for (size_t m = 0; m < zp.size(); ++m) {
+      const double mag = std::exp(lnm * 16.0 * (double)m), ph = std::remainder(arg * 16.0 * (double)m, 2.0 * M_PI);
+      zp[m] = mk((T)(mag * std::cos(ph)), (T)(mag * std::sin(ph)));
+    }
+    GM_TRY(dalloc(&iir_zp, zp.size()));
+    GM_TRY(upload(iir_zp, zp));
+    iir_zeta = mk((T)zeta.real(), (T)zeta.imag());
+    const cd csd = c * (dt * f_R);
+    iir_cs = mk((T)csd.real(), (T)csd.imag());
+    iir_omf = (T)(1.0 - f_R);
+    iir = true;
+    return 0;
+  }
+
+  template <int LOG2N>
+  int launch_pairs_iir_t(const C* A, long long a_ps, T* Vout, long long v_ps, int planes) {
+    constexpr int NT = (1 << LOG2N) / 16, NW = (NT + 31) / 32;
+    const size_t smem = sizeof(C) * (fft_smem_elems(1 << LOG2N) + 2 * NW + 2);
+    static bool configured = false;
+    if (!configured) {
+      GM_CUDA(cudaFuncSetAttribute(k_pair_iir<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      configured = true;
+    }
+    prof_begin(GMMNLSE_KIND_PAIR_CONV);
+    k_pair_iir<T, LOG2N><<<dim3((Q + 1) / 2, planes), NT, smem, stream>>>(A, a_ps, Vout, v_ps, pair_m, pair_n, Q,
+                                                                          iir_zeta, iir_cs, iir_omf, iir_zp);
+    prof_end();
+    GM_CUDA(cudaGetLastError());
+    return 0;
+  }
+  int launch_pairs_iir(const C* A, long long a_ps, T* Vout, long long v_ps, int planes) {
+#define GM_IIR_CASE(L) case L: return launch_pairs_iir_t<L>(A, a_ps, Vout, v_ps, planes);
+    switch (log2N) {
+      GM_IIR_CASE(5) GM_IIR_CASE(6) GM_IIR_CASE(7) GM_IIR_CASE(8) GM_IIR_CASE(9) GM_IIR_CASE(10) GM_IIR_CASE(11)
+      GM_IIR_CASE(12) GM_IIR_CASE(13)
+      case 14:
+        if constexpr (sizeof(T) == 4) return launch_pairs_iir_t<14>(A, a_ps, Vout, v_ps, planes);
+        return GMMNLSE_EUNSUPPORTED;
+    }
+#undef GM_IIR_CASE
+    return GMMNLSE_EUNSUPPORTED;
   }
 
   // ------------------------------------------------------------------ tcgen05 contraction setup
@@ -455,6 +542,7 @@ struct PlanT final : gmmnlse_plan {
     return 0;
   }
   int launch_pairs(const C* A, long long a_ps, T* Vout, long long v_ps, int planes) {
+    if (iir) return launch_pairs_iir(A, a_ps, Vout, v_ps, planes);
     const bool raman = f_R != 0.0;
 #define GM_PC_CASE(L)                                                               \
   case L:                                                                           \
@@ -692,6 +780,7 @@ struct PlanT final : gmmnlse_plan {
     return launch_pairs((const C*)A, PN, (T*)Vout, QN, n_planes);
   }
   int contraction_kind() const override { return tc_cg ? 1 + tc_cg : 1; }
+  int raman_kind() const override { return f_R == 0.0 ? 0 : (iir ? 2 : 1); }
   int set_tc_chunk(int k) override {
     if ((k & 0xFF) < 1) return GMMNLSE_EINVAL;
     tc_kchunk = k & 0xFF;
@@ -731,13 +820,14 @@ int gmmnlse_plan_create(gmmnlse_plan** out, int P, int N, int M, double dt, doub
                         const gmmnlse_options* opt) {
   if (!out) return GMMNLSE_EINVAL;
   *out = nullptr;
-  gmmnlse_options o = {0, 1, 1e-6, 0, 0, 0};
+  gmmnlse_options o = {0, 1, 1e-6, 0, 0, 0, 0};
   if (opt) o = *opt;
   if (P < 1 || N < 1 || M < 1 || n_beta < 1 || !beta || !S) return GMMNLSE_EINVAL;
   if (N & (N - 1)) return GMMNLSE_EINVAL;
   if (!(dt > 0) || !(dz > 0) || !(omega0 > 0) || !std::isfinite(n2) || !std::isfinite(f_R)) return GMMNLSE_EINVAL;
   if ((f_R != 0.0) != (h_R != nullptr)) return GMMNLSE_EINVAL;
   if (o.precision != 0 && o.precision != 1) return GMMNLSE_EINVAL;
+  if (o.raman < 0 || o.raman > 2) return GMMNLSE_EINVAL;
   if (o.shock && M_PI / dt >= omega0) return GMMNLSE_EINVAL;
   if (!(o.tol > 0)) o.tol = 1e-6;
   for (long long i = 0; i < (long long)P * n_beta; ++i)
@@ -771,6 +861,7 @@ int gmmnlse_plan_create(gmmnlse_plan** out, int P, int N, int M, double dt, doub
   pl->max_iter = o.max_iter > 0 ? o.max_iter : 2 * M + 4;
   pl->fixed_iter = o.fixed_iter > 0 ? o.fixed_iter : 0;
   pl->contraction = o.contraction;
+  pl->raman = o.raman;
   // Im D_w^(p) = beta0 + beta1 w + sum_{k>=2} beta_k w^k / k!
   pl->phi.assign((size_t)P * N, 0.0);
   for (int p = 0; p < P; ++p)
@@ -869,6 +960,8 @@ int gmmnlse_debug_contract(gmmnlse_plan* plan, const void* V, void* U, int n_pla
 }
 
 int gmmnlse_contraction_kind(const gmmnlse_plan* plan) { return plan ? plan->contraction_kind() : 0; }
+
+int gmmnlse_raman_kind(const gmmnlse_plan* plan) { return plan ? plan->raman_kind() : 0; }
 
 int gmmnlse_debug_set_tc_chunk(gmmnlse_plan* plan, int k) { return plan ? plan->set_tc_chunk(k) : GMMNLSE_EINVAL; }
 

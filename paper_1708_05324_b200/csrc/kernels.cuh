@@ -101,6 +101,107 @@ k_pair_conv(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restri
 }
 
 // ------------------------------------------------------------------------------------------
+// a4 + a5, recursive form.  When the sampled response is a damped oscillation, h_R[j] = Im(c zeta^j) (the
+// form BASELINE.json's tau1, tau2 give; detected at plan time from the samples themselves), the circular
+// convolution of Eq. 1 is a one-pole complex recurrence along t,
+//   w[i] = x[i] + zeta w[i-1],   (h_R (*) x)[i] = dt Im(c w[i]),
+// exact up to zeta^N (< 1e-14, checked).  Each thread owns 16 consecutive samples of two pair streams; chunk
+// carries are combined by a warp-shuffle scan of the recurrence (multipliers zeta^(16 d) from the table
+// zp[m] = zeta^(16 m)), warp totals through shared memory, and the periodic wrap w[-1] = w[N-1] closes the
+// circle.  No FFT: the kernel is one read of the field rows and one write of V.
+//   cs = c dt f_R,  omf = 1 - f_R;  V = omf x + Im(cs w).
+template <typename T, int LOG2N>
+__global__ void __launch_bounds__((1 << LOG2N) / 16)
+k_pair_iir(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restrict__ V, long long v_plane_stride,
+           const int* __restrict__ pair_m, const int* __restrict__ pair_n, int Q, cplx<T> zeta, cplx<T> cs, T omf,
+           const cplx<T>* __restrict__ zp) {
+  constexpr int N = 1 << LOG2N, NT = N / 16, NW = (NT + 31) / 32;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);         // fft_smem_elems(N) + 2 * (NW + 1) complex
+  cplx<T>* wt = sm + fft_smem_elems(N);                       // [2][NW] warp totals, then [2] row totals
+  const int q0 = 2 * blockIdx.x, q1 = q0 + 1, j = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const bool has1 = q1 < Q;
+  {
+    const cplx<T>* Aj = A + j * a_plane_stride;
+    const cplx<T>* am0 = Aj + (long long)pair_m[q0] * N;
+    const cplx<T>* an0 = Aj + (long long)pair_n[q0] * N;
+    const cplx<T>* am1 = Aj + (long long)pair_m[has1 ? q1 : q0] * N;
+    const cplx<T>* an1 = Aj + (long long)pair_n[has1 ? q1 : q0] * N;
+#pragma unroll 4
+    for (int e = 0; e < 16; ++e) {
+      const int n = tid + e * NT;
+      const cplx<T> a = am0[n], b = an0[n], c = am1[n], d = an1[n];
+      sm[fft_pad(n)] = mk(a.x * b.x + a.y * b.y, has1 ? c.x * d.x + c.y * d.y : (T)0);
+    }
+  }
+  __syncthreads();
+  cplx<T> x[16];                                              // x.x: stream q0, x.y: stream q1; samples 16 tid + e
+#pragma unroll
+  for (int e = 0; e < 16; ++e) x[e] = sm[17 * tid + e];       // fft_pad(16 k + e) = 17 k + e: conflict-free
+  cplx<T> w0 = mk((T)0, (T)0), w1 = w0;
+#pragma unroll
+  for (int e = 0; e < 16; ++e) {
+    w0 = mk(x[e].x + zeta.x * w0.x - zeta.y * w0.y, zeta.x * w0.y + zeta.y * w0.x);
+    w1 = mk(x[e].y + zeta.x * w1.x - zeta.y * w1.y, zeta.x * w1.y + zeta.y * w1.x);
+  }
+  // inclusive scan of the chunk totals inside the warp: T_k = sum_{i<=k} zeta^(16 (k-i)) E_i
+  const unsigned mask = NT >= 32 ? 0xffffffffu : ((1u << NT) - 1u);
+#pragma unroll
+  for (int d = 1; d < 32 && d < NT; d <<= 1) {
+    const cplx<T> p = zp[d];
+    const T r0x = __shfl_up_sync(mask, w0.x, d), r0y = __shfl_up_sync(mask, w0.y, d);
+    const T r1x = __shfl_up_sync(mask, w1.x, d), r1y = __shfl_up_sync(mask, w1.y, d);
+    if (lane >= d) {
+      w0 = mk(w0.x + p.x * r0x - p.y * r0y, w0.y + p.x * r0y + p.y * r0x);
+      w1 = mk(w1.x + p.x * r1x - p.y * r1y, w1.y + p.x * r1y + p.y * r1x);
+    }
+  }
+  if (lane == 31 || tid == NT - 1) { wt[warp] = w0; wt[NW + warp] = w1; }
+  // exclusive value inside the warp
+  cplx<T> e0 = mk(__shfl_up_sync(mask, w0.x, 1), __shfl_up_sync(mask, w0.y, 1));
+  cplx<T> e1 = mk(__shfl_up_sync(mask, w1.x, 1), __shfl_up_sync(mask, w1.y, 1));
+  if (lane == 0) { e0 = mk((T)0, (T)0); e1 = e0; }
+  __syncthreads();
+  // carry into this warp's first chunk from the warps before it (zero history): zeta^512 per warp step
+  cplx<T> g0 = mk((T)0, (T)0), g1 = g0;
+  const cplx<T> z32 = zp[NT >= 32 ? 32 : NT];
+  for (int i = 0; i < warp; ++i) {
+    const cplx<T> a0 = wt[i], a1 = wt[NW + i];
+    g0 = mk(a0.x + z32.x * g0.x - z32.y * g0.y, a0.y + z32.x * g0.y + z32.y * g0.x);
+    g1 = mk(a1.x + z32.x * g1.x - z32.y * g1.y, a1.y + z32.x * g1.y + z32.y * g1.x);
+  }
+  if (tid == NT - 1) {                                        // row total with zero history = w[N-1] = w[-1]
+    const cplx<T> pl = zp[lane + 1];
+    wt[2 * NW] = mk(w0.x + pl.x * g0.x - pl.y * g0.y, w0.y + pl.x * g0.y + pl.y * g0.x);
+    wt[2 * NW + 1] = mk(w1.x + pl.x * g1.x - pl.y * g1.y, w1.y + pl.x * g1.y + pl.y * g1.x);
+  }
+  __syncthreads();
+  {
+    const cplx<T> pl = zp[lane], pk = zp[tid], c0 = wt[2 * NW], c1 = wt[2 * NW + 1];
+    // carry into chunk tid: exclusive in-warp part + zeta^(16 lane) warp carry + zeta^(16 tid) wrap-around
+    w0 = mk(e0.x + pl.x * g0.x - pl.y * g0.y + pk.x * c0.x - pk.y * c0.y,
+            e0.y + pl.x * g0.y + pl.y * g0.x + pk.x * c0.y + pk.y * c0.x);
+    w1 = mk(e1.x + pl.x * g1.x - pl.y * g1.y + pk.x * c1.x - pk.y * c1.y,
+            e1.y + pl.x * g1.y + pl.y * g1.x + pk.x * c1.y + pk.y * c1.x);
+  }
+#pragma unroll
+  for (int e = 0; e < 16; ++e) {
+    w0 = mk(x[e].x + zeta.x * w0.x - zeta.y * w0.y, zeta.x * w0.y + zeta.y * w0.x);
+    w1 = mk(x[e].y + zeta.x * w1.x - zeta.y * w1.y, zeta.x * w1.y + zeta.y * w1.x);
+    sm[17 * tid + e] = mk(omf * x[e].x + cs.x * w0.y + cs.y * w0.x, omf * x[e].y + cs.x * w1.y + cs.y * w1.x);
+  }
+  __syncthreads();
+  T* v0 = V + j * v_plane_stride + (long long)q0 * N;
+#pragma unroll 4
+  for (int e = 0; e < 16; ++e) {
+    const int n = tid + e * NT;
+    const cplx<T> v = sm[fft_pad(n)];
+    v0[n] = v.x;
+    if (has1) v0[N + n] = v.y;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
 // a6 (CUDA-core form): U[j][r][t] = sum_q S2[r][q] V[j][q][t], r,q packed pairs (p<=l), (m<=n);
 // S2 holds S_plmn with off-diagonal (m<n) columns doubled.
 // Plain register-tiled GEMM, C[Q x N] = S2[Q x Q] * V_j[Q x N], one plane per blockIdx.z.

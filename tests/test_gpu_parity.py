@@ -80,13 +80,25 @@ def test_fft_tiny_vs_brute_force_dft(B):
 
 
 # ------------------------------------------------------------------------ a4/a5: pair streams
-@pytest.mark.parametrize("cfg,N,kw", [(2, 1024, {}), (3, 2048, {}), (2, 256, dict(max_group=1))])
-def test_pair_conv_vs_oracle(B, cfg, N, kw):
+@pytest.mark.parametrize("raman", [1, 2])            # 1: FFT . h~ . IFFT;  2: one-pole recurrence along t
+@pytest.mark.parametrize("cfg,N,kw", [(2, 1024, {}), (3, 2048, {}), (2, 256, dict(max_group=1)), (2, 32, {}),
+                                      (3, 16384, dict(max_group=1))])
+def test_pair_conv_vs_oracle(B, cfg, N, kw, raman):
     w = W.make_config(cfg, N=N, **kw)
     planes = 3
     rng = np.random.default_rng(11)
     A = np.stack([w.A0 * np.exp(2j * np.pi * rng.random((w.P, 1))) for _ in range(planes)])
-    with B.plan_from_workload(w) as plan:
+    # a pulse sitting on the window edge: the convolution is circular (reading S7), the recurrence must wrap
+    A[2] = np.roll(A[2], w.N // 2 - 3, axis=-1)
+    if raman == 2 and np.exp(-w.N * w.dt / W.TAU2) > 1e-14:
+        # window shorter than the response's decay: the N samples are not one damped oscillation's worth
+        # (the tail wraps), so the recurrence is refused and only the FFT path applies
+        with pytest.raises(B.GmmnlseError) as e:
+            B.plan_from_workload(w, raman=2)
+        assert e.value.status == B.EUNSUPPORTED
+        return
+    with B.plan_from_workload(w, raman=raman) as plan:
+        assert plan.raman_kind() == raman
         Ad = dev(A, np.complex64)
         Q = w.P * (w.P + 1) // 2
         V = torch.empty((planes, Q, w.N), dtype=torch.float32, device="cuda")
@@ -132,6 +144,25 @@ def test_nonlinear_op_vs_oracle(B, cfg, kw):
 def test_nonlinear_op_full_shape_large_P(B, cfg):
     w = W.make_config(cfg)
     assert _nonlinear_op_case(B, w) <= TOL_OP
+
+
+def test_raman_path_selection_and_general_response(B):
+    """auto picks the recurrence for the damped-oscillator samples and the FFT path for anything else; a
+    response that is not a single damped oscillation (two oscillators) still matches the oracle."""
+    w = W.make_config(2, N=1024)
+    with B.plan_from_workload(w) as plan:
+        assert plan.raman_kind() == 2
+    h2 = 0.7 * W.raman_response(w.N, w.dt) + 0.3 * W.raman_response(w.N, w.dt, tau1=20e-15, tau2=60e-15)
+    w.h_R = h2
+    with B.plan_from_workload(w) as plan:
+        assert plan.raman_kind() == 1
+    with pytest.raises(B.GmmnlseError) as e:
+        B.plan_from_workload(w, raman=2)
+    assert e.value.status == B.EUNSUPPORTED
+    assert _nonlinear_op_case(B, w) <= TOL_OP
+    w.f_R, w.h_R = 0.0, None
+    with B.plan_from_workload(w) as plan:
+        assert plan.raman_kind() == 0
 
 
 def test_nonlinear_op_kerr_only_and_no_shock(B):
