@@ -42,9 +42,12 @@ typedef struct {                /* pass NULL for defaults                       
   int    max_iter;              /* cap on iterations per large step; <=0 -> 2*M + 4               */
   int    fixed_iter;            /* >0: run exactly this many iterations per large step (parity)   */
   int    contraction;           /* a6 kernel: 0 = auto (3 when Q = P(P+1)/2 >= 64, complex64, N % 128 == 0; else 1),
-                                   1 = CUDA-core fp32/fp64 GEMM, 2 = tcgen05 3xTF32 on CTA pairs
-                                   (cta_group::2), 3 = tcgen05 3xTF32 single CTA.  2-3 need complex64 and
-                                   N % 128 == 0 (else EUNSUPPORTED)                                */
+                                   1 = CUDA-core fp32/fp64 GEMM; tcgen05 3xTF32 forms: 2 = CTA pairs
+                                   (cta_group::2), 3 = single CTA, both operands in shared memory, 4 = single
+                                   CTA, V_hi/V_lo operand in tensor memory, 5 = form 3 on clusters of two CTAs
+                                   that TMA-multicast the S tiles to each other.  2-5 need complex64 and
+                                   N % 128 == 0 (2, 5: N % 256 == 0), else EUNSUPPORTED.  Forms 2, 4, 5 are
+                                   kept for measurement: none beats form 3 on B200   */
   int    raman;                 /* a5 kernel: 0 = auto, 1 = FFT . h~_R . IFFT on the pair streams (any h_R),
                                    2 = one-pole recurrence along t, exact when the samples are a damped
                                    oscillation h_R[j] = Im(c zeta^j) (the tau1/tau2 form); auto picks 2 when
@@ -137,8 +140,9 @@ int gmmnlse_debug_pairs(gmmnlse_plan *plan, const void *A, void *V, int n_planes
 /*   contract: U[plane][r][t] = sum_q S2[r][q] V[plane][q][t] over packed pairs r = (p<=l), q = (m<=n),
  *          S2 = S_plmn with the m<n columns doubled (Eq. 1's sum over m,n); V, U DEVICE
  *          [n_planes][Q][N] real of the plan's precision, U must not alias V.
- *   contraction_kind: which a6 kernel the plan selected: 1 CUDA cores, 2 tcgen05 single CTA,
- *          3 tcgen05 CTA pairs.                                                              */
+ *   contraction_kind: which a6 kernel the plan selected: 1 CUDA cores, 2 tcgen05 single CTA (operands in
+ *          shared memory), 3 tcgen05 CTA pairs, 4 tcgen05 single CTA with the V operand in tensor memory,
+ *          5 tcgen05 multicast pairs.                                                            */
 int gmmnlse_debug_contract(gmmnlse_plan *plan, const void *V, void *U, int n_planes);
 int gmmnlse_contraction_kind(const gmmnlse_plan *plan);
 /*   raman_kind: which a5 kernel the plan selected: 0 none (f_R = 0), 1 FFT, 2 recursive.          */

@@ -183,7 +183,7 @@ class Plan:
         _check(self._lib, self._lib.gmmnlse_debug_contract(self._h, _ptr(V), _ptr(U), n_planes))
 
     def contraction_kind(self) -> int:
-        """1 = CUDA cores, 2 = tcgen05 single CTA, 3 = tcgen05 CTA pairs."""
+        """1 = CUDA cores, 2 = tcgen05 single CTA (SS), 3 = tcgen05 CTA pairs, 4 = tcgen05 single CTA (TS)."""
         return int(self._lib.gmmnlse_contraction_kind(self._h))
 
     def raman_kind(self) -> int:

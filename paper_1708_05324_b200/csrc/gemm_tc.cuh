@@ -64,7 +64,11 @@ inline size_t smem_bytes(int NT, int CG, int stages) {
   return 1024 /*alignment slack*/ + 1024 /*barriers*/ + (size_t)stages * stage_bytes(NT, CG);
 }
 
-template <int CG>
+// MC (needs CG == 1): clusters of two CTAs work on neighbouring t-tiles of the same r-tile; each loads half of the
+// S_hi / S_lo rows and TMA-multicasts it into both CTAs' shared memory, halving the L2 reads of the B operand
+// (77 % of the bytes a k-block needs).  MMAs stay per-CTA (cta_group::1); a stage is free when BOTH CTAs' MMAs
+// have released it (tcgen05.commit multicast onto both `empty` barriers, count 2).
+template <int CG, bool MC = false>
 __global__ void __launch_bounds__(NTHREADS, 1)
 k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmShi,
               const __grid_constant__ CUtensorMap tmSlo, const Params p) {
@@ -81,7 +85,9 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
   unsigned char* tiles_ptr = sm + 1024;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const uint32_t rank = CG == 2 ? cluster_ctarank() : 0u;
+  static_assert(!(MC && CG == 2), "multicast form uses per-CTA MMAs");
+  constexpr int CL = (CG == 2 || MC) ? 2 : 1;            // CTAs per cluster
+  const uint32_t rank = CL == 2 ? cluster_ctarank() : 0u;
   const int nb = b_bytes(p.NT, CG), sbytes = stage_bytes(p.NT, CG);
   const int stages = p.stages;
 
@@ -94,7 +100,7 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
     if (lane == 0) {
       for (int s = 0; s < MAX_STAGES; ++s) {
         mbar_init(bar_full + 8 * s, 1);
-        mbar_init(bar_empty + 8 * s, 1);
+        mbar_init(bar_empty + 8 * s, MC ? 2 : 1);
         mbar_init(bar_conv + 8 * s, 4 * CG);
       }
       for (int a = 0; a < 2; ++a) {
@@ -108,11 +114,11 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
     tmem_relinquish<CG>();
   }
   tc_fence_before();
-  if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
+  if constexpr (CL == 2) cluster_sync_all(); else __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
-  const int pair = blockIdx.x / CG, npairs = gridDim.x / CG;
+  const int pair = blockIdx.x / CL, npairs = gridDim.x / CL;
   const int tiles_per_plane = p.n_rt * p.t_tiles;
 
   if (warp == 0) {
@@ -123,8 +129,8 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
       for (int tile = pair; tile < p.total_tiles; tile += npairs) {
         const int pl = tile / tiles_per_plane, rem = tile - pl * tiles_per_plane;
         const int tt = rem / p.n_rt, rt = rem - tt * p.n_rt;
-        const int t0 = tt * (TM * CG) + (int)rank * TM;
-        const int r0 = rt * p.NT + (int)rank * (p.NT / CG);
+        const int t0 = tt * (TM * CL) + (int)rank * TM;
+        const int r0 = rt * p.NT + (int)rank * (p.NT / CL);
         for (int kb = 0; kb < p.KB; ++kb) {
           mbar_wait(bar_empty + 8 * stage, phase ^ 1u, 1);
           const uint32_t fb = bar_full + 8 * stage;
@@ -141,8 +147,14 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
                 tma_load_3d(sa + i * (BK * 128), &tmV, fb, t0 + 32 * i, kb * BK, p.plane0 + pl);
             }
             if (!skipB) {
-              tma_load_2d(sa + 2 * A_BYTES, &tmShi, fb, kb * BK, r0);
-              tma_load_2d(sa + 2 * A_BYTES + nb, &tmSlo, fb, kb * BK, r0);
+              if constexpr (MC) {                                  // my half of the rows, into both CTAs
+                const uint32_t half = (uint32_t)(nb / 2) * rank;
+                tma_load_2d_mc(sa + 2 * A_BYTES + half, &tmShi, fb, kb * BK, r0, (uint16_t)3);
+                tma_load_2d_mc(sa + 2 * A_BYTES + nb + half, &tmSlo, fb, kb * BK, r0, (uint16_t)3);
+              } else {
+                tma_load_2d(sa + 2 * A_BYTES, &tmShi, fb, kb * BK, r0);
+                tma_load_2d(sa + 2 * A_BYTES + nb, &tmSlo, fb, kb * BK, r0);
+              }
             }
           }
           if (++stage == stages) { stage = 0; phase ^= 1u; }
@@ -151,7 +163,7 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
     }
   } else if (warp == 1) {
     // ================================================================= MMA issuer (leader CTA)
-    if (lane == 0 && rank == 0) {
+    if (lane == 0 && (CG == 1 || rank == 0)) {             // CG == 2: only the leader CTA issues
       // instruction descriptor: D fp32, A/B tf32, A MN-major, B K-major, N = NT, M = 128 * CG
       const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 15) | ((uint32_t)(p.NT >> 3) << 17) |
                              ((uint32_t)((TM * CG) >> 4) << 24);
@@ -183,7 +195,8 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
             mma_tf32_ss<CG>(d, a_lo + da, b_hi + db, idesc, 1u);
             mma_tf32_ss<CG>(d, a_raw + da, b_hi + db, idesc, 1u);
           }
-          mma_commit<CG>(bar_empty + 8 * stage);                   // frees the smem stage (both CTAs)
+          if constexpr (MC) mma_commit_mc(bar_empty + 8 * stage);  // frees the smem stage in both CTAs
+          else mma_commit<CG>(bar_empty + 8 * stage);
           if (++stage == stages) { stage = 0; phase ^= 1u; }
           if (++inchunk == p.kchunk || kb == p.KB - 1) {           // chunk complete: hand it to the epilogue
             mma_commit<CG>(bar_tfull + 8 * acc);
@@ -242,7 +255,7 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
     for (int tile = pair; tile < p.total_tiles; tile += npairs) {
       const int pl = tile / tiles_per_plane, rem = tile - pl * tiles_per_plane;
       const int tt = rem / p.n_rt, rt = rem - tt * p.n_rt;
-      const int t = tt * (TM * CG) + (int)rank * TM + lg * 32 + lane;
+      const int t = tt * (TM * CL) + (int)rank * TM + lg * 32 + lane;
       float* Uout = p.U + (long long)pl * p.u_plane_stride + t;
 #pragma unroll
       for (int i = 0; i < EPI_COLS; ++i) accr[i] = 0.f;
@@ -286,7 +299,7 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
   // ------------------------------------------------------------------- teardown
   __syncwarp();
   tc_fence_before();
-  if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
+  if constexpr (CL == 2) cluster_sync_all(); else __syncthreads();
   tc_fence_after();
   if (warp == 1) tmem_dealloc<CG>(tmem_base, TMEM_COLS);
 }

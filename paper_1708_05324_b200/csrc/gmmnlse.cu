@@ -13,7 +13,7 @@
 #include <vector>
 
 #include "../../include/gmmnlse.h"
-#include "gemm_tc.cuh"
+#include "gemm_ts.cuh"
 #include "kernels.cuh"
 
 namespace {
@@ -196,6 +196,8 @@ struct PlanT final : gmmnlse_plan {
   // tcgen05 contraction (complex64 path only): TF32 hi/lo split of S2, zero-padded to [R_pad][Q_pad]
   float *S2hi = nullptr, *S2lo = nullptr;
   CUtensorMap tmV, tmShi, tmSlo;
+  bool tc_ts = false;          // A operand from tensor memory (gemm_ts.cuh)
+  bool tc_mc = false;          // clusters of two CTAs multicasting the S tiles (gemm_tc.cuh, MC)
   int tc_cg = 0, tc_NT = 0, tc_nrt = 0, tc_KB = 0, tc_stages = 0, tc_kchunk = 4, tc_probe = 0, tc_stage_cap = 0, n_sm = 0;
 
   ~PlanT() override {
@@ -384,10 +386,14 @@ struct PlanT final : gmmnlse_plan {
 
   // ------------------------------------------------------------------ tcgen05 contraction setup
   // contraction option: 0 auto (tensor cores when Q >= 64), 1 CUDA cores, 2 tcgen05 cta_group::2,
-  // 3 tcgen05 cta_group::1.
+  // 3 tcgen05 cta_group::1 with both operands in shared memory, 4 tcgen05 with V_hi/V_lo in tensor memory.
   int make_v_tmap(CUtensorMap* tm, const T* base, int planes) {
     const cuuint64_t dims[3] = {(cuuint64_t)N, (cuuint64_t)Q, (cuuint64_t)planes};
     const cuuint64_t strides[2] = {(cuuint64_t)N * 4, (cuuint64_t)QN * 4};
+    if (tc_ts) {                                     // TS form: one plain [BK q][128 t] box, read by threads only
+      const cuuint32_t box_ts[3] = {tc::TM, tc::BK, 1};
+      return encode_tmap_f32(tm, (void*)base, 3, dims, strides, box_ts, CU_TENSOR_MAP_SWIZZLE_NONE);
+    }
     const cuuint32_t box[3] = {32, tc::BK, 1};
     // t-contiguous operand: 32-byte swizzle atoms (the only MN-major layout kind::tf32 accepts)
     return encode_tmap_f32(tm, (void*)base, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B);
@@ -401,6 +407,11 @@ struct PlanT final : gmmnlse_plan {
       if (!want) return 0;
       // auto picks the single-CTA form: measured 1.76 ms against 1.86 ms for CTA pairs at config 5
       int cg = contraction == 2 ? 2 : 1;
+      // the tensor-memory (TS) form measured the same as the shared-memory (SS) form (1.68 vs 1.67 ms at config 5):
+      // auto keeps SS, the form the committed ncu profiles describe; 4 selects TS
+      tc_ts = contraction == 4;
+      tc_mc = contraction == 5 && N % (2 * tc::TM) == 0;
+      if (contraction == 5 && !tc_mc) return GMMNLSE_EUNSUPPORTED;
       if (N % (tc::TM * cg) != 0) {
         if (N % tc::TM == 0) cg = 1;
         else if (contraction >= 2) return GMMNLSE_EUNSUPPORTED;
@@ -416,8 +427,9 @@ struct PlanT final : gmmnlse_plan {
       int smax = 0;
       GM_CUDA(cudaDeviceGetAttribute(&smax, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
       tc_stages = tc::MAX_STAGES;
-      while (tc_stages > 1 && tc::smem_bytes(tc_NT, cg, tc_stages) > (size_t)smax) --tc_stages;
-      if (tc::smem_bytes(tc_NT, cg, tc_stages) > (size_t)smax) return GMMNLSE_EUNSUPPORTED;
+      auto need = [&](int st) { return tc_ts ? tc::ts_smem_bytes(tc_NT, st) : tc::smem_bytes(tc_NT, cg, st); };
+      while (tc_stages > 1 && need(tc_stages) > (size_t)smax) --tc_stages;
+      if (need(tc_stages) > (size_t)smax) return GMMNLSE_EUNSUPPORTED;
       std::vector<float> hi((size_t)Rp * Qp, 0.f), lo((size_t)Rp * Qp, 0.f);
       for (int r = 0; r < Q; ++r)
         for (int q = 0; q < Q; ++q) {
@@ -430,13 +442,17 @@ struct PlanT final : gmmnlse_plan {
       GM_TRY(dalloc(&S2lo, lo.size())); GM_TRY(upload(S2lo, lo));
       const cuuint64_t dims[2] = {(cuuint64_t)Qp, (cuuint64_t)Rp};
       const cuuint64_t strides[1] = {(cuuint64_t)Qp * 4};
-      const cuuint32_t box[2] = {tc::BK, (cuuint32_t)(tc_NT / cg)};
+      const cuuint32_t box[2] = {tc::BK, (cuuint32_t)(tc_NT / (tc_mc ? 2 : cg))};
       const CUtensorMapSwizzle bsw = tc::BK == 32 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B;
       GM_TRY(encode_tmap_f32(&tmShi, S2hi, 2, dims, strides, box, bsw));
       GM_TRY(encode_tmap_f32(&tmSlo, S2lo, 2, dims, strides, box, bsw));
       GM_TRY(make_v_tmap(&tmV, V, M + 1));
-      const int smem = (int)tc::smem_bytes(tc_NT, cg, tc_stages);
-      if (cg == 2)
+      const int smem = (int)need(tc_stages);
+      if (tc_ts)
+        GM_CUDA(cudaFuncSetAttribute(tc::k_contract_ts, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+      else if (tc_mc)
+        GM_CUDA(cudaFuncSetAttribute(tc::k_contract_tc<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+      else if (cg == 2)
         GM_CUDA(cudaFuncSetAttribute(tc::k_contract_tc<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
       else
         GM_CUDA(cudaFuncSetAttribute(tc::k_contract_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
@@ -453,27 +469,30 @@ struct PlanT final : gmmnlse_plan {
       prm.U = Uout;
       prm.u_plane_stride = QN;
       prm.Q = Q; prm.N = N; prm.NT = tc_NT; prm.KB = tc_KB; prm.n_rt = tc_nrt;
-      prm.t_tiles = N / (tc::TM * tc_cg);
+      const int cl = tc_mc ? 2 : tc_cg;                          // CTAs per cluster
+      prm.t_tiles = N / (tc::TM * cl);
       prm.total_tiles = planes * prm.t_tiles * tc_nrt;
       prm.plane0 = plane0; prm.stages = tc_stages; prm.kchunk = tc_kchunk;
       prm.probe = tc_probe;
       if (tc_stage_cap > 0 && tc_stage_cap < prm.stages) prm.stages = tc_stage_cap;
-      const int pairs = std::min(n_sm / tc_cg, prm.total_tiles);
+      const int pairs = std::min(n_sm / cl, prm.total_tiles);
       cudaLaunchConfig_t cfg = {};
-      cfg.gridDim = dim3((unsigned)(pairs * tc_cg));
+      cfg.gridDim = dim3((unsigned)(pairs * cl));
       cfg.blockDim = dim3(tc::NTHREADS);
-      cfg.dynamicSmemBytes = tc::smem_bytes(tc_NT, tc_cg, tc_stages);
+      cfg.dynamicSmemBytes = tc_ts ? tc::ts_smem_bytes(tc_NT, prm.stages) : tc::smem_bytes(tc_NT, tc_cg, tc_stages);
       cfg.stream = stream;
       cudaLaunchAttribute attr[1];
       attr[0].id = cudaLaunchAttributeClusterDimension;
-      attr[0].val.clusterDim.x = (unsigned)tc_cg;
+      attr[0].val.clusterDim.x = (unsigned)cl;
       attr[0].val.clusterDim.y = 1;
       attr[0].val.clusterDim.z = 1;
       cfg.attrs = attr;
       cfg.numAttrs = 1;
       prof_begin(GMMNLSE_KIND_CONTRACT);
       cudaError_t e;
-      if (tc_cg == 2) e = cudaLaunchKernelEx(&cfg, tc::k_contract_tc<2>, vmap, tmShi, tmSlo, prm);
+      if (tc_ts) e = cudaLaunchKernelEx(&cfg, tc::k_contract_ts, vmap, tmShi, tmSlo, prm);
+      else if (tc_mc) e = cudaLaunchKernelEx(&cfg, tc::k_contract_tc<1, true>, vmap, tmShi, tmSlo, prm);
+      else if (tc_cg == 2) e = cudaLaunchKernelEx(&cfg, tc::k_contract_tc<2>, vmap, tmShi, tmSlo, prm);
       else e = cudaLaunchKernelEx(&cfg, tc::k_contract_tc<1>, vmap, tmShi, tmSlo, prm);
       prof_end();
       GM_CUDA(e);
@@ -779,7 +798,7 @@ struct PlanT final : gmmnlse_plan {
     if (n_planes < 1) return GMMNLSE_EINVAL;
     return launch_pairs((const C*)A, PN, (T*)Vout, QN, n_planes);
   }
-  int contraction_kind() const override { return tc_cg ? 1 + tc_cg : 1; }
+  int contraction_kind() const override { return tc_cg ? (tc_ts ? 4 : (tc_mc ? 5 : 1 + tc_cg)) : 1; }
   int raman_kind() const override { return f_R == 0.0 ? 0 : (iir ? 2 : 1); }
   int set_tc_chunk(int k) override {
     if ((k & 0xFF) < 1) return GMMNLSE_EINVAL;
@@ -827,7 +846,7 @@ int gmmnlse_plan_create(gmmnlse_plan** out, int P, int N, int M, double dt, doub
   if (!(dt > 0) || !(dz > 0) || !(omega0 > 0) || !std::isfinite(n2) || !std::isfinite(f_R)) return GMMNLSE_EINVAL;
   if ((f_R != 0.0) != (h_R != nullptr)) return GMMNLSE_EINVAL;
   if (o.precision != 0 && o.precision != 1) return GMMNLSE_EINVAL;
-  if (o.raman < 0 || o.raman > 2) return GMMNLSE_EINVAL;
+  if (o.raman < 0 || o.raman > 2 || o.contraction < 0 || o.contraction > 5) return GMMNLSE_EINVAL;
   if (o.shock && M_PI / dt >= omega0) return GMMNLSE_EINVAL;
   if (!(o.tol > 0)) o.tol = 1e-6;
   for (long long i = 0; i < (long long)P * n_beta; ++i)

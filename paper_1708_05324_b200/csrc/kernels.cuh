@@ -14,7 +14,7 @@ namespace gm {
 //   out_k = X_k * scale * (post_vec ? post_vec[k] : 1) * (post_tab ? conj(post_tab[j][p][k]) : 1)
 //                                                        Eq. 12: K(w) exp(-D j dz) F{N_p}
 template <typename T, int LOG2N, int DIR>
-__global__ void __launch_bounds__((1 << LOG2N) / 16)
+__global__ void __launch_bounds__((1 << LOG2N) / 16, ((1 << LOG2N) / 16 == 512 && sizeof(T) == 4) ? 2 : 1)
 k_fft_rows(const cplx<T>* __restrict__ in, long long in_plane_stride, cplx<T>* __restrict__ out,
            long long out_plane_stride, const cplx<T>* __restrict__ pre, const cplx<T>* __restrict__ post_vec,
            const cplx<T>* __restrict__ post_tab, long long tab_plane_stride, T scale,

@@ -334,10 +334,11 @@ def _packed_S2(S):
 
 
 @pytest.mark.parametrize("cfg,N,kw,kind", [
-    (3, 1024, {}, 1), (3, 1024, {}, 3), (3, 1024, {}, 2),          # Q = 120: one r-tile of 128, K = 4 blocks
-    (4, 512, {}, 3), (4, 512, {}, 2),                              # Q = 210: two r-tiles of 112
-    (5, 256, {}, 3), (5, 256, {}, 2), (5, 256, {}, 1),             # Q = 1035: five r-tiles of 208, ragged K
-    (3, 128, dict(max_group=3), 3),                                # Q = 55 < 64: tensor path forced, N = 128
+    (3, 1024, {}, 1), (3, 1024, {}, 3), (3, 1024, {}, 2), (3, 1024, {}, 4),   # Q = 120: one r-tile of 128
+    (4, 512, {}, 3), (4, 512, {}, 2), (4, 512, {}, 4),             # Q = 210: two r-tiles of 112
+    (5, 256, {}, 3), (5, 256, {}, 2), (5, 256, {}, 1), (5, 256, {}, 4), (5, 256, {}, 5),   # Q = 1035: 5 r-tiles of 208
+    (3, 1024, {}, 5), (4, 512, {}, 5),                              # multicast pairs
+    (3, 128, dict(max_group=3), 3), (3, 128, dict(max_group=3), 4),       # Q = 55 < 64: tensor path forced, N = 128
 ])
 def test_contraction_vs_fp64_matmul(B, cfg, N, kw, kind):
     w = W.make_config(cfg, N=N, **kw)
@@ -347,7 +348,7 @@ def test_contraction_vs_fp64_matmul(B, cfg, N, kw, kind):
     # pair streams with the dynamic range of |A|^2 products: peak to 1e-6 of peak along t
     V = (rng.standard_normal((planes, Q, N)) * np.exp(rng.uniform(-7, 7, (planes, 1, N)))).astype(np.float32)
     with B.plan_from_workload(w, contraction=kind) as plan:
-        assert plan.contraction_kind() == {1: 1, 2: 3, 3: 2}[kind]
+        assert plan.contraction_kind() == {1: 1, 2: 3, 3: 2, 4: 4, 5: 5}[kind]
         Vd = torch.from_numpy(V).cuda()
         U = torch.full((planes, Q, N), float("nan"), dtype=torch.float32, device="cuda")
         plan.debug_contract(Vd, U, planes)
