@@ -33,7 +33,8 @@ __all__ = [
     "dft_direct", "fft_radix2", "to_freq", "to_time", "omega_grid",
     "dispersion_operator", "raman_transfer", "pair_products",
     "raman_convolve_direct", "raman_convolve", "nonlinear_term",
-    "nonlinear_term_literal", "nonlinear_op", "nonlinear_op_freq",
+    "nonlinear_term_literal", "nonlinear_term_general", "nonlinear_term_general_literal",
+    "nonlinear_op", "nonlinear_op_freq",
     "rk4ip_step", "rk4ip_propagate", "mpa_large_step", "mpa_propagate",
     "energy", "photon_number", "conserved_quantity",
 ]
@@ -142,6 +143,8 @@ def nonlinear_term(A, S, f_R=0.0, h_R=None, dt=1.0, direct_conv=False):
     T_mn, their Raman convolution, the blend, the sum over (m,n) (a matmul
     step), the sum over l.  No symmetry of S is used.
     """
+    if isinstance(S, tuple):                              # (S^K, S^R): the general form of Eq. 1
+        return nonlinear_term_general(A, S[0], S[1], f_R, h_R, dt, direct_conv)
     A = np.asarray(A, dtype=np.complex128)
     S = np.asarray(S, dtype=np.float64)
     P, N = A.shape
@@ -182,6 +185,50 @@ def nonlinear_term_literal(A, S, f_R=0.0, h_R=None, dt=1.0):
                             R[i] = dt * acc
                         term = term + f_R * R
                     out[p] += s * A[l] * term
+    return out
+
+
+def nonlinear_term_general(A, SK, SR, f_R=0.0, h_R=None, dt=1.0, direct_conv=False):
+    """N_p(t) = sum_{lmn} A_l [(1-fR) S^K_plmn A_m A_n* + fR S^R_plmn (h_R (*) A_m A_n*)].
+
+    Eq. 1 before the scalar-mode simplification of Eq. 2: separate Kerr and Raman
+    tensors, real or complex, with no index symmetry assumed (S^K and S^R differ once the
+    modes carry polarisation).  Two polarisations per spatial mode are 2P fields
+    with the corresponding (2P)^4 tensors.  Staged as the definition reads: all P^2 ordered pair
+    streams, their convolution, one matmul per tensor, the sum over l.
+    """
+    A = np.asarray(A, dtype=np.complex128)
+    SK = np.asarray(SK, dtype=np.complex128)
+    SR = np.asarray(SR, dtype=np.complex128)
+    P, N = A.shape
+    T = pair_products(A).reshape(P * P, N)                # [(m n)][t]
+    U = (1.0 - f_R) * (SK.reshape(P * P, P * P) @ T)
+    if f_R != 0.0:
+        R = (raman_convolve_direct if direct_conv else raman_convolve)(T, h_R, dt)
+        U = U + f_R * (SR.reshape(P * P, P * P) @ R)
+    return np.einsum("plt,lt->pt", U.reshape(P, P, N), A)
+
+
+def nonlinear_term_general_literal(A, SK, SR, f_R=0.0, h_R=None, dt=1.0):
+    """Four nested loops + the literal convolution for the general form (tiny P, N only)."""
+    A = np.asarray(A, dtype=np.complex128)
+    P, N = A.shape
+    out = np.zeros((P, N), dtype=np.complex128)
+    for p in range(P):
+        for l in range(P):
+            for m in range(P):
+                for n in range(P):
+                    T = A[m] * np.conj(A[n])
+                    term = (1.0 - f_R) * SK[p, l, m, n] * T
+                    if f_R != 0.0:
+                        R = np.zeros(N, dtype=np.complex128)
+                        for i in range(N):
+                            acc = 0.0
+                            for j in range(N):
+                                acc += h_R[j] * T[(i - j) % N]
+                            R[i] = dt * acc
+                        term = term + f_R * SR[p, l, m, n] * R
+                    out[p] += A[l] * term
     return out
 
 

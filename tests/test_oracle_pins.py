@@ -294,3 +294,45 @@ def test_mpa_ragged_last_step_and_fixed_iter():
     st = {}
     O.mpa_propagate(wl.A0, 10 * 50e-6, 50e-6, 5, *args, fixed_iter=3, stats=st)
     assert st["iterations"] == 6
+
+
+# ------------------------------------------------------------ general form (S^K != S^R, complex, no symmetry)
+@pytest.mark.parametrize("P,N,fR,cplx", [(2, 8, 0.0, False), (3, 8, 0.18, False), (3, 8, 0.3, True)])
+def test_general_term_vs_literal_loop_and_reductions(P, N, fR, cplx):
+    rng = np.random.default_rng(7 * P + N)
+    A = rng.standard_normal((P, N)) + 1j * rng.standard_normal((P, N))
+    mk = lambda: rng.standard_normal((P,) * 4) + (1j * rng.standard_normal((P,) * 4) if cplx else 0)
+    SK, SR = mk(), mk()
+    h = rng.standard_normal(N) if fR else None
+    dt = 0.41
+    a = O.nonlinear_term_general(A, SK, SR, fR, h, dt)
+    assert rel(a, O.nonlinear_term_general_literal(A, SK, SR, fR, h, dt)) < 1e-13
+    # tuple dispatch through the common entry, and S^K = S^R = real S reduces to the scalar-mode term (Eq. 2)
+    assert rel(O.nonlinear_term(A, (SK, SR), fR, h, dt), a) < 1e-15
+    S = rng.standard_normal((P,) * 4)
+    assert rel(O.nonlinear_term_general(A, S, S, fR, h, dt), O.nonlinear_term(A, S, fR, h, dt)) < 1e-13
+    if fR:
+        # linear in each tensor; the Raman tensor acts only through h_R (*) T: CW fields see the blended tensor
+        z = np.zeros_like(SK)
+        assert rel(O.nonlinear_term_general(A, SK, z, fR, h, dt) + O.nonlinear_term_general(A, z, SR, fR, h, dt), a) < 1e-13
+        Acw = (rng.standard_normal((P, 1)) + 1j * rng.standard_normal((P, 1))) * np.ones((1, N))
+        hn = np.abs(rng.standard_normal(N)); hn /= dt * hn.sum()           # dt sum h = 1
+        blend = (1 - fR) * SK + fR * SR
+        assert rel(O.nonlinear_term_general(Acw, SK, SR, fR, hn, dt),
+                   O.nonlinear_term_general(Acw, blend, blend, 0.0, None, dt)) < 1e-12
+
+
+def test_general_form_conserves_energy_for_a_hermitian_tensor():
+    """With S_plmn = conj(S_lpnm) (what an overlap integral of F_p* F_l F_m* F_n-type products gives) and no shock,
+    sum_p int A_p* N_p is real, so the energy is conserved: an invariant of the general path's integrators."""
+    rng = np.random.default_rng(5)
+    P, N = 3, 64
+    dt = 5e-15
+    S0 = rng.standard_normal((P,) * 4) + 1j * rng.standard_normal((P,) * 4)
+    S = 0.5 * (S0 + np.conj(S0.transpose(1, 0, 3, 2))) * 1e9
+    t = (np.arange(N) - N // 2) * dt
+    A0 = (rng.standard_normal((P, 1)) + 1j * rng.standard_normal((P, 1))) * np.exp(-(t / 40e-15) ** 2)[None, :] * 30.0
+    beta = np.zeros((P, 3)); beta[:, 2] = 2e-26
+    out = O.rk4ip_propagate(A0, 0.02, 0.0005, beta, (S, S), KAPPA, W.OMEGA0, 0.0, None, dt, shock=False)
+    assert abs(O.energy(out, dt) / O.energy(A0, dt) - 1) < 1e-8
+    assert rel(out, A0) > 1e-3            # the propagation did something
