@@ -75,6 +75,18 @@ int gmmnlse_plan_create(gmmnlse_plan **out, int P, int N, int M, double dt, doub
                         double f_R, const double *h_R, double omega0, double n2,
                         const gmmnlse_options *opt);
 
+/* Plan for the GENERAL form of Eq. 1: separate Kerr and Raman tensors,
+ *   N_p = sum_lmn A_l [(1-fR) S^K_plmn A_m A_n* + fR S^R_plmn (h_R (*) A_m A_n*)],
+ * real or complex, with NO index symmetry assumed.  Two polarisations per spatial mode are 2P fields with the
+ * corresponding (2P)^4 tensors.  S_K, S_R: HOST [P][P][P][P] (index as S above), doubles; if tensors_complex != 0
+ * each entry is (re, im) interleaved.  Everything else as gmmnlse_plan_create; all other calls work on the plan
+ * unchanged.  The contraction runs on 2 ceil(P^2/2) x 2 real pair streams (Re and Im of A_m A_n*, Kerr- and
+ * Raman-weighted) instead of the P(P+1)/2 packed ones: about 8x the work of the scalar-mode path at equal P.   */
+int gmmnlse_plan_create_general(gmmnlse_plan **out, int P, int N, int M, double dt, double dz,
+                                const double *beta, int n_beta, const double *S_K, const double *S_R,
+                                int tensors_complex, double f_R, const double *h_R, double omega0, double n2,
+                                const gmmnlse_options *opt);
+
 /* Integrate Eq. 1 from z0 to z0 + L with the MPA.
  *   A_in, A_out  DEVICE [P][N] interleaved (re,im), float2 or double2 per precision, time
  *                domain, sqrt(W); A_out may alias A_in; never freed by the library.

@@ -39,6 +39,9 @@ SIGNATURES = {
     "gmmnlse_plan_create": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
                                       _DP, C.c_int, _DP, C.c_double, _DP, C.c_double, C.c_double,
                                       C.POINTER(Options)]),
+    "gmmnlse_plan_create_general": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_double,
+                                              C.c_double, _DP, C.c_int, _DP, _DP, C.c_int, C.c_double, _DP,
+                                              C.c_double, C.c_double, C.POINTER(Options)]),
     "gmmnlse_propagate": (C.c_int, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]),
     "gmmnlse_propagate_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]),
     "gmmnlse_propagate_rk4ip": (C.c_int, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]),
@@ -108,16 +111,30 @@ class Plan:
         self._lib = load_library()
         self._h = C.c_void_p()
         beta = np.ascontiguousarray(beta, dtype=np.float64).reshape(P, -1)
-        S = np.ascontiguousarray(S, dtype=np.float64)
-        if S.size != P ** 4:
-            raise GmmnlseError(EINVAL, "S must hold P^4 entries")
+        general = isinstance(S, tuple)          # (S_K, S_R): the general form of Eq. 1
+        if general:
+            cplx = any(np.iscomplexobj(x) for x in S)
+            SK, SR = (np.ascontiguousarray(x, dtype=np.complex128 if cplx else np.float64) for x in S)
+            if SK.size != P ** 4 or SR.size != P ** 4:
+                raise GmmnlseError(EINVAL, "S_K and S_R must hold P^4 entries each")
+        else:
+            S = np.ascontiguousarray(S, dtype=np.float64)
+            if S.size != P ** 4:
+                raise GmmnlseError(EINVAL, "S must hold P^4 entries")
         hR = None if h_R is None else np.ascontiguousarray(h_R, dtype=np.float64)
         if hR is not None and hR.size != N:
             raise GmmnlseError(EINVAL, "h_R must hold N samples")
         opt = Options(int(precision), int(bool(shock)), float(tol), int(max_iter), int(fixed_iter), int(contraction), int(raman))
-        st = self._lib.gmmnlse_plan_create(
-            C.byref(self._h), P, N, M, dt, dz, beta.ctypes.data_as(_DP), beta.shape[1], S.ctypes.data_as(_DP),
-            f_R, None if hR is None else hR.ctypes.data_as(_DP), omega0, n2, C.byref(opt))
+        hp = None if hR is None else hR.ctypes.data_as(_DP)
+        if general:
+            st = self._lib.gmmnlse_plan_create_general(
+                C.byref(self._h), P, N, M, dt, dz, beta.ctypes.data_as(_DP), beta.shape[1],
+                C.cast(SK.ctypes.data, _DP), C.cast(SR.ctypes.data, _DP), int(cplx), f_R, hp, omega0, n2,
+                C.byref(opt))
+        else:
+            st = self._lib.gmmnlse_plan_create(
+                C.byref(self._h), P, N, M, dt, dz, beta.ctypes.data_as(_DP), beta.shape[1], S.ctypes.data_as(_DP),
+                f_R, hp, omega0, n2, C.byref(opt))
         _check(self._lib, st)
         self.P, self.N, self.M, self.precision = P, N, M, int(precision)
         self.np_dtype = np.complex128 if precision else np.complex64

@@ -109,6 +109,9 @@ int ilog2(int n) {
 struct gmmnlse_plan {
   int P = 0, N = 0, M = 0, log2N = 0, Q = 0, precision = 0, shock = 1, max_iter = 0, fixed_iter = 0;
   int contraction = 0, raman = 0;
+  // general form of Eq. 1 (gmmnlse_plan_create_general): separate, possibly complex tensors, no symmetry
+  bool general = false, gen_complex = false;
+  const double* gen_SR = nullptr;          // host, valid during init only
   double dt = 0, dz = 0, f_R = 0, omega0 = 0, n2 = 0, tol = 1e-6;
   cudaStream_t stream = nullptr;
   long long n_large = 0, n_iter = 0, n_noconv = 0, n_launch = 0;
@@ -186,6 +189,10 @@ struct PlanT final : gmmnlse_plan {
   C* d_io = nullptr;
   std::map<int, double2*> EM_ragged;
   long long PN = 0, QN = 0;
+  int Bp = 0;                              // general mode: rows per Re / Im block of U, streams per Kerr / Raman block
+  int* st_kind = nullptr;
+  T *st_wk = nullptr, *st_wr = nullptr;
+  StreamSpec<T> spec() const { return StreamSpec<T>{st_kind, st_wk, st_wr}; }
   // recursive Raman path (k_pair_iir): h_R[j] = Im(c zeta^j) detected from the samples
   bool iir = false;
   C iir_zeta, iir_cs, *iir_zp = nullptr;
@@ -205,7 +212,7 @@ struct PlanT final : gmmnlse_plan {
     cudaFree(pair_m); cudaFree(pair_n); cudaFree(psi0_d); cudaFree(psi); cudaFree(At); cudaFree(G);
     cudaFree(V); cudaFree(U); cudaFree(errbuf); cudaFree(d_err); cudaFree(d_io);
     cudaFree(S2hi); cudaFree(S2lo);
-    cudaFree(iir_zp); cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
+    cudaFree(st_kind); cudaFree(st_wk); cudaFree(st_wr); cudaFree(iir_zp); cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
     if (h_err) cudaFreeHost(h_err);
     if (h_in) cudaFreeHost(h_in);
     if (h_out) cudaFreeHost(h_out);
@@ -235,7 +242,9 @@ struct PlanT final : gmmnlse_plan {
 
   int init(const double* S, const double* h_R) override {
     PN = (long long)P * N;
-    Q = P * (P + 1) / 2;
+    const int Qs = P * (P + 1) / 2;                  // unordered pairs m <= n
+    Bp = (P * P + 1) & ~1;                           // P^2 rounded up to even
+    Q = general ? 2 * Bp : Qs;
     QN = (long long)Q * N;
     // ---- tables (fp64 on the host, rounded once to T) ----
     std::vector<double> omega(N);
@@ -254,7 +263,8 @@ struct PlanT final : gmmnlse_plan {
         host_fft(hh, +1);
       }
       for (int k = 0; k < N; ++k) {
-        const cd v = ((1.0 - f_R) + f_R * dt * hh[k]) / (double)N;
+        // scalar-mode path: the blended transfer function; general path: ht_R / N alone (weights per stream)
+        const cd v = general ? dt * hh[k] / (double)N : ((1.0 - f_R) + f_R * dt * hh[k]) / (double)N;
         h_H[k] = mk((T)v.real(), (T)v.imag());
       }
     }
@@ -266,20 +276,62 @@ struct PlanT final : gmmnlse_plan {
         h_E[(size_t)j * PN + i] = mk((T)std::cos(ph), (T)std::sin(ph));
       }
     // ---- packed coupling matrix: rows (p<=l), columns (m<=n), off-diagonal columns doubled ----
-    std::vector<int> pm(Q), pn(Q);
-    {
+    std::vector<int> pm(Q, 0), pn(Q, 0);
+    std::vector<T> h_S2((size_t)Q * Q);
+    std::vector<double> h_S2d((size_t)Q * Q, 0.0);
+    if (!general) {
       int q = 0;
       for (int m = 0; m < P; ++m)
         for (int n = m; n < P; ++n, ++q) { pm[q] = m; pn[q] = n; }
-    }
-    std::vector<T> h_S2((size_t)Q * Q);
-    std::vector<double> h_S2d((size_t)Q * Q);
-    for (int r = 0; r < Q; ++r)
-      for (int q = 0; q < Q; ++q) {
-        const size_t idx = (((size_t)pm[r] * P + pn[r]) * P + pm[q]) * P + pn[q];
-        h_S2d[(size_t)r * Q + q] = S[idx] * (pm[q] == pn[q] ? 1.0 : 2.0);
-        h_S2[(size_t)r * Q + q] = (T)h_S2d[(size_t)r * Q + q];
+      for (int r = 0; r < Q; ++r)
+        for (int qq = 0; qq < Q; ++qq) {
+          const size_t idx = (((size_t)pm[r] * P + pn[r]) * P + pm[qq]) * P + pn[qq];
+          h_S2d[(size_t)r * Q + qq] = S[idx] * (pm[qq] == pn[qq] ? 1.0 : 2.0);
+        }
+    } else {
+      // General form.  Streams (columns), two blocks of Bp: [Kerr | Raman]; inside a block the Qs streams
+      // X_mn = Re(A_m A_n*), m <= n, then the Qs - P streams Y_mn = Im(A_m A_n*), m < n (T_nm = conj T_mn).
+      // Rows, two blocks of Bp: Re U_pl then Im U_pl, (p, l) ordered, row p P + l.  With s = S_plmn (complex):
+      //   sum_mn s_mn T_mn = sum_{m<=n} alpha_mn X_mn + sum_{m<n} beta_mn Y_mn,
+      //   alpha = s_mm (m = n) or s_mn + s_nm,  beta = i (s_mn - s_nm).
+      std::vector<int> kind(Q, 0);
+      std::vector<T> wk(Q, (T)0), wr(Q, (T)0);
+      for (int b = 0; b < 2; ++b) {
+        int q = b * Bp;
+        for (int m = 0; m < P; ++m)
+          for (int n = m; n < P; ++n, ++q) { pm[q] = m; pn[q] = n; kind[q] = 0; }
+        for (int m = 0; m < P; ++m)
+          for (int n = m + 1; n < P; ++n, ++q) { pm[q] = m; pn[q] = n; kind[q] = 1; }
+        for (int qq = b * Bp; qq < (b + 1) * Bp; ++qq) {
+          wk[qq] = b == 0 ? (T)(1.0 - f_R) : (T)0;
+          wr[qq] = b == 0 ? (T)0 : (T)f_R;
+        }
       }
+      const int stride = gen_complex ? 2 : 1;
+      auto tens = [&](const double* Sx, int p, int l, int m, int n) {
+        const size_t idx = ((((size_t)p * P + l) * P + m) * P + n) * stride;
+        return cd(Sx[idx], gen_complex ? Sx[idx + 1] : 0.0);
+      };
+      for (int b = 0; b < 2; ++b) {
+        const double* Sx = b == 0 ? S : gen_SR;
+        for (int p = 0; p < P; ++p)
+          for (int l = 0; l < P; ++l) {
+            const size_t rr = (size_t)p * P + l, ri = (size_t)Bp + rr;
+            for (int q = b * Bp; q < b * Bp + P * P; ++q) {
+              const int m = pm[q], n = pn[q];
+              cd c;
+              if (kind[q] == 0) c = m == n ? tens(Sx, p, l, m, m) : tens(Sx, p, l, m, n) + tens(Sx, p, l, n, m);
+              else c = cd(0, 1) * (tens(Sx, p, l, m, n) - tens(Sx, p, l, n, m));
+              h_S2d[rr * Q + q] = c.real();
+              h_S2d[ri * Q + q] = c.imag();
+            }
+          }
+      }
+      GM_TRY(dalloc(&st_kind, Q)); GM_TRY(upload(st_kind, kind));
+      GM_TRY(dalloc(&st_wk, Q)); GM_TRY(upload(st_wk, wk));
+      GM_TRY(dalloc(&st_wr, Q)); GM_TRY(upload(st_wr, wr));
+    }
+    for (size_t i = 0; i < h_S2.size(); ++i) h_S2[i] = (T)h_S2d[i];
     GM_TRY(dalloc(&tw, N)); GM_TRY(upload(tw, h_tw));
     GM_TRY(dalloc(&Kw, N)); GM_TRY(upload(Kw, h_K));
     GM_TRY(dalloc(&H, N)); GM_TRY(upload(H, h_H));
@@ -348,7 +400,7 @@ struct PlanT final : gmmnlse_plan {
     GM_TRY(dalloc(&iir_zp, zp.size()));
     GM_TRY(upload(iir_zp, zp));
     iir_zeta = mk((T)zeta.real(), (T)zeta.imag());
-    const cd csd = c * (dt * f_R);
+    const cd csd = general ? c * dt : c * (dt * f_R);      // general mode: f_R sits in the per-stream weights
     iir_cs = mk((T)csd.real(), (T)csd.imag());
     iir_omf = (T)(1.0 - f_R);
     iir = true;
@@ -366,7 +418,7 @@ struct PlanT final : gmmnlse_plan {
     }
     prof_begin(GMMNLSE_KIND_PAIR_CONV);
     k_pair_iir<T, LOG2N><<<dim3((Q + 1) / 2, planes), NT, smem, stream>>>(A, a_ps, Vout, v_ps, pair_m, pair_n, Q,
-                                                                          iir_zeta, iir_cs, iir_omf, iir_zp);
+                                                                          iir_zeta, iir_cs, iir_omf, iir_zp, spec());
     prof_end();
     GM_CUDA(cudaGetLastError());
     return 0;
@@ -555,7 +607,7 @@ struct PlanT final : gmmnlse_plan {
     }
     prof_begin(GMMNLSE_KIND_PAIR_CONV);
     k_pair_conv<T, LOG2N, RAMAN><<<dim3((Q + 1) / 2, planes), NT, smem, stream>>>(A, a_ps, Vout, v_ps, pair_m,
-                                                                                  pair_n, Q, H, tw);
+                                                                                  pair_n, Q, H, tw, spec());
     prof_end();
     GM_CUDA(cudaGetLastError());
     return 0;
@@ -605,6 +657,21 @@ struct PlanT final : gmmnlse_plan {
   }
 
   int launch_mode_reduce(const T* Uin, const C* A, C* Nout, int planes) {
+    if (general) {
+      const size_t smem = sizeof(C) * P * 128;
+      static size_t configured_g = 0;
+      if (smem > configured_g) {
+        GM_CUDA(cudaFuncSetAttribute(k_mode_reduce_gen<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured_g = smem;
+      }
+      const int Gg = P >= 12 ? 4 : (P >= 4 ? 2 : 1);
+      prof_begin(GMMNLSE_KIND_MODE_REDUCE);
+      k_mode_reduce_gen<T><<<dim3((N + 127) / 128, planes), 128 * Gg, smem, stream>>>(Uin, QN, A, PN, Nout, PN, P, Bp,
+                                                                                        N);
+      prof_end();
+      GM_CUDA(cudaGetLastError());
+      return 0;
+    }
     const size_t smem = sizeof(C) * P * 128;
     static size_t configured = 0;
     if (smem > configured) {
@@ -834,9 +901,9 @@ const char* gmmnlse_status_string(int s) {
   return "unknown status";
 }
 
-int gmmnlse_plan_create(gmmnlse_plan** out, int P, int N, int M, double dt, double dz, const double* beta,
-                        int n_beta, const double* S, double f_R, const double* h_R, double omega0, double n2,
-                        const gmmnlse_options* opt) {
+static int create_plan(gmmnlse_plan** out, int P, int N, int M, double dt, double dz, const double* beta,
+                       int n_beta, const double* S, const double* S_R, bool general, bool tensors_complex,
+                       double f_R, const double* h_R, double omega0, double n2, const gmmnlse_options* opt) {
   if (!out) return GMMNLSE_EINVAL;
   *out = nullptr;
   gmmnlse_options o = {0, 1, 1e-6, 0, 0, 0, 0};
@@ -851,10 +918,11 @@ int gmmnlse_plan_create(gmmnlse_plan** out, int P, int N, int M, double dt, doub
   if (!(o.tol > 0)) o.tol = 1e-6;
   for (long long i = 0; i < (long long)P * n_beta; ++i)
     if (!std::isfinite(beta[i])) return GMMNLSE_EINVAL;
-  const long long P4 = (long long)P * P * P * P;
+  if (general && !S_R) return GMMNLSE_EINVAL;
+  const long long P4 = (long long)P * P * P * P * (general && tensors_complex ? 2 : 1);
   double smax = 0;
   for (long long i = 0; i < P4; ++i) {
-    if (!std::isfinite(S[i])) return GMMNLSE_EINVAL;
+    if (!std::isfinite(S[i]) || (general && !std::isfinite(S_R[i]))) return GMMNLSE_EINVAL;
     smax = std::fmax(smax, std::fabs(S[i]));
   }
   if (h_R)
@@ -862,7 +930,7 @@ int gmmnlse_plan_create(gmmnlse_plan** out, int P, int N, int M, double dt, doub
       if (!std::isfinite(h_R[i])) return GMMNLSE_EINVAL;
   if (N < 16 || N > (o.precision ? 8192 : 16384)) return GMMNLSE_EUNSUPPORTED;
   // the packed-pair path needs S symmetric under m<->n and p<->l (Eq. 2 gives all 24 permutations)
-  for (int p = 0; p < P; ++p)
+  for (int p = 0; p < (general ? 0 : P); ++p)
     for (int l = 0; l < P; ++l)
       for (int m = 0; m < P; ++m)
         for (int n = 0; n < P; ++n) {
@@ -881,6 +949,9 @@ int gmmnlse_plan_create(gmmnlse_plan** out, int P, int N, int M, double dt, doub
   pl->fixed_iter = o.fixed_iter > 0 ? o.fixed_iter : 0;
   pl->contraction = o.contraction;
   pl->raman = o.raman;
+  pl->general = general;
+  pl->gen_complex = general && tensors_complex;
+  pl->gen_SR = S_R;
   // Im D_w^(p) = beta0 + beta1 w + sum_{k>=2} beta_k w^k / k!
   pl->phi.assign((size_t)P * N, 0.0);
   for (int p = 0; p < P; ++p)
@@ -894,9 +965,23 @@ int gmmnlse_plan_create(gmmnlse_plan** out, int P, int N, int M, double dt, doub
       pl->phi[(size_t)p * N + k] = acc;
     }
   const int st = pl->init(S, h_R);
+  pl->gen_SR = nullptr;
   if (st < 0) { delete pl; return st; }
   *out = pl;
   return GMMNLSE_OK;
+}
+
+int gmmnlse_plan_create(gmmnlse_plan** out, int P, int N, int M, double dt, double dz, const double* beta,
+                        int n_beta, const double* S, double f_R, const double* h_R, double omega0, double n2,
+                        const gmmnlse_options* opt) {
+  return create_plan(out, P, N, M, dt, dz, beta, n_beta, S, nullptr, false, false, f_R, h_R, omega0, n2, opt);
+}
+
+int gmmnlse_plan_create_general(gmmnlse_plan** out, int P, int N, int M, double dt, double dz, const double* beta,
+                                int n_beta, const double* S_K, const double* S_R, int tensors_complex, double f_R,
+                                const double* h_R, double omega0, double n2, const gmmnlse_options* opt) {
+  return create_plan(out, P, N, M, dt, dz, beta, n_beta, S_K, S_R, true, tensors_complex != 0, f_R, h_R, omega0, n2,
+                     opt);
 }
 
 int gmmnlse_propagate(gmmnlse_plan* plan, const void* A_in, double L, void* A_out, void* stream) {

@@ -43,6 +43,20 @@ k_fft_rows(const cplx<T>* __restrict__ in, long long in_plane_stride, cplx<T>* _
       });
 }
 
+// Per-stream description of the general form of Eq. 1 (S^K != S^R, complex, no symmetry; NEXT-2): stream q is
+// Re (kind 0) or Im (kind 1) of A_m A_n*, weighted wk[q] on its instantaneous part and wr[q] on its Raman-
+// convolved part.  All-null = the scalar-mode path (every stream Re, weights folded into H / cs, omf).
+// The two streams of one CTA (q0 = 2 bx, q0 + 1) always share their weights (blocks are padded to even size).
+template <typename T> struct StreamSpec {
+  const int* kind;
+  const T* wk;
+  const T* wr;
+};
+template <typename C>
+__device__ __forceinline__ auto pair_stream(C a, C b, bool imag) -> decltype(a.x) {
+  return imag ? a.y * b.x - a.x * b.y : a.x * b.x + a.y * b.y;       // Im / Re of a b*
+}
+
 // ------------------------------------------------------------------------------------------
 // a4 + a5: pair products and Raman convolution, two real pair streams per complex FFT.
 //   grid = (ceil(Q/2), n_planes).  CTA (qq, j) handles packed pairs q0 = 2 qq, q1 = q0 + 1:
@@ -53,7 +67,7 @@ template <typename T, int LOG2N, bool HAS_RAMAN>
 __global__ void __launch_bounds__((1 << LOG2N) / 16)
 k_pair_conv(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restrict__ V, long long v_plane_stride,
             const int* __restrict__ pair_m, const int* __restrict__ pair_n, int Q,
-            const cplx<T>* __restrict__ H, const cplx<T>* __restrict__ tw) {
+            const cplx<T>* __restrict__ H, const cplx<T>* __restrict__ tw, StreamSpec<T> gs) {
   constexpr int N = 1 << LOG2N, NT = N / 16;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
@@ -70,24 +84,31 @@ k_pair_conv(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restri
     const cplx<T>* an1 = Aj + (long long)pair_n[has1 ? q1 : q0] * N;
     T* v0 = V + j * v_plane_stride + (long long)q0 * N;
     T* v1 = V + j * v_plane_stride + (long long)q1 * N;
+    const bool im0 = gs.kind && gs.kind[q0], im1 = gs.kind && has1 && gs.kind[q1];
+    const T wk = gs.wk ? gs.wk[q0] : (T)1;
 #pragma unroll 4
     for (int e = 0; e < 16; ++e) {
       const int n = threadIdx.x + e * NT;
       const cplx<T> a = am0[n], b = an0[n], c = am1[n], d = an1[n];
-      const cplx<T> z = mk(a.x * b.x + a.y * b.y, has1 ? c.x * d.x + c.y * d.y : (T)0);
+      const cplx<T> z = mk(pair_stream(a, b, im0), has1 ? pair_stream(c, d, im1) : (T)0);
       if constexpr (HAS_RAMAN) {
         sm[fft_pad(n)] = z;
       } else {
-        v0[n] = z.x;
-        if (has1) v1[n] = z.y;
+        v0[n] = wk * z.x;
+        if (has1) v1[n] = wk * z.y;
       }
     }
   }
   if constexpr (HAS_RAMAN) {
     __syncthreads();
-    // phase 2: Z = F{z} . H   (H = ((1-fR) + fR ht_R)/N), in place in shared memory
+    // phase 2: Z = F{z} . H   (H = ((1-fR) + fR ht_R)/N; general streams: H_q = wk_q/N + wr_q ht_R/N), in place
+    const T wkN = gs.wk ? gs.wk[q0] / (T)N : (T)0, wr = gs.wr ? gs.wr[q0] : (T)0;
     block_fft<T, LOG2N, +1>(sm, tw, [&](int n) { return sm[fft_pad(n)]; },
-                            [&](int k, cplx<T> Z) { sm[fft_pad(k)] = cmul(Z, H[k]); });
+                            [&](int k, cplx<T> Z) {
+                              cplx<T> h = H[k];
+                              if (gs.wk) h = mk(wkN + wr * h.x, wr * h.y);     // H holds ht_R/N in general mode
+                              sm[fft_pad(k)] = cmul(Z, h);
+                            });
     __syncthreads();
     // phase 3: v = F^-1{Z};  V[q0] = Re v, V[q1] = Im v
     T* v0 = V + j * v_plane_stride + (long long)q0 * N;
@@ -114,7 +135,7 @@ template <typename T, int LOG2N>
 __global__ void __launch_bounds__((1 << LOG2N) / 16)
 k_pair_iir(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restrict__ V, long long v_plane_stride,
            const int* __restrict__ pair_m, const int* __restrict__ pair_n, int Q, cplx<T> zeta, cplx<T> cs, T omf,
-           const cplx<T>* __restrict__ zp) {
+           const cplx<T>* __restrict__ zp, StreamSpec<T> gs) {
   constexpr int N = 1 << LOG2N, NT = N / 16, NW = (NT + 31) / 32;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);         // fft_smem_elems(N) + 2 * (NW + 1) complex
@@ -127,12 +148,17 @@ k_pair_iir(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restric
     const cplx<T>* an0 = Aj + (long long)pair_n[q0] * N;
     const cplx<T>* am1 = Aj + (long long)pair_m[has1 ? q1 : q0] * N;
     const cplx<T>* an1 = Aj + (long long)pair_n[has1 ? q1 : q0] * N;
+    const bool im0 = gs.kind && gs.kind[q0], im1 = gs.kind && has1 && gs.kind[q1];
 #pragma unroll 4
     for (int e = 0; e < 16; ++e) {
       const int n = tid + e * NT;
       const cplx<T> a = am0[n], b = an0[n], c = am1[n], d = an1[n];
-      sm[fft_pad(n)] = mk(a.x * b.x + a.y * b.y, has1 ? c.x * d.x + c.y * d.y : (T)0);
+      sm[fft_pad(n)] = mk(pair_stream(a, b, im0), has1 ? pair_stream(c, d, im1) : (T)0);
     }
+  }
+  if (gs.wk) {                                                // general streams: per-stream Kerr / Raman weights
+    omf = gs.wk[q0];
+    cs = cscale(cs, gs.wr[q0]);
   }
   __syncthreads();
   cplx<T> x[16];                                              // x.x: stream q0, x.y: stream q1; samples 16 tid + e
@@ -301,6 +327,42 @@ k_mode_reduce(const T* __restrict__ U, long long u_plane_stride, const cplx<T>* 
       const cplx<T> a = at[l * 128];
       sx += u * a.x;
       sy += u * a.y;
+    }
+    Nt[j * n_plane_stride + (long long)p * N + t] = mk(sx, sy);
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// a7, general form: N_p(t) = sum_l A_l(t) U_pl(t) with complex, unsymmetric U stored as two blocks of real
+// rows: Re U_pl at row p P + l, Im U_pl at row Bp + p P + l.  grid = (N / 128, n_planes), blockDim = 128 G.
+template <typename T>
+__global__ void __launch_bounds__(512)
+k_mode_reduce_gen(const T* __restrict__ U, long long u_plane_stride, const cplx<T>* __restrict__ A,
+                  long long a_plane_stride, cplx<T>* __restrict__ Nt, long long n_plane_stride, int P, int Bp, int N) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx<T>* a_s = reinterpret_cast<cplx<T>*>(smem_raw);        // [P][128]
+  const int tx = threadIdx.x & 127, g = threadIdx.x >> 7, G = blockDim.x >> 7, j = blockIdx.y;
+  const int t0 = blockIdx.x * 128;
+  const cplx<T>* Aj = A + j * a_plane_stride + t0;
+  for (int i = threadIdx.x; i < P * 128; i += blockDim.x) {
+    const int x = i & 127;
+    a_s[i] = t0 + x < N ? Aj[(long long)(i >> 7) * N + x] : mk((T)0, (T)0);
+  }
+  __syncthreads();
+  const int t = t0 + tx;
+  if (t >= N) return;
+  const T* Ur = U + j * u_plane_stride + t;
+  const T* Ui = Ur + (long long)Bp * N;
+  const cplx<T>* at = a_s + tx;
+  for (int p = g; p < P; p += G) {
+    T sx = 0, sy = 0;
+#pragma unroll 4
+    for (int l = 0; l < P; ++l) {
+      const long long r = (long long)(p * P + l) * N;
+      const T ur = Ur[r], ui = Ui[r];
+      const cplx<T> a = at[l * 128];
+      sx += ur * a.x - ui * a.y;
+      sy += ur * a.y + ui * a.x;
     }
     Nt[j * n_plane_stride + (long long)p * N + t] = mk(sx, sy);
   }

@@ -480,3 +480,89 @@ def test_rk4ip_gpu_zero_length_and_bad_length(B):
         assert rel(out.cpu().numpy(), Ad.cpu().numpy()) <= 1e-6
         with pytest.raises(B.GmmnlseError):
             plan.propagate_rk4ip(Ad, 0.5 * w.dz, out)
+
+
+# ------------------------------------- NEXT-2: general form of Eq. 1 (S^K != S^R, complex, no index symmetry)
+def _general_tensors(w, seed, cplx):
+    rng = np.random.default_rng(seed)
+    smax = np.abs(w.S).max()
+    pert = lambda: 0.3 * smax * rng.standard_normal(w.S.shape) + (0.2j * smax * rng.standard_normal(w.S.shape)
+                                                                  if cplx else 0.0)
+    return w.S + pert(), w.S + pert()
+
+
+def _general_plan(B, w, SK, SR, **kw):
+    opts = dict(precision=w.precision, shock=w.shock, tol=w.tol)
+    opts.update(kw)
+    M = opts.pop("M", w.M)
+    return B.Plan(w.P, w.N, M, w.dt, w.dz, w.beta, (SK, SR), w.f_R, w.h_R, w.omega0, w.n2, **opts)
+
+
+@pytest.mark.parametrize("cfg,kw,cplx,raman,kind", [
+    (2, dict(N=1024, max_group=1), False, 0, 0),      # P = 3: 20 streams, CUDA-core contraction, recurrence
+    (2, dict(N=1024), False, 1, 0),                   # P = 6: 72 streams -> tcgen05 contraction, FFT convolution
+    (2, dict(N=1024), True, 2, 0),                    # complex tensors, recurrence
+    (2, dict(N=1024), True, 0, 1),                    # complex tensors on the CUDA-core contraction
+    (3, dict(N=512, max_group=3), True, 0, 0),        # P = 10: 200 streams, one r-tile of 208
+    (1, dict(N=256), False, 0, 0),                    # P = 1, complex128, Kerr only
+])
+def test_general_form_nonlinear_op_vs_oracle(B, cfg, kw, cplx, raman, kind):
+    w = W.make_config(cfg, **kw)
+    SK, SR = _general_tensors(w, 31 + cfg, cplx)
+    dt = np.complex128 if w.precision else np.complex64
+    Ad = dev(w.A0, dt)
+    dA = torch.empty_like(Ad)
+    with _general_plan(B, w, SK, SR, raman=raman, contraction=kind) as plan:
+        plan.nonlinear_op(Ad, dA)
+        torch.cuda.synchronize()
+    A_in = Ad.cpu().numpy().astype(np.complex128)
+    ref = O.nonlinear_op(A_in, (SK, SR), w.kappa, w.omega0, w.f_R, w.h_R, w.dt, w.shock)
+    assert rel(dA.cpu().numpy(), ref) <= (1e-12 if w.precision else TOL_OP)
+
+
+def test_general_form_reduces_to_scalar_mode_path(B):
+    w = W.make_config(2, N=512)
+    Ad = dev(w.A0, np.complex64)
+    d1, d2 = torch.empty_like(Ad), torch.empty_like(Ad)
+    with B.plan_from_workload(w) as plan:
+        plan.nonlinear_op(Ad, d1)
+    with _general_plan(B, w, w.S, w.S) as plan:
+        plan.nonlinear_op(Ad, d2)
+    torch.cuda.synchronize()
+    assert rel(d2.cpu().numpy(), d1.cpu().numpy()) <= 2e-6
+
+
+def test_general_form_mpa_and_rk4ip_vs_oracle(B):
+    w = W.make_config(2, N=512, L=20 * 50e-6, max_group=1)
+    # hermitian tensors (S_plmn = conj S_lpnm) keep the energy bounded; the Raman tensor differs from the Kerr one
+    SK, SR = _general_tensors(w, 77, True)
+    herm = lambda S: 0.5 * (S + np.conj(S.transpose(1, 0, 3, 2)))
+    SK, SR = herm(SK), herm(SR)
+    Ad = dev(w.A0, np.complex64)
+    out, out_rk = torch.empty_like(Ad), torch.empty_like(Ad)
+    with _general_plan(B, w, SK, SR) as plan:
+        st = plan.propagate(Ad, w.L, out)
+        plan.propagate_rk4ip(Ad, w.L, out_rk)
+        torch.cuda.synchronize()
+        stats = plan.stats()
+    assert st == 0
+    A_in = Ad.cpu().numpy().astype(np.complex128)
+    args = (w.beta, (SK, SR), w.kappa, w.omega0, w.f_R, w.h_R, w.dt)
+    ost = {}
+    ref_mpa = O.mpa_propagate(A_in, w.L, w.dz, w.M, *args, shock=w.shock, tol=w.tol, stats=ost)
+    ref_rk = O.rk4ip_propagate(A_in, w.L, w.dz, *args, shock=w.shock)
+    assert rel(out.cpu().numpy(), ref_mpa) <= 1e-4
+    assert rel(out_rk.cpu().numpy(), ref_rk) <= 2e-5
+    assert rel(out.cpu().numpy(), ref_rk) <= TOL_FIELD
+    assert stats["large_steps"] == ost["large_steps"]
+
+
+def test_general_form_rejects_bad_arguments(B):
+    w = W.make_config(2, N=256, max_group=1)
+    with pytest.raises(B.GmmnlseError):
+        B.Plan(w.P, w.N, w.M, w.dt, w.dz, w.beta, (w.S, w.S[:2]), w.f_R, w.h_R, w.omega0, w.n2)
+    bad = w.S.copy()
+    bad[0, 0, 0, 0] = np.nan
+    with pytest.raises(B.GmmnlseError) as e:
+        B.Plan(w.P, w.N, w.M, w.dt, w.dz, w.beta, (w.S, bad), w.f_R, w.h_R, w.omega0, w.n2)
+    assert e.value.status == B.EINVAL
