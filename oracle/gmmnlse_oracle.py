@@ -31,7 +31,7 @@ import numpy as np
 
 __all__ = [
     "dft_direct", "fft_radix2", "to_freq", "to_time", "omega_grid",
-    "dispersion_operator", "raman_transfer", "pair_products",
+    "dispersion_operator", "coupling_term", "raman_transfer", "pair_products",
     "raman_convolve_direct", "raman_convolve", "nonlinear_term",
     "nonlinear_term_literal", "nonlinear_term_general", "nonlinear_term_general_literal",
     "nonlinear_op", "nonlinear_op_freq",
@@ -90,8 +90,11 @@ def omega_grid(N: int, dt: float) -> np.ndarray:
 
 
 # ------------------------------------------------------------------ linear part
-def dispersion_operator(beta: np.ndarray, omega: np.ndarray) -> np.ndarray:
-    """D_w^(p) = i[dbeta0 + dbeta1 w + sum_{k>=2} beta_k w^k / k!].
+def dispersion_operator(beta: np.ndarray, omega: np.ndarray, gain=None) -> np.ndarray:
+    """D_w^(p) = i[dbeta0 + dbeta1 w + sum_{k>=2} beta_k w^k / k!]  [+ g_p].
+
+    ``gain[p]`` (optional, 1/m): the small-signal FIELD gain (loss if negative) of the added term
+    ``g_p A_p`` (section F.2); being linear and diagonal it joins D as its real part.
 
     ``beta[p][k]`` = beta_k^(p) in s^k/m (k=0: dbeta0 [1/m], k=1: dbeta1 [s/m]).
     Follows from Eq. 1's first three terms with d_t -> -i w:
@@ -102,7 +105,16 @@ def dispersion_operator(beta: np.ndarray, omega: np.ndarray) -> np.ndarray:
     D = np.zeros((P, omega.shape[0]), dtype=np.float64)
     for k in range(nb):
         D += beta[:, k:k + 1] * omega[None, :] ** k / math.factorial(k)
+    if gain is not None:
+        return 1j * D + np.asarray(gain, dtype=np.float64).reshape(P, 1)
     return 1j * D
+
+
+def coupling_term(At: np.ndarray, Qc) -> np.ndarray:
+    """C_p = i sum_n Q_np A_n  (section F.1; Eq. 13 defines Q_np): the linear mode-coupling term added
+    to the right-hand side.  ``Qc[n][p]`` = Q_np [1/m], constant over the call and over frequency, so the sum
+    reads the same in the time and the frequency domain."""
+    return 1j * (np.asarray(Qc, dtype=np.complex128).T @ At)
 
 
 # ---------------------------------------------------------------- nonlinear part
@@ -265,15 +277,19 @@ def rk4ip_step(At, h, D, nl):
     return E * (AI + k1 / 6.0 + k2 / 3.0 + k3 / 3.0) + k4 / 6.0
 
 
-def rk4ip_propagate(A0, L, dz, beta, S, kappa, omega0, f_R, h_R, dt, shock=True, n_steps=None):
-    """Propagate A0[p][t] over L with fixed step dz using RK4IP; returns A(L)[p][t]."""
+def rk4ip_propagate(A0, L, dz, beta, S, kappa, omega0, f_R, h_R, dt, shock=True, n_steps=None,
+                    gain=None, coupling=None):
+    """Propagate A0[p][t] over L with fixed step dz using RK4IP; returns A(L)[p][t].
+
+    ``gain`` joins D; ``coupling`` (Q_np) is integrated with the nonlinear term (it does not commute with D)."""
     A0 = np.asarray(A0, dtype=np.complex128)
     N = A0.shape[-1]
     omega = omega_grid(N, dt)
-    D = dispersion_operator(beta, omega)
+    D = dispersion_operator(beta, omega, gain)
     if n_steps is None:
         n_steps = int(round(L / dz))
-    nl = lambda X: nonlinear_op_freq(X, S, kappa, omega, omega0, f_R, h_R, dt, shock)
+    nl0 = lambda X: nonlinear_op_freq(X, S, kappa, omega, omega0, f_R, h_R, dt, shock)
+    nl = nl0 if coupling is None else (lambda X: nl0(X) + coupling_term(X, coupling))
     At = to_freq(A0)
     for _ in range(n_steps):
         At = rk4ip_step(At, dz, D, nl)
@@ -282,7 +298,7 @@ def rk4ip_propagate(A0, L, dz, beta, S, kappa, omega0, f_R, h_R, dt, shock=True,
 
 # --------------------------------------------------------------------- O4: MPA
 def mpa_large_step(psi0, M, dz, D, nl_time, K, tol=1e-6, max_iter=None, fixed_iter=0,
-                   history=None):
+                   history=None, coupling=None):
     """One MPA large step z0 -> z0 + M dz  (Eqs. 11-12).
 
     psi0[p][w] = At(z0).  Planes j = 0..M (reading S10).  ``nl_time(A_t)`` returns
@@ -301,12 +317,14 @@ def mpa_large_step(psi0, M, dz, D, nl_time, K, tol=1e-6, max_iter=None, fixed_it
         max_iter = 2 * M + 4
     psi = np.broadcast_to(psi0, (M + 1, P, N)).copy()
     G = np.zeros((M + 1, P, N), dtype=np.complex128)
-    G[0] = K * to_freq(nl_time(to_time(psi0)))             # depends on psi_0 only (S10)
+    # extra right-hand-side term in the frequency domain (linear coupling), rotated like the nonlinear one
+    extra = (lambda Af: 0.0) if coupling is None else (lambda Af: coupling_term(Af, coupling))
+    G[0] = K * to_freq(nl_time(to_time(psi0))) + extra(psi0)   # depends on psi_0 only (S10)
     n_iter, err, converged = 0, np.inf, False
     while True:
         for j in range(1, M + 1):
-            Aj = to_time(psi[j] * np.exp(D * (j * dz)))
-            G[j] = K * np.exp(-D * (j * dz)) * to_freq(nl_time(Aj))
+            Afj = psi[j] * np.exp(D * (j * dz))
+            G[j] = np.exp(-D * (j * dz)) * (K * to_freq(nl_time(to_time(Afj))) + extra(Afj))
         new = np.empty_like(psi)
         new[0] = psi0
         for j in range(1, M + 1):
@@ -336,12 +354,12 @@ def mpa_large_step(psi0, M, dz, D, nl_time, K, tol=1e-6, max_iter=None, fixed_it
 
 
 def mpa_propagate(A0, L, dz, M, beta, S, kappa, omega0, f_R, h_R, dt, shock=True,
-                  tol=1e-6, max_iter=None, fixed_iter=0, stats=None, history=None):
+                  tol=1e-6, max_iter=None, fixed_iter=0, stats=None, history=None, gain=None, coupling=None):
     """Propagate with MPA; the last large step uses M' = (L/dz) mod M planes."""
     A0 = np.asarray(A0, dtype=np.complex128)
     N = A0.shape[-1]
     omega = omega_grid(N, dt)
-    D = dispersion_operator(beta, omega)
+    D = dispersion_operator(beta, omega, gain)
     K = 1j * kappa * _shock_factor(omega, omega0, shock)
     nl_time = lambda A: nonlinear_term(A, S, f_R, h_R, dt)
     n_small = int(round(L / dz))
@@ -352,7 +370,7 @@ def mpa_propagate(A0, L, dz, M, beta, S, kappa, omega0, f_R, h_R, dt, shock=True
         Mc = min(M, n_small - done)
         hist = [] if history is not None else None
         psi0, it, last_err, conv = mpa_large_step(psi0, Mc, dz, D, nl_time, K, tol,
-                                                   max_iter, fixed_iter, hist)
+                                                   max_iter, fixed_iter, hist, coupling)
         if history is not None:
             history.append(hist)
         tot_it += it

@@ -336,3 +336,48 @@ def test_general_form_conserves_energy_for_a_hermitian_tensor():
     out = O.rk4ip_propagate(A0, 0.02, 0.0005, beta, (S, S), KAPPA, W.OMEGA0, 0.0, None, dt, shock=False)
     assert abs(O.energy(out, dt) / O.energy(A0, dt) - 1) < 1e-8
     assert rel(out, A0) > 1e-3            # the propagation did something
+
+
+# ------------------------------------------------------------ NEXT-3: gain g_p A_p and linear coupling i Q_np A_n
+def test_gain_closed_form_with_dispersion():
+    """g_p A_p is linear and diagonal: the Gaussian of Eq. 9 broadens exactly as without gain and its
+    field grows as exp(g z); a negative g is loss."""
+    N, dt, T0, b2, z = 1024, 4e-15, 60e-15, 2e-26, 0.08
+    t = (np.arange(N) - N // 2) * dt
+    A0 = np.stack([np.exp(-t ** 2 / (2 * T0 ** 2)), 0.5 * np.exp(-t ** 2 / (2 * T0 ** 2))]).astype(complex)
+    g = np.array([3.0, -7.0])
+    beta = np.array([[0, 0, b2], [0, 0, b2]])
+    S0 = np.zeros((2, 2, 2, 2))
+    q = T0 ** 2 - 1j * b2 * z
+    exact = T0 / np.sqrt(q) * np.exp(-t ** 2 / (2 * q))
+    for out in (O.rk4ip_propagate(A0, z, z / 8, beta, S0, KAPPA, W.OMEGA0, 0.0, None, dt, shock=False, gain=g),
+                O.mpa_propagate(A0, z, z / 8, 4, beta, S0, KAPPA, W.OMEGA0, 0.0, None, dt, shock=False, gain=g)):
+        assert rel(out[0], np.exp(g[0] * z) * exact) < 1e-10
+        assert rel(out[1], 0.5 * np.exp(g[1] * z) * exact) < 1e-10
+
+
+def test_linear_coupling_two_mode_coupler_closed_form():
+    """i sum_n Q_np A_n with Q = [[0, k], [k, 0]] and a propagation-constant mismatch D: the
+    textbook directional coupler, P_2(z) = k^2/(k^2 + (D/2)^2) sin^2(sqrt(k^2 + (D/2)^2) z); energy conserved
+    for a hermitian Q; the sign (A_2 leads by +i for D = 0) fixes the 'i' of the term."""
+    N, dt = 64, 5e-15
+    A0 = np.zeros((2, N), complex); A0[0] = 1.0
+    kap, Dm, z = 40.0, 50.0, 0.03
+    Qc = np.array([[0, kap], [kap, 0]], dtype=complex)
+    S0 = np.zeros((2, 2, 2, 2))
+    for Dm_ in (0.0, Dm):
+        beta = np.array([[0.0], [Dm_]])
+        Om = np.hypot(kap, Dm_ / 2)
+        p2 = kap ** 2 / Om ** 2 * np.sin(Om * z) ** 2
+        rk = O.rk4ip_propagate(A0, z, z / 400, beta, S0, KAPPA, W.OMEGA0, 0.0, None, dt, shock=False, coupling=Qc)
+        mp = O.mpa_propagate(A0, z, z / 400, 8, beta, S0, KAPPA, W.OMEGA0, 0.0, None, dt, shock=False, coupling=Qc,
+                             tol=1e-12)
+        for out, tol in ((rk, 1e-9), (mp, 2e-5)):
+            assert abs(np.abs(out[1, 0]) ** 2 - p2) < tol
+            assert abs(np.sum(np.abs(out[:, 0]) ** 2) - 1.0) < tol
+        if Dm_ == 0.0:
+            assert abs(rk[1, 0] - 1j * np.sin(kap * z)) < 1e-9 and abs(rk[0, 0] - np.cos(kap * z)) < 1e-9
+    # index order: Q[n][p] couples n -> p; a one-way (non-hermitian) Q feeds only its target mode
+    Q1 = np.zeros((2, 2), complex); Q1[0, 1] = kap
+    out = O.rk4ip_propagate(A0, z, z / 100, np.zeros((2, 1)), S0, KAPPA, W.OMEGA0, 0.0, None, dt, shock=False, coupling=Q1)
+    assert abs(out[0, 0] - 1.0) < 1e-12 and abs(out[1, 0] - 1j * kap * z) < 1e-9
