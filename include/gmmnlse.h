@@ -109,6 +109,20 @@ int gmmnlse_propagate_host(gmmnlse_plan *plan, const void *A_in_host, double L, 
  * plane per launch.  Arguments, layout and errors as gmmnlse_propagate; fully asynchronous (no read-back).  */
 int gmmnlse_propagate_rk4ip(gmmnlse_plan *plan, const void *A_in, double L, void *A_out, void *stream);
 
+/* Other effects within the GMMNLSE (section F), both integrators:
+ *   set_gain:     small-signal FIELD gain g_p A_p; g: HOST [P] in 1/m (negative = loss), NULL or all
+ *                 zero = none.  Linear and diagonal, so it joins D_w as its real part: the rotation tables
+ *                 exp(+-D_w j dz) get the factors exp(+-g_p j dz).  Frequency-independent gain only; the
+ *                 Taylor-expanded saturation term of section F.2 is not built.
+ *   set_coupling: linear mode coupling C_p = i sum_n Q_np A_n (Eq. 13 for Q_np); Q: HOST [P][P]
+ *                 (re, im) interleaved, entry (n P + p) = Q_np in 1/m, NULL or all zero = none.  Constant over
+ *                 a call and over frequency; a z-dependent Q(z) (disorder, gratings) is propagated in segments
+ *                 with set_coupling between the calls.  Integrated with the nonlinear term (same trapezoid /
+ *                 RK4 stages).  gmmnlse_nonlinear_op does not include it.
+ * Both synchronise the plan's stream, copy their argument, and return EINVAL on non-finite input.               */
+int gmmnlse_set_gain(gmmnlse_plan *plan, const double *g);
+int gmmnlse_set_coupling(gmmnlse_plan *plan, const double *Q);
+
 /* One evaluation of the last term of Eq. 1:
  *   dA_p(t) = i n2 w0/c (1 + i/w0 d_t) sum_lmn S_plmn A_l [(1-fR) A_m A_n* + fR (h_R (*) A_m A_n*)]
  * A, dA: DEVICE [P][N] as above (dA must not alias A); enqueued on the plan's stream.      */

@@ -46,6 +46,8 @@ SIGNATURES = {
     "gmmnlse_propagate_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]),
     "gmmnlse_propagate_rk4ip": (C.c_int, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]),
     "gmmnlse_nonlinear_op": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "gmmnlse_set_gain": (C.c_int, [C.c_void_p, _DP]),
+    "gmmnlse_set_coupling": (C.c_int, [C.c_void_p, _DP]),
     "gmmnlse_set_stream": (C.c_int, [C.c_void_p, C.c_void_p]),
     "gmmnlse_get_stats": (C.c_int, [C.c_void_p, _LLP, _LLP, _DP, _LLP]),
     "gmmnlse_launch_count": (C.c_longlong, [C.c_void_p]),
@@ -159,6 +161,26 @@ class Plan:
 
     def nonlinear_op(self, A, dA) -> int:
         return _check(self._lib, self._lib.gmmnlse_nonlinear_op(self._h, _ptr(A), _ptr(dA)))
+
+    def set_gain(self, g) -> None:
+        """gmmnlse_set_gain: g[P] field gain in 1/m (None clears it)."""
+        if g is None:
+            _check(self._lib, self._lib.gmmnlse_set_gain(self._h, None))
+            return
+        g = np.ascontiguousarray(g, dtype=np.float64)
+        if g.size != self.P:
+            raise GmmnlseError(EINVAL, "gain must hold P entries")
+        _check(self._lib, self._lib.gmmnlse_set_gain(self._h, g.ctypes.data_as(_DP)))
+
+    def set_coupling(self, Q) -> None:
+        """gmmnlse_set_coupling: Q[n][p] = Q_np complex [P][P] in 1/m (None clears it)."""
+        if Q is None:
+            _check(self._lib, self._lib.gmmnlse_set_coupling(self._h, None))
+            return
+        Q = np.ascontiguousarray(Q, dtype=np.complex128)
+        if Q.size != self.P * self.P:
+            raise GmmnlseError(EINVAL, "Q must hold P x P entries")
+        _check(self._lib, self._lib.gmmnlse_set_coupling(self._h, C.cast(Q.ctypes.data, _DP)))
 
     # -- helpers -----------------------------------------------------------------------------------
     def set_stream(self, stream) -> None:

@@ -158,6 +158,8 @@ struct gmmnlse_plan {
   virtual int propagate(const void* A_in, double L, void* A_out) = 0;
   virtual int propagate_host(const void* A_in, double L, void* A_out) = 0;
   virtual int propagate_rk4ip(const void* A_in, double L, void* A_out) = 0;
+  virtual int set_gain(const double* g) = 0;
+  virtual int set_coupling(const double* Qri) = 0;
   virtual int nonlinear_op(const void* A, void* dA) = 0;
   virtual int get_planes(void* out) = 0;
   virtual int debug_fft(const void* in, void* out, int rows, int dir) = 0;
@@ -189,6 +191,10 @@ struct PlanT final : gmmnlse_plan {
   C* d_io = nullptr;
   std::map<int, double2*> EM_ragged;
   long long PN = 0, QN = 0;
+  // NEXT-3: small-signal gain g_p (joins D as its real part) and constant linear coupling Q_np
+  std::vector<double> gain;                // [P], 1/m; empty = none
+  T *gfwd = nullptr, *ginv = nullptr;      // [(M+1)][P]: exp(+g_p j dz), exp(-g_p j dz)
+  C* Qc = nullptr;                         // [P][P], Qc[n P + p] = Q_np
   int Bp = 0;                              // general mode: rows per Re / Im block of U, streams per Kerr / Raman block
   int* st_kind = nullptr;
   T *st_wk = nullptr, *st_wr = nullptr;
@@ -212,7 +218,7 @@ struct PlanT final : gmmnlse_plan {
     cudaFree(pair_m); cudaFree(pair_n); cudaFree(psi0_d); cudaFree(psi); cudaFree(At); cudaFree(G);
     cudaFree(V); cudaFree(U); cudaFree(errbuf); cudaFree(d_err); cudaFree(d_io);
     cudaFree(S2hi); cudaFree(S2lo);
-    cudaFree(st_kind); cudaFree(st_wk); cudaFree(st_wr); cudaFree(iir_zp); cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
+    cudaFree(gfwd); cudaFree(ginv); cudaFree(Qc); cudaFree(st_kind); cudaFree(st_wk); cudaFree(st_wr); cudaFree(iir_zp); cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
     if (h_err) cudaFreeHost(h_err);
     if (h_in) cudaFreeHost(h_in);
     if (h_out) cudaFreeHost(h_out);
@@ -234,7 +240,8 @@ struct PlanT final : gmmnlse_plan {
     std::vector<double2> em((size_t)PN);
     for (long long i = 0; i < PN; ++i) {
       const double ph = std::remainder(phi[i] * (Mc * dz), 2.0 * M_PI);
-      em[i] = make_double2(std::cos(ph), std::sin(ph));
+      const double mag = gain.empty() ? 1.0 : std::exp(gain[(size_t)(i / N)] * (Mc * dz));
+      em[i] = make_double2(mag * std::cos(ph), mag * std::sin(ph));
     }
     GM_TRY(dalloc(out, (size_t)PN));
     return upload(*out, em);
@@ -413,12 +420,20 @@ struct PlanT final : gmmnlse_plan {
     const size_t smem = sizeof(C) * (fft_smem_elems(1 << LOG2N) + 2 * NW + 2);
     static bool configured = false;
     if (!configured) {
-      GM_CUDA(cudaFuncSetAttribute(k_pair_iir<T, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      GM_CUDA(cudaFuncSetAttribute(k_pair_iir<T, LOG2N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)smem));
+      GM_CUDA(cudaFuncSetAttribute(k_pair_iir<T, LOG2N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)smem));
       configured = true;
     }
     prof_begin(GMMNLSE_KIND_PAIR_CONV);
-    k_pair_iir<T, LOG2N><<<dim3((Q + 1) / 2, planes), NT, smem, stream>>>(A, a_ps, Vout, v_ps, pair_m, pair_n, Q,
-                                                                          iir_zeta, iir_cs, iir_omf, iir_zp, spec());
+    const dim3 grid((Q + 1) / 2, planes);
+    if (general)
+      k_pair_iir<T, LOG2N, true><<<grid, NT, smem, stream>>>(A, a_ps, Vout, v_ps, pair_m, pair_n, Q, iir_zeta, iir_cs,
+                                                             iir_omf, iir_zp, spec());
+    else
+      k_pair_iir<T, LOG2N, false><<<grid, NT, smem, stream>>>(A, a_ps, Vout, v_ps, pair_m, pair_n, Q, iir_zeta,
+                                                              iir_cs, iir_omf, iir_zp, spec());
     prof_end();
     GM_CUDA(cudaGetLastError());
     return 0;
@@ -555,7 +570,7 @@ struct PlanT final : gmmnlse_plan {
   // ------------------------------------------------------------------ kernel launchers
   template <int LOG2N, int DIR>
   int launch_fft_t(const C* in, long long in_ps, C* out, long long out_ps, const C* pre, const C* post_vec,
-                   const C* post_tab, long long tab_ps, T scale, int rows, int planes) {
+                   const C* post_tab, long long tab_ps, T scale, int rows, int planes, const T* rscale) {
     constexpr int NT = (1 << LOG2N) / 16;
     const size_t smem = sizeof(C) * fft_smem_elems(1 << LOG2N);
     static bool configured = false;
@@ -566,28 +581,28 @@ struct PlanT final : gmmnlse_plan {
     }
     prof_begin(DIR > 0 ? GMMNLSE_KIND_FFT_TO_FREQ : GMMNLSE_KIND_FFT_TO_TIME);
     k_fft_rows<T, LOG2N, DIR><<<dim3(rows, planes), NT, smem, stream>>>(in, in_ps, out, out_ps, pre, post_vec,
-                                                                         post_tab, tab_ps, scale, tw);
+                                                                         post_tab, tab_ps, scale, tw, rscale);
     prof_end();
     GM_CUDA(cudaGetLastError());
     return 0;
   }
   int launch_fft(int dir, const C* in, long long in_ps, C* out, long long out_ps, const C* pre, const C* post_vec,
-                 const C* post_tab, long long tab_ps, T scale, int rows, int planes) {
+                 const C* post_tab, long long tab_ps, T scale, int rows, int planes, const T* rscale = nullptr) {
 #define GM_FFT_CASE(L)                                                                                       \
   case L:                                                                                                    \
     return dir > 0 ? launch_fft_t<L, +1>(in, in_ps, out, out_ps, pre, post_vec, post_tab, tab_ps, scale, rows, \
-                                         planes)                                                             \
+                                         planes, rscale)                                                     \
                    : launch_fft_t<L, -1>(in, in_ps, out, out_ps, pre, post_vec, post_tab, tab_ps, scale, rows, \
-                                         planes);
+                                         planes, rscale);
     switch (log2N) {
       GM_FFT_CASE(4) GM_FFT_CASE(5) GM_FFT_CASE(6) GM_FFT_CASE(7) GM_FFT_CASE(8) GM_FFT_CASE(9)
       GM_FFT_CASE(10) GM_FFT_CASE(11) GM_FFT_CASE(12) GM_FFT_CASE(13)
       case 14:
         if constexpr (sizeof(T) == 4) {
           return dir > 0 ? launch_fft_t<14, +1>(in, in_ps, out, out_ps, pre, post_vec, post_tab, tab_ps, scale,
-                                                rows, planes)
+                                                rows, planes, rscale)
                          : launch_fft_t<14, -1>(in, in_ps, out, out_ps, pre, post_vec, post_tab, tab_ps, scale,
-                                                rows, planes);
+                                                rows, planes, rscale);
         }
         return GMMNLSE_EUNSUPPORTED;
     }
@@ -724,10 +739,14 @@ struct PlanT final : gmmnlse_plan {
       const int j0 = it == 0 ? 0 : 1, np = Mc + 1 - j0;
       // a3: A_j(t) = F^-1{psi_j exp(+D j dz)}; first iterate psi_j = psi_0
       GM_TRY(launch_fft(-1, it == 0 ? psi : psi + j0 * PN, it == 0 ? 0 : PN, At + j0 * PN, PN, E + j0 * PN, nullptr,
-                        nullptr, PN, (T)(1.0 / N), P, np));
+                        nullptr, PN, (T)(1.0 / N), P, np, gfwd ? gfwd + j0 * P : nullptr));
       GM_TRY(nonlinear_term(j0, np));                                        // a4-a7
       // a8: G_j = K(w) exp(-D j dz) F{N_p}
-      GM_TRY(launch_fft(+1, G + j0 * PN, PN, G + j0 * PN, PN, nullptr, Kw, E + j0 * PN, PN, (T)1, P, np));
+      GM_TRY(launch_fft(+1, G + j0 * PN, PN, G + j0 * PN, PN, nullptr, Kw, E + j0 * PN, PN, (T)1, P, np,
+                        ginv ? ginv + j0 * P : nullptr));
+      if (Qc)                                                                 // + exp(-D j dz) i Q^T (psi_j exp(D j dz))
+        GM_TRY(launch_couple(it == 0 ? psi : psi + j0 * PN, it == 0 ? 0 : PN, E + j0 * PN,
+                             gfwd ? gfwd + j0 * P : nullptr, ginv ? ginv + j0 * P : nullptr, G + j0 * PN, np));
       // a9 + a10
       prof_begin(GMMNLSE_KIND_SCAN);
       k_trapz_scan<T><<<sblocks, 256, sizeof(double) * 2 * (Mc + 1), stream>>>(psi, G, psi, PN, Mc, (T)dz,
@@ -806,7 +825,66 @@ struct PlanT final : gmmnlse_plan {
     GM_TRY(launch_fft(-1, Xf, 0, At, 0, nullptr, nullptr, nullptr, 0, (T)(1.0 / N), P, 1));
     GM_TRY(nonlinear_term(0, 1));
     GM_TRY(launch_fft(+1, G, 0, G, 0, nullptr, Kw, nullptr, 0, (T)1, P, 1));
+    if (Qc) GM_TRY(launch_couple(Xf, 0, nullptr, nullptr, nullptr, G, 1));
     return 0;
+  }
+
+  int launch_couple(const C* src, long long src_ps, const C* Etab, const T* gf, const T* gi, C* Gout, int planes) {
+    const size_t smem = sizeof(C) * P * 64;
+    static size_t configured = 0;
+    if (smem > configured) {
+      GM_CUDA(cudaFuncSetAttribute(k_couple<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      configured = smem;
+    }
+    prof_begin(GMMNLSE_KIND_MISC);
+    k_couple<T><<<dim3((N + 63) / 64, planes), 256, smem, stream>>>(src, src_ps, Etab, gf, gi, Qc, Gout, PN, P, N);
+    prof_end();
+    GM_CUDA(cudaGetLastError());
+    return 0;
+  }
+
+  int set_gain(const double* g) override {
+    GM_CUDA(cudaStreamSynchronize(stream));
+    bool any = false;
+    if (g)
+      for (int p = 0; p < P; ++p) {
+        if (!std::isfinite(g[p])) return GMMNLSE_EINVAL;
+        any = any || g[p] != 0.0;
+      }
+    cudaFree(gfwd); cudaFree(ginv); cudaFree(EM_d); cudaFree(EH_d);
+    gfwd = ginv = nullptr; EM_d = nullptr; EH_d = nullptr;
+    for (auto& kv : EM_ragged) cudaFree(kv.second);
+    EM_ragged.clear();
+    gain.clear();
+    if (any) {
+      gain.assign(g, g + P);
+      std::vector<T> f((size_t)(M + 1) * P), b((size_t)(M + 1) * P);
+      for (int jn = 0; jn <= M; ++jn)
+        for (int p = 0; p < P; ++p) {
+          f[(size_t)jn * P + p] = (T)std::exp(gain[p] * (jn * dz));
+          b[(size_t)jn * P + p] = (T)std::exp(-gain[p] * (jn * dz));
+        }
+      GM_TRY(dalloc(&gfwd, f.size())); GM_TRY(upload(gfwd, f));
+      GM_TRY(dalloc(&ginv, b.size())); GM_TRY(upload(ginv, b));
+    }
+    return make_EM(M, &EM_d);
+  }
+
+  int set_coupling(const double* Qri) override {
+    GM_CUDA(cudaStreamSynchronize(stream));
+    cudaFree(Qc);
+    Qc = nullptr;
+    if (!Qri) return 0;
+    std::vector<C> q((size_t)P * P);
+    bool any = false;
+    for (size_t i = 0; i < q.size(); ++i) {
+      if (!std::isfinite(Qri[2 * i]) || !std::isfinite(Qri[2 * i + 1])) return GMMNLSE_EINVAL;
+      q[i] = mk((T)Qri[2 * i], (T)Qri[2 * i + 1]);
+      any = any || Qri[2 * i] != 0.0 || Qri[2 * i + 1] != 0.0;
+    }
+    if (!any) return 0;
+    GM_TRY(dalloc(&Qc, q.size()));
+    return upload(Qc, q);
   }
 
   int propagate_rk4ip(const void* A_in, double L, void* A_out) override {
@@ -816,10 +894,13 @@ struct PlanT final : gmmnlse_plan {
     if (!rk_X) {
       GM_TRY(dalloc(&rk_X, (size_t)PN)); GM_TRY(dalloc(&rk_AI, (size_t)PN)); GM_TRY(dalloc(&rk_K1, (size_t)PN));
       GM_TRY(dalloc(&rk_K2, (size_t)PN)); GM_TRY(dalloc(&rk_K3, (size_t)PN));
+    }
+    if (!EH_d) {
       std::vector<double2> eh((size_t)PN);
       for (long long i = 0; i < PN; ++i) {
         const double ph = std::remainder(phi[i] * (0.5 * dz), 2.0 * M_PI);
-        eh[i] = make_double2(std::cos(ph), std::sin(ph));
+        const double mag = gain.empty() ? 1.0 : std::exp(gain[(size_t)(i / N)] * (0.5 * dz));
+        eh[i] = make_double2(mag * std::cos(ph), mag * std::sin(ph));
       }
       GM_TRY(dalloc(&EH_d, (size_t)PN));
       GM_TRY(upload(EH_d, eh));
@@ -1001,6 +1082,12 @@ int gmmnlse_propagate_rk4ip(gmmnlse_plan* plan, const void* A_in, double L, void
   if (!plan || !A_in || !A_out) return GMMNLSE_EINVAL;
   if (stream) plan->stream = (cudaStream_t)stream;
   return plan->propagate_rk4ip(A_in, L, A_out);
+}
+
+int gmmnlse_set_gain(gmmnlse_plan* plan, const double* g) { return plan ? plan->set_gain(g) : GMMNLSE_EINVAL; }
+
+int gmmnlse_set_coupling(gmmnlse_plan* plan, const double* Q) {
+  return plan ? plan->set_coupling(Q) : GMMNLSE_EINVAL;
 }
 
 int gmmnlse_nonlinear_op(gmmnlse_plan* plan, const void* A, void* dA) {

@@ -18,7 +18,7 @@ __global__ void __launch_bounds__((1 << LOG2N) / 16, ((1 << LOG2N) / 16 == 512 &
 k_fft_rows(const cplx<T>* __restrict__ in, long long in_plane_stride, cplx<T>* __restrict__ out,
            long long out_plane_stride, const cplx<T>* __restrict__ pre, const cplx<T>* __restrict__ post_vec,
            const cplx<T>* __restrict__ post_tab, long long tab_plane_stride, T scale,
-           const cplx<T>* __restrict__ tw) {
+           const cplx<T>* __restrict__ tw, const T* __restrict__ row_scale) {
   constexpr int N = 1 << LOG2N;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
@@ -28,6 +28,7 @@ k_fft_rows(const cplx<T>* __restrict__ in, long long in_plane_stride, cplx<T>* _
   const long long toff = j * tab_plane_stride + (long long)p * N;
   const cplx<T>* pre_r = pre ? pre + toff : nullptr;
   const cplx<T>* post_r = post_tab ? post_tab + toff : nullptr;
+  if (row_scale) scale *= row_scale[j * gridDim.x + p];     // gain: exp(+-g_p j dz), one factor per (plane, mode)
   block_fft<T, LOG2N, DIR>(
       sm, tw,
       [&](int n) {
@@ -131,7 +132,7 @@ k_pair_conv(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restri
 // zp[m] = zeta^(16 m)), warp totals through shared memory, and the periodic wrap w[-1] = w[N-1] closes the
 // circle.  No FFT: the kernel is one read of the field rows and one write of V.
 //   cs = c dt f_R,  omf = 1 - f_R;  V = omf x + Im(cs w).
-template <typename T, int LOG2N>
+template <typename T, int LOG2N, bool GEN>
 __global__ void __launch_bounds__((1 << LOG2N) / 16)
 k_pair_iir(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restrict__ V, long long v_plane_stride,
            const int* __restrict__ pair_m, const int* __restrict__ pair_n, int Q, cplx<T> zeta, cplx<T> cs, T omf,
@@ -148,7 +149,7 @@ k_pair_iir(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restric
     const cplx<T>* an0 = Aj + (long long)pair_n[q0] * N;
     const cplx<T>* am1 = Aj + (long long)pair_m[has1 ? q1 : q0] * N;
     const cplx<T>* an1 = Aj + (long long)pair_n[has1 ? q1 : q0] * N;
-    const bool im0 = gs.kind && gs.kind[q0], im1 = gs.kind && has1 && gs.kind[q1];
+    const bool im0 = GEN && gs.kind[q0], im1 = GEN && has1 && gs.kind[q1];
 #pragma unroll 4
     for (int e = 0; e < 16; ++e) {
       const int n = tid + e * NT;
@@ -156,7 +157,7 @@ k_pair_iir(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restric
       sm[fft_pad(n)] = mk(pair_stream(a, b, im0), has1 ? pair_stream(c, d, im1) : (T)0);
     }
   }
-  if (gs.wk) {                                                // general streams: per-stream Kerr / Raman weights
+  if constexpr (GEN) {                                        // general streams: per-stream Kerr / Raman weights
     omf = gs.wk[q0];
     cs = cscale(cs, gs.wr[q0]);
   }
@@ -504,6 +505,49 @@ k_rk4_stage(int stage, double2* __restrict__ At_d, cplx<T>* __restrict__ At, con
     const double2 r = make_double2(sx * e.x - sy * e.y + gx / 6.0, sx * e.y + sy * e.x + gy / 6.0);
     At_d[i] = r;
     At[i] = mk((T)r.x, (T)r.y);
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// Linear mode coupling (section F.1): G_j[p] += R-_j[p] i sum_n Q_np (R+_j[n] src_j[n])
+// per frequency, where R+-_j = exp(+-D_w j dz) = E^(+-1) x gain factor rotates between the interaction picture of
+// plane j and the field (tables null: no rotation, the RK4IP stages).  Q[n][p] constant over the call.
+//   grid = (N / 64, n_planes), block = 256: 64 frequencies x 4 mode groups; the rotated field tile sits in smem.
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_couple(const cplx<T>* __restrict__ src, long long src_plane_stride, const cplx<T>* __restrict__ E,
+         const T* __restrict__ gfwd, const T* __restrict__ ginv, const cplx<T>* __restrict__ Qc,
+         cplx<T>* __restrict__ G, long long plane_stride, int P, int N) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx<T>* a_s = reinterpret_cast<cplx<T>*>(smem_raw);        // [P][64]
+  const int x = threadIdx.x & 63, g = threadIdx.x >> 6, j = blockIdx.y;
+  const int w0 = blockIdx.x * 64, w = w0 + x;
+  const cplx<T>* sj = src + j * src_plane_stride;
+  const cplx<T>* Ej = E ? E + j * plane_stride : nullptr;
+  for (int i = threadIdx.x; i < P * 64; i += blockDim.x) {
+    const int n = i >> 6, xx = i & 63;
+    cplx<T> a = mk((T)0, (T)0);
+    if (w0 + xx < N) {
+      a = sj[(long long)n * N + w0 + xx];
+      if (Ej) a = cmul(a, Ej[(long long)n * N + w0 + xx]);
+      if (gfwd) a = cscale(a, gfwd[j * P + n]);
+    }
+    a_s[i] = a;
+  }
+  __syncthreads();
+  if (w >= N) return;
+  for (int p = g; p < P; p += 4) {
+    T sx = 0, sy = 0;
+    for (int n = 0; n < P; ++n) {
+      const cplx<T> q = Qc[n * P + p], a = a_s[n * 64 + x];
+      sx += q.x * a.x - q.y * a.y;
+      sy += q.x * a.y + q.y * a.x;
+    }
+    cplx<T> c = mk(-sy, sx);                                    // times i
+    if (Ej) c = cmulc(c, Ej[(long long)p * N + w]);
+    if (ginv) c = cscale(c, ginv[j * P + p]);
+    cplx<T>* out = G + j * plane_stride + (long long)p * N + w;
+    *out = cadd(*out, c);
   }
 }
 

@@ -566,3 +566,89 @@ def test_general_form_rejects_bad_arguments(B):
     with pytest.raises(B.GmmnlseError) as e:
         B.Plan(w.P, w.N, w.M, w.dt, w.dz, w.beta, (w.S, bad), w.f_R, w.h_R, w.omega0, w.n2)
     assert e.value.status == B.EINVAL
+
+
+# ------------------------------------------------ NEXT-3: gain g_p A_p and linear coupling i sum_n Q_np A_n
+def test_gain_and_coupling_closed_forms_on_gpu(B):
+    """Amplified Gaussian (PAPER.md:299 with Eq. 9) and the two-mode directional coupler, no
+    nonlinearity, both GPU integrators, complex64 and complex128."""
+    N, dt, T0, b2 = 1024, 4e-15, 60e-15, 2e-26
+    t = (np.arange(N) - N // 2) * dt
+    A0 = np.stack([np.exp(-t ** 2 / (2 * T0 ** 2)), 0.5 * np.exp(-t ** 2 / (2 * T0 ** 2))]).astype(np.complex128)
+    S0 = np.zeros((2, 2, 2, 2))
+    for precision, tol in ((0, 5e-6), (1, 1e-10)):
+        cdt = np.complex128 if precision else np.complex64
+        # gain with dispersion: exact
+        z, dz, g = 0.08, 0.01, np.array([3.0, -7.0])
+        beta = np.array([[0, 0, b2], [0, 0, b2]])
+        q = T0 ** 2 - 1j * b2 * z
+        exact = T0 / np.sqrt(q) * np.exp(-t ** 2 / (2 * q))
+        with B.Plan(2, N, 4, dt, dz, beta, S0, 0.0, None, W.OMEGA0, W.N2, precision=precision, shock=False) as plan:
+            plan.set_gain(g)
+            for fn in (plan.propagate, plan.propagate_rk4ip):
+                Ad = dev(A0, cdt); out = torch.empty_like(Ad)
+                fn(Ad, z, out); torch.cuda.synchronize()
+                o = out.cpu().numpy()
+                assert rel(o[0], np.exp(g[0] * z) * exact) <= tol
+                assert rel(o[1], 0.5 * np.exp(g[1] * z) * exact) <= tol
+            plan.set_gain(None)                      # cleared: plain dispersion again
+            Ad = dev(A0, cdt); out = torch.empty_like(Ad)
+            plan.propagate(Ad, z, out); torch.cuda.synchronize()
+            assert rel(out.cpu().numpy()[0], exact) <= tol
+        # coupler with mismatch: P_2(z) = k^2/Om^2 sin^2(Om z), Om^2 = k^2 + (D/2)^2
+        kap, Dm, z, nst = 40.0, 50.0, 0.03, 240
+        Qc = np.array([[0, kap], [kap, 0]], dtype=complex)
+        Ac = np.zeros((2, N), np.complex128); Ac[0] = 1.0
+        Om = np.hypot(kap, Dm / 2)
+        p2 = kap ** 2 / Om ** 2 * np.sin(Om * z) ** 2
+        with B.Plan(2, N, 8, dt, z / nst, np.array([[0.0], [Dm]]), S0, 0.0, None, W.OMEGA0, W.N2, precision=precision,
+                    shock=False, tol=1e-9) as plan:
+            plan.set_coupling(Qc)
+            for fn, tl in ((plan.propagate_rk4ip, max(tol, 1e-8)), (plan.propagate, 5e-5)):
+                Ad = dev(Ac, cdt); out = torch.empty_like(Ad)
+                fn(Ad, z, out); torch.cuda.synchronize()
+                o = out.cpu().numpy().astype(np.complex128)
+                assert abs(np.abs(o[1, 7]) ** 2 - p2) <= tl
+                assert abs(np.sum(np.abs(o[:, 7]) ** 2) - 1.0) <= tl
+
+
+@pytest.mark.parametrize("general", [False, True])
+def test_gain_and_coupling_with_nonlinearity_vs_oracle(B, general):
+    w = W.make_config(2, N=512, L=20 * 50e-6)
+    rng = np.random.default_rng(9)
+    g = rng.uniform(-20.0, 20.0, w.P)
+    Q0 = rng.standard_normal((w.P, w.P)) + 1j * rng.standard_normal((w.P, w.P))
+    Qc = 60.0 * (Q0 + Q0.conj().T)                   # hermitian, a few 1e2 /m (stronger coupling only raises the
+                                                     # MPA's own O(dz^2) distance from RK4IP, oracle and GPU alike)
+    S = w.S
+    if general:
+        SK, SR = _general_tensors(w, 5, True)
+        herm = lambda X: 0.5 * (X + np.conj(X.transpose(1, 0, 3, 2)))
+        S = (herm(SK), herm(SR))
+    Ad = dev(w.A0, np.complex64)
+    out, out_rk = torch.empty_like(Ad), torch.empty_like(Ad)
+    with B.Plan(w.P, w.N, w.M, w.dt, w.dz, w.beta, S, w.f_R, w.h_R, w.omega0, w.n2, tol=w.tol) as plan:
+        plan.set_gain(g)
+        plan.set_coupling(Qc)
+        plan.propagate(Ad, w.L, out)
+        plan.propagate_rk4ip(Ad, w.L, out_rk)
+        torch.cuda.synchronize()
+    A_in = Ad.cpu().numpy().astype(np.complex128)
+    args = (w.beta, S, w.kappa, w.omega0, w.f_R, w.h_R, w.dt)
+    ref_rk = O.rk4ip_propagate(A_in, w.L, w.dz, *args, shock=w.shock, gain=g, coupling=Qc)
+    ref_mpa = O.mpa_propagate(A_in, w.L, w.dz, w.M, *args, shock=w.shock, tol=w.tol, gain=g, coupling=Qc)
+    assert rel(out_rk.cpu().numpy(), ref_rk) <= 2e-5
+    assert rel(out.cpu().numpy(), ref_mpa) <= 1e-4
+    assert rel(out.cpu().numpy(), ref_rk) <= TOL_FIELD
+
+
+def test_gain_coupling_reject_bad_input(B):
+    w = W.make_config(2, N=256, max_group=1)
+    with B.plan_from_workload(w) as plan:
+        with pytest.raises(B.GmmnlseError):
+            plan.set_gain(np.array([1.0, np.nan, 0.0]))
+        with pytest.raises(B.GmmnlseError):
+            plan.set_gain(np.zeros(w.P + 1))
+        bad = np.zeros((w.P, w.P), complex); bad[0, 1] = np.inf
+        with pytest.raises(B.GmmnlseError):
+            plan.set_coupling(bad)
