@@ -150,7 +150,7 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def measure(cfg, K, Wm, with_events, host_path=False, seed_offset=0):
+    def measure(cfg, K, Wm, with_events, host_path=False, seed_offset=0, contraction=None):
         w = workloads.make_config(cfg)
         n_large = LARGE_PER_STEP[cfg]
         L_step = n_large * w.M * w.dz
@@ -158,7 +158,8 @@ def run_gpu(args):
         tdt = torch.complex128 if w.precision else torch.complex64
         A0 = w.A0.astype(cdt)
         A0 = replica_launch_field(A0, seed_offset, workloads.SEED_BASE)
-        plan = binding.plan_from_workload(w)
+        plan = binding.plan_from_workload(w, contraction=args.contraction if contraction is None else contraction)
+        ckind, crank = plan.contraction_kind(), plan.lowrank_rank()
         stream = torch.cuda.current_stream()
         A = torch.from_numpy(A0).cuda()
         h_a, h_b = A0.copy(), np.empty_like(A0)
@@ -201,7 +202,7 @@ def run_gpu(args):
         ls = s1["large_steps"] - s0["large_steps"]
         return dict(w=w, ms=ms, wall_ms=wall_ms, z_steps=K * n_large * w.M, iters=it, large=ls, prof=prof,
                     launches=l1 - l0, not_conv=s1["not_converged"] - s0["not_converged"], finite=finite,
-                    bytes_io=int(A0.nbytes))
+                    bytes_io=int(A0.nbytes), ckind=ckind, crank=crank)
 
     cfg, K, Wm = args.config, args.steps, max(args.warmup, 3)
     peaks = _peaks()
@@ -254,6 +255,8 @@ def run_gpu(args):
         roof = dict(bound="hbm", kernel=dom, achieved=round(ach, 1), peak=peaks["hbm"], unit="GB/s",
                     frac=round(ach / peaks["hbm"], 4), traffic=traffic,
                     note=f"algorithmic bytes / event-timed duration; peak = {peaks['source']} copy bandwidth")
+    if main["ckind"] == 6:
+        roof["note"] += "; low-rank form selected: flop rates are dense-equivalent, not executed"
     roof["avg_launch_ms"] = round(dom_ms / dom_n, 4)
     roof["kernels"] = shares
 
@@ -277,6 +280,18 @@ def run_gpu(args):
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = oracle_sample(cfg, 1, 0)
+    out["config"]["contraction_kind"] = main["ckind"]
+    if rank == 0 and world == 1 and args.contraction == 0 and cfg >= 3 and not args.no_variants:
+        # SURVEY.md 8(f) NEXT-4, reported beside the headline, never as it: the same propagation with the exact
+        # low-rank form of the contraction (BASELINE.json names the dense one, which `value` measures)
+        try:
+            lr = measure(cfg, K, Wm, with_events=False, contraction=6)
+            out["variants"] = {"lowrank_contraction": {
+                "value": round(lr["z_steps"] / (lr["ms"] * 1e-3), 2), "unit": UNIT, "rank": lr["crank"],
+                "Q": w.P * (w.P + 1) // 2, "ms_per_step": round(lr["ms"] / K, 4),
+                "iterations_per_large_step": round(lr["iters"] / max(lr["large"], 1), 3)}}
+        except binding.GmmnlseError as exc:
+            out["variants"] = {"lowrank_contraction": {"unavailable": str(exc)}}
     if rank == 0 and args.all_configs and world == 1:
         others = []
         for c in (1, 2, 3, 4):
@@ -415,6 +430,9 @@ def main():
     ap.add_argument("--impl", default="graft", choices=["graft", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--all-configs", action="store_true", help="also time configs 1-4 briefly (other_workloads)")
+    ap.add_argument("--contraction", type=int, default=0,
+                    help="options.contraction for every measurement (0 auto = the dense tcgen05 form; 6 low-rank)")
+    ap.add_argument("--no-variants", action="store_true", help="skip the low-rank variant measurement")
     ap.add_argument("--sweep-M", action="store_true", help="serial RK4IP vs MPA(M) on a 10-mode GRIN (Fig. 3 shape)")
     args = ap.parse_args()
     if args.sweep_M:

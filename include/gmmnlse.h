@@ -45,7 +45,12 @@ typedef struct {                /* pass NULL for defaults                       
                                    1 = CUDA-core fp32/fp64 GEMM; tcgen05 3xTF32 forms: 2 = CTA pairs
                                    (cta_group::2), 3 = single CTA, both operands in shared memory, 4 = single
                                    CTA, V_hi/V_lo operand in tensor memory, 5 = form 3 on clusters of two CTAs
-                                   that TMA-multicast the S tiles to each other.  2-5 need complex64 and
+                                   that TMA-multicast the S tiles to each other; 6 = exact low-rank form
+                                   (SURVEY.md 8(f) NEXT-4): S_(pl),(mn) = sum_k L_(pl),k L_(mn),k by pivoted
+                                   Cholesky at plan time (Eq. 2 makes S a Gram matrix; rank 153 of 1035 for 45
+                                   Hermite-Gauss modes), two tcgen05 GEMMs Q x R and R x Q instead of Q x Q;
+                                   EUNSUPPORTED if S is not positive semi-definite.  Never chosen by auto:
+                                   BASELINE.json names the dense contraction.  2-6 need complex64 and
                                    N % 128 == 0 (2, 5: N % 256 == 0), else EUNSUPPORTED.  Forms 2, 4, 5 are
                                    kept for measurement: none beats form 3 on B200   */
   int    raman;                 /* a5 kernel: 0 = auto, 1 = FFT . h~_R . IFFT on the pair streams (any h_R),
@@ -168,9 +173,11 @@ int gmmnlse_debug_pairs(gmmnlse_plan *plan, const void *A, void *V, int n_planes
  *          [n_planes][Q][N] real of the plan's precision, U must not alias V.
  *   contraction_kind: which a6 kernel the plan selected: 1 CUDA cores, 2 tcgen05 single CTA (operands in
  *          shared memory), 3 tcgen05 CTA pairs, 4 tcgen05 single CTA with the V operand in tensor memory,
- *          5 tcgen05 multicast pairs.                                                            */
+ *          5 tcgen05 multicast pairs, 6 low-rank pair of tcgen05 GEMMs.                                                            */
 int gmmnlse_debug_contract(gmmnlse_plan *plan, const void *V, void *U, int n_planes);
 int gmmnlse_contraction_kind(const gmmnlse_plan *plan);
+/*   lowrank_rank: rank R of the factorisation when contraction_kind is 6, else 0.                 */
+int gmmnlse_lowrank_rank(const gmmnlse_plan *plan);
 /*   raman_kind: which a5 kernel the plan selected: 0 none (f_R = 0), 1 FFT, 2 recursive.          */
 int gmmnlse_raman_kind(const gmmnlse_plan *plan);
 /*   set_tc_chunk: k-blocks (16 packed pairs each) a tensor-memory accumulator holds before the epilogue

@@ -59,6 +59,7 @@ SIGNATURES = {
     "gmmnlse_debug_contract": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
     "gmmnlse_contraction_kind": (C.c_int, [C.c_void_p]),
     "gmmnlse_raman_kind": (C.c_int, [C.c_void_p]),
+    "gmmnlse_lowrank_rank": (C.c_int, [C.c_void_p]),
     "gmmnlse_debug_set_tc_chunk": (C.c_int, [C.c_void_p, C.c_int]),
     "gmmnlse_plan_destroy": (None, [C.c_void_p]),
     "gmmnlse_status_string": (C.c_char_p, [C.c_int]),
@@ -224,6 +225,9 @@ class Plan:
     def contraction_kind(self) -> int:
         """1 = CUDA cores, 2 = tcgen05 single CTA (SS), 3 = tcgen05 CTA pairs, 4 = tcgen05 single CTA (TS)."""
         return int(self._lib.gmmnlse_contraction_kind(self._h))
+
+    def lowrank_rank(self) -> int:
+        return int(self._lib.gmmnlse_lowrank_rank(self._h))
 
     def raman_kind(self) -> int:
         """0 = no Raman term, 1 = FFT convolution, 2 = recursive (damped-oscillator) form."""

@@ -168,6 +168,7 @@ struct gmmnlse_plan {
   virtual int contraction_kind() const = 0;
   virtual int set_tc_chunk(int k) = 0;
   virtual int raman_kind() const = 0;
+  virtual int lowrank_rank() const = 0;
 };
 
 namespace {
@@ -209,6 +210,17 @@ struct PlanT final : gmmnlse_plan {
   // tcgen05 contraction (complex64 path only): TF32 hi/lo split of S2, zero-padded to [R_pad][Q_pad]
   float *S2hi = nullptr, *S2lo = nullptr;
   CUtensorMap tmV, tmShi, tmSlo;
+  // NEXT-4: exact low-rank form of the contraction, S_(pl),(mn) = sum_k L_(pl),k L_(mn),k (pivoted Cholesky)
+  struct TcGemm {              // one rows x K operand of the single-CTA shared-memory tcgen05 kernel
+    float *hi = nullptr, *lo = nullptr;
+    CUtensorMap tmHi, tmLo;
+    int rows = 0, K = 0, NT = 0, nrt = 0, KB = 0, stages = 0;
+  };
+  bool lowrank = false;
+  int lr_R = 0;
+  TcGemm lr1, lr2;             // Z = (L^T D) V  [R x Q],  U = L Z  [Q x R]
+  T* Zb = nullptr;             // [(M+1)][R][N]
+  CUtensorMap tmZ;
   bool tc_ts = false;          // A operand from tensor memory (gemm_ts.cuh)
   bool tc_mc = false;          // clusters of two CTAs multicasting the S tiles (gemm_tc.cuh, MC)
   int tc_cg = 0, tc_NT = 0, tc_nrt = 0, tc_KB = 0, tc_stages = 0, tc_kchunk = 4, tc_probe = 0, tc_stage_cap = 0, n_sm = 0;
@@ -218,6 +230,7 @@ struct PlanT final : gmmnlse_plan {
     cudaFree(pair_m); cudaFree(pair_n); cudaFree(psi0_d); cudaFree(psi); cudaFree(At); cudaFree(G);
     cudaFree(V); cudaFree(U); cudaFree(errbuf); cudaFree(d_err); cudaFree(d_io);
     cudaFree(S2hi); cudaFree(S2lo);
+    cudaFree(lr1.hi); cudaFree(lr1.lo); cudaFree(lr2.hi); cudaFree(lr2.lo); cudaFree(Zb);
     cudaFree(gfwd); cudaFree(ginv); cudaFree(Qc); cudaFree(st_kind); cudaFree(st_wk); cudaFree(st_wr); cudaFree(iir_zp); cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
     if (h_err) cudaFreeHost(h_err);
     if (h_in) cudaFreeHost(h_in);
@@ -465,6 +478,121 @@ struct PlanT final : gmmnlse_plan {
     // t-contiguous operand: 32-byte swizzle atoms (the only MN-major layout kind::tf32 accepts)
     return encode_tmap_f32(tm, (void*)base, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B);
   }
+  // A-operand map (shared-memory form) over [planes][Krows][N] streams
+  int make_a_tmap(CUtensorMap* tm, const T* base, int Krows, int planes) {
+    const cuuint64_t dims[3] = {(cuuint64_t)N, (cuuint64_t)Krows, (cuuint64_t)planes};
+    const cuuint64_t strides[2] = {(cuuint64_t)N * 4, (cuuint64_t)Krows * N * 4};
+    const cuuint32_t box[3] = {32, tc::BK, 1};
+    return encode_tmap_f32(tm, (void*)base, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B);
+  }
+  int tc_build(TcGemm& g, const std::vector<double>& mat, int rows, int K, int smax) {
+    g.rows = rows; g.K = K;
+    g.nrt = (rows + 207) / 208;
+    g.NT = (((rows + g.nrt - 1) / g.nrt) + 15) / 16 * 16;
+    g.KB = (K + tc::BK - 1) / tc::BK;
+    g.stages = tc::MAX_STAGES;
+    while (g.stages > 1 && tc::smem_bytes(g.NT, 1, g.stages) > (size_t)smax) --g.stages;
+    const int Rp = g.nrt * g.NT, Kp = g.KB * tc::BK;
+    std::vector<float> hi((size_t)Rp * Kp, 0.f), lo((size_t)Rp * Kp, 0.f);
+    for (int r = 0; r < rows; ++r)
+      for (int q = 0; q < K; ++q) {
+        const double v = mat[(size_t)r * K + q];
+        const float h = round_tf32(v);
+        hi[(size_t)r * Kp + q] = h;
+        lo[(size_t)r * Kp + q] = round_tf32(v - (double)h);
+      }
+    GM_TRY(dalloc(&g.hi, hi.size())); GM_TRY(upload(g.hi, hi));
+    GM_TRY(dalloc(&g.lo, lo.size())); GM_TRY(upload(g.lo, lo));
+    const cuuint64_t dims[2] = {(cuuint64_t)Kp, (cuuint64_t)Rp};
+    const cuuint64_t strides[1] = {(cuuint64_t)Kp * 4};
+    const cuuint32_t box[2] = {tc::BK, (cuuint32_t)g.NT};
+    const CUtensorMapSwizzle bsw = tc::BK == 32 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B;
+    GM_TRY(encode_tmap_f32(&g.tmHi, g.hi, 2, dims, strides, box, bsw));
+    return encode_tmap_f32(&g.tmLo, g.lo, 2, dims, strides, box, bsw);
+  }
+  int tc_run(const TcGemm& g, const CUtensorMap& amap, int plane0, T* out, long long out_ps, int planes) {
+    if constexpr (sizeof(T) != 4) {
+      return GMMNLSE_EUNSUPPORTED;
+    } else {
+      tc::Params prm;
+      prm.U = out; prm.u_plane_stride = out_ps;
+      prm.Q = g.rows; prm.N = N; prm.NT = g.NT; prm.KB = g.KB; prm.n_rt = g.nrt;
+      prm.t_tiles = N / tc::TM;
+      prm.total_tiles = planes * prm.t_tiles * g.nrt;
+      prm.plane0 = plane0; prm.stages = g.stages; prm.kchunk = tc_kchunk; prm.probe = 0;
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)std::min(n_sm, prm.total_tiles));
+      cfg.blockDim = dim3(tc::NTHREADS);
+      cfg.dynamicSmemBytes = tc::smem_bytes(g.NT, 1, g.stages);
+      cfg.stream = stream;
+      prof_begin(GMMNLSE_KIND_CONTRACT);
+      cudaError_t e = cudaLaunchKernelEx(&cfg, tc::k_contract_tc<1>, amap, g.tmHi, g.tmLo, prm);
+      prof_end();
+      GM_CUDA(e);
+      return 0;
+    }
+  }
+  // Pivoted Cholesky of the (p<=l) x (m<=n) symmetric matrix Ms = S_plmn (Eq. 2 makes it a Gram matrix of the
+  // pair functions F_p F_l, hence positive semi-definite and, for Hermite-Gauss modes, of rank << Q).  Exact to
+  // fp64 rounding: stops when the largest remaining diagonal is < 1e-13 of the largest, then verifies
+  // max |Ms - L L^T| <= 1e-11 max |Ms| (a tensor that is not PSD fails here: EUNSUPPORTED).
+  int init_lowrank(const std::vector<double>& h_S2, int smax) {
+    std::vector<double> dbl(Q);
+    for (int q = 0, m = 0; m < P; ++m)
+      for (int n = m; n < P; ++n, ++q) dbl[q] = m == n ? 1.0 : 2.0;
+    std::vector<double> Ms((size_t)Q * Q);
+    double amax = 0;
+    for (int r = 0; r < Q; ++r)
+      for (int q = 0; q < Q; ++q) {
+        Ms[(size_t)r * Q + q] = h_S2[(size_t)r * Q + q] / dbl[q];
+        amax = std::fmax(amax, std::fabs(Ms[(size_t)r * Q + q]));
+      }
+    std::vector<double> d(Q), L;                       // L column-major by factor: L[k * Q + r]
+    double dmax0 = 0;
+    for (int r = 0; r < Q; ++r) { d[r] = Ms[(size_t)r * Q + r]; dmax0 = std::fmax(dmax0, d[r]); }
+    if (!(dmax0 > 0)) return GMMNLSE_EUNSUPPORTED;
+    int R = 0;
+    while (R < Q) {
+      int piv = 0;
+      for (int r = 1; r < Q; ++r) if (d[r] > d[piv]) piv = r;
+      if (d[piv] <= 1e-13 * dmax0) break;
+      L.resize((size_t)(R + 1) * Q);
+      double* col = &L[(size_t)R * Q];
+      const double inv = 1.0 / std::sqrt(d[piv]);
+      for (int r = 0; r < Q; ++r) {
+        double v = Ms[(size_t)r * Q + piv];
+        for (int k = 0; k < R; ++k) v -= L[(size_t)k * Q + r] * L[(size_t)k * Q + piv];
+        col[r] = v * inv;
+      }
+      for (int r = 0; r < Q; ++r) d[r] -= col[r] * col[r];
+      ++R;
+    }
+    double res = 0;
+    for (int r = 0; r < Q; ++r)
+      for (int q = r; q < Q; ++q) {
+        double v = Ms[(size_t)r * Q + q];
+        for (int k = 0; k < R; ++k) v -= L[(size_t)k * Q + r] * L[(size_t)k * Q + q];
+        res = std::fmax(res, std::fabs(v));
+      }
+    if (R == 0 || res > 1e-11 * amax) return GMMNLSE_EUNSUPPORTED;
+    lr_R = R;
+    std::vector<double> W1((size_t)R * Q), W2((size_t)Q * R);
+    for (int k = 0; k < R; ++k)
+      for (int q = 0; q < Q; ++q) {
+        W1[(size_t)k * Q + q] = L[(size_t)k * Q + q] * dbl[q];     // (L^T D)[k][q]
+        W2[(size_t)q * R + k] = L[(size_t)k * Q + q];              // L[q][k]
+      }
+    GM_TRY(tc_build(lr1, W1, R, Q, smax));
+    GM_TRY(tc_build(lr2, W2, Q, R, smax));
+    GM_TRY(dalloc(&Zb, (size_t)(M + 1) * R * N));
+    GM_TRY(make_a_tmap(&tmZ, Zb, R, M + 1));
+    GM_TRY(make_a_tmap(&tmV, V, Q, M + 1));
+    if constexpr (sizeof(T) == 4)
+      GM_CUDA(cudaFuncSetAttribute(tc::k_contract_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smax));
+    lowrank = true;
+    return 0;
+  }
+
   int init_tc(const std::vector<double>& h_S2) {
     if constexpr (sizeof(T) != 4) {
       if (contraction >= 2) return GMMNLSE_EUNSUPPORTED;
@@ -472,6 +600,14 @@ struct PlanT final : gmmnlse_plan {
     } else {
       const bool want = contraction >= 2 || (contraction == 0 && Q >= 64);
       if (!want) return 0;
+      if (contraction == 6) {                          // exact low-rank form (NEXT-4), scalar-mode path only
+        if (general || N % tc::TM != 0) return GMMNLSE_EUNSUPPORTED;
+        int dev0 = 0, smax0 = 0;
+        GM_CUDA(cudaGetDevice(&dev0));
+        GM_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev0));
+        GM_CUDA(cudaDeviceGetAttribute(&smax0, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev0));
+        return init_lowrank(h_S2, smax0);
+      }
       // auto picks the single-CTA form: measured 1.76 ms against 1.86 ms for CTA pairs at config 5
       int cg = contraction == 2 ? 2 : 1;
       // the tensor-memory (TS) form measured the same as the shared-memory (SS) form (1.68 vs 1.67 ms at config 5):
@@ -649,6 +785,17 @@ struct PlanT final : gmmnlse_plan {
   }
 
   int launch_contract(const T* Vin, T* Uout, int planes) {
+    if (lowrank) {
+      if (planes > M + 1) return GMMNLSE_EINVAL;
+      if (Vin >= V && Vin < V + (size_t)(M + 1) * QN) {
+        GM_TRY(tc_run(lr1, tmV, (int)((Vin - V) / QN), Zb, (long long)lr_R * N, planes));
+      } else {
+        CUtensorMap tmp;
+        GM_TRY(make_a_tmap(&tmp, Vin, Q, planes));
+        GM_TRY(tc_run(lr1, tmp, 0, Zb, (long long)lr_R * N, planes));
+      }
+      return tc_run(lr2, tmZ, 0, Uout, QN, planes);
+    }
     if (tc_cg) {
       if (Vin >= V && Vin < V + (size_t)(M + 1) * QN)              // the plan's own buffer
         return launch_contract_tc(tmV, (int)((Vin - V) / QN), Uout, planes);
@@ -946,7 +1093,10 @@ struct PlanT final : gmmnlse_plan {
     if (n_planes < 1) return GMMNLSE_EINVAL;
     return launch_pairs((const C*)A, PN, (T*)Vout, QN, n_planes);
   }
-  int contraction_kind() const override { return tc_cg ? (tc_ts ? 4 : (tc_mc ? 5 : 1 + tc_cg)) : 1; }
+  int contraction_kind() const override {
+    return lowrank ? 6 : (tc_cg ? (tc_ts ? 4 : (tc_mc ? 5 : 1 + tc_cg)) : 1);
+  }
+  int lowrank_rank() const override { return lowrank ? lr_R : 0; }
   int raman_kind() const override { return f_R == 0.0 ? 0 : (iir ? 2 : 1); }
   int set_tc_chunk(int k) override {
     if ((k & 0xFF) < 1) return GMMNLSE_EINVAL;
@@ -994,7 +1144,7 @@ static int create_plan(gmmnlse_plan** out, int P, int N, int M, double dt, doubl
   if (!(dt > 0) || !(dz > 0) || !(omega0 > 0) || !std::isfinite(n2) || !std::isfinite(f_R)) return GMMNLSE_EINVAL;
   if ((f_R != 0.0) != (h_R != nullptr)) return GMMNLSE_EINVAL;
   if (o.precision != 0 && o.precision != 1) return GMMNLSE_EINVAL;
-  if (o.raman < 0 || o.raman > 2 || o.contraction < 0 || o.contraction > 5) return GMMNLSE_EINVAL;
+  if (o.raman < 0 || o.raman > 2 || o.contraction < 0 || o.contraction > 6) return GMMNLSE_EINVAL;
   if (o.shock && M_PI / dt >= omega0) return GMMNLSE_EINVAL;
   if (!(o.tol > 0)) o.tol = 1e-6;
   for (long long i = 0; i < (long long)P * n_beta; ++i)
@@ -1153,6 +1303,8 @@ int gmmnlse_debug_contract(gmmnlse_plan* plan, const void* V, void* U, int n_pla
 int gmmnlse_contraction_kind(const gmmnlse_plan* plan) { return plan ? plan->contraction_kind() : 0; }
 
 int gmmnlse_raman_kind(const gmmnlse_plan* plan) { return plan ? plan->raman_kind() : 0; }
+
+int gmmnlse_lowrank_rank(const gmmnlse_plan* plan) { return plan ? plan->lowrank_rank() : 0; }
 
 int gmmnlse_debug_set_tc_chunk(gmmnlse_plan* plan, int k) { return plan ? plan->set_tc_chunk(k) : GMMNLSE_EINVAL; }
 

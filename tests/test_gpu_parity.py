@@ -114,14 +114,14 @@ def test_pair_conv_vs_oracle(B, cfg, N, kw, raman):
 
 
 # --------------------------------------------------------------------------- a12: nonlinear_op
-def _nonlinear_op_case(B, w, seed=0):
+def _nonlinear_op_case(B, w, seed=0, **plan_kw):
     rng = np.random.default_rng(seed)
     # a developed field: the launch field with random per-mode spectral phases (still seeded)
     A = w.A0
     dt = np.complex128 if w.precision else np.complex64
     Ad = dev(A, dt)
     dA = torch.empty_like(Ad)
-    with B.plan_from_workload(w) as plan:
+    with B.plan_from_workload(w, **plan_kw) as plan:
         plan.nonlinear_op(Ad, dA)
         torch.cuda.synchronize()
     A_in = Ad.cpu().numpy().astype(np.complex128)
@@ -338,6 +338,7 @@ def _packed_S2(S):
     (4, 512, {}, 3), (4, 512, {}, 2), (4, 512, {}, 4),             # Q = 210: two r-tiles of 112
     (5, 256, {}, 3), (5, 256, {}, 2), (5, 256, {}, 1), (5, 256, {}, 4), (5, 256, {}, 5),   # Q = 1035: 5 r-tiles of 208
     (3, 1024, {}, 5), (4, 512, {}, 5),                              # multicast pairs
+    (3, 1024, {}, 6), (4, 512, {}, 6), (5, 256, {}, 6),             # exact low-rank form (rank 45 / ~120 / 153)
     (3, 128, dict(max_group=3), 3), (3, 128, dict(max_group=3), 4),       # Q = 55 < 64: tensor path forced, N = 128
 ])
 def test_contraction_vs_fp64_matmul(B, cfg, N, kw, kind):
@@ -348,7 +349,7 @@ def test_contraction_vs_fp64_matmul(B, cfg, N, kw, kind):
     # pair streams with the dynamic range of |A|^2 products: peak to 1e-6 of peak along t
     V = (rng.standard_normal((planes, Q, N)) * np.exp(rng.uniform(-7, 7, (planes, 1, N)))).astype(np.float32)
     with B.plan_from_workload(w, contraction=kind) as plan:
-        assert plan.contraction_kind() == {1: 1, 2: 3, 3: 2, 4: 4, 5: 5}[kind]
+        assert plan.contraction_kind() == {1: 1, 2: 3, 3: 2, 4: 4, 5: 5, 6: 6}[kind]
         Vd = torch.from_numpy(V).cuda()
         U = torch.full((planes, Q, N), float("nan"), dtype=torch.float32, device="cuda")
         plan.debug_contract(Vd, U, planes)
@@ -367,6 +368,28 @@ def test_contraction_vs_fp64_matmul(B, cfg, N, kw, kind):
     # column-wise (per time sample and plane): no sample may be off by more than a few fp32 ulps of its scale
     col = np.linalg.norm(Uh - ref, axis=1) / np.linalg.norm(ref, axis=1)
     assert col.max() <= 3e-6, col.max()
+
+
+def test_lowrank_form_rank_operator_and_propagation(B):
+    """NEXT-4: the Gram structure of Eq. 2's tensor.  Products of Hermite-Gauss modes of order <= g span the
+    polynomials of degree <= 2g times a Gaussian: rank (2g+1)(2g+2)/2 (45 at P = 15, 153 at P = 45)."""
+    w = W.make_config(3, N=1024, L=2 * 10 * 100e-6)
+    with B.plan_from_workload(w, contraction=6) as plan:
+        assert plan.contraction_kind() == 6 and plan.lowrank_rank() == 45
+    assert _nonlinear_op_case(B, w, contraction=6) <= TOL_OP
+    out_lr = _propagate(B, w, contraction=6)[1]
+    out_d = _propagate(B, w, contraction=3)[1]
+    assert rel(out_lr, out_d) <= 2e-5
+    w5 = W.make_config(5, N=256)
+    with B.plan_from_workload(w5, contraction=6) as plan:
+        assert plan.lowrank_rank() == 153
+    assert _nonlinear_op_case(B, w5, contraction=6) <= TOL_OP
+    # a tensor that is not a Gram matrix (indefinite) has no such factorisation
+    S_bad = w.S.copy()
+    S_bad[0, 0, 0, 0] = -abs(S_bad[0, 0, 0, 0])
+    with pytest.raises(B.GmmnlseError) as e:
+        B.Plan(w.P, w.N, w.M, w.dt, w.dz, w.beta, S_bad, w.f_R, w.h_R, w.omega0, w.n2, contraction=6)
+    assert e.value.status == B.EUNSUPPORTED
 
 
 def test_contraction_auto_selects_tensor_cores_for_large_P(B):
