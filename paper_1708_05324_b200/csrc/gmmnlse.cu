@@ -223,7 +223,7 @@ struct PlanT final : gmmnlse_plan {
   CUtensorMap tmZ;
   bool tc_ts = false;          // A operand from tensor memory (gemm_ts.cuh)
   bool tc_mc = false;          // clusters of two CTAs multicasting the S tiles (gemm_tc.cuh, MC)
-  int tc_cg = 0, tc_NT = 0, tc_nrt = 0, tc_KB = 0, tc_stages = 0, tc_kchunk = 4, tc_probe = 0, tc_stage_cap = 0, n_sm = 0;
+  int tc_cg = 0, tc_NT = 0, tc_nrt = 0, tc_KB = 0, tc_stages = 0, tc_kchunk = 4, tc_probe = 0, tc_stage_cap = 0, n_sm = 0, mr_tile = 0;
 
   ~PlanT() override {
     cudaFree(tw); cudaFree(Kw); cudaFree(H); cudaFree(E); cudaFree(EM_d); cudaFree(S2);
@@ -834,15 +834,20 @@ struct PlanT final : gmmnlse_plan {
       GM_CUDA(cudaGetLastError());
       return 0;
     }
-    const size_t smem = sizeof(C) * P * 128;
+    const int tw = mr_tile > 0 ? mr_tile : (P >= 32 && N >= 64 ? 32 : 128);
+    const int G = tw == 128 ? (P >= 12 ? 4 : (P >= 4 ? 2 : 1)) : (tw == 64 ? 8 : 8);   // mode groups per CTA
+    const size_t smem = sizeof(C) * P * tw;
     static size_t configured = 0;
     if (smem > configured) {
-      GM_CUDA(cudaFuncSetAttribute(k_mode_reduce<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      configured = smem;
+      GM_CUDA(cudaFuncSetAttribute(k_mode_reduce<T, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)(sizeof(C) * P * 128)));
+      configured = sizeof(C) * P * 128;
     }
-    const int G = P >= 12 ? 4 : (P >= 4 ? 2 : 1);              // mode groups per CTA
+    const dim3 grid((N + tw - 1) / tw, planes);
     prof_begin(GMMNLSE_KIND_MODE_REDUCE);
-    k_mode_reduce<T><<<dim3((N + 127) / 128, planes), 128 * G, smem, stream>>>(Uin, QN, A, PN, Nout, PN, P, N);
+    if (tw == 32) k_mode_reduce<T, 32><<<grid, 32 * G, smem, stream>>>(Uin, QN, A, PN, Nout, PN, P, N);
+    else if (tw == 64) k_mode_reduce<T, 64><<<grid, 64 * G, smem, stream>>>(Uin, QN, A, PN, Nout, PN, P, N);
+    else k_mode_reduce<T, 128><<<grid, 128 * G, smem, stream>>>(Uin, QN, A, PN, Nout, PN, P, N);
     prof_end();
     GM_CUDA(cudaGetLastError());
     return 0;
@@ -1103,6 +1108,7 @@ struct PlanT final : gmmnlse_plan {
     tc_kchunk = k & 0xFF;
     tc_probe = (k >> 8) & 0xFF;          // timing probes (gemm_tc.cuh Params::probe); results are wrong when set
     tc_stage_cap = (k >> 16) & 0xFF;     // cap on smem stages (0 = as many as fit)
+    mr_tile = ((k >> 24) & 0x3) == 1 ? 32 : (((k >> 24) & 0x3) == 2 ? 64 : (((k >> 24) & 0x3) == 3 ? 128 : 0));   // a7 tile probe
     return 0;
   }
   int debug_contract(const void* Vin, void* Uout, int n_planes) override {

@@ -289,22 +289,24 @@ k_contract(const T* __restrict__ S2, const T* __restrict__ V, long long v_plane_
 
 // ------------------------------------------------------------------------------------------
 // a7: N_p(t) = sum_l U_pl(t) A_l(t), U real symmetric, stored packed: row r(p,l) = p P - p(p-1)/2 + (l-p)
-// for p <= l.  grid = (N / 128, n_planes); blockDim = 128 * G: thread (tx, g) owns sample t = 128 bx + tx
-// and modes p = g, g + G, ...; the A tile [P][128] is staged in shared memory, the accumulator of one
+// for p <= l.  grid = (N / TW, n_planes); blockDim = TW * G: thread (tx, g) owns sample t = TW bx + tx
+// and modes p = g, g + G, ...; the A tile [P][TW] is staged in shared memory, the accumulator of one
 // (p, t) lives in registers, so the U loads of a row are independent and pipeline freely.  Each U value
 // is read twice (once as U_pl, once as U_lp) by threads of the same CTA: the second read hits L1/L2.
-template <typename T>
+template <typename T, int TW>
 __global__ void __launch_bounds__(512)
 k_mode_reduce(const T* __restrict__ U, long long u_plane_stride, const cplx<T>* __restrict__ A,
               long long a_plane_stride, cplx<T>* __restrict__ Nt, long long n_plane_stride, int P, int N) {
+  // TW = samples per CTA (32 / 64 / 128): a narrow tile keeps the CTA's slice of U (Q x TW x 4 B) small enough
+  // that its second read (U_lp) still finds the first (U_pl) in L2
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  cplx<T>* a_s = reinterpret_cast<cplx<T>*>(smem_raw);        // [P][128]
-  const int tx = threadIdx.x & 127, g = threadIdx.x >> 7, G = blockDim.x >> 7, j = blockIdx.y;
-  const int t0 = blockIdx.x * 128;
+  cplx<T>* a_s = reinterpret_cast<cplx<T>*>(smem_raw);        // [P][TW]
+  const int tx = threadIdx.x % TW, g = threadIdx.x / TW, G = blockDim.x / TW, j = blockIdx.y;
+  const int t0 = blockIdx.x * TW;
   const cplx<T>* Aj = A + j * a_plane_stride + t0;
-  for (int i = threadIdx.x; i < P * 128; i += blockDim.x) {
-    const int x = i & 127;
-    a_s[i] = t0 + x < N ? Aj[(long long)(i >> 7) * N + x] : mk((T)0, (T)0);
+  for (int i = threadIdx.x; i < P * TW; i += blockDim.x) {
+    const int x = i % TW;
+    a_s[i] = t0 + x < N ? Aj[(long long)(i / TW) * N + x] : mk((T)0, (T)0);
   }
   __syncthreads();
   const int t = t0 + tx;
@@ -317,7 +319,7 @@ k_mode_reduce(const T* __restrict__ U, long long u_plane_stride, const cplx<T>* 
 #pragma unroll 8
     for (int l = 0; l < p; ++l) {                     // column part: U_lp, l < p
       const T u = Ut[r * N];
-      const cplx<T> a = at[l * 128];
+      const cplx<T> a = at[l * TW];
       sx += u * a.x;
       sy += u * a.y;
       r += P - l - 1;                                 // r(l+1, p) - r(l, p)
@@ -325,7 +327,7 @@ k_mode_reduce(const T* __restrict__ U, long long u_plane_stride, const cplx<T>* 
 #pragma unroll 8
     for (int l = p; l < P; ++l, ++r) {                // row part: U_pl, l >= p; r == r(p, p) here
       const T u = Ut[r * N];
-      const cplx<T> a = at[l * 128];
+      const cplx<T> a = at[l * TW];
       sx += u * a.x;
       sy += u * a.y;
     }
