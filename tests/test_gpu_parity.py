@@ -675,3 +675,58 @@ def test_gain_coupling_reject_bad_input(B):
         bad = np.zeros((w.P, w.P), complex); bad[0, 1] = np.inf
         with pytest.raises(B.GmmnlseError):
             plan.set_coupling(bad)
+
+
+# ------------------------------------------ full-length propagation against stored oracle outputs (tests/golden)
+def _golden(fname):
+    import importlib.util
+    import os
+    gdir = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    path = os.path.join(gdir, fname)
+    if not os.path.exists(path):
+        pytest.skip(f"{fname} not generated (python tests/golden/make_golden.py)")
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(gdir, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)
+    meta = {}
+    with open(path) as fh:
+        for line in fh:
+            if not line.startswith("#"):
+                break
+            for tok in line[1:].split():
+                if "=" in tok:
+                    k, v = tok.split("=", 1)
+                    meta[k] = v
+    data = np.loadtxt(path)
+    return mg, meta, data
+
+
+@pytest.mark.parametrize("fname,cfg,tol_rk,tol_mpa", [
+    ("config2_rk4ip_3000steps.txt", 2, 1e-4, TOL_FIELD),     # BASELINE config 2 at its full length (15 cm)
+    ("config3_rk4ip_200steps.txt", 3, 1e-4, 5e-3),           # first 2 cm of config 3
+])
+def test_long_propagation_vs_stored_oracle_rk4ip(B, fname, cfg, tol_rk, tol_mpa):
+    mg, meta, data = _golden(fname)
+    w = W.make_config(cfg)
+    L, steps = float(meta["L_m"]), int(meta["steps"])
+    assert abs(steps * w.dz - L) < 1e-12 and int(meta["N"]) == w.N and int(meta["P"]) == w.P
+    A_in = w.A0.astype(np.complex64).astype(np.complex128)
+    assert mg.input_checksum(w, A_in) == meta["input_sha256_32"], "golden is stale: inputs changed"
+    modes, samples = data[:, 0].astype(int), data[:, 1].astype(int)
+    ref = data[:, 2] + 1j * data[:, 3]
+    Ad = dev(w.A0, np.complex64)
+    out_mpa, out_rk = torch.empty_like(Ad), torch.empty_like(Ad)
+    with B.plan_from_workload(w) as plan:
+        st = plan.propagate(Ad, L, out_mpa)
+        plan.propagate_rk4ip(Ad, L, out_rk)
+        torch.cuda.synchronize()
+        stats = plan.stats()
+    assert st == 0 and stats["not_converged"] == 0
+    o_rk = out_rk.cpu().numpy().astype(np.complex128)
+    o_mpa = out_mpa.cpu().numpy().astype(np.complex128)
+    assert rel(o_rk[modes, samples], ref) <= tol_rk
+    assert rel(o_mpa[modes, samples], ref) <= tol_mpa
+    # conserved quantity of the full field against the oracle's own drift (stored in the header), same scheme (S15)
+    pn_ref = float(meta["photon_number_ratio"])
+    pn = O.photon_number(o_rk, w.dt, w.omega0) / O.photon_number(A_in, w.dt, w.omega0)
+    assert abs(pn - pn_ref) <= TOL_DRIFT

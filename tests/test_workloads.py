@@ -85,3 +85,30 @@ def test_configs_shapes_and_seeding(idx):
         t = (np.arange(4096) - 2048) * a.dt
         above = t[I >= 0.5 * I.max()]
         assert abs((above[-1] - above[0]) / a.meta["fwhm"] - 1) < 0.05
+
+
+def test_stored_goldens_match_current_inputs():
+    """Every stored oracle output under tests/golden names the inputs it was computed from (checksum of the launch
+    field, S, beta, h_R); a change of the seeded generators must regenerate them."""
+    import glob
+    import importlib.util
+    import os
+    gdir = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(gdir, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)
+    for path in glob.glob(os.path.join(gdir, "config*_rk4ip_*steps.txt")):
+        meta = {}
+        with open(path) as fh:
+            for line in fh:
+                if not line.startswith("#"):
+                    break
+                for tok in line[1:].split():
+                    if "=" in tok:
+                        k, v = tok.split("=", 1)
+                        meta[k] = v
+        cfg = int(os.path.basename(path)[len("config")])
+        w = W.make_config(cfg)
+        A_in = w.A0.astype(np.complex64).astype(np.complex128)
+        assert mg.input_checksum(w, A_in) == meta["input_sha256_32"], path
+        assert int(meta["steps"]) == int(round(float(meta["L_m"]) / w.dz))
