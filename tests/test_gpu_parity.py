@@ -704,6 +704,8 @@ def _golden(fname):
 @pytest.mark.parametrize("fname,cfg,tol_rk,tol_mpa", [
     ("config2_rk4ip_3000steps.txt", 2, 1e-4, TOL_FIELD),     # BASELINE config 2 at its full length (15 cm)
     ("config3_rk4ip_200steps.txt", 3, 1e-4, 5e-3),           # first 2 cm of config 3
+    ("config4_rk4ip_100steps.txt", 4, 1e-4, 5e-3),           # first 5 mm of config 4 (5 large steps, full shape)
+    ("config5_rk4ip_40steps.txt", 5, 1e-4, 2e-2),            # first 1 mm of config 5 (2 large steps, full shape)
 ])
 def test_long_propagation_vs_stored_oracle_rk4ip(B, fname, cfg, tol_rk, tol_mpa):
     mg, meta, data = _golden(fname)
@@ -711,7 +713,7 @@ def test_long_propagation_vs_stored_oracle_rk4ip(B, fname, cfg, tol_rk, tol_mpa)
     L, steps = float(meta["L_m"]), int(meta["steps"])
     assert abs(steps * w.dz - L) < 1e-12 and int(meta["N"]) == w.N and int(meta["P"]) == w.P
     A_in = w.A0.astype(np.complex64).astype(np.complex128)
-    assert mg.input_checksum(w, A_in) == meta["input_sha256_32"], "golden is stale: inputs changed"
+    assert mg.fingerprint_matches(meta, w, A_in), "golden is stale: inputs changed"
     modes, samples = data[:, 0].astype(int), data[:, 1].astype(int)
     ref = data[:, 2] + 1j * data[:, 3]
     Ad = dev(w.A0, np.complex64)

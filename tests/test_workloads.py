@@ -88,7 +88,7 @@ def test_configs_shapes_and_seeding(idx):
 
 
 def test_stored_goldens_match_current_inputs():
-    """Every stored oracle output under tests/golden names the inputs it was computed from (checksum of the launch
+    """Every stored oracle output under tests/golden names the inputs it was computed from (fingerprint of the launch
     field, S, beta, h_R); a change of the seeded generators must regenerate them."""
     import glob
     import importlib.util
@@ -110,5 +110,5 @@ def test_stored_goldens_match_current_inputs():
         cfg = int(os.path.basename(path)[len("config")])
         w = W.make_config(cfg)
         A_in = w.A0.astype(np.complex64).astype(np.complex128)
-        assert mg.input_checksum(w, A_in) == meta["input_sha256_32"], path
+        assert mg.fingerprint_matches(meta, w, A_in), path
         assert int(meta["steps"]) == int(round(float(meta["L_m"]) / w.dz))
