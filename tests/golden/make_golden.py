@@ -44,6 +44,8 @@ def main():
     ap.add_argument("--config", type=int, required=True)
     ap.add_argument("--length", type=float, default=None, help="propagation length in m (default: the full L)")
     ap.add_argument("--stride", type=int, default=8)
+    ap.add_argument("--integrator", default="rk4ip", choices=["rk4ip", "mpa"],
+                    help="oracle O3 (RK4IP, default) or O4 (plain MPA with the configuration's M and tol)")
     ap.add_argument("--out", default=None)
     args = ap.parse_args()
     w = W.make_config(args.config)
@@ -53,19 +55,28 @@ def main():
     omega = O.omega_grid(w.N, w.dt)
     D = O.dispersion_operator(w.beta, omega)
     nl = lambda X: O.nonlinear_op_freq(X, w.S, w.kappa, omega, w.omega0, w.f_R, w.h_R, w.dt, w.shock)
-    At = O.to_freq(A_in)
     t0 = time.time()
-    for i in range(steps):
-        At = O.rk4ip_step(At, w.dz, D, nl)
-        if (i + 1) % 100 == 0:
-            print(f"step {i + 1}/{steps}  {time.time() - t0:.0f} s", flush=True)
-    out = O.to_time(At)
+    extra = ""
+    if args.integrator == "mpa":
+        st = {}
+        out = O.mpa_propagate(A_in, L, w.dz, w.M, w.beta, w.S, w.kappa, w.omega0, w.f_R, w.h_R, w.dt, shock=w.shock,
+                              tol=w.tol, stats=st)
+        extra = f"M={w.M} tol={float(w.tol)!r} large_steps={st['large_steps']} iterations={st['iterations']}\n"
+    else:
+        At = O.to_freq(A_in)
+        for i in range(steps):
+            At = O.rk4ip_step(At, w.dz, D, nl)
+            if (i + 1) % 100 == 0:
+                print(f"step {i + 1}/{steps}  {time.time() - t0:.0f} s", flush=True)
+        out = O.to_time(At)
     name = args.out or os.path.join(os.path.dirname(os.path.abspath(__file__)),
-                                    f"config{args.config}_rk4ip_{steps}steps.txt")
+                                    f"config{args.config}_{args.integrator}_{steps}steps.txt")
     idx = np.arange(0, w.N, args.stride)
     rows = [(p, n, out[p, n].real, out[p, n].imag) for p in range(w.P) for n in idx]
     pn = float(O.photon_number(out, w.dt, w.omega0) / O.photon_number(A_in, w.dt, w.omega0))
-    header = (f"oracle RK4IP (oracle/gmmnlse_oracle.py rk4ip_step), BASELINE.json config {args.config}\n"
+    which = "RK4IP (oracle/gmmnlse_oracle.py rk4ip_step)" if args.integrator == "rk4ip" else \
+        "plain MPA (oracle/gmmnlse_oracle.py mpa_propagate)"
+    header = (f"oracle {which}, BASELINE.json config {args.config}\n" + extra +
               f"L_m={float(L)!r} dz_m={float(w.dz)!r} steps={steps} P={w.P} N={w.N} stride={args.stride}\n"              + " ".join(f"{k}={v!r}" for k, v in input_fingerprint(w, A_in).items()) + "\n" +
               f"energy_in={float(O.energy(A_in, w.dt))!r} energy_out={float(O.energy(out, w.dt))!r}\n"
               f"photon_number_ratio={pn!r}\n"

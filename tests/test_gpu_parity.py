@@ -734,3 +734,29 @@ def test_long_propagation_vs_stored_oracle_rk4ip(B, fname, cfg, tol_rk, tol_mpa)
     pn_ref = float(meta["photon_number_ratio"])
     pn = O.photon_number(o_rk, w.dt, w.omega0) / O.photon_number(A_in, w.dt, w.omega0)
     assert abs(pn - pn_ref) <= TOL_DRIFT
+
+
+def test_long_mpa_vs_stored_oracle_mpa(B):
+    """Config 3 at full shape over 20 large steps against the oracle's own MPA (O4, stored): same scheme, so the
+    distance is fp32 rounding plus at most one iteration of difference per large step, not the O(dz^2) of the
+    RK4IP comparison."""
+    mg, meta, data = _golden("config3_mpa_200steps.txt")
+    w = W.make_config(3)
+    L = float(meta["L_m"])
+    A_in = w.A0.astype(np.complex64).astype(np.complex128)
+    assert mg.fingerprint_matches(meta, w, A_in), "golden is stale: inputs changed"
+    assert int(meta["M"]) == w.M and float(meta["tol"]) == w.tol
+    modes, samples = data[:, 0].astype(int), data[:, 1].astype(int)
+    ref = data[:, 2] + 1j * data[:, 3]
+    Ad = dev(w.A0, np.complex64)
+    out = torch.empty_like(Ad)
+    with B.plan_from_workload(w) as plan:
+        st = plan.propagate(Ad, L, out)
+        torch.cuda.synchronize()
+        stats = plan.stats()
+    assert st == 0 and stats["large_steps"] == int(meta["large_steps"])
+    assert abs(stats["iterations"] - int(meta["iterations"])) <= stats["large_steps"]
+    o = out.cpu().numpy().astype(np.complex128)
+    assert rel(o[modes, samples], ref) <= 1e-4
+    pn = O.photon_number(o, w.dt, w.omega0) / O.photon_number(A_in, w.dt, w.omega0)
+    assert abs(pn - float(meta["photon_number_ratio"])) <= TOL_DRIFT

@@ -97,7 +97,7 @@ def test_stored_goldens_match_current_inputs():
     spec = importlib.util.spec_from_file_location("make_golden", os.path.join(gdir, "make_golden.py"))
     mg = importlib.util.module_from_spec(spec)
     spec.loader.exec_module(mg)
-    for path in glob.glob(os.path.join(gdir, "config*_rk4ip_*steps.txt")):
+    for path in glob.glob(os.path.join(gdir, "config*_*steps.txt")):
         meta = {}
         with open(path) as fh:
             for line in fh:
