@@ -182,8 +182,14 @@ int gmmnlse_lowrank_rank(const gmmnlse_plan *plan);
 int gmmnlse_raman_kind(const gmmnlse_plan *plan);
 /*   set_tc_chunk: k-blocks (16 packed pairs each) a tensor-memory accumulator holds before the epilogue
  *          drains it into fp32 registers (default 4); bounds the bias of the tensor core's truncating
- *          accumulate.  k >= 1.                          */
+ *          accumulate.  1 <= k <= 255.                        */
 int gmmnlse_debug_set_tc_chunk(gmmnlse_plan *plan, int k);
+/*   set_probe: measurement knobs behind profiles/r01c-r01h.  probe_bits: timing probes of the tcgen05 contraction
+ *          (1 skip the V_lo conversion, 2 / 8 / 16 skip all / A / B TMA loads after the first fill, 4 skip the U
+ *          stores, 32 skip the MMAs) -- RESULTS ARE WRONG when non-zero, time only; stage_cap: cap on its
+ *          shared-memory stages (0 = as many as fit); a7_tile: samples per CTA of the mode reduction (0 auto, 32,
+ *          64, 128).  EINVAL on other values.                                                   */
+int gmmnlse_debug_set_probe(gmmnlse_plan *plan, int probe_bits, int stage_cap, int a7_tile);
 
 void gmmnlse_plan_destroy(gmmnlse_plan *plan);
 const char *gmmnlse_status_string(int status);

@@ -61,6 +61,7 @@ SIGNATURES = {
     "gmmnlse_raman_kind": (C.c_int, [C.c_void_p]),
     "gmmnlse_lowrank_rank": (C.c_int, [C.c_void_p]),
     "gmmnlse_debug_set_tc_chunk": (C.c_int, [C.c_void_p, C.c_int]),
+    "gmmnlse_debug_set_probe": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int]),
     "gmmnlse_plan_destroy": (None, [C.c_void_p]),
     "gmmnlse_status_string": (C.c_char_p, [C.c_int]),
     "gmmnlse_last_cuda_error": (C.c_char_p, []),
@@ -235,6 +236,9 @@ class Plan:
 
     def debug_set_tc_chunk(self, k: int) -> None:
         _check(self._lib, self._lib.gmmnlse_debug_set_tc_chunk(self._h, int(k)))
+
+    def debug_set_probe(self, probe_bits: int = 0, stage_cap: int = 0, a7_tile: int = 0) -> None:
+        _check(self._lib, self._lib.gmmnlse_debug_set_probe(self._h, int(probe_bits), int(stage_cap), int(a7_tile)))
 
     def destroy(self) -> None:
         if self._h:

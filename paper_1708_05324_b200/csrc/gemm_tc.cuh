@@ -54,8 +54,8 @@ struct Params {
   float* U;                    // [plane][Q][N]
   long long u_plane_stride;    // elements
   int Q, N, NT, KB, n_rt, t_tiles, total_tiles, plane0, stages, kchunk;
-  int probe;                   // timing probes only (results wrong): 1 skip V_lo conversion, 2 skip TMA after the first
-                               // fill, 4 skip the U stores
+  int probe;                   // timing probes only (results wrong): 1 skip V_lo conversion, 2 / 8 / 16 skip all / A /
+                               // B TMA loads after the first fill, 4 skip the U stores, 32 skip the MMAs
 };
 
 __host__ __device__ inline int b_bytes(int NT, int CG) { return (NT / CG) * BK * 4; }

@@ -167,6 +167,7 @@ struct gmmnlse_plan {
   virtual int debug_contract(const void* V, void* U, int n_planes) = 0;
   virtual int contraction_kind() const = 0;
   virtual int set_tc_chunk(int k) = 0;
+  virtual int set_probe(int probe_bits, int stage_cap, int a7_tile) = 0;
   virtual int raman_kind() const = 0;
   virtual int lowrank_rank() const = 0;
 };
@@ -1104,11 +1105,16 @@ struct PlanT final : gmmnlse_plan {
   int lowrank_rank() const override { return lowrank ? lr_R : 0; }
   int raman_kind() const override { return f_R == 0.0 ? 0 : (iir ? 2 : 1); }
   int set_tc_chunk(int k) override {
-    if ((k & 0xFF) < 1) return GMMNLSE_EINVAL;
-    tc_kchunk = k & 0xFF;
-    tc_probe = (k >> 8) & 0xFF;          // timing probes (gemm_tc.cuh Params::probe); results are wrong when set
-    tc_stage_cap = (k >> 16) & 0xFF;     // cap on smem stages (0 = as many as fit)
-    mr_tile = ((k >> 24) & 0x3) == 1 ? 32 : (((k >> 24) & 0x3) == 2 ? 64 : (((k >> 24) & 0x3) == 3 ? 128 : 0));   // a7 tile probe
+    if (k < 1 || k > 255) return GMMNLSE_EINVAL;
+    tc_kchunk = k;
+    return 0;
+  }
+  int set_probe(int probe_bits, int stage_cap, int a7_tile) override {
+    if (probe_bits < 0 || stage_cap < 0 || (a7_tile != 0 && a7_tile != 32 && a7_tile != 64 && a7_tile != 128))
+      return GMMNLSE_EINVAL;
+    tc_probe = probe_bits;               // timing probes (gemm_tc.cuh Params::probe); results are wrong when set
+    tc_stage_cap = stage_cap;            // cap on smem stages (0 = as many as fit)
+    mr_tile = a7_tile;                   // a7 samples per CTA (0 = auto)
     return 0;
   }
   int debug_contract(const void* Vin, void* Uout, int n_planes) override {
@@ -1313,6 +1319,10 @@ int gmmnlse_raman_kind(const gmmnlse_plan* plan) { return plan ? plan->raman_kin
 int gmmnlse_lowrank_rank(const gmmnlse_plan* plan) { return plan ? plan->lowrank_rank() : 0; }
 
 int gmmnlse_debug_set_tc_chunk(gmmnlse_plan* plan, int k) { return plan ? plan->set_tc_chunk(k) : GMMNLSE_EINVAL; }
+
+int gmmnlse_debug_set_probe(gmmnlse_plan* plan, int probe_bits, int stage_cap, int a7_tile) {
+  return plan ? plan->set_probe(probe_bits, stage_cap, a7_tile) : GMMNLSE_EINVAL;
+}
 
 void gmmnlse_plan_destroy(gmmnlse_plan* plan) { delete plan; }
 
