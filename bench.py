@@ -235,27 +235,36 @@ def run_gpu(args):
         traffic = json.load(open(tpath)).get(f"cfg{cfg}", {}).get(dom)
     dom_ms, dom_n = prof[dom]
     if dom == "contract":
-        # a6: `achieved` counts the method's useful packed-real flops (2 Q^2 N per plane)
-        # against the TF32 dense peak = measured bf16 sustained x 0.5 (the guide's nominal ratio).  The
-        # kernel reaches fp32-grade accuracy by issuing three TF32 MMAs per product (3xTF32), so the
-        # tensor pipe executes 3x the useful flops: `executed_*` reports that utilisation.
+        # a6: `achieved` counts the method's useful packed-real flops (2 Q^2 N per plane).
+        # The tcgen05 kernels reach fp32-grade accuracy by issuing three MMAs per product on hi/lo splits of the
+        # operands, so the tensor pipe executes 3x the useful flops: `executed_*` reports that utilisation.
+        # Peak: the measured bf16 sustained rate for the kind::f16 forms (fp16 = bf16 rate), x 0.5 (the guide's
+        # nominal ratio) for the TF32 forms.
         ach = fl / (dom_ms * 1e-3) / 1e12
-        peak = peaks["bf16_sustained"] * 0.5
-        tc = w.P * (w.P + 1) // 2 >= 64 and not w.precision
-        roof = dict(bound="tensor", kernel="k_contract_tc (a6, tcgen05 3xTF32)" if tc else "k_contract (a6, fp32 FFMA)",
+        ck = main["ckind"]
+        if ck in (7, 8):
+            kname, peak, mult = "k_contract_h (a6, tcgen05 kind::f16 on fp16 hi/lo splits)", peaks["bf16_sustained"], 3
+            pnote = f"peak = {peaks['source']} bf16 sustained (fp16 runs at the bf16 rate)"
+        elif ck >= 2:
+            kname, peak, mult = "k_contract_tc (a6, tcgen05 3xTF32)", peaks["bf16_sustained"] * 0.5, 3
+            pnote = (f"peak = {peaks['source']} bf16 sustained x 0.5 (TF32 nominal ratio); cuBLAS TF32 8192^3 on the "
+                     "same box: 756 burst / 658 sustained TFLOP/s (profiles/r01c_summary.md)")
+        else:
+            kname, peak, mult = "k_contract (a6, fp32 FFMA)", peaks["bf16_sustained"] * 0.5, 1
+            pnote = f"peak = {peaks['source']} bf16 sustained x 0.5"
+        roof = dict(bound="tensor", kernel=kname,
                     achieved=round(ach, 3), peak=round(peak, 1), unit="TFLOP/s", frac=round(ach / peak, 4),
                     traffic=traffic,
-                    executed_tflops=round((3 if tc else 1) * ach, 2),
-                    executed_frac=round((3 if tc else 1) * ach / peak, 4),
-                    note=f"useful flops 2*Q^2*N per plane; peak = {peaks['source']} bf16 sustained x 0.5 (TF32 nominal "
-                         "ratio); executed = 3x useful (three TF32 MMAs per product); cuBLAS TF32 8192^3 on the same "
-                         "box: 756 burst / 658 sustained TFLOP/s (profiles/r01c_summary.md)")
+                    executed_tflops=round(mult * ach, 2),
+                    executed_frac=round(mult * ach / peak, 4),
+                    note=f"useful flops 2*Q^2*N per plane; {pnote}; executed = {mult}x useful"
+                         + (" (three MMAs per product: hi.lo, lo.hi, hi.hi)" if mult == 3 else ""))
     else:
         ach = by / (dom_ms * 1e-3) / 1e9
         roof = dict(bound="hbm", kernel=dom, achieved=round(ach, 1), peak=peaks["hbm"], unit="GB/s",
                     frac=round(ach / peaks["hbm"], 4), traffic=traffic,
                     note=f"algorithmic bytes / event-timed duration; peak = {peaks['source']} copy bandwidth")
-    if main["ckind"] == 6:
+    if main["ckind"] in (6, 8):
         roof["note"] += "; low-rank form selected: flop rates are dense-equivalent, not executed"
     roof["avg_launch_ms"] = round(dom_ms / dom_n, 4)
     roof["kernels"] = shares
@@ -284,14 +293,23 @@ def run_gpu(args):
     if rank == 0 and world == 1 and args.contraction == 0 and cfg >= 3 and not args.no_variants:
         # SURVEY.md 8(f) NEXT-4, reported beside the headline, never as it: the same propagation with the exact
         # low-rank form of the contraction (BASELINE.json names the dense one, which `value` measures)
+        out["variants"] = {}
         try:
-            lr = measure(cfg, K, Wm, with_events=False, contraction=6)
-            out["variants"] = {"lowrank_contraction": {
+            lr = measure(cfg, K, Wm, with_events=False, contraction=8)
+            out["variants"]["lowrank_contraction"] = {
                 "value": round(lr["z_steps"] / (lr["ms"] * 1e-3), 2), "unit": UNIT, "rank": lr["crank"],
-                "Q": w.P * (w.P + 1) // 2, "ms_per_step": round(lr["ms"] / K, 4),
-                "iterations_per_large_step": round(lr["iters"] / max(lr["large"], 1), 3)}}
+                "Q": w.P * (w.P + 1) // 2, "ms_per_step": round(lr["ms"] / K, 4), "contraction_kind": lr["ckind"],
+                "iterations_per_large_step": round(lr["iters"] / max(lr["large"], 1), 3)}
         except binding.GmmnlseError as exc:
-            out["variants"] = {"lowrank_contraction": {"unavailable": str(exc)}}
+            out["variants"]["lowrank_contraction"] = {"unavailable": str(exc)}
+        try:                                         # the dense contraction on the 3xTF32 kernel (r01c-r01i's default)
+            tf = measure(cfg, K, Wm, with_events=False, contraction=3)
+            out["variants"]["tf32_contraction"] = {
+                "value": round(tf["z_steps"] / (tf["ms"] * 1e-3), 2), "unit": UNIT,
+                "ms_per_step": round(tf["ms"] / K, 4), "contraction_kind": tf["ckind"],
+                "iterations_per_large_step": round(tf["iters"] / max(tf["large"], 1), 3)}
+        except binding.GmmnlseError as exc:
+            out["variants"]["tf32_contraction"] = {"unavailable": str(exc)}
     if rank == 0 and args.all_configs and world == 1:
         others = []
         for c in (1, 2, 3, 4):
@@ -431,7 +449,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--all-configs", action="store_true", help="also time configs 1-4 briefly (other_workloads)")
     ap.add_argument("--contraction", type=int, default=0,
-                    help="options.contraction for every measurement (0 auto = the dense tcgen05 form; 6 low-rank)")
+                    help="options.contraction for every measurement (0 auto = the dense kind::f16 tcgen05 form; 3 dense 3xTF32; "
+                         "6 / 8 low-rank on the TF32 / f16 kernel)")
     ap.add_argument("--no-variants", action="store_true", help="skip the low-rank variant measurement")
     ap.add_argument("--sweep-M", action="store_true", help="serial RK4IP vs MPA(M) on a 10-mode GRIN (Fig. 3 shape)")
     args = ap.parse_args()

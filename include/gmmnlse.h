@@ -41,18 +41,25 @@ typedef struct {                /* pass NULL for defaults                       
   double tol;                   /* MPA convergence threshold, default 1e-6         */
   int    max_iter;              /* cap on iterations per large step; <=0 -> 2*M + 4               */
   int    fixed_iter;            /* >0: run exactly this many iterations per large step (parity)   */
-  int    contraction;           /* a6 kernel: 0 = auto (3 when Q = P(P+1)/2 >= 64, complex64, N % 128 == 0; else 1),
-                                   1 = CUDA-core fp32/fp64 GEMM; tcgen05 3xTF32 forms: 2 = CTA pairs
-                                   (cta_group::2), 3 = single CTA, both operands in shared memory, 4 = single
-                                   CTA, V_hi/V_lo operand in tensor memory, 5 = form 3 on clusters of two CTAs
-                                   that TMA-multicast the S tiles to each other; 6 = exact low-rank form
-                                   (SURVEY.md 8(f) NEXT-4): S_(pl),(mn) = sum_k L_(pl),k L_(mn),k by pivoted
-                                   Cholesky at plan time (Eq. 2 makes S a Gram matrix; rank 153 of 1035 for 45
-                                   Hermite-Gauss modes), two tcgen05 GEMMs Q x R and R x Q instead of Q x Q;
+  int    contraction;           /* a6 kernel: 0 = auto (7 when Q = P(P+1)/2 >= 64, complex64, N % 128 == 0; else 1),
+                                   1 = CUDA-core fp32/fp64 GEMM;
+                                   7 = tcgen05 kind::f16 GEMM on fp16 hi/lo splits of both operands (22 mantissa
+                                   bits, as 3xTF32, at twice its MMA rate): the pair kernels write V scaled by a
+                                   power of two into fp16 range as two fp16 arrays, S is split per row at plan
+                                   time, the scales are undone exactly in the epilogue;
+                                   tcgen05 3xTF32 forms: 2 = CTA pairs (cta_group::2), 3 = single CTA, both
+                                   operands in shared memory, 4 = single CTA, V_hi/V_lo operand in tensor
+                                   memory, 5 = form 3 on clusters of two CTAs that TMA-multicast the S tiles to
+                                   each other;
+                                   6 = exact low-rank form on the 3xTF32 kernel,
+                                   8 = the same on the kind::f16 kernel: S_(pl),(mn) = sum_k L_(pl),k L_(mn),k
+                                   by pivoted Cholesky at plan time (Eq. 2 makes S a Gram matrix; rank 153 of
+                                   1035 for 45 Hermite-Gauss modes), two GEMMs Q x R and R x Q instead of Q x Q;
                                    EUNSUPPORTED if S is not positive semi-definite.  Never chosen by auto:
-                                   BASELINE.json names the dense contraction.  2-6 need complex64 and
-                                   N % 128 == 0 (2, 5: N % 256 == 0), else EUNSUPPORTED.  Forms 2, 4, 5 are
-                                   kept for measurement: none beats form 3 on B200   */
+                                   BASELINE.json names the dense contraction.  2-8 need complex64 and
+                                   N % 128 == 0 (2, 5: N % 256 == 0), else EUNSUPPORTED.  Forms 2-5 are kept
+                                   for measurement: none beats form 3, and form 7 is twice as fast as form 3
+                                   on B200                                     */
   int    raman;                 /* a5 kernel: 0 = auto, 1 = FFT . h~_R . IFFT on the pair streams (any h_R),
                                    2 = one-pole recurrence along t, exact when the samples are a damped
                                    oscillation h_R[j] = Im(c zeta^j) (the tau1/tau2 form); auto picks 2 when
@@ -173,14 +180,17 @@ int gmmnlse_debug_pairs(gmmnlse_plan *plan, const void *A, void *V, int n_planes
  *          [n_planes][Q][N] real of the plan's precision, U must not alias V.
  *   contraction_kind: which a6 kernel the plan selected: 1 CUDA cores, 2 tcgen05 single CTA (operands in
  *          shared memory), 3 tcgen05 CTA pairs, 4 tcgen05 single CTA with the V operand in tensor memory,
- *          5 tcgen05 multicast pairs, 6 low-rank pair of tcgen05 GEMMs.                                                            */
+ *          5 tcgen05 multicast pairs, 6 low-rank pair of 3xTF32 GEMMs, 7 tcgen05 kind::f16 on fp16 hi/lo
+ *          splits, 8 low-rank pair of kind::f16 GEMMs.  With 7 and 8 debug_pairs still writes fp32 V, and
+ *          debug_contract splits the caller's fp32 V into fp16 pairs first (scaled by its own max |V|).                                                            */
 int gmmnlse_debug_contract(gmmnlse_plan *plan, const void *V, void *U, int n_planes);
 int gmmnlse_contraction_kind(const gmmnlse_plan *plan);
-/*   lowrank_rank: rank R of the factorisation when contraction_kind is 6, else 0.                 */
+/*   lowrank_rank: rank R of the factorisation when contraction_kind is 6 or 8, else 0.            */
 int gmmnlse_lowrank_rank(const gmmnlse_plan *plan);
 /*   raman_kind: which a5 kernel the plan selected: 0 none (f_R = 0), 1 FFT, 2 recursive.          */
 int gmmnlse_raman_kind(const gmmnlse_plan *plan);
-/*   set_tc_chunk: k-blocks (16 packed pairs each) a tensor-memory accumulator holds before the epilogue
+/*   set_tc_chunk: k-blocks (16 packed pairs each in the 3xTF32 forms, 32 in the kind::f16 forms: 24
+ *          tensor-core accumulates either way) a tensor-memory accumulator holds before the epilogue
  *          drains it into fp32 registers (default 4); bounds the bias of the tensor core's truncating
  *          accumulate.  1 <= k <= 255.                        */
 int gmmnlse_debug_set_tc_chunk(gmmnlse_plan *plan, int k);

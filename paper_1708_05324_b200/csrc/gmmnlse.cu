@@ -14,6 +14,7 @@
 
 #include "../../include/gmmnlse.h"
 #include "gemm_ts.cuh"
+#include "gemm_h.cuh"
 #include "kernels.cuh"
 
 namespace {
@@ -73,8 +74,8 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 // fp32 tensor map, 128-byte swizzle span (16- or 32-byte atoms); dims/box innermost first; strides in bytes for dims 1..rank-1
-int encode_tmap_f32(CUtensorMap* out, void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides,
-                    const cuuint32_t* box, CUtensorMapSwizzle swz) {
+int encode_tmap(CUtensorMap* out, CUtensorMapDataType dtype, void* base, int rank, const cuuint64_t* dims,
+                const cuuint64_t* strides, const cuuint32_t* box, CUtensorMapSwizzle swz) {
   static EncodeTiledFn fn = nullptr;
   if (!fn) {
     void* ptr = nullptr;
@@ -87,7 +88,7 @@ int encode_tmap_f32(CUtensorMap* out, void* base, int rank, const cuuint64_t* di
     fn = (EncodeTiledFn)ptr;
   }
   const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
-  CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, (cuuint32_t)rank, base, dims, strides, box, estr,
+  CUresult r = fn(out, dtype, (cuuint32_t)rank, base, dims, strides, box, estr,
                   CU_TENSOR_MAP_INTERLEAVE_NONE, swz, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
@@ -95,6 +96,11 @@ int encode_tmap_f32(CUtensorMap* out, void* base, int rank, const cuuint64_t* di
     return GMMNLSE_ECUDA;
   }
   return 0;
+}
+
+int encode_tmap_f32(CUtensorMap* out, void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides,
+                    const cuuint32_t* box, CUtensorMapSwizzle swz) {
+  return encode_tmap(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, base, rank, dims, strides, box, swz);
 }
 
 int ilog2(int n) {
@@ -222,6 +228,20 @@ struct PlanT final : gmmnlse_plan {
   TcGemm lr1, lr2;             // Z = (L^T D) V  [R x Q],  U = L Z  [Q x R]
   T* Zb = nullptr;             // [(M+1)][R][N]
   CUtensorMap tmZ;
+  // kind::f16 forms (gemm_h.cuh; options 7 dense, 8 low-rank): fp16 hi/lo split of both operands
+  struct HGemm {
+    __half *hi = nullptr, *lo = nullptr;
+    float* rscale = nullptr;   // [nrt * NT] 1 / sS[r]
+    CUtensorMap tmHi, tmLo;
+    int rows = 0, K = 0, NT = 0, nrt = 0, KB = 0, stages = 0;
+    double gain = 0;           // max_r sum_q |mat[r][q]|: |out| <= gain max |in|
+  };
+  bool tc_h = false;
+  HGemm hg, hl1, hl2;
+  float* d_vbound = nullptr;   // device scalar: bound on |V| of the current launch
+  float v_gain = 1.f;          // |V| <= v_gain max |A|^2
+  HalfOut cur_ho = {nullptr, 0, 0, 0, nullptr};
+  CUtensorMap tmVh, tmVl, tmZh, tmZl;
   bool tc_ts = false;          // A operand from tensor memory (gemm_ts.cuh)
   bool tc_mc = false;          // clusters of two CTAs multicasting the S tiles (gemm_tc.cuh, MC)
   int tc_cg = 0, tc_NT = 0, tc_nrt = 0, tc_KB = 0, tc_stages = 0, tc_kchunk = 4, tc_probe = 0, tc_stage_cap = 0, n_sm = 0, mr_tile = 0;
@@ -232,6 +252,8 @@ struct PlanT final : gmmnlse_plan {
     cudaFree(V); cudaFree(U); cudaFree(errbuf); cudaFree(d_err); cudaFree(d_io);
     cudaFree(S2hi); cudaFree(S2lo);
     cudaFree(lr1.hi); cudaFree(lr1.lo); cudaFree(lr2.hi); cudaFree(lr2.lo); cudaFree(Zb);
+    for (HGemm* g : {&hg, &hl1, &hl2}) { cudaFree(g->hi); cudaFree(g->lo); cudaFree(g->rscale); }
+    cudaFree(d_vbound);
     cudaFree(gfwd); cudaFree(ginv); cudaFree(Qc); cudaFree(st_kind); cudaFree(st_wk); cudaFree(st_wr); cudaFree(iir_zp); cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
     if (h_err) cudaFreeHost(h_err);
     if (h_in) cudaFreeHost(h_in);
@@ -280,8 +302,11 @@ struct PlanT final : gmmnlse_plan {
     {
       std::vector<cd> hh(N, cd(0, 0));
       if (f_R != 0.0) {
-        for (int k = 0; k < N; ++k) hh[k] = h_R[k];
+        double hsum = 0;
+        for (int k = 0; k < N; ++k) { hh[k] = h_R[k]; hsum += std::fabs(h_R[k]); }
         host_fft(hh, +1);
+        // |(1 - f_R) x + f_R dt (h_R (*) x)| <= v_gain max |x|: the range bound of the fp16 pair streams
+        v_gain = (float)(1.0001 * ((1.0 - f_R) + f_R * dt * hsum));
       }
       for (int k = 0; k < N; ++k) {
         // scalar-mode path: the blended transfer function; general path: ht_R / N alone (weights per stream)
@@ -444,10 +469,10 @@ struct PlanT final : gmmnlse_plan {
     const dim3 grid((Q + 1) / 2, planes);
     if (general)
       k_pair_iir<T, LOG2N, true><<<grid, NT, smem, stream>>>(A, a_ps, Vout, v_ps, pair_m, pair_n, Q, iir_zeta, iir_cs,
-                                                             iir_omf, iir_zp, spec());
+                                                             iir_omf, iir_zp, spec(), cur_ho);
     else
       k_pair_iir<T, LOG2N, false><<<grid, NT, smem, stream>>>(A, a_ps, Vout, v_ps, pair_m, pair_n, Q, iir_zeta,
-                                                              iir_cs, iir_omf, iir_zp, spec());
+                                                              iir_cs, iir_omf, iir_zp, spec(), cur_ho);
     prof_end();
     GM_CUDA(cudaGetLastError());
     return 0;
@@ -533,6 +558,98 @@ struct PlanT final : gmmnlse_plan {
       return 0;
     }
   }
+  // ------------------------------------------------------------------ kind::f16 form (gemm_h.cuh)
+  int h_build(HGemm& g, const std::vector<double>& mat, int rows, int K, int smax) {
+    g.rows = rows; g.K = K;
+    g.nrt = (rows + 207) / 208;
+    g.NT = (((rows + g.nrt - 1) / g.nrt) + 15) / 16 * 16;
+    g.KB = (K + hc::BK - 1) / hc::BK;
+    g.stages = hc::MAX_STAGES;
+    while (g.stages > 1 && hc::smem_bytes(g.NT, g.stages) > (size_t)smax) --g.stages;
+    if (hc::smem_bytes(g.NT, g.stages) > (size_t)smax) return GMMNLSE_EUNSUPPORTED;
+    const int Rp = g.nrt * g.NT, Kp = g.KB * hc::BK;
+    std::vector<__half> hi((size_t)Rp * Kp, __float2half_rn(0.f)), lo((size_t)Rp * Kp, __float2half_rn(0.f));
+    std::vector<float> rs((size_t)Rp, 1.f);
+    g.gain = 0;
+    for (int r = 0; r < rows; ++r) {
+      double amax = 0, asum = 0;
+      for (int q = 0; q < K; ++q) {
+        const double a = std::fabs(mat[(size_t)r * K + q]);
+        amax = std::fmax(amax, a);
+        asum += a;
+      }
+      g.gain = std::fmax(g.gain, asum);
+      int e = 0;
+      if (amax > 0) std::frexp(amax, &e);                       // amax = m 2^e, m in [0.5, 1): scaled row max in [2^13, 2^14)
+      const int sh = amax > 0 ? std::max(-120, std::min(120, hc::V_RANGE_LOG2 - e)) : 0;
+      rs[r] = (float)std::ldexp(1.0, -sh);
+      for (int q = 0; q < K; ++q) {
+        const double v = std::ldexp(mat[(size_t)r * K + q], sh);
+        const __half h = __float2half_rn((float)v);
+        hi[(size_t)r * Kp + q] = h;
+        lo[(size_t)r * Kp + q] = __float2half_rn((float)(v - (double)__half2float(h)));
+      }
+    }
+    g.gain *= 1.0001;
+    GM_TRY(dalloc(&g.hi, hi.size())); GM_TRY(upload(g.hi, hi));
+    GM_TRY(dalloc(&g.lo, lo.size())); GM_TRY(upload(g.lo, lo));
+    GM_TRY(dalloc(&g.rscale, rs.size())); GM_TRY(upload(g.rscale, rs));
+    const cuuint64_t dims[2] = {(cuuint64_t)Kp, (cuuint64_t)Rp};
+    const cuuint64_t strides[1] = {(cuuint64_t)Kp * 2};
+    const cuuint32_t box[2] = {hc::BK, (cuuint32_t)g.NT};
+    GM_TRY(encode_tmap(&g.tmHi, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, g.hi, 2, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_64B));
+    return encode_tmap(&g.tmLo, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, g.lo, 2, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_64B);
+  }
+  // A-operand maps over fp16 split planes: plane = [Krows][N] hi rows then [Krows][N] lo rows
+  int h_a_tmaps(CUtensorMap* mhi, CUtensorMap* mlo, const void* base, int Krows, int planes) {
+    const cuuint64_t dims[3] = {(cuuint64_t)N, (cuuint64_t)Krows, (cuuint64_t)planes};
+    const cuuint64_t strides[2] = {(cuuint64_t)N * 2, (cuuint64_t)Krows * N * 4};
+    const cuuint32_t box[3] = {64, hc::BK, 1};
+    __half* b = reinterpret_cast<__half*>(const_cast<void*>(base));
+    GM_TRY(encode_tmap(mhi, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, b, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B));
+    return encode_tmap(mlo, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, b + (size_t)Krows * N, 3, dims, strides, box,
+                       CU_TENSOR_MAP_SWIZZLE_128B);
+  }
+  int h_run(const HGemm& g, const CUtensorMap& mhi, const CUtensorMap& mlo, int plane0, T* outU, __half* outZ,
+            long long out_ps, int planes, float bound_gain, float zgain) {
+    if constexpr (sizeof(T) != 4) {
+      return GMMNLSE_EUNSUPPORTED;
+    } else {
+      hc::Params prm;
+      prm.U = outU; prm.Zh = outZ; prm.u_plane_stride = out_ps;
+      prm.rscale = g.rscale; prm.vbound = d_vbound; prm.bound_gain = bound_gain; prm.zgain = zgain;
+      prm.Q = g.rows; prm.N = N; prm.NT = g.NT; prm.KB = g.KB; prm.n_rt = g.nrt;
+      prm.t_tiles = N / hc::TM;
+      prm.total_tiles = planes * prm.t_tiles * g.nrt;
+      prm.plane0 = plane0; prm.stages = g.stages;
+      prm.kchunk = tc_kchunk;                                    // k-blocks of 32 q here (16 q in the TF32 forms)
+      prm.probe = tc_probe;
+      if (tc_stage_cap > 0 && tc_stage_cap < prm.stages) prm.stages = tc_stage_cap;
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)std::min(n_sm, prm.total_tiles));
+      cfg.blockDim = dim3(hc::NTHREADS);
+      cfg.dynamicSmemBytes = hc::smem_bytes(g.NT, g.stages);
+      cfg.stream = stream;
+      prof_begin(GMMNLSE_KIND_CONTRACT);
+      cudaError_t e = outZ ? cudaLaunchKernelEx(&cfg, hc::k_contract_h<true>, mhi, mlo, g.tmHi, g.tmLo, prm)
+                           : cudaLaunchKernelEx(&cfg, hc::k_contract_h<false>, mhi, mlo, g.tmHi, g.tmLo, prm);
+      prof_end();
+      GM_CUDA(e);
+      return 0;
+    }
+  }
+  int init_h_common(int smax) {
+    GM_TRY(dalloc(&d_vbound, 1));
+    GM_CUDA(cudaMemset(d_vbound, 0, sizeof(float)));
+    GM_TRY(h_a_tmaps(&tmVh, &tmVl, V, Q, M + 1));
+    if constexpr (sizeof(T) == 4) {
+      GM_CUDA(cudaFuncSetAttribute(hc::k_contract_h<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smax));
+      GM_CUDA(cudaFuncSetAttribute(hc::k_contract_h<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smax));
+    }
+    tc_h = true;
+    return 0;
+  }
+
   // Pivoted Cholesky of the (p<=l) x (m<=n) symmetric matrix Ms = S_plmn (Eq. 2 makes it a Gram matrix of the
   // pair functions F_p F_l, hence positive semi-definite and, for Hermite-Gauss modes, of rank << Q).  Exact to
   // fp64 rounding: stops when the largest remaining diagonal is < 1e-13 of the largest, then verifies
@@ -583,6 +700,15 @@ struct PlanT final : gmmnlse_plan {
         W1[(size_t)k * Q + q] = L[(size_t)k * Q + q] * dbl[q];     // (L^T D)[k][q]
         W2[(size_t)q * R + k] = L[(size_t)k * Q + q];              // L[q][k]
       }
+    if (contraction == 8) {                            // both GEMMs on the kind::f16 kernel, Z kept as fp16 hi / lo
+      GM_TRY(h_build(hl1, W1, R, Q, smax));
+      GM_TRY(h_build(hl2, W2, Q, R, smax));
+      GM_TRY(dalloc(&Zb, (size_t)(M + 1) * R * N));
+      GM_TRY(h_a_tmaps(&tmZh, &tmZl, Zb, R, M + 1));
+      GM_TRY(init_h_common(smax));
+      lowrank = true;
+      return 0;
+    }
     GM_TRY(tc_build(lr1, W1, R, Q, smax));
     GM_TRY(tc_build(lr2, W2, Q, R, smax));
     GM_TRY(dalloc(&Zb, (size_t)(M + 1) * R * N));
@@ -601,7 +727,17 @@ struct PlanT final : gmmnlse_plan {
     } else {
       const bool want = contraction >= 2 || (contraction == 0 && Q >= 64);
       if (!want) return 0;
-      if (contraction == 6) {                          // exact low-rank form (NEXT-4), scalar-mode path only
+      // auto: the kind::f16 form (0.82 ms per 20-plane launch at config 5 against 1.66 ms for the 3xTF32 form)
+      if (contraction == 7 || (contraction == 0 && N % hc::TM == 0)) {   // dense, fp16 hi / lo operands
+        if (N % hc::TM != 0) return GMMNLSE_EUNSUPPORTED;
+        int dev0 = 0, smax0 = 0;
+        GM_CUDA(cudaGetDevice(&dev0));
+        GM_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev0));
+        GM_CUDA(cudaDeviceGetAttribute(&smax0, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev0));
+        GM_TRY(h_build(hg, h_S2, Q, Q, smax0));
+        return init_h_common(smax0);
+      }
+      if (contraction == 6 || contraction == 8) {      // exact low-rank form (NEXT-4), scalar-mode path only
         if (general || N % tc::TM != 0) return GMMNLSE_EUNSUPPORTED;
         int dev0 = 0, smax0 = 0;
         GM_CUDA(cudaGetDevice(&dev0));
@@ -759,12 +895,27 @@ struct PlanT final : gmmnlse_plan {
     }
     prof_begin(GMMNLSE_KIND_PAIR_CONV);
     k_pair_conv<T, LOG2N, RAMAN><<<dim3((Q + 1) / 2, planes), NT, smem, stream>>>(A, a_ps, Vout, v_ps, pair_m,
-                                                                                  pair_n, Q, H, tw, spec());
+                                                                                  pair_n, Q, H, tw, spec(), cur_ho);
     prof_end();
     GM_CUDA(cudaGetLastError());
     return 0;
   }
+  bool own_v(const T* p) const { return p >= V && p < V + (size_t)(M + 1) * QN; }
   int launch_pairs(const C* A, long long a_ps, T* Vout, long long v_ps, int planes) {
+    cur_ho.Vh = nullptr;
+    if constexpr (sizeof(T) == 4) {
+      if (tc_h && own_v(Vout)) {                    // the f16 contraction follows: V as fp16 hi / lo planes
+        GM_CUDA(cudaMemsetAsync(d_vbound, 0, sizeof(float), stream));
+        prof_begin(GMMNLSE_KIND_PAIR_CONV);
+        k_bound_field<T><<<dim3(32, planes), 256, 0, stream>>>(A, a_ps, PN, v_gain, d_vbound);
+        prof_end();
+        GM_CUDA(cudaGetLastError());
+        cur_ho = HalfOut{reinterpret_cast<__half*>(Vout), 2 * QN, QN, N, d_vbound};
+      }
+    }
+    return launch_pairs_impl(A, a_ps, Vout, v_ps, planes);
+  }
+  int launch_pairs_impl(const C* A, long long a_ps, T* Vout, long long v_ps, int planes) {
     if (iir) return launch_pairs_iir(A, a_ps, Vout, v_ps, planes);
     const bool raman = f_R != 0.0;
 #define GM_PC_CASE(L)                                                               \
@@ -786,6 +937,30 @@ struct PlanT final : gmmnlse_plan {
   }
 
   int launch_contract(const T* Vin, T* Uout, int planes) {
+    if constexpr (sizeof(T) == 4) {
+      if (tc_h) {
+        if (planes > M + 1) return GMMNLSE_EINVAL;
+        int plane0 = 0;
+        if (own_v(Vin)) {
+          plane0 = (int)((Vin - V) / QN);
+        } else {                                    // caller's fp32 V: bound, split into the plan's V planes
+          const long long total = (long long)planes * QN;
+          GM_CUDA(cudaMemsetAsync(d_vbound, 0, sizeof(float), stream));
+          prof_begin(GMMNLSE_KIND_CONTRACT);
+          k_bound_real<T><<<592, 256, 0, stream>>>(Vin, total, d_vbound);
+          k_v_encode<<<1184, 256, 0, stream>>>(Vin, QN, total,
+                                               HalfOut{reinterpret_cast<__half*>(V), 2 * QN, QN, N, d_vbound});
+          prof_end();
+          GM_CUDA(cudaGetLastError());
+        }
+        if (lowrank) {
+          GM_TRY(h_run(hl1, tmVh, tmVl, plane0, nullptr, reinterpret_cast<__half*>(Zb), 2LL * lr_R * N, planes, 1.f,
+                       (float)hl1.gain));
+          return h_run(hl2, tmZh, tmZl, 0, Uout, nullptr, QN, planes, (float)hl1.gain, 0.f);
+        }
+        return h_run(hg, tmVh, tmVl, plane0, Uout, nullptr, QN, planes, 1.f, 0.f);
+      }
+    }
     if (lowrank) {
       if (planes > M + 1) return GMMNLSE_EINVAL;
       if (Vin >= V && Vin < V + (size_t)(M + 1) * QN) {
@@ -1100,6 +1275,7 @@ struct PlanT final : gmmnlse_plan {
     return launch_pairs((const C*)A, PN, (T*)Vout, QN, n_planes);
   }
   int contraction_kind() const override {
+    if (tc_h) return lowrank ? 8 : 7;
     return lowrank ? 6 : (tc_cg ? (tc_ts ? 4 : (tc_mc ? 5 : 1 + tc_cg)) : 1);
   }
   int lowrank_rank() const override { return lowrank ? lr_R : 0; }
@@ -1156,7 +1332,7 @@ static int create_plan(gmmnlse_plan** out, int P, int N, int M, double dt, doubl
   if (!(dt > 0) || !(dz > 0) || !(omega0 > 0) || !std::isfinite(n2) || !std::isfinite(f_R)) return GMMNLSE_EINVAL;
   if ((f_R != 0.0) != (h_R != nullptr)) return GMMNLSE_EINVAL;
   if (o.precision != 0 && o.precision != 1) return GMMNLSE_EINVAL;
-  if (o.raman < 0 || o.raman > 2 || o.contraction < 0 || o.contraction > 6) return GMMNLSE_EINVAL;
+  if (o.raman < 0 || o.raman > 2 || o.contraction < 0 || o.contraction > 8) return GMMNLSE_EINVAL;
   if (o.shock && M_PI / dt >= omega0) return GMMNLSE_EINVAL;
   if (!(o.tol > 0)) o.tol = 1e-6;
   for (long long i = 0; i < (long long)P * n_beta; ++i)

@@ -2,6 +2,7 @@
 // T (float: complex64 path, double: complex128 path) and on log2 N.
 #pragma once
 #include "fft.cuh"
+#include "gemm_h.cuh"
 
 namespace gm {
 
@@ -44,6 +45,62 @@ k_fft_rows(const cplx<T>* __restrict__ in, long long in_plane_stride, cplx<T>* _
       });
 }
 
+// fp16 split output of the pair kernels for the kind::f16 contraction (gemm_h.cuh): V' = sV V as Vh + Vl, two
+// fp16 arrays per plane ([Q][N] hi rows, then [Q][N] lo rows: the bytes of the fp32 V plane they replace).
+// sV = hc::v_scale(*vbound): a power of two that puts the launch's largest |V| below 2^14.  Vh == nullptr: fp32 V.
+struct HalfOut {
+  __half* Vh;
+  long long plane_stride;      // halves between planes (2 Q N)
+  long long lo_offset;         // halves from a hi row to its lo row (Q N)
+  int N;
+  const float* vbound;
+  __device__ __forceinline__ void store(int j, int q, int n, float v) const {
+    const float x = v * hc::v_scale(*vbound, false);
+    const __half h = __float2half_rn(x);
+    __half* d = Vh + j * plane_stride + (long long)q * N + n;
+    d[0] = h;
+    d[lo_offset] = __float2half_rn(x - __half2float(h));
+  }
+};
+
+// bound[0] = max(bound[0], gain * max |A|^2) over `planes` planes of n complex samples (bound zeroed before the
+// launch; non-negative floats order like their bit patterns).  |Re / Im (A_m A_n*)| <= max |A|^2, and `gain`
+// bounds the instantaneous + Raman-convolved weights of a stream, so bound >= every |V| the pair kernel writes.
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_bound_field(const cplx<T>* __restrict__ A, long long a_plane_stride, long long n, float gain, float* bound) {
+  const cplx<T>* a = A + blockIdx.y * a_plane_stride;
+  float m = 0.f;
+  for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256) {
+    const cplx<T> v = a[i];
+    m = fmaxf(m, (float)(v.x * v.x + v.y * v.y));
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, d));
+  if ((threadIdx.x & 31) == 0 && m > 0.f) atomicMax(reinterpret_cast<unsigned int*>(bound), __float_as_uint(m * gain));
+}
+// same for an array of n real samples: bound[0] = max(bound[0], max |V|)
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_bound_real(const T* __restrict__ V, long long n, float* bound) {
+  float m = 0.f;
+  for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256)
+    m = fmaxf(m, fabsf((float)V[i]));
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, d));
+  if ((threadIdx.x & 31) == 0 && m > 0.f) atomicMax(reinterpret_cast<unsigned int*>(bound), __float_as_uint(m * 1.0001f));
+}
+
+// fp32 V[planes][Q][N] -> fp16 split planes (for a caller-supplied V: gmmnlse_debug_contract)
+__global__ void __launch_bounds__(256)
+k_v_encode(const float* __restrict__ Vin, long long QN, long long total, HalfOut ho) {
+  for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < total; i += (long long)gridDim.x * 256) {
+    const int j = (int)(i / QN);
+    const long long r = i - j * QN;
+    ho.store(j, (int)(r / ho.N), (int)(r % ho.N), Vin[i]);
+  }
+}
+
 // Per-stream description of the general form of Eq. 1 (S^K != S^R, complex, no symmetry; NEXT-2): stream q is
 // Re (kind 0) or Im (kind 1) of A_m A_n*, weighted wk[q] on its instantaneous part and wr[q] on its Raman-
 // convolved part.  All-null = the scalar-mode path (every stream Re, weights folded into H / cs, omf).
@@ -68,7 +125,7 @@ template <typename T, int LOG2N, bool HAS_RAMAN>
 __global__ void __launch_bounds__((1 << LOG2N) / 16)
 k_pair_conv(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restrict__ V, long long v_plane_stride,
             const int* __restrict__ pair_m, const int* __restrict__ pair_n, int Q,
-            const cplx<T>* __restrict__ H, const cplx<T>* __restrict__ tw, StreamSpec<T> gs) {
+            const cplx<T>* __restrict__ H, const cplx<T>* __restrict__ tw, StreamSpec<T> gs, HalfOut ho) {
   constexpr int N = 1 << LOG2N, NT = N / 16;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
@@ -94,6 +151,9 @@ k_pair_conv(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restri
       const cplx<T> z = mk(pair_stream(a, b, im0), has1 ? pair_stream(c, d, im1) : (T)0);
       if constexpr (HAS_RAMAN) {
         sm[fft_pad(n)] = z;
+      } else if (ho.Vh) {
+        ho.store(j, q0, n, (float)(wk * z.x));
+        if (has1) ho.store(j, q1, n, (float)(wk * z.y));
       } else {
         v0[n] = wk * z.x;
         if (has1) v1[n] = wk * z.y;
@@ -116,8 +176,13 @@ k_pair_conv(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restri
     block_fft<T, LOG2N, -1>(
         sm, tw, [&](int k) { return sm[fft_pad(k)]; },
         [&](int n, cplx<T> v) {
-          v0[n] = v.x;
-          if (has1) v0[N + n] = v.y;
+          if (ho.Vh) {
+            ho.store(j, q0, n, (float)v.x);
+            if (has1) ho.store(j, q1, n, (float)v.y);
+          } else {
+            v0[n] = v.x;
+            if (has1) v0[N + n] = v.y;
+          }
         });
   }
 }
@@ -136,7 +201,7 @@ template <typename T, int LOG2N, bool GEN>
 __global__ void __launch_bounds__((1 << LOG2N) / 16)
 k_pair_iir(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restrict__ V, long long v_plane_stride,
            const int* __restrict__ pair_m, const int* __restrict__ pair_n, int Q, cplx<T> zeta, cplx<T> cs, T omf,
-           const cplx<T>* __restrict__ zp, StreamSpec<T> gs) {
+           const cplx<T>* __restrict__ zp, StreamSpec<T> gs, HalfOut ho) {
   constexpr int N = 1 << LOG2N, NT = N / 16, NW = (NT + 31) / 32;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);         // fft_smem_elems(N) + 2 * (NW + 1) complex
@@ -218,6 +283,26 @@ k_pair_iir(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restric
     sm[17 * tid + e] = mk(omf * x[e].x + cs.x * w0.y + cs.y * w0.x, omf * x[e].y + cs.x * w1.y + cs.y * w1.x);
   }
   __syncthreads();
+  if (ho.Vh) {                                                // fp16 hi / lo pairs, two samples per thread and store
+    const float sv = hc::v_scale(*ho.vbound, false);
+    __half2* h0 = reinterpret_cast<__half2*>(ho.Vh + j * ho.plane_stride + (long long)q0 * N);
+    __half2* l0 = reinterpret_cast<__half2*>(ho.Vh + j * ho.plane_stride + ho.lo_offset + (long long)q0 * N);
+#pragma unroll 4
+    for (int e = 0; e < 8; ++e) {
+      const int n2 = tid + e * NT;                            // samples 2 n2, 2 n2 + 1
+      const cplx<T> a = sm[fft_pad(2 * n2)], b = sm[fft_pad(2 * n2 + 1)];
+      const float2 s0 = make_float2((float)a.x * sv, (float)b.x * sv), s1 = make_float2((float)a.y * sv, (float)b.y * sv);
+      const __half2 hh0 = __float22half2_rn(s0), hh1 = __float22half2_rn(s1);
+      const float2 f0 = __half22float2(hh0), f1 = __half22float2(hh1);
+      h0[n2] = hh0;
+      l0[n2] = __float22half2_rn(make_float2(s0.x - f0.x, s0.y - f0.y));
+      if (has1) {
+        h0[N / 2 + n2] = hh1;
+        l0[N / 2 + n2] = __float22half2_rn(make_float2(s1.x - f1.x, s1.y - f1.y));
+      }
+    }
+    return;
+  }
   T* v0 = V + j * v_plane_stride + (long long)q0 * N;
 #pragma unroll 4
   for (int e = 0; e < 16; ++e) {
