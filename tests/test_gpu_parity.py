@@ -775,12 +775,13 @@ def test_long_propagation_vs_stored_oracle_rk4ip(B, fname, cfg, tol_rk, tol_mpa)
     assert abs(pn - pn_ref) <= TOL_DRIFT
 
 
-def test_long_mpa_vs_stored_oracle_mpa(B):
-    """Config 3 at full shape over 20 large steps against the oracle's own MPA (O4, stored): same scheme, so the
-    distance is fp32 rounding plus at most one iteration of difference per large step, not the O(dz^2) of the
-    RK4IP comparison."""
-    mg, meta, data = _golden("config3_mpa_200steps.txt")
-    w = W.make_config(3)
+@pytest.mark.parametrize("cfg,fname", [(3, "config3_mpa_200steps.txt"), (5, "config5_mpa_40steps.txt")])
+def test_long_mpa_vs_stored_oracle_mpa(B, cfg, fname):
+    """Configs 3 (20 large steps) and 5 (the shape bench.py times, 2 large steps) at full shape against the oracle's
+    own MPA (O4, stored): same scheme, so the distance is fp32 rounding plus at most one iteration of difference
+    per large step, not the O(dz^2) of the RK4IP comparison."""
+    mg, meta, data = _golden(fname)
+    w = W.make_config(cfg)
     L = float(meta["L_m"])
     A_in = w.A0.astype(np.complex64).astype(np.complex128)
     assert mg.fingerprint_matches(meta, w, A_in), "golden is stale: inputs changed"
