@@ -402,9 +402,12 @@ def test_lowrank_form_rank_operator_and_propagation(B, kind):
 
 
 def test_contraction_auto_selects_tensor_cores_for_large_P(B):
-    w = W.make_config(3, N=1024)
+    w = W.make_config(4, N=1024)                       # Q = 210: kind::f16
     with B.plan_from_workload(w) as plan:
         assert plan.contraction_kind() == 7
+    w = W.make_config(3, N=1024)                       # Q = 120: 3xTF32 (the f16 form's extra launches do not pay)
+    with B.plan_from_workload(w) as plan:
+        assert plan.contraction_kind() == 2
     w = W.make_config(2, N=1024)
     with B.plan_from_workload(w) as plan:
         assert plan.contraction_kind() == 1
