@@ -158,7 +158,8 @@ def run_gpu(args):
         tdt = torch.complex128 if w.precision else torch.complex64
         A0 = w.A0.astype(cdt)
         A0 = replica_launch_field(A0, seed_offset, workloads.SEED_BASE)
-        plan = binding.plan_from_workload(w, contraction=args.contraction if contraction is None else contraction)
+        plan = binding.plan_from_workload(w, contraction=args.contraction if contraction is None else contraction,
+                                          graph=1 if args.host_loop else 0)
         ckind, crank = plan.contraction_kind(), plan.lowrank_rank()
         stream = torch.cuda.current_stream()
         A = torch.from_numpy(A0).cuda()
@@ -194,6 +195,7 @@ def run_gpu(args):
         if with_events:
             plan.profile_enable(False)
         s1, l1 = plan.stats(), plan.launch_count()
+        loop_kind = plan.loop_kind()
         barrier()
         ms = max_over_ranks(ms, world, "cuda")
         finite = bool(np.isfinite(h_a).all()) if host_path else bool(torch.isfinite(torch.view_as_real(A)).all())
@@ -201,18 +203,21 @@ def run_gpu(args):
         it = s1["iterations"] - s0["iterations"]
         ls = s1["large_steps"] - s0["large_steps"]
         return dict(w=w, ms=ms, wall_ms=wall_ms, z_steps=K * n_large * w.M, iters=it, large=ls, prof=prof,
+                    loop=loop_kind,
                     launches=l1 - l0, not_conv=s1["not_converged"] - s0["not_converged"], finite=finite,
                     bytes_io=int(A0.nbytes), ckind=ckind, crank=crank)
 
     cfg, K, Wm = args.config, args.steps, max(args.warmup, 3)
     peaks = _peaks()
+    # `value`: the call a user makes (no per-kernel events; the MPA loop runs on the device as a CUDA graph).
+    # `main`: the same region with the library's per-kernel CUDA events on (host loop), for the roofline object.
     with ClockSampler(local) as clk:
+        plain = measure(cfg, K, Wm, with_events=False, seed_offset=rank)
         main = measure(cfg, K, Wm, with_events=True, seed_offset=rank)
     clocks = clk.summary()
-    plain = measure(cfg, K, Wm, with_events=False, seed_offset=rank)          # same region, no per-kernel events
     e2e = measure(cfg, K, Wm, with_events=False, host_path=True, seed_offset=rank)
     w = main["w"]
-    value = world * main["z_steps"] / (main["ms"] * 1e-3)
+    value = world * plain["z_steps"] / (plain["ms"] * 1e-3)
 
     # ---- roofline of the dominant kernel class, from the per-launch CUDA events of the timed region
     prof = {k: v for k, v in main["prof"].items() if v[1] > 0}
@@ -271,7 +276,7 @@ def run_gpu(args):
 
     out = {
         "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
-        "ms_per_step": round(main["ms"] / K, 4), "higher_is_better": True, "scaling": "weak",
+        "ms_per_step": round(plain["ms"] / K, 4), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "c128" if w.precision else "c64 (f32)", "data": "synthetic",
         "config": {"workload": w.name, "baseline_config_index": cfg, "P": w.P, "N": w.N, "M": w.M,
                    "dz_m": w.dz, "z_steps_per_step": LARGE_PER_STEP[cfg] * w.M,
@@ -279,17 +284,19 @@ def run_gpu(args):
                    "l2": "working set per MPA iteration exceeds L2 (no flush)" if cfg >= 4 else
                          "working set is L2-resident by nature of the workload (no flush); not an HBM measurement"},
         "mode_sample_updates_per_s": round(value * w.P * w.N, 1),
-        "iterations_per_large_step": round(main["iters"] / max(main["large"], 1), 3),
-        "not_converged": main["not_conv"], "finite": main["finite"],
-        "ms_per_step_without_kernel_events": round(plain["ms"] / K, 4),
+        "iterations_per_large_step": round(plain["iters"] / max(plain["large"], 1), 3),
+        "not_converged": plain["not_conv"], "finite": plain["finite"] and main["finite"],
+        "ms_per_step_with_kernel_events": round(main["ms"] / K, 4),
         "e2e": {"value": round(world * e2e["z_steps"] / (e2e["ms"] * 1e-3), 2), "unit": UNIT,
-                "h2d_bytes_per_step": e2e["bytes_io"], "d2h_bytes_per_step": e2e["bytes_io"] + 8 * e2e["iters"] // K},
-        "gpu_launches": main["launches"],
+                "h2d_bytes_per_step": e2e["bytes_io"], "d2h_bytes_per_step": e2e["bytes_io"] + (24 if e2e["loop"] == 1 else 8 * e2e["iters"] // K)},
+        "gpu_launches": plain["launches"],
         "clocks": clocks, "roofline": roof,
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = oracle_sample(cfg, 1, 0)
     out["config"]["contraction_kind"] = main["ckind"]
+    out["config"]["mpa_loop"] = ("device (one CUDA graph per large step, WHILE node)" if plain["loop"] == 1
+                                 else "host (read-back per iteration)")
     if rank == 0 and world == 1 and args.contraction == 0 and cfg >= 3 and not args.no_variants:
         # SURVEY.md 8(f) NEXT-4, reported beside the headline, never as it: the same propagation with the exact
         # low-rank form of the contraction (BASELINE.json names the dense one, which `value` measures)
@@ -318,7 +325,8 @@ def run_gpu(args):
             m = measure(c, 3, 3, with_events=False)
             others.append({"workload": m["w"].name, "z_steps_per_s": round(m["z_steps"] / (m["ms"] * 1e-3), 1),
                            "ms_per_step": round(m["ms"] / 3, 4), "z_steps_per_step": LARGE_PER_STEP[c] * m["w"].M,
-                           "iterations_per_large_step": round(m["iters"] / max(m["large"], 1), 3)})
+                           "iterations_per_large_step": round(m["iters"] / max(m["large"], 1), 3),
+                           "mpa_loop": "device" if m["loop"] == 1 else "host"})
         out["other_workloads"] = others
     if rank == 0:
         print(json.dumps(out))
@@ -448,6 +456,9 @@ def main():
     ap.add_argument("--impl", default="graft", choices=["graft", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--all-configs", action="store_true", help="also time configs 1-4 briefly (other_workloads)")
+    ap.add_argument("--host-loop", action="store_true",
+                    help="options.graph = 1: take the MPA convergence decision on the host (read-back per iteration) "
+                         "instead of in the CUDA-graph WHILE loop")
     ap.add_argument("--contraction", type=int, default=0,
                     help="options.contraction for every measurement (0 auto = the dense kind::f16 tcgen05 form; 3 dense 3xTF32; "
                          "6 / 8 low-rank on the TF32 / f16 kernel)")

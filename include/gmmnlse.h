@@ -66,6 +66,15 @@ typedef struct {                /* pass NULL for defaults                       
                                    oscillation h_R[j] = Im(c zeta^j) (the tau1/tau2 form); auto picks 2 when
                                    all N samples fit that form to 1e-10 of the peak, else 1; 2 on a response
                                    that does not fit is EUNSUPPORTED                                */
+  int    graph;                 /* MPA iteration loop: 0 (default) = on the device -- every full
+                                   large step is one CUDA graph (iteration 0, a WHILE node whose body is one
+                                   further iteration, a11); the convergence test err < tol and the max_iter cap
+                                   are evaluated by a kernel that sets the node's condition, and the host reads
+                                   the counters back once per gmmnlse_propagate call.  1 = host loop: one 8-byte
+                                   D2H and a stream synchronise per iteration.  Same kernels, same arithmetic,
+                                   same iteration counts.  The first large step of a plan, a ragged last step
+                                   ((L/dz) mod M planes) and calls under gmmnlse_profile_enable use the host
+                                   loop in either case                                               */
 } gmmnlse_options;
 
 /* Build a plan: precompute D_w^(p), the rotation tables exp(+-D_w j dz) (j = 0..M) in
@@ -106,9 +115,12 @@ int gmmnlse_plan_create_general(gmmnlse_plan **out, int P, int N, int M, double 
  *   L            [m], an integer multiple of dz (1e-9 relative) else EINVAL; the last large
  *                step uses (L/dz) mod M planes.
  *   stream       cudaStream_t as void* (NULL = the plan's current stream).  Work is enqueued
- *                on it; the call returns after the last convergence decision was read back
- *                (one 8-byte D2H per iteration) -- A_out is complete only
- *                after the stream is synchronised.                                         */
+ *                on it.  Device loop (options.graph = 0): the call returns after one
+ *                read-back of the loop counters that follows the last kernel, so A_out is
+ *                complete on return.  Host loop: it returns after the last convergence
+ *                decision was read back (one 8-byte D2H per iteration) and A_out is
+ *                complete only after the stream is synchronised.  `stream` must not be
+ *                capturing.                                                                */
 int gmmnlse_propagate(gmmnlse_plan *plan, const void *A_in, double L, void *A_out, void *stream);
 
 /* Same as gmmnlse_propagate but A_in / A_out are HOST [P][N] buffers of the plan's
@@ -188,6 +200,10 @@ int gmmnlse_debug_contract(gmmnlse_plan *plan, const void *V, void *U, int n_pla
 int gmmnlse_contraction_kind(const gmmnlse_plan *plan);
 /*   lowrank_rank: rank R of the factorisation when contraction_kind is 6 or 8, else 0.            */
 int gmmnlse_lowrank_rank(const gmmnlse_plan *plan);
+/*   loop_kind: how the MPA iteration loop of the last gmmnlse_propagate ran: 1 = on the device (CUDA-graph
+ *          WHILE node, options.graph = 0), 0 = host loop only so far, -1 = the graph could not be built on this
+ *          driver and the plan fell back to the host loop (gmmnlse_last_cuda_error() says why).          */
+int gmmnlse_loop_kind(const gmmnlse_plan *plan);
 /*   raman_kind: which a5 kernel the plan selected: 0 none (f_R = 0), 1 FFT, 2 recursive.          */
 int gmmnlse_raman_kind(const gmmnlse_plan *plan);
 /*   set_tc_chunk: k-blocks (16 packed pairs each in the 3xTF32 forms, 32 in the kind::f16 forms: 24

@@ -27,7 +27,7 @@ class GmmnlseError(RuntimeError):
 
 class Options(C.Structure):
     _fields_ = [("precision", C.c_int), ("shock", C.c_int), ("tol", C.c_double), ("max_iter", C.c_int),
-                ("fixed_iter", C.c_int), ("contraction", C.c_int), ("raman", C.c_int)]
+                ("fixed_iter", C.c_int), ("contraction", C.c_int), ("raman", C.c_int), ("graph", C.c_int)]
 
 
 _LIB = None
@@ -60,6 +60,7 @@ SIGNATURES = {
     "gmmnlse_contraction_kind": (C.c_int, [C.c_void_p]),
     "gmmnlse_raman_kind": (C.c_int, [C.c_void_p]),
     "gmmnlse_lowrank_rank": (C.c_int, [C.c_void_p]),
+    "gmmnlse_loop_kind": (C.c_int, [C.c_void_p]),
     "gmmnlse_debug_set_tc_chunk": (C.c_int, [C.c_void_p, C.c_int]),
     "gmmnlse_debug_set_probe": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int]),
     "gmmnlse_plan_destroy": (None, [C.c_void_p]),
@@ -111,7 +112,7 @@ class Plan:
     """Owner of one ``gmmnlse_plan``; methods mirror the C calls one to one."""
 
     def __init__(self, P, N, M, dt, dz, beta, S, f_R, h_R, omega0, n2, *, precision=0, shock=True,
-                 tol=1e-6, max_iter=0, fixed_iter=0, contraction=0, raman=0):
+                 tol=1e-6, max_iter=0, fixed_iter=0, contraction=0, raman=0, graph=0):
         self._lib = load_library()
         self._h = C.c_void_p()
         beta = np.ascontiguousarray(beta, dtype=np.float64).reshape(P, -1)
@@ -128,7 +129,8 @@ class Plan:
         hR = None if h_R is None else np.ascontiguousarray(h_R, dtype=np.float64)
         if hR is not None and hR.size != N:
             raise GmmnlseError(EINVAL, "h_R must hold N samples")
-        opt = Options(int(precision), int(bool(shock)), float(tol), int(max_iter), int(fixed_iter), int(contraction), int(raman))
+        opt = Options(int(precision), int(bool(shock)), float(tol), int(max_iter), int(fixed_iter), int(contraction),
+                      int(raman), int(graph))
         hp = None if hR is None else hR.ctypes.data_as(_DP)
         if general:
             st = self._lib.gmmnlse_plan_create_general(
@@ -229,6 +231,9 @@ class Plan:
 
     def lowrank_rank(self) -> int:
         return int(self._lib.gmmnlse_lowrank_rank(self._h))
+
+    def loop_kind(self) -> int:
+        return int(self._lib.gmmnlse_loop_kind(self._h))
 
     def raman_kind(self) -> int:
         """0 = no Raman term, 1 = FFT convolution, 2 = recursive (damped-oscillator) form."""

@@ -114,7 +114,8 @@ int ilog2(int n) {
 // ============================================================================================
 struct gmmnlse_plan {
   int P = 0, N = 0, M = 0, log2N = 0, Q = 0, precision = 0, shock = 1, max_iter = 0, fixed_iter = 0;
-  int contraction = 0, raman = 0;
+  int contraction = 0, raman = 0, graph = 0;
+  int loop_state = 0;                      // 0 host loop so far, 1 device loop (CUDA graph) in use, -1 graph build failed
   // general form of Eq. 1 (gmmnlse_plan_create_general): separate, possibly complex tensors, no symmetry
   bool general = false, gen_complex = false;
   const double* gen_SR = nullptr;          // host, valid during init only
@@ -176,6 +177,7 @@ struct gmmnlse_plan {
   virtual int set_probe(int probe_bits, int stage_cap, int a7_tile) = 0;
   virtual int raman_kind() const = 0;
   virtual int lowrank_rank() const = 0;
+  virtual void drop_loop_graph() = 0;
 };
 
 namespace {
@@ -198,6 +200,14 @@ struct PlanT final : gmmnlse_plan {
   void *h_in = nullptr, *h_out = nullptr;          // pinned staging for propagate_host
   C* d_io = nullptr;
   std::map<int, double2*> EM_ragged;
+  // device-side MPA loop: one CUDA graph per full large step = iteration 0, a WHILE node whose body is one further
+  // iteration, a11.  k_err_finalize_loop takes the convergence decision; the host reads LoopStats once per call.
+  cudaGraph_t lg = nullptr;
+  cudaGraphExec_t lg_exec = nullptr;
+  cudaStream_t cap_stream = nullptr;
+  LoopStats *d_stats = nullptr, *h_stats = nullptr;
+  long long lg_c0 = 0, lg_cb = 0, lg_ca = 0;       // kernel launches in iteration 0, the loop body, a11
+  bool warmed = false;                             // one host-loop large step has run (function attributes set)
   long long PN = 0, QN = 0;
   // NEXT-3: small-signal gain g_p (joins D as its real part) and constant linear coupling Q_np
   std::vector<double> gain;                // [P], 1/m; empty = none
@@ -254,6 +264,10 @@ struct PlanT final : gmmnlse_plan {
     cudaFree(lr1.hi); cudaFree(lr1.lo); cudaFree(lr2.hi); cudaFree(lr2.lo); cudaFree(Zb);
     for (HGemm* g : {&hg, &hl1, &hl2}) { cudaFree(g->hi); cudaFree(g->lo); cudaFree(g->rscale); }
     cudaFree(d_vbound);
+    drop_loop_graph();
+    if (cap_stream) cudaStreamDestroy(cap_stream);
+    cudaFree(d_stats);
+    if (h_stats) cudaFreeHost(h_stats);
     cudaFree(gfwd); cudaFree(ginv); cudaFree(Qc); cudaFree(st_kind); cudaFree(st_wk); cudaFree(st_wr); cudaFree(iir_zp); cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
     if (h_err) cudaFreeHost(h_err);
     if (h_in) cudaFreeHost(h_in);
@@ -1049,6 +1063,38 @@ struct PlanT final : gmmnlse_plan {
     return 0;
   }
 
+  // a3-a9 of one MPA iteration over planes j0..Mc (j0 = 0 on the first iterate, which starts every plane from psi_0)
+  int enqueue_iteration(int Mc, bool first) {
+    const int j0 = first ? 0 : 1, np = Mc + 1 - j0;
+    const unsigned sblocks = (unsigned)((PN + 255) / 256);
+    // a3: A_j(t) = F^-1{psi_j exp(+D j dz)}; first iterate psi_j = psi_0
+    GM_TRY(launch_fft(-1, first ? psi : psi + j0 * PN, first ? 0 : PN, At + j0 * PN, PN, E + j0 * PN, nullptr,
+                      nullptr, PN, (T)(1.0 / N), P, np, gfwd ? gfwd + j0 * P : nullptr));
+    GM_TRY(nonlinear_term(j0, np));                                        // a4-a7
+    // a8: G_j = K(w) exp(-D j dz) F{N_p}
+    GM_TRY(launch_fft(+1, G + j0 * PN, PN, G + j0 * PN, PN, nullptr, Kw, E + j0 * PN, PN, (T)1, P, np,
+                      ginv ? ginv + j0 * P : nullptr));
+    if (Qc)                                                                 // + exp(-D j dz) i Q^T (psi_j exp(D j dz))
+      GM_TRY(launch_couple(first ? psi : psi + j0 * PN, first ? 0 : PN, E + j0 * PN,
+                           gfwd ? gfwd + j0 * P : nullptr, ginv ? ginv + j0 * P : nullptr, G + j0 * PN, np));
+    // a9 + a10
+    prof_begin(GMMNLSE_KIND_SCAN);
+    k_trapz_scan<T><<<sblocks, 256, sizeof(double) * 2 * (Mc + 1), stream>>>(psi, G, psi, PN, Mc, (T)dz,
+                                                                             first ? 1 : 0, errbuf, PN);
+    prof_end();
+    GM_CUDA(cudaGetLastError());
+    return 0;
+  }
+
+  int enqueue_advance(int Mc, const double2* EM) {                           // a11
+    const unsigned sblocks = (unsigned)((PN + 255) / 256);
+    prof_begin(GMMNLSE_KIND_ADVANCE);
+    k_advance<T><<<sblocks, 256, 0, stream>>>(psi0_d, psi, G, PN, Mc, dz, EM, PN);
+    prof_end();
+    GM_CUDA(cudaGetLastError());
+    return 0;
+  }
+
   int large_step(int Mc, bool* converged) {
     double2* EM = EM_d;
     if (Mc != M) {
@@ -1065,24 +1111,8 @@ struct PlanT final : gmmnlse_plan {
     const int cap = fixed_iter > 0 ? fixed_iter : max_iter;
     int it = 0;
     *converged = false;
-    const unsigned sblocks = (unsigned)((PN + 255) / 256);
     while (true) {
-      const int j0 = it == 0 ? 0 : 1, np = Mc + 1 - j0;
-      // a3: A_j(t) = F^-1{psi_j exp(+D j dz)}; first iterate psi_j = psi_0
-      GM_TRY(launch_fft(-1, it == 0 ? psi : psi + j0 * PN, it == 0 ? 0 : PN, At + j0 * PN, PN, E + j0 * PN, nullptr,
-                        nullptr, PN, (T)(1.0 / N), P, np, gfwd ? gfwd + j0 * P : nullptr));
-      GM_TRY(nonlinear_term(j0, np));                                        // a4-a7
-      // a8: G_j = K(w) exp(-D j dz) F{N_p}
-      GM_TRY(launch_fft(+1, G + j0 * PN, PN, G + j0 * PN, PN, nullptr, Kw, E + j0 * PN, PN, (T)1, P, np,
-                        ginv ? ginv + j0 * P : nullptr));
-      if (Qc)                                                                 // + exp(-D j dz) i Q^T (psi_j exp(D j dz))
-        GM_TRY(launch_couple(it == 0 ? psi : psi + j0 * PN, it == 0 ? 0 : PN, E + j0 * PN,
-                             gfwd ? gfwd + j0 * P : nullptr, ginv ? ginv + j0 * P : nullptr, G + j0 * PN, np));
-      // a9 + a10
-      prof_begin(GMMNLSE_KIND_SCAN);
-      k_trapz_scan<T><<<sblocks, 256, sizeof(double) * 2 * (Mc + 1), stream>>>(psi, G, psi, PN, Mc, (T)dz,
-                                                                               it == 0 ? 1 : 0, errbuf, PN);
-      prof_end();
+      GM_TRY(enqueue_iteration(Mc, it == 0));
       prof_begin(GMMNLSE_KIND_MISC);
       k_err_finalize<<<1, 32, 0, stream>>>(errbuf, Mc, d_err);
       prof_end();
@@ -1099,12 +1129,99 @@ struct PlanT final : gmmnlse_plan {
       if (last_err < tol) { *converged = true; break; }
       if (it >= cap) break;
     }
-    // a11
-    prof_begin(GMMNLSE_KIND_ADVANCE);
-    k_advance<T><<<sblocks, 256, 0, stream>>>(psi0_d, psi, G, PN, Mc, dz, EM, PN);
-    prof_end();
-    GM_CUDA(cudaGetLastError());
+    GM_TRY(enqueue_advance(Mc, EM));
     ++n_large;
+    if (Mc == M) warmed = true;
+    return 0;
+  }
+
+  // ---- device-side loop (options.graph = 0): the large step above as one CUDA graph, no host decision inside
+  void drop_loop_graph() override {
+    if (lg_exec) cudaGraphExecDestroy(lg_exec);
+    if (lg) cudaGraphDestroy(lg);
+    lg_exec = nullptr;
+    lg = nullptr;
+    if (loop_state > 0) loop_state = 0;
+  }
+
+  int capture_loop_graph() {     // runs with `stream` = cap_stream
+    const int cap = fixed_iter > 0 ? fixed_iter : max_iter;
+    const cudaStreamCaptureMode mode = cudaStreamCaptureModeRelaxed;
+    cudaGraph_t got = nullptr;
+    GM_CUDA(cudaGraphCreate(&lg, 0));
+    cudaGraphConditionalHandle handle;
+    GM_CUDA(cudaGraphConditionalHandleCreate(&handle, lg, 0, 0));
+    auto finalize = [&]() -> int {
+      prof_begin(GMMNLSE_KIND_MISC);
+      k_err_finalize_loop<<<1, 32, 0, stream>>>(errbuf, M, d_err, tol, cap, fixed_iter > 0 ? 1 : 0, handle, d_stats);
+      prof_end();
+      GM_CUDA(cudaGetLastError());
+      return 0;
+    };
+    // iteration 0
+    GM_CUDA(cudaStreamBeginCaptureToGraph(stream, lg, nullptr, nullptr, 0, mode));
+    GM_CUDA(cudaMemsetAsync(&d_stats->it, 0, sizeof(int), stream));
+    long long c = n_launch;
+    GM_TRY(enqueue_iteration(M, true));
+    GM_TRY(finalize());
+    lg_c0 = n_launch - c;
+    cudaStreamCaptureStatus cs;
+    unsigned long long id = 0;
+    const cudaGraphNode_t* deps = nullptr;
+    size_t nd = 0;
+    GM_CUDA(cudaStreamGetCaptureInfo(stream, &cs, &id, &got, &deps, &nd));
+    std::vector<cudaGraphNode_t> tail(deps, deps + nd);
+    GM_CUDA(cudaStreamEndCapture(stream, &got));
+    // while (continue) { one further iteration }
+    cudaGraphNodeParams cp = {};
+    cp.type = cudaGraphNodeTypeConditional;
+    cp.conditional.handle = handle;
+    cp.conditional.type = cudaGraphCondTypeWhile;
+    cp.conditional.size = 1;
+    cudaGraphNode_t loop_node;
+    GM_CUDA(cudaGraphAddNode(&loop_node, lg, tail.data(), tail.size(), &cp));
+    cudaGraph_t body = cp.conditional.phGraph_out[0];
+    GM_CUDA(cudaStreamBeginCaptureToGraph(stream, body, nullptr, nullptr, 0, mode));
+    c = n_launch;
+    GM_TRY(enqueue_iteration(M, false));
+    GM_TRY(finalize());
+    lg_cb = n_launch - c;
+    GM_CUDA(cudaStreamEndCapture(stream, &got));
+    // a11
+    GM_CUDA(cudaStreamBeginCaptureToGraph(stream, lg, &loop_node, nullptr, 1, mode));
+    c = n_launch;
+    GM_TRY(enqueue_advance(M, EM_d));
+    lg_ca = n_launch - c;
+    GM_CUDA(cudaStreamEndCapture(stream, &got));
+    GM_CUDA(cudaGraphInstantiate(&lg_exec, lg, 0));
+    return 0;
+  }
+
+  int build_loop_graph() {
+    if (!cap_stream) GM_CUDA(cudaStreamCreateWithFlags(&cap_stream, cudaStreamNonBlocking));
+    if (!d_stats) {
+      GM_CUDA(cudaMalloc(&d_stats, sizeof(LoopStats)));
+      GM_CUDA(cudaMallocHost(&h_stats, sizeof(LoopStats)));
+    }
+    GM_CUDA(cudaStreamSynchronize(stream));
+    cudaStream_t user = stream;
+    const long long nl = n_launch;
+    stream = cap_stream;
+    const int st = capture_loop_graph();
+    stream = user;
+    n_launch = nl;
+    if (st != 0) {
+      cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+      if (cudaStreamIsCapturing(cap_stream, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone) {
+        cudaGraph_t tmp = nullptr;
+        cudaStreamEndCapture(cap_stream, &tmp);
+      }
+      drop_loop_graph();
+      cudaGetLastError();
+      loop_state = -1;
+      return st;
+    }
+    loop_state = 1;
     return 0;
   }
 
@@ -1115,22 +1232,43 @@ struct PlanT final : gmmnlse_plan {
     // a1: psi_0 = F{A(z0)}
     GM_TRY(launch_fft(+1, (const C*)A_in, 0, psi, 0, nullptr, nullptr, nullptr, 0, (T)1, P, 1));
     GM_TRY(to_master(psi));
-    long long done = 0;
+    long long done = 0, gsteps = 0;
     int status = GMMNLSE_OK;
+    bool last_on_device = false;
     while (done < nsteps) {
       const int Mc = (int)std::min<long long>(M, nsteps - done);
-      bool conv = false;
-      GM_TRY(large_step(Mc, &conv));
-      if (!conv) { ++n_noconv; status = GMMNLSE_WARN_NOCONV; }
+      // full large steps run as one graph launch each once a host-loop step has set the kernels up; the ragged
+      // last step, per-kernel event timing and options.graph = 1 keep the host loop
+      bool on_device = graph == 0 && !prof_on && Mc == M && warmed && loop_state >= 0;
+      if (on_device && !lg_exec && build_loop_graph() != 0) on_device = false;
+      if (on_device) {
+        if (gsteps == 0) GM_CUDA(cudaMemsetAsync(d_stats, 0, sizeof(LoopStats), stream));
+        GM_CUDA(cudaGraphLaunch(lg_exec, stream));
+        ++gsteps;
+        ++n_large;
+        last_on_device = true;
+      } else {
+        bool conv = false;
+        GM_TRY(large_step(Mc, &conv));
+        if (!conv) { ++n_noconv; status = GMMNLSE_WARN_NOCONV; }
+        last_on_device = false;
+      }
       done += Mc;
     }
-    if (fixed_iter > 0) {
+    // A_out = F^-1{psi_0}
+    GM_TRY(launch_fft(-1, psi, 0, (C*)A_out, 0, nullptr, nullptr, nullptr, 0, (T)(1.0 / N), P, 1));
+    if (gsteps > 0) {            // one read-back per call: iteration count, unconverged steps, last error
+      GM_CUDA(cudaMemcpyAsync(h_stats, d_stats, sizeof(LoopStats), cudaMemcpyDeviceToHost, stream));
+      GM_CUDA(cudaStreamSynchronize(stream));
+      n_iter += h_stats->iters;
+      n_launch += gsteps * (lg_c0 - lg_cb + lg_ca) + lg_cb * h_stats->iters;
+      if (h_stats->noconv > 0) { n_noconv += h_stats->noconv; status = GMMNLSE_WARN_NOCONV; }
+      if (last_on_device) last_err = h_stats->last_err;
+    } else if (fixed_iter > 0) {
       GM_CUDA(cudaMemcpyAsync(h_err, d_err, sizeof(double), cudaMemcpyDeviceToHost, stream));
       GM_CUDA(cudaStreamSynchronize(stream));
       last_err = nsteps > 0 ? *h_err : 0.0;
     }
-    // A_out = F^-1{psi_0}
-    GM_TRY(launch_fft(-1, psi, 0, (C*)A_out, 0, nullptr, nullptr, nullptr, 0, (T)(1.0 / N), P, 1));
     return status;
   }
 
@@ -1176,6 +1314,7 @@ struct PlanT final : gmmnlse_plan {
 
   int set_gain(const double* g) override {
     GM_CUDA(cudaStreamSynchronize(stream));
+    drop_loop_graph();
     bool any = false;
     if (g)
       for (int p = 0; p < P; ++p) {
@@ -1203,6 +1342,7 @@ struct PlanT final : gmmnlse_plan {
 
   int set_coupling(const double* Qri) override {
     GM_CUDA(cudaStreamSynchronize(stream));
+    drop_loop_graph();
     cudaFree(Qc);
     Qc = nullptr;
     if (!Qri) return 0;
@@ -1285,12 +1425,16 @@ struct PlanT final : gmmnlse_plan {
   int raman_kind() const override { return f_R == 0.0 ? 0 : (iir ? 2 : 1); }
   int set_tc_chunk(int k) override {
     if (k < 1 || k > 255) return GMMNLSE_EINVAL;
+    cudaStreamSynchronize(stream);
+    drop_loop_graph();
     tc_kchunk = k;
     return 0;
   }
   int set_probe(int probe_bits, int stage_cap, int a7_tile) override {
     if (probe_bits < 0 || stage_cap < 0 || (a7_tile != 0 && a7_tile != 32 && a7_tile != 64 && a7_tile != 128))
       return GMMNLSE_EINVAL;
+    cudaStreamSynchronize(stream);
+    drop_loop_graph();
     tc_probe = probe_bits;               // timing probes (gemm_tc.cuh Params::probe); results are wrong when set
     tc_stage_cap = stage_cap;            // cap on smem stages (0 = as many as fit)
     mr_tile = a7_tile;                   // a7 samples per CTA (0 = auto)
@@ -1328,7 +1472,7 @@ static int create_plan(gmmnlse_plan** out, int P, int N, int M, double dt, doubl
                        double f_R, const double* h_R, double omega0, double n2, const gmmnlse_options* opt) {
   if (!out) return GMMNLSE_EINVAL;
   *out = nullptr;
-  gmmnlse_options o = {0, 1, 1e-6, 0, 0, 0, 0};
+  gmmnlse_options o = {0, 1, 1e-6, 0, 0, 0, 0, 0};
   if (opt) o = *opt;
   if (P < 1 || N < 1 || M < 1 || n_beta < 1 || !beta || !S) return GMMNLSE_EINVAL;
   if (N & (N - 1)) return GMMNLSE_EINVAL;
@@ -1336,6 +1480,7 @@ static int create_plan(gmmnlse_plan** out, int P, int N, int M, double dt, doubl
   if ((f_R != 0.0) != (h_R != nullptr)) return GMMNLSE_EINVAL;
   if (o.precision != 0 && o.precision != 1) return GMMNLSE_EINVAL;
   if (o.raman < 0 || o.raman > 2 || o.contraction < 0 || o.contraction > 8) return GMMNLSE_EINVAL;
+  if (o.graph < 0 || o.graph > 1) return GMMNLSE_EINVAL;
   if (o.shock && M_PI / dt >= omega0) return GMMNLSE_EINVAL;
   if (!(o.tol > 0)) o.tol = 1e-6;
   for (long long i = 0; i < (long long)P * n_beta; ++i)
@@ -1371,6 +1516,7 @@ static int create_plan(gmmnlse_plan** out, int P, int N, int M, double dt, doubl
   pl->fixed_iter = o.fixed_iter > 0 ? o.fixed_iter : 0;
   pl->contraction = o.contraction;
   pl->raman = o.raman;
+  pl->graph = o.graph;
   pl->general = general;
   pl->gen_complex = general && tensors_complex;
   pl->gen_SR = S_R;
@@ -1496,6 +1642,8 @@ int gmmnlse_contraction_kind(const gmmnlse_plan* plan) { return plan ? plan->con
 int gmmnlse_raman_kind(const gmmnlse_plan* plan) { return plan ? plan->raman_kind() : 0; }
 
 int gmmnlse_lowrank_rank(const gmmnlse_plan* plan) { return plan ? plan->lowrank_rank() : 0; }
+
+int gmmnlse_loop_kind(const gmmnlse_plan* plan) { return plan ? plan->loop_state : 0; }
 
 int gmmnlse_debug_set_tc_chunk(gmmnlse_plan* plan, int k) { return plan ? plan->set_tc_chunk(k) : GMMNLSE_EINVAL; }
 

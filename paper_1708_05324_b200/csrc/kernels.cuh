@@ -525,6 +525,43 @@ __global__ void k_err_finalize(double* __restrict__ errbuf, int Mc, double* __re
   }
 }
 
+// a10 taken on the device (the loop of PAPER.md:218 as a CUDA-graph WHILE node): the same
+// error as k_err_finalize, then the decision the host loop takes after its read-back -- stop when err < tol or
+// at the iteration cap -- written to the conditional handle that gates the next pass of the loop body.
+// st->it is zeroed by a memset node at the head of every large step; iters / noconv accumulate over a call.
+struct LoopStats {
+  int it, noconv;
+  long long iters;
+  double last_err;
+};
+__global__ void k_err_finalize_loop(double* __restrict__ errbuf, int Mc, double* __restrict__ out, double tol, int cap,
+                                    int fixed, cudaGraphConditionalHandle handle, LoopStats* __restrict__ st) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) {
+    double e = 0.0;
+    for (int j = 1; j <= Mc; ++j) {
+      const double num = errbuf[2 * j], den = errbuf[2 * j + 1];
+      const double r = den > 0.0 ? sqrt(num / den) : 0.0;
+      e = fmax(e, r);
+      errbuf[2 * j] = 0.0;
+      errbuf[2 * j + 1] = 0.0;
+    }
+    out[0] = e;
+    const int it = st->it + 1;
+    st->it = it;
+    st->iters += 1;
+    st->last_err = e;
+    bool cont;
+    if (fixed) {
+      cont = it < cap;
+    } else {
+      const bool conv = e < tol;
+      cont = !conv && it < cap;
+      if (!conv && !cont) st->noconv += 1;
+    }
+    cudaGraphSetConditional(handle, cont ? 1u : 0u);
+  }
+}
+
 // ------------------------------------------------------------------------------------------
 // a11: advance the fp64 master state by one large step and refresh its working-precision copy.
 //   psi0_d <- (psi0_d + dz [G_0/2 + G_1 + .. + G_{Mc-1} + G_Mc/2]) * exp(D Mc dz)

@@ -264,6 +264,87 @@ def test_host_entry_matches_device_entry(B):
     assert np.array_equal(h_out, out.astype(np.complex64))
 
 
+# ------------------------------------------------------- device-side iteration loop (options.graph)
+def _run_loop(B, w, graph, calls=1, **plan_kw):
+    Ad = dev(w.A0, np.complex128 if w.precision else np.complex64)
+    sts = []
+    with B.plan_from_workload(w, graph=graph, **plan_kw) as plan:
+        for _ in range(calls):
+            sts.append(plan.propagate(Ad, w.L, Ad))
+        torch.cuda.synchronize()
+        return Ad.cpu().numpy(), sts, plan.stats(), plan.loop_kind(), plan.launch_count()
+
+
+@pytest.mark.parametrize("cfg,kw,plan_kw", [
+    (2, dict(N=1024, L=60 * 50e-6), {}),                       # 6 full large steps (CUDA-core contraction)
+    (2, dict(N=512, L=47 * 50e-6), {}),                        # 4 full + a 7-plane tail on the host loop
+    (3, dict(N=1024, L=0.004, max_group=2), {}),               # Raman + shock
+    (3, dict(N=1024, L=0.003), dict(contraction=7)),           # tcgen05 kind::f16 contraction inside the graph
+    (3, dict(N=1024, L=0.003), dict(contraction=3)),           # 3xTF32
+    (1, dict(), {}),                                           # complex128
+    (2, dict(N=512, L=40 * 50e-6), dict(fixed_iter=3)),
+    (2, dict(N=512, L=40 * 50e-6), dict(max_iter=2, tol=1e-12)),
+])
+def test_device_loop_is_the_host_loop(B, cfg, kw, plan_kw):
+    """The CUDA-graph WHILE loop takes the decisions of PAPER.md:218 that the host loop takes after its read-back:
+    same kernels in the same order, so fields are bit-identical and every counter agrees."""
+    w = W.make_config(cfg, **kw)
+    if cfg == 1:
+        w.L = 40 * w.dz
+    out_d, st_d, stats_d, kind_d, launches_d = _run_loop(B, w, 0, calls=2, **plan_kw)
+    out_h, st_h, stats_h, kind_h, launches_h = _run_loop(B, w, 1, calls=2, **plan_kw)
+    assert kind_d == 1 and kind_h == 0
+    assert np.array_equal(out_d, out_h)
+    assert st_d == st_h
+    assert stats_d == stats_h
+    assert launches_d == launches_h
+    if plan_kw.get("max_iter"):
+        assert st_d[0] == B.WARN_NOCONV and stats_d["not_converged"] == stats_d["large_steps"]
+
+
+def test_device_loop_follows_gain_and_coupling_changes(B):
+    w = W.make_config(2, N=512, L=30 * 50e-6)
+    rng = np.random.default_rng(5)
+    g = rng.uniform(-2.0, 2.0, w.P)
+    Q = rng.normal(size=(w.P, w.P)) * 20.0
+    Q = Q + Q.T
+    outs = []
+    for graph in (0, 1):
+        Ad = dev(w.A0, np.complex64)
+        with B.plan_from_workload(w, graph=graph) as plan:
+            plan.propagate(Ad, w.L, Ad)             # builds the graph without gain
+            plan.set_gain(g)
+            plan.set_coupling(Q.astype(np.complex128))
+            plan.propagate(Ad, w.L, Ad)             # must rebuild: new tables, extra kernel
+            plan.set_gain(None)
+            plan.set_coupling(None)
+            plan.propagate(Ad, w.L, Ad)
+            torch.cuda.synchronize()
+            assert plan.loop_kind() == (1 if graph == 0 else 0)
+        outs.append(Ad.cpu().numpy())
+    assert np.array_equal(outs[0], outs[1])
+
+
+def test_device_loop_on_a_user_stream_and_under_profiling(B):
+    w = W.make_config(2, N=512, L=30 * 50e-6)
+    ref, _, stats_ref, _, _ = _run_loop(B, w, 1)
+    Ad = dev(w.A0, np.complex64)
+    s = torch.cuda.Stream()
+    with B.plan_from_workload(w) as plan:
+        with torch.cuda.stream(s):
+            plan.propagate(Ad, w.L, Ad, s)
+        s.synchronize()
+        assert plan.loop_kind() == 1 and plan.stats() == stats_ref
+        assert np.array_equal(Ad.cpu().numpy(), ref)
+        plan.profile_enable(True)                   # per-kernel events: host loop, same result
+        Bd = dev(w.A0, np.complex64)
+        plan.propagate(Bd, w.L, Bd)
+        prof = plan.profile_get()
+        plan.profile_enable(False)
+        assert np.array_equal(Bd.cpu().numpy(), ref)
+        assert sum(v[1] for v in prof.values()) > 0
+
+
 # ----------------------------------------------------------------------------------- edge cases
 def test_zero_length_is_identity(B):
     w = W.make_config(2, N=256)
