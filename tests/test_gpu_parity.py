@@ -296,6 +296,8 @@ def test_device_loop_is_the_host_loop(B, cfg, kw, plan_kw):
     assert kind_d == 1 and kind_h == 0
     assert np.array_equal(out_d, out_h)
     assert st_d == st_h
+    # last_err comes from fp64 atomics whose order differs between launches: last bits only
+    assert stats_d.pop("last_err") == pytest.approx(stats_h.pop("last_err"), rel=1e-9)
     assert stats_d == stats_h
     assert launches_d == launches_h
     if plan_kw.get("max_iter"):
@@ -334,7 +336,9 @@ def test_device_loop_on_a_user_stream_and_under_profiling(B):
         with torch.cuda.stream(s):
             plan.propagate(Ad, w.L, Ad, s)
         s.synchronize()
-        assert plan.loop_kind() == 1 and plan.stats() == stats_ref
+        st = plan.stats()
+        assert plan.loop_kind() == 1 and st.pop("last_err") == pytest.approx(stats_ref.pop("last_err"), rel=1e-9)
+        assert st == stats_ref
         assert np.array_equal(Ad.cpu().numpy(), ref)
         plan.profile_enable(True)                   # per-kernel events: host loop, same result
         Bd = dev(w.A0, np.complex64)
