@@ -215,10 +215,14 @@ k_pair_iir(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restric
     const cplx<T>* am1 = Aj + (long long)pair_m[has1 ? q1 : q0] * N;
     const cplx<T>* an1 = Aj + (long long)pair_n[has1 ? q1 : q0] * N;
     const bool im0 = GEN && gs.kind[q0], im1 = GEN && has1 && gs.kind[q1];
+    // consecutive packed pairs (m, n), (m, n + 1) share row m except across a row end: read it once (the kernel is
+    // bound by L1 throughput, and a quarter of its global loads were this second read)
+    const bool same_m = am1 == am0;
 #pragma unroll 4
     for (int e = 0; e < 16; ++e) {
       const int n = tid + e * NT;
-      const cplx<T> a = am0[n], b = an0[n], c = am1[n], d = an1[n];
+      const cplx<T> a = am0[n], b = an0[n], d = an1[n];
+      const cplx<T> c = same_m ? a : am1[n];
       sm[fft_pad(n)] = mk(pair_stream(a, b, im0), has1 ? pair_stream(c, d, im1) : (T)0);
     }
   }
