@@ -364,17 +364,19 @@ def run_sweep(args):
         return best
 
     out_rk = torch.empty_like(A)
-    with binding.plan_from_workload(w, M=1) as plan:
+    g = 1 if args.host_loop else 0
+    with binding.plan_from_workload(w, M=1, graph=g) as plan:
         ms = timed(lambda: plan.propagate_rk4ip(A, L, out_rk, stream))
     ref = out_rk.cpu().numpy().astype(np.complex128)
     res = {"sweep": "fig3-like", "workload": "10-mode GRIN (config-3 fibre, groups 0-3), N=8192, 200 kW 300 fs, "
                                              "Kerr+Raman+shock", "P": w.P, "N": w.N, "dz_m": w.dz,
            "z_nl_over_dz": 200.0, "small_steps": n_small, "unit": UNIT,
+           "loops": "host (options.graph = 1)" if g else "device (CUDA graphs: MPA WHILE loop, replayed RK4IP step)",
            "serial_rk4ip": {"z_steps_per_s": round(n_small / (ms * 1e-3), 1), "ms": round(ms, 3),
                             "nonlinear_evals_per_step": 4}, "mpa": []}
     for M in (1, 2, 4, 5, 10, 20, 40):
         out = torch.empty_like(A)
-        with binding.plan_from_workload(w, M=M) as plan:
+        with binding.plan_from_workload(w, M=M, graph=g) as plan:
             ms = timed(lambda: plan.propagate(A, L, out, stream))
             s0 = plan.stats()
             plan.propagate(A, L, out, stream); torch.cuda.synchronize()

@@ -208,6 +208,11 @@ struct PlanT final : gmmnlse_plan {
   LoopStats *d_stats = nullptr, *h_stats = nullptr;
   long long lg_c0 = 0, lg_cb = 0, lg_ca = 0;       // kernel launches in iteration 0, the loop body, a11
   bool warmed = false;                             // one host-loop large step has run (function attributes set)
+  // serial RK4IP: one step (4 stages) as a graph, replayed; no decision inside, so no conditional node
+  cudaGraph_t rkg = nullptr;
+  cudaGraphExec_t rkg_exec = nullptr;
+  long long rk_c = 0;                              // kernel launches per RK4IP step
+  bool rk_warmed = false;
   long long PN = 0, QN = 0;
   // NEXT-3: small-signal gain g_p (joins D as its real part) and constant linear coupling Q_np
   std::vector<double> gain;                // [P], 1/m; empty = none
@@ -1141,6 +1146,11 @@ struct PlanT final : gmmnlse_plan {
     if (lg) cudaGraphDestroy(lg);
     lg_exec = nullptr;
     lg = nullptr;
+    if (rkg_exec) cudaGraphExecDestroy(rkg_exec);
+    if (rkg) cudaGraphDestroy(rkg);
+    rkg_exec = nullptr;
+    rkg = nullptr;
+    warmed = rk_warmed = false;      // the kernel set may change (coupling): next call starts on the host path
     if (loop_state > 0) loop_state = 0;
   }
 
@@ -1358,6 +1368,43 @@ struct PlanT final : gmmnlse_plan {
     return upload(Qc, q);
   }
 
+  int enqueue_rk4_step() {
+    const unsigned blocks = (unsigned)((PN + 255) / 256);
+    for (int stage = 1; stage <= 4; ++stage) {
+      GM_TRY(nonlinear_freq(stage == 1 ? psi : rk_X));
+      prof_begin(GMMNLSE_KIND_ADVANCE);
+      k_rk4_stage<T><<<blocks, 256, 0, stream>>>(stage, psi0_d, psi, EH_d, G, rk_AI, rk_K1, rk_K2, rk_K3, rk_X, dz, PN);
+      prof_end();
+      GM_CUDA(cudaGetLastError());
+    }
+    return 0;
+  }
+
+  int build_rk4_graph() {
+    if (!cap_stream) GM_CUDA(cudaStreamCreateWithFlags(&cap_stream, cudaStreamNonBlocking));
+    GM_CUDA(cudaStreamSynchronize(stream));
+    cudaStream_t user = stream;
+    const long long nl = n_launch;
+    stream = cap_stream;
+    int st = cudaStreamBeginCapture(stream, cudaStreamCaptureModeRelaxed) == cudaSuccess ? 0 : GMMNLSE_ECUDA;
+    if (st == 0) {
+      st = enqueue_rk4_step();
+      rk_c = n_launch - nl;
+      if (cudaStreamEndCapture(stream, &rkg) != cudaSuccess) st = GMMNLSE_ECUDA;
+    }
+    if (st == 0 && cudaGraphInstantiate(&rkg_exec, rkg, 0) != cudaSuccess) st = GMMNLSE_ECUDA;
+    stream = user;
+    n_launch = nl;
+    if (st != 0) {
+      if (rkg) cudaGraphDestroy(rkg);
+      rkg = nullptr;
+      rkg_exec = nullptr;
+      cudaGetLastError();
+      loop_state = -1;
+    }
+    return st;
+  }
+
   int propagate_rk4ip(const void* A_in, double L, void* A_out) override {
     const double ns = L / dz;
     const long long nsteps = llround(ns);
@@ -1378,15 +1425,19 @@ struct PlanT final : gmmnlse_plan {
     }
     GM_TRY(launch_fft(+1, (const C*)A_in, 0, psi, 0, nullptr, nullptr, nullptr, 0, (T)1, P, 1));
     GM_TRY(to_master(psi));
-    const unsigned blocks = (unsigned)((PN + 255) / 256);
-    for (long long s = 0; s < nsteps; ++s) {
-      for (int stage = 1; stage <= 4; ++stage) {
-        GM_TRY(nonlinear_freq(stage == 1 ? psi : rk_X));
-        prof_begin(GMMNLSE_KIND_ADVANCE);
-        k_rk4_stage<T><<<blocks, 256, 0, stream>>>(stage, psi0_d, psi, EH_d, G, rk_AI, rk_K1, rk_K2, rk_K3, rk_X, dz,
-                                                    PN);
-        prof_end();
-        GM_CUDA(cudaGetLastError());
+    long long s = 0;
+    if (nsteps > 0 && !rk_warmed) {                  // first step of a plan on the host path: sets kernel attributes
+      GM_TRY(enqueue_rk4_step());
+      rk_warmed = true;
+      s = 1;
+    }
+    const bool replay = graph == 0 && !prof_on && loop_state >= 0 && s < nsteps && (rkg_exec || build_rk4_graph() == 0);
+    for (; s < nsteps; ++s) {
+      if (replay) {
+        GM_CUDA(cudaGraphLaunch(rkg_exec, stream));
+        n_launch += rk_c;
+      } else {
+        GM_TRY(enqueue_rk4_step());
       }
     }
     GM_TRY(launch_fft(-1, psi, 0, (C*)A_out, 0, nullptr, nullptr, nullptr, 0, (T)(1.0 / N), P, 1));

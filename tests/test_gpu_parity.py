@@ -327,6 +327,22 @@ def test_device_loop_follows_gain_and_coupling_changes(B):
     assert np.array_equal(outs[0], outs[1])
 
 
+def test_rk4ip_step_graph_is_the_host_path(B):
+    """The serial integrator replays one captured step; same kernels, so the field is bit-identical."""
+    w = W.make_config(2, N=512, L=25 * 50e-6)
+    outs, launches = [], []
+    for graph in (0, 1):
+        Ad = dev(w.A0, np.complex64)
+        with B.plan_from_workload(w, graph=graph) as plan:
+            plan.propagate_rk4ip(Ad, w.L, Ad)
+            plan.propagate_rk4ip(Ad, w.L, Ad)
+            torch.cuda.synchronize()
+            launches.append(plan.launch_count())
+        outs.append(Ad.cpu().numpy())
+    assert np.array_equal(outs[0], outs[1])
+    assert launches[0] == launches[1]
+
+
 def test_device_loop_on_a_user_stream_and_under_profiling(B):
     w = W.make_config(2, N=512, L=30 * 50e-6)
     ref, _, stats_ref, _, _ = _run_loop(B, w, 1)
