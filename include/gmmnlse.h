@@ -124,8 +124,10 @@ int gmmnlse_plan_create_general(gmmnlse_plan **out, int P, int N, int M, double 
 int gmmnlse_propagate(gmmnlse_plan *plan, const void *A_in, double L, void *A_out, void *stream);
 
 /* Same as gmmnlse_propagate but A_in / A_out are HOST [P][N] buffers of the plan's
- * precision; the call stages them through plan-owned pinned memory, copies, propagates and
- * synchronises.  This is the end-to-end entry bench.py times.                              */
+ * precision: H2D copy, propagate, D2H copy on the plan's stream, one synchronise; A_out is
+ * complete on return.  Page-locked buffers (cudaMallocHost / cudaHostRegister) are copied
+ * from and to directly; pageable ones are staged through plan-owned pinned memory.  This is
+ * the end-to-end entry bench.py times (with page-locked buffers).                          */
 int gmmnlse_propagate_host(gmmnlse_plan *plan, const void *A_in_host, double L, void *A_out_host);
 
 /* Serial comparison integrator (the role of the split-step code the paper times the

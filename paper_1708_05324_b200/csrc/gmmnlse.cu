@@ -199,6 +199,8 @@ struct PlanT final : gmmnlse_plan {
   double *errbuf = nullptr, *d_err = nullptr, *h_err = nullptr;
   void *h_in = nullptr, *h_out = nullptr;          // pinned staging for propagate_host
   C* d_io = nullptr;
+  void* d2h_dst = nullptr;                         // set by propagate_host around its propagate() call
+  size_t d2h_bytes = 0;
   std::map<int, double2*> EM_ragged;
   // device-side MPA loop: one CUDA graph per full large step = iteration 0, a WHILE node whose body is one further
   // iteration, a11.  k_err_finalize_loop takes the convergence decision; the host reads LoopStats once per call.
@@ -1267,6 +1269,7 @@ struct PlanT final : gmmnlse_plan {
     }
     // A_out = F^-1{psi_0}
     GM_TRY(launch_fft(-1, psi, 0, (C*)A_out, 0, nullptr, nullptr, nullptr, 0, (T)(1.0 / N), P, 1));
+    if (d2h_dst) GM_CUDA(cudaMemcpyAsync(d2h_dst, A_out, d2h_bytes, cudaMemcpyDeviceToHost, stream));   // host entry
     if (gsteps > 0) {            // one read-back per call: iteration count, unconverged steps, last error
       GM_CUDA(cudaMemcpyAsync(h_stats, d_stats, sizeof(LoopStats), cudaMemcpyDeviceToHost, stream));
       GM_CUDA(cudaStreamSynchronize(stream));
@@ -1282,20 +1285,31 @@ struct PlanT final : gmmnlse_plan {
     return status;
   }
 
+  static bool is_pinned(const void* p) {          // page-locked (cudaMallocHost / cudaHostRegister) host memory?
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeHost;
+  }
+
+  // Host entry: H2D, propagate, D2H on the plan's stream, one synchronise.  Page-locked caller buffers are copied
+  // from and to directly; pageable ones are staged through plan-owned pinned memory (two host memcpys more).
   int propagate_host(const void* A_in, double L, void* A_out) override {
     const size_t bytes = sizeof(C) * (size_t)PN;
-    if (!h_in) {
+    if (!d_io) GM_TRY(dalloc(&d_io, (size_t)PN));
+    const bool pin_in = is_pinned(A_in), pin_out = is_pinned(A_out);
+    if ((!pin_in || !pin_out) && !h_in) {
       GM_CUDA(cudaMallocHost(&h_in, bytes));
       GM_CUDA(cudaMallocHost(&h_out, bytes));
-      GM_TRY(dalloc(&d_io, (size_t)PN));
     }
-    std::memcpy(h_in, A_in, bytes);
-    GM_CUDA(cudaMemcpyAsync(d_io, h_in, bytes, cudaMemcpyHostToDevice, stream));
+    if (!pin_in) std::memcpy(h_in, A_in, bytes);
+    GM_CUDA(cudaMemcpyAsync(d_io, pin_in ? A_in : h_in, bytes, cudaMemcpyHostToDevice, stream));
+    d2h_dst = pin_out ? A_out : h_out;             // propagate() enqueues this copy ahead of its own read-back
+    d2h_bytes = bytes;
     const int st = propagate(d_io, L, d_io);
+    d2h_dst = nullptr;
     if (st < 0) return st;
-    GM_CUDA(cudaMemcpyAsync(h_out, d_io, bytes, cudaMemcpyDeviceToHost, stream));
     GM_CUDA(cudaStreamSynchronize(stream));
-    std::memcpy(A_out, h_out, bytes);
+    if (!pin_out) std::memcpy(A_out, h_out, bytes);
     return st;
   }
 

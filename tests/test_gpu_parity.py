@@ -262,6 +262,17 @@ def test_host_entry_matches_device_entry(B):
     with B.plan_from_workload(w) as plan:
         plan.propagate_host(h_in, w.L, h_out)
     assert np.array_equal(h_out, out.astype(np.complex64))
+    # page-locked caller buffers take the direct-copy path; a mixed pair too
+    p_in = torch.from_numpy(h_in.copy()).pin_memory().numpy()
+    p_out = torch.from_numpy(np.zeros_like(h_in)).pin_memory().numpy()
+    with B.plan_from_workload(w) as plan:
+        plan.propagate_host(p_in, w.L, p_out)
+        assert np.array_equal(p_out, h_out)
+        h2 = np.zeros_like(h_in)
+        plan.propagate_host(p_in, w.L, h2)
+        assert np.array_equal(h2, h_out)
+        plan.propagate_host(p_in, w.L, p_in)          # aliased in/out
+        assert np.array_equal(p_in, h_out)
 
 
 # ------------------------------------------------------- device-side iteration loop (options.graph)
