@@ -28,15 +28,35 @@ def test_fft_vs_direct_dft(N, sign):
     assert np.allclose(O.fft_radix2(x, sign), O.dft_direct(x, sign), rtol=0, atol=1e-12 * N)
 
 
-def test_fft_convention_matches_library_witness():
-    # to_freq uses exp(+i...) un-normalised == N * numpy.ifft ; to_time == numpy.fft / N
+@pytest.mark.parametrize("N", [1, 2, 8, 64])
+def test_transforms_vs_direct_dft(N):
+    # to_freq / to_time (library FFT as the step) against the O(N^2) definition, sign and 1/N included
+    rng = np.random.default_rng(N + 11)
+    x = rng.standard_normal((3, N)) + 1j * rng.standard_normal((3, N))
+    assert np.allclose(O.to_freq(x), O.dft_direct(x, +1), rtol=0, atol=1e-12 * N)
+    assert np.allclose(O.to_time(x), O.dft_direct(x, -1) / N, rtol=0, atol=1e-12)
+
+
+@pytest.mark.parametrize("log2N", range(0, 15))
+def test_transforms_vs_written_out_radix2(log2N):
+    # every power of two the configurations use (up to 16384): library transform == the recursion written out above it
+    N = 1 << log2N
+    rng = np.random.default_rng(100 + log2N)
+    x = rng.standard_normal((2, N)) + 1j * rng.standard_normal((2, N))
+    assert rel(O.to_freq(x), O.fft_radix2(x, +1)) < 1e-14 * max(1, log2N)
+    assert rel(O.to_time(x), O.fft_radix2(x, -1) / N) < 1e-14 * max(1, log2N)
+
+
+def test_fft_convention_round_trip_and_parseval():
     rng = np.random.default_rng(1)
     x = rng.standard_normal((2, 256)) + 1j * rng.standard_normal((2, 256))
-    assert rel(O.to_freq(x), 256 * np.fft.ifft(x)) < 1e-13
-    assert rel(O.to_time(x), np.fft.fft(x) / 256) < 1e-13
     assert rel(O.to_time(O.to_freq(x)), x) < 1e-13
     # Parseval: sum |X|^2 = N sum |x|^2
     assert abs(np.sum(abs(O.to_freq(x)) ** 2) / (256 * np.sum(abs(x) ** 2)) - 1) < 1e-13
+    # a real, even input has a real spectrum; a delta at n=1 gives exp(+2 pi i k/N)  (sign of the exponent)
+    d = np.zeros(16); d[1] = 1.0
+    assert np.allclose(O.to_freq(d), np.exp(+2j * np.pi * np.arange(16) / 16), atol=1e-14)
+    assert np.allclose(O.fft_radix2(d, +1), np.exp(+2j * np.pi * np.arange(16) / 16), atol=1e-14)
 
 
 def test_single_tone_lands_in_expected_bin():
