@@ -29,7 +29,8 @@ if ROOT not in sys.path:
 METRIC = "GMMNLSE z-steps/s (P modes, N samples, M planes)"
 UNIT = "z-steps/s"
 LARGE_PER_STEP = {1: 100, 2: 30, 3: 10, 4: 2, 5: 1}
-ORACLE_SAMPLE_N = {1: 1024, 2: 4096, 3: 8192, 4: 4096, 5: 2048}      # time-grid samples of the CPU sample
+ORACLE_MIN_SECONDS = 10.0             # the CPU sample runs whole RK4IP steps at the full (P, N) until this much time
+ORACLE_MAX_STEPS = 400                 # ... or this many steps (configs 1-2 take milliseconds per step)
 DEFAULT_CONFIG = 5
 
 
@@ -129,7 +130,36 @@ def replica_launch_field(A0, rank: int, seed_base: int):
     return (A0 * np.exp(2j * np.pi * rng.random((A0.shape[0], 1)))).astype(A0.dtype)
 
 
+def job_value(world: int, z_steps_per_rank: int, ms_max_over_ranks: float) -> float:
+    """Whole-job z-steps/s of `world` replicas: every rank advances its own field by z_steps_per_rank small steps in
+    the slowest rank's time (weak scaling, no data-path collective)."""
+    return world * z_steps_per_rank / (ms_max_over_ranks * 1e-3)
+
+
+def run_launch_stub(args, stub_ms: float):
+    """tests/test_bench_ranks.py only (GMMNLSE_BENCH_STUB_MS set): the N-rank launch of this script -- rendezvous,
+    barrier, max over ranks, whole-job value, rank 0 printing -- with the measurement replaced by a fixed per-rank
+    time, on CPU over gloo.  Nothing of the GPU path runs."""
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("gloo")
+        dist.barrier()
+    ms = max_over_ranks(stub_ms * (1 + rank), world, "cpu")
+    z = args.steps * LARGE_PER_STEP[args.config] * 20
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": job_value(world, z, ms), "unit": UNIT, "n_gpus": world,
+                          "steps": args.steps, "ms_per_step": ms / args.steps, "scaling": "weak", "stub": True}))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
 def run_gpu(args):
+    if os.environ.get("GMMNLSE_BENCH_STUB_MS"):
+        return run_launch_stub(args, float(os.environ["GMMNLSE_BENCH_STUB_MS"]))
     import torch
     import torch.distributed as dist
     from paper_1708_05324_b200 import binding, workloads
@@ -219,7 +249,7 @@ def run_gpu(args):
     clocks = clk.summary()
     e2e = measure(cfg, K, Wm, with_events=False, host_path=True, seed_offset=rank)
     w = main["w"]
-    value = world * plain["z_steps"] / (plain["ms"] * 1e-3)
+    value = job_value(world, plain["z_steps"], plain["ms"])
 
     # ---- roofline of the dominant kernel class, from the per-launch CUDA events of the timed region
     prof = {k: v for k, v in main["prof"].items() if v[1] > 0}
@@ -236,10 +266,12 @@ def run_gpu(args):
         shares[k] = dict(ms=round(ms_k, 4), launches=n_k, share=round(ms_k / tot_ms, 4),
                          GBps=round(by / (ms_k * 1e-3) / 1e9, 1), TFLOPs=round(fl / (ms_k * 1e-3) / 1e12, 3))
     by, fl = algorithmic(dom, w, planes_total[dom])
-    traffic = None
+    traffic, traffic_src = None, None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")     # written from an ncu --set full capture
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(f"cfg{cfg}", {}).get(dom)
+        tj = json.load(open(tpath))
+        traffic = tj.get(f"cfg{cfg}", {}).get(dom)
+        traffic_src = tj.get("_source", "profiles/traffic.json") + " (an earlier ncu --set full capture, replayed here: not measured by this run)"
     dom_ms, dom_n = prof[dom]
     if dom == "contract":
         # a6: `achieved` counts the method's useful packed-real flops (2 Q^2 N per plane).
@@ -249,27 +281,31 @@ def run_gpu(args):
         # nominal ratio) for the TF32 forms.
         ach = fl / (dom_ms * 1e-3) / 1e12
         ck = main["ckind"]
+        # the timed region is a fraction of a second at full clock, so the BURST figure is the denominator of
+        # `frac`; the sustained one is printed beside it
         if ck in (7, 8):
-            kname, peak, mult = "k_contract_h (a6, tcgen05 kind::f16 on fp16 hi/lo splits)", peaks["bf16_sustained"], 3
-            pnote = f"peak = {peaks['source']} bf16 sustained (fp16 runs at the bf16 rate)"
-        elif ck >= 2:
-            kname, peak, mult = "k_contract_tc (a6, tcgen05 3xTF32)", peaks["bf16_sustained"] * 0.5, 3
-            pnote = (f"peak = {peaks['source']} bf16 sustained x 0.5 (TF32 nominal ratio); cuBLAS TF32 8192^3 on the "
-                     "same box: 756 burst / 658 sustained TFLOP/s (profiles/r01c_summary.md)")
+            kname, ratio, mult = "k_contract_h (a6 + a7, tcgen05 kind::f16 on fp16 hi/lo splits)", 1.0, 3
+            pnote = f"peak = {peaks['source']} bf16 burst (fp16 runs at the bf16 rate)"
+        elif ck in (3, 6):
+            kname, ratio, mult = "k_contract_tc (a6, tcgen05 3xTF32)", 0.5, 3
+            pnote = f"peak = {peaks['source']} bf16 burst x 0.5 (TF32 nominal ratio)"
         else:
-            kname, peak, mult = "k_contract (a6, fp32 FFMA)", peaks["bf16_sustained"] * 0.5, 1
-            pnote = f"peak = {peaks['source']} bf16 sustained x 0.5"
+            kname, ratio, mult = "k_contract (a6, fp32 FFMA)", 0.5, 1
+            pnote = f"peak = {peaks['source']} bf16 burst x 0.5"
+        peak, peak_s = peaks["bf16_burst"] * ratio, peaks["bf16_sustained"] * ratio
         roof = dict(bound="tensor", kernel=kname,
                     achieved=round(ach, 3), peak=round(peak, 1), unit="TFLOP/s", frac=round(ach / peak, 4),
-                    traffic=traffic,
+                    peak_sustained=round(peak_s, 1), frac_of_sustained=round(ach / peak_s, 4),
+                    traffic=traffic, traffic_source=traffic_src,
                     executed_tflops=round(mult * ach, 2),
                     executed_frac=round(mult * ach / peak, 4),
+                    executed_frac_of_sustained=round(mult * ach / peak_s, 4),
                     note=f"useful flops 2*Q^2*N per plane; {pnote}; executed = {mult}x useful"
                          + (" (three MMAs per product: hi.lo, lo.hi, hi.hi)" if mult == 3 else ""))
     else:
         ach = by / (dom_ms * 1e-3) / 1e9
         roof = dict(bound="hbm", kernel=dom, achieved=round(ach, 1), peak=peaks["hbm"], unit="GB/s",
-                    frac=round(ach / peaks["hbm"], 4), traffic=traffic,
+                    frac=round(ach / peaks["hbm"], 4), traffic=traffic, traffic_source=traffic_src,
                     note=f"algorithmic bytes / event-timed duration; peak = {peaks['source']} copy bandwidth")
     if main["ckind"] in (6, 8):
         roof["note"] += "; low-rank form selected: flop rates are dense-equivalent, not executed"
@@ -289,13 +325,13 @@ def run_gpu(args):
         "iterations_per_large_step": round(plain["iters"] / max(plain["large"], 1), 3),
         "not_converged": plain["not_conv"], "finite": plain["finite"] and main["finite"],
         "ms_per_step_with_kernel_events": round(main["ms"] / K, 4),
-        "e2e": {"value": round(world * e2e["z_steps"] / (e2e["ms"] * 1e-3), 2), "unit": UNIT,
+        "e2e": {"value": round(job_value(world, e2e["z_steps"], e2e["ms"]), 2), "unit": UNIT,
                 "h2d_bytes_per_step": e2e["bytes_io"], "d2h_bytes_per_step": e2e["bytes_io"] + (24 if e2e["loop"] == 1 else 8 * e2e["iters"] // K)},
         "gpu_launches": plain["launches"],
         "clocks": clocks, "roofline": roof,
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = oracle_sample(cfg, 1, 0)
+        out["cpu_baseline"] = oracle_sample(cfg, 0, 0)
     out["config"]["contraction_kind"] = main["ckind"]
     out["config"]["mpa_loop"] = ("device (one CUDA graph per large step, WHILE node)" if plain["loop"] == 1
                                  else "host (read-back per iteration)")
@@ -395,60 +431,100 @@ def run_sweep(args):
 
 
 # ------------------------------------------------------------------------------ oracle (CPU) leg
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for line in fh:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def oracle_sample(cfg, K, Wm):
-    """Time the fp64 oracle as it stands (RK4IP, oracle/gmmnlse_oracle.py) on a bounded sample of the
-    workload: K RK4IP small steps on the first ORACLE_SAMPLE_N[cfg] samples of the time grid (same dt,
-    same fibre, same pulse); cost is linear in N up to the FFT's log factor, so z-steps/s at the full
-    grid = sample z-steps/s x (N_sample / N)."""
+    """Time the fp64 oracle as it stands (oracle/gmmnlse_oracle.py) at the configuration's FULL (P, N): one
+    nonlinear-operator evaluation (O2), then whole RK4IP small steps (O3, 4 evaluations each).  K > 0: exactly K
+    timed steps after Wm warm-up steps (the --impl reference arm); K == 0: as many steps as it takes to pass
+    ORACLE_MIN_SECONDS (at least one).  Nothing is extrapolated: value = steps done / seconds taken."""
     from oracle import gmmnlse_oracle as O
     from paper_1708_05324_b200 import workloads
-    full = workloads.make_config(cfg)
-    Ns = min(ORACLE_SAMPLE_N[cfg], full.N)
-    w = workloads.make_config(cfg, N=Ns)
+    w = workloads.make_config(cfg)
     omega = O.omega_grid(w.N, w.dt)
     D = O.dispersion_operator(w.beta, omega)
     nl = lambda X: O.nonlinear_op_freq(X, w.S, w.kappa, omega, w.omega0, w.f_R, w.h_R, w.dt, w.shock)
+    t0 = time.perf_counter()
+    O.nonlinear_op(w.A0, w.S, w.kappa, w.omega0, w.f_R, w.h_R, w.dt, w.shock)
+    op_sec = time.perf_counter() - t0
     At = O.to_freq(w.A0)
     for _ in range(Wm):
         At = O.rk4ip_step(At, w.dz, D, nl)
+    done, step_secs = 0, []
     t0 = time.perf_counter()
-    for _ in range(K):
+    while True:
+        t1 = time.perf_counter()
         At = O.rk4ip_step(At, w.dz, D, nl)
+        step_secs.append(time.perf_counter() - t1)
+        done += 1
+        if (K > 0 and done >= K) or (K == 0 and (time.perf_counter() - t0 >= ORACLE_MIN_SECONDS
+                                                   or done >= ORACLE_MAX_STEPS)):
+            break
     sec = time.perf_counter() - t0
     try:
         import threadpoolctl
         cores = max([p["num_threads"] for p in threadpoolctl.threadpool_info()] or [1])
     except Exception:
         cores = os.cpu_count() or 1
-    v = K / sec * (Ns / full.N)
-    return {"value": round(v, 4), "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{K} RK4IP step(s) (4 nonlinear-operator evaluations each) of {full.name} on N={Ns} of "
-                      f"{full.N} time samples, {sec:.1f} s CPU, scaled by {Ns}/{full.N}",
+    return {"value": round(done / sec, 5), "unit": UNIT, "cores": cores, "cpu_model": cpu_model(),
+            "host_cpus": os.cpu_count(), "kind": "oracle",
+            "sample": f"{done} RK4IP small step(s) (4 nonlinear-operator evaluations each) of {w.name} at its full "
+                      f"shape P={w.P}, N={w.N}: {sec:.1f} s; one nonlinear-operator evaluation alone: {op_sec:.2f} s",
+            "steps": done, "seconds": round(sec, 2), "ms_per_rk4ip_step": round(1e3 * float(np.mean(step_secs)), 1),
+            "nonlinear_op_evals_per_s": round(1.0 / op_sec, 4),
             "finite": bool(np.isfinite(At).all())}
 
 
 def run_reference(args):
+    """The reference arm of this tier is the oracle: one "step" = one RK4IP small step (dz) at the full shape, so
+    value = steps / seconds is the same z-steps/s metric and ms_per_step x steps is the time the timed loop took."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     from paper_1708_05324_b200 import workloads
-    K, Wm = args.steps, args.warmup
-    K = min(K, 3)                               # each step is already a bounded sample
-    Wm = min(Wm, 1)
-    t0 = time.perf_counter()
-    cb = oracle_sample(args.config, K, Wm)
     w = workloads.make_config(args.config)
+    # bound the run to a few minutes: one probe step sets the cap on the timed steps
+    t0 = time.perf_counter()
+    probe = oracle_sample(args.config, 1, 0)
+    per_step = probe["seconds"]
+    K = max(1, min(args.steps, int(150.0 / max(per_step, 1e-3))))
+    Wm = min(args.warmup, 1 if per_step > 1.0 else 3)
+    cb = oracle_sample(args.config, K, Wm)
     out = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT,
            "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": K, "warmup": Wm,
-           "ms_per_step": round(1e3 / cb["value"] * LARGE_PER_STEP[args.config] * w.M, 1) if cb["value"] else None,
+           "ms_per_step": round(1e3 * cb["seconds"] / K, 1),
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "c128 (f64)",
            "data": "synthetic",
            "config": {"workload": w.name, "baseline_config_index": args.config, "P": w.P, "N": w.N, "M": w.M,
-                      "dz_m": w.dz, "integrator": "RK4IP (oracle O3), fixed step dz"},
+                      "dz_m": w.dz, "integrator": "RK4IP (oracle O3), fixed step dz", "z_steps_per_step": 1,
+                      "steps_requested": args.steps, "steps_run": K,
+                      "note": "a step is one RK4IP small step at the full shape; the step count is capped so the run "
+                              "ends within a few minutes"},
            "cpu_baseline": cb,
            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "wall_s": round(time.perf_counter() - t0, 1)}
     print(json.dumps(out))
+
+
+def spawn_ranks(n: int) -> int:
+    """`python bench.py --gpus N` outside torchrun: start the N ranks ourselves, exactly the way the driver would
+    (one process per GPU, NCCL rendezvous on 127.0.0.1), and pass their output through."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -469,6 +545,8 @@ def main():
     ap.add_argument("--no-variants", action="store_true", help="skip the low-rank variant measurement")
     ap.add_argument("--sweep-M", action="store_true", help="serial RK4IP vs MPA(M) on a 10-mode GRIN (Fig. 3 shape)")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "graft" and not args.sweep_M:
+        raise SystemExit(spawn_ranks(args.gpus))
     if args.sweep_M:
         run_sweep(args)
     elif args.impl == "reference":

@@ -44,23 +44,20 @@ typedef struct {                /* pass NULL for defaults                       
   int    contraction;           /* a6 kernel: 0 = auto (complex64 and N % 128 == 0: 7 when Q = P(P+1)/2 >= 160,
                                    3 when 64 <= Q < 160; else 1),
                                    1 = CUDA-core fp32/fp64 GEMM;
+                                   3 = tcgen05 3xTF32 GEMM (kind::tf32 on hi/lo splits, both operands in shared memory);
                                    7 = tcgen05 kind::f16 GEMM on fp16 hi/lo splits of both operands (22 mantissa
                                    bits, as 3xTF32, at twice its MMA rate): the pair kernels write V scaled by a
                                    power of two into fp16 range as two fp16 arrays, S is split per row at plan
-                                   time, the scales are undone exactly in the epilogue;
-                                   tcgen05 3xTF32 forms: 2 = CTA pairs (cta_group::2), 3 = single CTA, both
-                                   operands in shared memory, 4 = single CTA, V_hi/V_lo operand in tensor
-                                   memory, 5 = form 3 on clusters of two CTAs that TMA-multicast the S tiles to
-                                   each other;
+                                   time, the scales are undone exactly in the epilogue, and a7 (sum_l U_pl A_l,
+                                   PAPER.md:53) runs in the same epilogue, so U never reaches HBM (DESIGN.md
+                                   section 7);
                                    6 = exact low-rank form on the 3xTF32 kernel,
                                    8 = the same on the kind::f16 kernel: S_(pl),(mn) = sum_k L_(pl),k L_(mn),k
                                    by pivoted Cholesky at plan time (Eq. 2 makes S a Gram matrix; rank 153 of
                                    1035 for 45 Hermite-Gauss modes), two GEMMs Q x R and R x Q instead of Q x Q;
                                    EUNSUPPORTED if S is not positive semi-definite.  Never chosen by auto:
-                                   BASELINE.json names the dense contraction.  2-8 need complex64 and
-                                   N % 128 == 0 (2, 5: N % 256 == 0), else EUNSUPPORTED.  Forms 2-5 are kept
-                                   for measurement: none beats form 3, and form 7 is twice as fast as form 3
-                                   on B200                                     */
+                                   BASELINE.json names the dense contraction.  3-8 need complex64 and
+                                   N % 128 == 0, else EUNSUPPORTED.  Other values: EINVAL                */
   int    raman;                 /* a5 kernel: 0 = auto, 1 = FFT . h~_R . IFFT on the pair streams (any h_R),
                                    2 = one-pole recurrence along t, exact when the samples are a damped
                                    oscillation h_R[j] = Im(c zeta^j) (the tau1/tau2 form); auto picks 2 when
@@ -90,8 +87,10 @@ typedef struct {                /* pass NULL for defaults                       
  *             symmetric under m<->n and p<->l (true for Eq. 2); otherwise EUNSUPPORTED.
  *   f_R, h_R  Raman fraction; HOST [N] samples h_R(j dt) in 1/s (NULL iff f_R == 0)
  *   omega0    carrier [rad/s];  n2 [m^2/W]
- * Host arrays are copied; the caller keeps ownership.  EINVAL: sizes < 1, N not a power of
- * two, pi/dt >= omega0 with shock on, NULL pointers, non-finite beta/S/h_R.               */
+ * Host arrays are copied; the caller keeps ownership.  The plan lives on the CUDA device that is
+ * current at creation; every later call runs there whatever the caller's current device.
+ * EINVAL: sizes < 1, N not a power of two, pi/dt >= omega0 with shock on, NULL pointers,
+ * non-finite beta/S/h_R, f_R outside [0, 1].                                              */
 int gmmnlse_plan_create(gmmnlse_plan **out, int P, int N, int M, double dt, double dz,
                         const double *beta, int n_beta, const double *S,
                         double f_R, const double *h_R, double omega0, double n2,
@@ -114,20 +113,21 @@ int gmmnlse_plan_create_general(gmmnlse_plan **out, int P, int N, int M, double 
  *                domain, sqrt(W); A_out may alias A_in; never freed by the library.
  *   L            [m], an integer multiple of dz (1e-9 relative) else EINVAL; the last large
  *                step uses (L/dz) mod M planes.
- *   stream       cudaStream_t as void* (NULL = the plan's current stream).  Work is enqueued
- *                on it.  Device loop (options.graph = 0): the call returns after one
- *                read-back of the loop counters that follows the last kernel, so A_out is
- *                complete on return.  Host loop: it returns after the last convergence
- *                decision was read back (one 8-byte D2H per iteration) and A_out is
- *                complete only after the stream is synchronised.  `stream` must not be
- *                capturing.                                                                */
+ *   stream       cudaStream_t as void*; applies to THIS call only (NULL = the plan's stream, see
+ *                gmmnlse_set_stream).  Work is enqueued on it and the call returns after one
+ *                synchronise that follows the last kernel: A_out is complete on return and the
+ *                counters of gmmnlse_get_stats are current (the return code WARN_NOCONV needs
+ *                them).  Device loop (options.graph = 0): that is the only synchronise of the
+ *                call; host loop: one 8-byte D2H + synchronise per iteration as well.  `stream`
+ *                must not be capturing.                                                     */
 int gmmnlse_propagate(gmmnlse_plan *plan, const void *A_in, double L, void *A_out, void *stream);
 
 /* Same as gmmnlse_propagate but A_in / A_out are HOST [P][N] buffers of the plan's
  * precision: H2D copy, propagate, D2H copy on the plan's stream, one synchronise; A_out is
  * complete on return.  Page-locked buffers (cudaMallocHost / cudaHostRegister) are copied
- * from and to directly; pageable ones are staged through plan-owned pinned memory.  This is
- * the end-to-end entry bench.py times (with page-locked buffers).                          */
+ * from and to directly; pageable ones are staged through plan-owned pinned memory; device or
+ * managed pointers are EINVAL (use gmmnlse_propagate).  This is the end-to-end entry
+ * bench.py times (with page-locked buffers).                                               */
 int gmmnlse_propagate_host(gmmnlse_plan *plan, const void *A_in_host, double L, void *A_out_host);
 
 /* Serial comparison integrator (the role of the split-step code the paper times the
@@ -155,6 +155,8 @@ int gmmnlse_set_coupling(gmmnlse_plan *plan, const double *Q);
  * A, dA: DEVICE [P][N] as above (dA must not alias A); enqueued on the plan's stream.      */
 int gmmnlse_nonlinear_op(gmmnlse_plan *plan, const void *A, void *dA);
 
+/* Bind the plan to a stream: every later call that is given no stream of its own (NULL, or calls without a
+ * stream argument: nonlinear_op, propagate_host, the debug_* stages) enqueues there.  Default: the NULL stream. */
 int gmmnlse_set_stream(gmmnlse_plan *plan, void *stream);
 
 /* Counters accumulated since plan creation (any pointer may be NULL).                      */
@@ -193,10 +195,9 @@ int gmmnlse_debug_pairs(gmmnlse_plan *plan, const void *A, void *V, int n_planes
 /*   contract: U[plane][r][t] = sum_q S2[r][q] V[plane][q][t] over packed pairs r = (p<=l), q = (m<=n),
  *          S2 = S_plmn with the m<n columns doubled (Eq. 1's sum over m,n); V, U DEVICE
  *          [n_planes][Q][N] real of the plan's precision, U must not alias V.
- *   contraction_kind: which a6 kernel the plan selected: 1 CUDA cores, 2 tcgen05 single CTA (operands in
- *          shared memory), 3 tcgen05 CTA pairs, 4 tcgen05 single CTA with the V operand in tensor memory,
- *          5 tcgen05 multicast pairs, 6 low-rank pair of 3xTF32 GEMMs, 7 tcgen05 kind::f16 on fp16 hi/lo
- *          splits, 8 low-rank pair of kind::f16 GEMMs.  With 7 and 8 debug_pairs still writes fp32 V, and
+ *   contraction_kind: which a6 kernel the plan selected (the values of options.contraction): 1 CUDA cores,
+ *          3 tcgen05 3xTF32, 6 low-rank pair of 3xTF32 GEMMs, 7 tcgen05 kind::f16 on fp16 hi/lo splits,
+ *          8 low-rank pair of kind::f16 GEMMs.  With 7 and 8 debug_pairs still writes fp32 V, and
  *          debug_contract splits the caller's fp32 V into fp16 pairs first (scaled by its own max |V|).                                                            */
 int gmmnlse_debug_contract(gmmnlse_plan *plan, const void *V, void *U, int n_planes);
 int gmmnlse_contraction_kind(const gmmnlse_plan *plan);
@@ -213,12 +214,6 @@ int gmmnlse_raman_kind(const gmmnlse_plan *plan);
  *          drains it into fp32 registers (default 4); bounds the bias of the tensor core's truncating
  *          accumulate.  1 <= k <= 255.                        */
 int gmmnlse_debug_set_tc_chunk(gmmnlse_plan *plan, int k);
-/*   set_probe: measurement knobs behind profiles/r01c-r01h.  probe_bits: timing probes of the tcgen05 contraction
- *          (1 skip the V_lo conversion, 2 / 8 / 16 skip all / A / B TMA loads after the first fill, 4 skip the U
- *          stores, 32 skip the MMAs) -- RESULTS ARE WRONG when non-zero, time only; stage_cap: cap on its
- *          shared-memory stages (0 = as many as fit); a7_tile: samples per CTA of the mode reduction (0 auto, 32,
- *          64, 128).  EINVAL on other values.                                                   */
-int gmmnlse_debug_set_probe(gmmnlse_plan *plan, int probe_bits, int stage_cap, int a7_tile);
 
 void gmmnlse_plan_destroy(gmmnlse_plan *plan);
 const char *gmmnlse_status_string(int status);

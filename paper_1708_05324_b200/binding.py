@@ -62,7 +62,6 @@ SIGNATURES = {
     "gmmnlse_lowrank_rank": (C.c_int, [C.c_void_p]),
     "gmmnlse_loop_kind": (C.c_int, [C.c_void_p]),
     "gmmnlse_debug_set_tc_chunk": (C.c_int, [C.c_void_p, C.c_int]),
-    "gmmnlse_debug_set_probe": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int]),
     "gmmnlse_plan_destroy": (None, [C.c_void_p]),
     "gmmnlse_status_string": (C.c_char_p, [C.c_int]),
     "gmmnlse_last_cuda_error": (C.c_char_p, []),
@@ -226,7 +225,7 @@ class Plan:
         _check(self._lib, self._lib.gmmnlse_debug_contract(self._h, _ptr(V), _ptr(U), n_planes))
 
     def contraction_kind(self) -> int:
-        """1 = CUDA cores, 2 = tcgen05 single CTA (SS), 3 = tcgen05 CTA pairs, 4 = tcgen05 single CTA (TS)."""
+        """1 CUDA cores, 3 tcgen05 3xTF32, 7 tcgen05 kind::f16 (a7 fused), 6 / 8 the low-rank pairs of those."""
         return int(self._lib.gmmnlse_contraction_kind(self._h))
 
     def lowrank_rank(self) -> int:
@@ -241,9 +240,6 @@ class Plan:
 
     def debug_set_tc_chunk(self, k: int) -> None:
         _check(self._lib, self._lib.gmmnlse_debug_set_tc_chunk(self._h, int(k)))
-
-    def debug_set_probe(self, probe_bits: int = 0, stage_cap: int = 0, a7_tile: int = 0) -> None:
-        _check(self._lib, self._lib.gmmnlse_debug_set_probe(self._h, int(probe_bits), int(stage_cap), int(a7_tile)))
 
     def destroy(self) -> None:
         if self._h:

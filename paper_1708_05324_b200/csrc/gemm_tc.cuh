@@ -3,7 +3,7 @@
 // as a split-precision ("3xTF32") tcgen05 GEMM with fp32 accumulation in tensor memory.
 //
 // Orientation: D[t][r] = sum_q A[t][q] B[r][q] with A = V_j^T and B = S2.
-//   * M = t: 128 samples per CTA (256 per CTA pair with cta_group::2) -- N is a power of two, so
+//   * M = t: 128 samples per CTA -- N is a power of two, so
 //     the M tiles have no ragged edge; each TMEM lane is one time sample, so the epilogue's stores
 //     (one column r at a time, 32 lanes = 32 consecutive t) are coalesced into U[r][t].
 //   * N = r: NT packed pair rows per tile, NT = 16-multiple <= 256 chosen so that n_rt*NT >= Q with
@@ -28,8 +28,6 @@
 // Warp roles (576 threads): warp 0 TMA producer, warp 1 MMA issuer + TMEM allocator, warps 2-5
 // converters, warps 6-17 epilogue (three per TMEM lane group, each owning a third of the NT columns).
 // Pipelines: smem stages (full -> conv -> empty) and two TMEM accumulators (tmem_full / tmem_empty).
-// With CG == 2 the kernel runs as clusters of two CTAs: each loads its own 128 t of A and half of
-// the NT rows of B, the leader issues tcgen05.mma.cta_group::2 (M = 256) for both.
 #pragma once
 #include <cuda.h>
 
@@ -54,21 +52,14 @@ struct Params {
   float* U;                    // [plane][Q][N]
   long long u_plane_stride;    // elements
   int Q, N, NT, KB, n_rt, t_tiles, total_tiles, plane0, stages, kchunk;
-  int probe;                   // timing probes only (results wrong): 1 skip V_lo conversion, 2 / 8 / 16 skip all / A /
-                               // B TMA loads after the first fill, 4 skip the U stores, 32 skip the MMAs
 };
 
-__host__ __device__ inline int b_bytes(int NT, int CG) { return (NT / CG) * BK * 4; }
-__host__ __device__ inline int stage_bytes(int NT, int CG) { return 2 * A_BYTES + 2 * b_bytes(NT, CG); }
-inline size_t smem_bytes(int NT, int CG, int stages) {
-  return 1024 /*alignment slack*/ + 1024 /*barriers*/ + (size_t)stages * stage_bytes(NT, CG);
+__host__ __device__ inline int b_bytes(int NT) { return NT * BK * 4; }
+__host__ __device__ inline int stage_bytes(int NT) { return 2 * A_BYTES + 2 * b_bytes(NT); }
+inline size_t smem_bytes(int NT, int stages) {
+  return 1024 /*alignment slack*/ + 1024 /*barriers*/ + (size_t)stages * stage_bytes(NT);
 }
 
-// MC (needs CG == 1): clusters of two CTAs work on neighbouring t-tiles of the same r-tile; each loads half of the
-// S_hi / S_lo rows and TMA-multicasts it into both CTAs' shared memory, halving the L2 reads of the B operand
-// (77 % of the bytes a k-block needs).  MMAs stay per-CTA (cta_group::1); a stage is free when BOTH CTAs' MMAs
-// have released it (tcgen05.commit multicast onto both `empty` barriers, count 2).
-template <int CG, bool MC = false>
 __global__ void __launch_bounds__(NTHREADS, 1)
 k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmShi,
               const __grid_constant__ CUtensorMap tmSlo, const Params p) {
@@ -85,10 +76,7 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
   unsigned char* tiles_ptr = sm + 1024;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  static_assert(!(MC && CG == 2), "multicast form uses per-CTA MMAs");
-  constexpr int CL = (CG == 2 || MC) ? 2 : 1;            // CTAs per cluster
-  const uint32_t rank = CL == 2 ? cluster_ctarank() : 0u;
-  const int nb = b_bytes(p.NT, CG), sbytes = stage_bytes(p.NT, CG);
+  const int nb = b_bytes(p.NT), sbytes = stage_bytes(p.NT);
   const int stages = p.stages;
 
   if (warp == 0 && lane == 0) {
@@ -100,25 +88,25 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
     if (lane == 0) {
       for (int s = 0; s < MAX_STAGES; ++s) {
         mbar_init(bar_full + 8 * s, 1);
-        mbar_init(bar_empty + 8 * s, MC ? 2 : 1);
-        mbar_init(bar_conv + 8 * s, 4 * CG);
+        mbar_init(bar_empty + 8 * s, 1);
+        mbar_init(bar_conv + 8 * s, 4);
       }
       for (int a = 0; a < 2; ++a) {
         mbar_init(bar_tfull + 8 * a, 1);
-        mbar_init(bar_tempty + 8 * a, NUM_EPI_WARPS * CG);
+        mbar_init(bar_tempty + 8 * a, NUM_EPI_WARPS);
       }
       fence_barrier_init();
     }
     __syncwarp();
-    tmem_alloc<CG>(slot_addr, TMEM_COLS);
-    tmem_relinquish<CG>();
+    tmem_alloc<1>(slot_addr, TMEM_COLS);
+    tmem_relinquish<1>();
   }
   tc_fence_before();
-  if constexpr (CL == 2) cluster_sync_all(); else __syncthreads();
+  __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
-  const int pair = blockIdx.x / CL, npairs = gridDim.x / CL;
+  const int pair = blockIdx.x, npairs = gridDim.x;
   const int tiles_per_plane = p.n_rt * p.t_tiles;
 
   if (warp == 0) {
@@ -129,54 +117,38 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
       for (int tile = pair; tile < p.total_tiles; tile += npairs) {
         const int pl = tile / tiles_per_plane, rem = tile - pl * tiles_per_plane;
         const int tt = rem / p.n_rt, rt = rem - tt * p.n_rt;
-        const int t0 = tt * (TM * CL) + (int)rank * TM;
-        const int r0 = rt * p.NT + (int)rank * (p.NT / CL);
+        const int t0 = tt * TM;
+        const int r0 = rt * p.NT;
         for (int kb = 0; kb < p.KB; ++kb) {
           mbar_wait(bar_empty + 8 * stage, phase ^ 1u, 1);
           const uint32_t fb = bar_full + 8 * stage;
           const uint32_t sa = tiles_addr + stage * sbytes;
-          const bool warm = tile != pair || kb >= stages;
-          const bool skipA = warm && (p.probe & (2 | 8)), skipB = warm && (p.probe & (2 | 16));
-          if (skipA && skipB) {
-            mbar_arrive(fb);
-          } else {
-            mbar_arrive_expect_tx(fb, (skipA ? 0u : (uint32_t)A_BYTES) + (skipB ? 0u : (uint32_t)(2 * nb)));
-            if (!skipA) {
+          mbar_arrive_expect_tx(fb, (uint32_t)(A_BYTES + 2 * nb));
 #pragma unroll
-              for (int i = 0; i < TM / 32; ++i)                   // 4 boxes of 32 t x BK q
-                tma_load_3d(sa + i * (BK * 128), &tmV, fb, t0 + 32 * i, kb * BK, p.plane0 + pl);
-            }
-            if (!skipB) {
-              if constexpr (MC) {                                  // my half of the rows, into both CTAs
-                const uint32_t half = (uint32_t)(nb / 2) * rank;
-                tma_load_2d_mc(sa + 2 * A_BYTES + half, &tmShi, fb, kb * BK, r0, (uint16_t)3);
-                tma_load_2d_mc(sa + 2 * A_BYTES + nb + half, &tmSlo, fb, kb * BK, r0, (uint16_t)3);
-              } else {
-                tma_load_2d(sa + 2 * A_BYTES, &tmShi, fb, kb * BK, r0);
-                tma_load_2d(sa + 2 * A_BYTES + nb, &tmSlo, fb, kb * BK, r0);
-              }
-            }
-          }
+          for (int i = 0; i < TM / 32; ++i)                       // 4 boxes of 32 t x BK q
+            tma_load_3d(sa + i * (BK * 128), &tmV, fb, t0 + 32 * i, kb * BK, p.plane0 + pl);
+          tma_load_2d(sa + 2 * A_BYTES, &tmShi, fb, kb * BK, r0);
+          tma_load_2d(sa + 2 * A_BYTES + nb, &tmSlo, fb, kb * BK, r0);
           if (++stage == stages) { stage = 0; phase ^= 1u; }
         }
       }
     }
   } else if (warp == 1) {
-    // ================================================================= MMA issuer (leader CTA)
-    if (lane == 0 && (CG == 1 || rank == 0)) {             // CG == 2: only the leader CTA issues
-      // instruction descriptor: D fp32, A/B tf32, A MN-major, B K-major, N = NT, M = 128 * CG
+    // ================================================================= MMA issuer
+    if (lane == 0) {
+      // instruction descriptor: D fp32, A/B tf32, A MN-major, B K-major, N = NT, M = 128
       const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 15) | ((uint32_t)(p.NT >> 3) << 17) |
-                             ((uint32_t)((TM * CG) >> 4) << 24);
+                             ((uint32_t)(TM >> 4) << 24);
       int stage = 0, acc = 0;
       uint32_t phase = 0, acc_phase = 0;
       for (int tile = pair; tile < p.total_tiles; tile += npairs) {
         for (int kb = 0, inchunk = 0; kb < p.KB; ++kb) {
           if (inchunk == 0) {                                      // new chunk: claim a TMEM accumulator
-            mbar_wait<CG == 2>(bar_tempty + 8 * acc, acc_phase ^ 1u, 2);
+            mbar_wait(bar_tempty + 8 * acc, acc_phase ^ 1u, 2);
             tc_fence_after();
           }
           const uint32_t d = tmem_base + (uint32_t)(acc * ACC_COLS);
-          mbar_wait<CG == 2>(bar_conv + 8 * stage, phase, 3);
+          mbar_wait(bar_conv + 8 * stage, phase, 3);
           tc_fence_after();
           const uint32_t sa = tiles_addr + stage * sbytes;
           // A: MN-major, 128-byte swizzle with 32-byte atoms (TMA SWIZZLE_128B_ATOM_32B): rows of 32 t
@@ -186,20 +158,18 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
           // B: K-major rows of BK q (64 B: SWIZZLE_64B), 8-row groups B_SBO apart; LBO unused when swizzled
           const uint64_t b_hi = make_smem_desc(sa + 2 * A_BYTES, 16, B_SBO, B_LAYOUT);
           const uint64_t b_lo = make_smem_desc(sa + 2 * A_BYTES + nb, 16, B_SBO, B_LAYOUT);
-          if (!(p.probe & 32))
 #pragma unroll
           for (int kk = 0; kk < BK / 8; ++kk) {
             const uint64_t da = (uint64_t)(kk * (1024 >> 4));      // next 8 q of A: +1024 B
             const uint64_t db = (uint64_t)(kk * (32 >> 4));        // next 8 q of B: +32 B in the row
-            mma_tf32_ss<CG>(d, a_raw + da, b_lo + db, idesc, (inchunk | kk) != 0 ? 1u : 0u);
-            mma_tf32_ss<CG>(d, a_lo + da, b_hi + db, idesc, 1u);
-            mma_tf32_ss<CG>(d, a_raw + da, b_hi + db, idesc, 1u);
+            mma_tf32_ss<1>(d, a_raw + da, b_lo + db, idesc, (inchunk | kk) != 0 ? 1u : 0u);
+            mma_tf32_ss<1>(d, a_lo + da, b_hi + db, idesc, 1u);
+            mma_tf32_ss<1>(d, a_raw + da, b_hi + db, idesc, 1u);
           }
-          if constexpr (MC) mma_commit_mc(bar_empty + 8 * stage);  // frees the smem stage in both CTAs
-          else mma_commit<CG>(bar_empty + 8 * stage);
+          mma_commit<1>(bar_empty + 8 * stage);
           if (++stage == stages) { stage = 0; phase ^= 1u; }
           if (++inchunk == p.kchunk || kb == p.KB - 1) {           // chunk complete: hand it to the epilogue
-            mma_commit<CG>(bar_tfull + 8 * acc);
+            mma_commit<1>(bar_tfull + 8 * acc);
             inchunk = 0;
             if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
           }
@@ -216,7 +186,6 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
         mbar_wait(bar_full + 8 * stage, phase, 4);
         float4* raw = reinterpret_cast<float4*>(tiles_ptr + (size_t)stage * sbytes);
         float4* lo = reinterpret_cast<float4*>(tiles_ptr + (size_t)stage * sbytes + A_BYTES);
-        if (!(p.probe & 1))
 #pragma unroll
         for (int j = 0; j < A_BYTES / 16 / 128; ++j) {
           const int idx = tid_c + 128 * j;
@@ -234,10 +203,7 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
         }
         fence_proxy_async_smem();                 // generic-proxy writes -> visible to the MMA's async reads
         __syncwarp();
-        if (lane == 0) {
-          if (CG == 2) mbar_arrive_cluster(bar_conv + 8 * stage, 0);
-          else mbar_arrive(bar_conv + 8 * stage);
-        }
+        if (lane == 0) mbar_arrive(bar_conv + 8 * stage);
         if (++stage == stages) { stage = 0; phase ^= 1u; }
       }
     }
@@ -255,7 +221,7 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
     for (int tile = pair; tile < p.total_tiles; tile += npairs) {
       const int pl = tile / tiles_per_plane, rem = tile - pl * tiles_per_plane;
       const int tt = rem / p.n_rt, rt = rem - tt * p.n_rt;
-      const int t = tt * (TM * CL) + (int)rank * TM + lg * 32 + lane;
+      const int t = tt * TM + lg * 32 + lane;
       float* Uout = p.U + (long long)pl * p.u_plane_stride + t;
 #pragma unroll
       for (int i = 0; i < EPI_COLS; ++i) accr[i] = 0.f;
@@ -281,17 +247,14 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
         }
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) {
-          if (CG == 2) mbar_arrive_cluster(bar_tempty + 8 * acc, 0);
-          else mbar_arrive(bar_tempty + 8 * acc);
-        }
+        if (lane == 0) mbar_arrive(bar_tempty + 8 * acc);
         if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
       }
       const int rbase = rt * p.NT + cbeg;
 #pragma unroll
       for (int c = 0; c < EPI_COLS; ++c) {
         const int r = rbase + c;
-        if (c < ncols && r < p.Q && !(p.probe & 4)) Uout[(long long)r * p.N] = accr[c];
+        if (c < ncols && r < p.Q) Uout[(long long)r * p.N] = accr[c];
       }
     }
   }
@@ -299,9 +262,9 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
   // ------------------------------------------------------------------- teardown
   __syncwarp();
   tc_fence_before();
-  if constexpr (CL == 2) cluster_sync_all(); else __syncthreads();
+  __syncthreads();
   tc_fence_after();
-  if (warp == 1) tmem_dealloc<CG>(tmem_base, TMEM_COLS);
+  if (warp == 1) tmem_dealloc<1>(tmem_base, TMEM_COLS);
 }
 
 }  // namespace tc

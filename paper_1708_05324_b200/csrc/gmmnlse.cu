@@ -8,13 +8,14 @@
 #include <cstdio>
 #include <cstring>
 #include <map>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
 
 #include "../../include/gmmnlse.h"
-#include "gemm_ts.cuh"
 #include "gemm_h.cuh"
+#include "gemm_tc.cuh"
 #include "kernels.cuh"
 
 namespace {
@@ -103,6 +104,30 @@ int encode_tmap_f32(CUtensorMap* out, void* base, int rank, const cuuint64_t* di
   return encode_tmap(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, base, rank, dims, strides, box, swz);
 }
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a property of (device, kernel), not of the process: remember the
+// largest size granted per pair and only ever raise it (plans on several devices, or of several shapes, share kernels).
+std::mutex g_attr_mu;
+std::map<std::pair<int, const void*>, size_t> g_attr;
+int ensure_dyn_smem(int device, const void* fn, size_t bytes) {
+  std::lock_guard<std::mutex> lk(g_attr_mu);
+  size_t& have = g_attr[std::make_pair(device, fn)];
+  if (bytes <= have || bytes <= 48 * 1024) return 0;
+  GM_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+  have = bytes;
+  return 0;
+}
+
+struct DeviceGuard {            // run a call on the plan's device, restore the caller's current device afterwards
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+};
+
 int ilog2(int n) {
   int l = 0;
   while ((1 << l) < n) ++l;
@@ -116,6 +141,7 @@ struct gmmnlse_plan {
   int P = 0, N = 0, M = 0, log2N = 0, Q = 0, precision = 0, shock = 1, max_iter = 0, fixed_iter = 0;
   int contraction = 0, raman = 0, graph = 0;
   int loop_state = 0;                      // 0 host loop so far, 1 device loop (CUDA graph) in use, -1 graph build failed
+  int device = 0;                          // the CUDA device the plan was created on (every call runs there)
   // general form of Eq. 1 (gmmnlse_plan_create_general): separate, possibly complex tensors, no symmetry
   bool general = false, gen_complex = false;
   const double* gen_SR = nullptr;          // host, valid during init only
@@ -145,8 +171,9 @@ struct gmmnlse_plan {
   void prof_end() {
     if (prof_on) cudaEventRecord(prof_ev[prof_used++], stream);
   }
-  int prof_collect() {   // synchronises the stream
-    if (cudaStreamSynchronize(stream) != cudaSuccess) return GMMNLSE_ECUDA;
+  int prof_collect() {   // waits for the recorded events
+    // wait for the last recorded event, not for `stream`: a per-call stream argument is no longer bound to the plan
+    if (prof_used > 0 && cudaEventSynchronize(prof_ev[prof_used - 1]) != cudaSuccess) return GMMNLSE_ECUDA;
     for (size_t i = 0; i + 1 < prof_used; i += 2) {
       float ms = 0;
       if (cudaEventElapsedTime(&ms, prof_ev[i], prof_ev[i + 1]) != cudaSuccess) return GMMNLSE_ECUDA;
@@ -174,7 +201,6 @@ struct gmmnlse_plan {
   virtual int debug_contract(const void* V, void* U, int n_planes) = 0;
   virtual int contraction_kind() const = 0;
   virtual int set_tc_chunk(int k) = 0;
-  virtual int set_probe(int probe_bits, int stage_cap, int a7_tile) = 0;
   virtual int raman_kind() const = 0;
   virtual int lowrank_rank() const = 0;
   virtual void drop_loop_graph() = 0;
@@ -214,7 +240,7 @@ struct PlanT final : gmmnlse_plan {
   cudaGraph_t rkg = nullptr;
   cudaGraphExec_t rkg_exec = nullptr;
   long long rk_c = 0;                              // kernel launches per RK4IP step
-  bool rk_warmed = false;
+  bool rk_warmed = false, rk_graph_failed = false;
   long long PN = 0, QN = 0;
   // NEXT-3: small-signal gain g_p (joins D as its real part) and constant linear coupling Q_np
   std::vector<double> gain;                // [P], 1/m; empty = none
@@ -259,9 +285,9 @@ struct PlanT final : gmmnlse_plan {
   float v_gain = 1.f;          // |V| <= v_gain max |A|^2
   HalfOut cur_ho = {nullptr, 0, 0, 0, nullptr};
   CUtensorMap tmVh, tmVl, tmZh, tmZl;
-  bool tc_ts = false;          // A operand from tensor memory (gemm_ts.cuh)
-  bool tc_mc = false;          // clusters of two CTAs multicasting the S tiles (gemm_tc.cuh, MC)
-  int tc_cg = 0, tc_NT = 0, tc_nrt = 0, tc_KB = 0, tc_stages = 0, tc_kchunk = 4, tc_probe = 0, tc_stage_cap = 0, n_sm = 0, mr_tile = 0;
+  bool tc_on = false;          // dense 3xTF32 form (gemm_tc.cuh)
+  int tc_NT = 0, tc_nrt = 0, tc_KB = 0, tc_stages = 0, tc_kchunk = 4, n_sm = 0;
+  template <typename F> int ensure_smem(F fn, size_t bytes) { return ensure_dyn_smem(device, (const void*)fn, bytes); }
 
   ~PlanT() override {
     cudaFree(tw); cudaFree(Kw); cudaFree(H); cudaFree(E); cudaFree(EM_d); cudaFree(S2);
@@ -478,14 +504,7 @@ struct PlanT final : gmmnlse_plan {
   int launch_pairs_iir_t(const C* A, long long a_ps, T* Vout, long long v_ps, int planes) {
     constexpr int NT = (1 << LOG2N) / 16, NW = (NT + 31) / 32;
     const size_t smem = sizeof(C) * (fft_smem_elems(1 << LOG2N) + 2 * NW + 2);
-    static bool configured = false;
-    if (!configured) {
-      GM_CUDA(cudaFuncSetAttribute(k_pair_iir<T, LOG2N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)smem));
-      GM_CUDA(cudaFuncSetAttribute(k_pair_iir<T, LOG2N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)smem));
-      configured = true;
-    }
+    GM_TRY(general ? ensure_smem(k_pair_iir<T, LOG2N, true>, smem) : ensure_smem(k_pair_iir<T, LOG2N, false>, smem));
     prof_begin(GMMNLSE_KIND_PAIR_CONV);
     const dim3 grid((Q + 1) / 2, planes);
     if (general)
@@ -517,10 +536,6 @@ struct PlanT final : gmmnlse_plan {
   int make_v_tmap(CUtensorMap* tm, const T* base, int planes) {
     const cuuint64_t dims[3] = {(cuuint64_t)N, (cuuint64_t)Q, (cuuint64_t)planes};
     const cuuint64_t strides[2] = {(cuuint64_t)N * 4, (cuuint64_t)QN * 4};
-    if (tc_ts) {                                     // TS form: one plain [BK q][128 t] box, read by threads only
-      const cuuint32_t box_ts[3] = {tc::TM, tc::BK, 1};
-      return encode_tmap_f32(tm, (void*)base, 3, dims, strides, box_ts, CU_TENSOR_MAP_SWIZZLE_NONE);
-    }
     const cuuint32_t box[3] = {32, tc::BK, 1};
     // t-contiguous operand: 32-byte swizzle atoms (the only MN-major layout kind::tf32 accepts)
     return encode_tmap_f32(tm, (void*)base, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B);
@@ -538,7 +553,7 @@ struct PlanT final : gmmnlse_plan {
     g.NT = (((rows + g.nrt - 1) / g.nrt) + 15) / 16 * 16;
     g.KB = (K + tc::BK - 1) / tc::BK;
     g.stages = tc::MAX_STAGES;
-    while (g.stages > 1 && tc::smem_bytes(g.NT, 1, g.stages) > (size_t)smax) --g.stages;
+    while (g.stages > 1 && tc::smem_bytes(g.NT, g.stages) > (size_t)smax) --g.stages;
     const int Rp = g.nrt * g.NT, Kp = g.KB * tc::BK;
     std::vector<float> hi((size_t)Rp * Kp, 0.f), lo((size_t)Rp * Kp, 0.f);
     for (int r = 0; r < rows; ++r)
@@ -566,14 +581,14 @@ struct PlanT final : gmmnlse_plan {
       prm.Q = g.rows; prm.N = N; prm.NT = g.NT; prm.KB = g.KB; prm.n_rt = g.nrt;
       prm.t_tiles = N / tc::TM;
       prm.total_tiles = planes * prm.t_tiles * g.nrt;
-      prm.plane0 = plane0; prm.stages = g.stages; prm.kchunk = tc_kchunk; prm.probe = 0;
+      prm.plane0 = plane0; prm.stages = g.stages; prm.kchunk = tc_kchunk;
       cudaLaunchConfig_t cfg = {};
       cfg.gridDim = dim3((unsigned)std::min(n_sm, prm.total_tiles));
       cfg.blockDim = dim3(tc::NTHREADS);
-      cfg.dynamicSmemBytes = tc::smem_bytes(g.NT, 1, g.stages);
+      cfg.dynamicSmemBytes = tc::smem_bytes(g.NT, g.stages);
       cfg.stream = stream;
       prof_begin(GMMNLSE_KIND_CONTRACT);
-      cudaError_t e = cudaLaunchKernelEx(&cfg, tc::k_contract_tc<1>, amap, g.tmHi, g.tmLo, prm);
+      cudaError_t e = cudaLaunchKernelEx(&cfg, tc::k_contract_tc, amap, g.tmHi, g.tmLo, prm);
       prof_end();
       GM_CUDA(e);
       return 0;
@@ -644,8 +659,6 @@ struct PlanT final : gmmnlse_plan {
       prm.total_tiles = planes * prm.t_tiles * g.nrt;
       prm.plane0 = plane0; prm.stages = g.stages;
       prm.kchunk = tc_kchunk;                                    // k-blocks of 32 q here (16 q in the TF32 forms)
-      prm.probe = tc_probe;
-      if (tc_stage_cap > 0 && tc_stage_cap < prm.stages) prm.stages = tc_stage_cap;
       cudaLaunchConfig_t cfg = {};
       cfg.gridDim = dim3((unsigned)std::min(n_sm, prm.total_tiles));
       cfg.blockDim = dim3(hc::NTHREADS);
@@ -664,8 +677,8 @@ struct PlanT final : gmmnlse_plan {
     GM_CUDA(cudaMemset(d_vbound, 0, sizeof(float)));
     GM_TRY(h_a_tmaps(&tmVh, &tmVl, V, Q, M + 1));
     if constexpr (sizeof(T) == 4) {
-      GM_CUDA(cudaFuncSetAttribute(hc::k_contract_h<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smax));
-      GM_CUDA(cudaFuncSetAttribute(hc::k_contract_h<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smax));
+      GM_TRY(ensure_smem(hc::k_contract_h<false>, (size_t)smax));
+      GM_TRY(ensure_smem(hc::k_contract_h<true>, (size_t)smax));
     }
     tc_h = true;
     return 0;
@@ -735,8 +748,7 @@ struct PlanT final : gmmnlse_plan {
     GM_TRY(dalloc(&Zb, (size_t)(M + 1) * R * N));
     GM_TRY(make_a_tmap(&tmZ, Zb, R, M + 1));
     GM_TRY(make_a_tmap(&tmV, V, Q, M + 1));
-    if constexpr (sizeof(T) == 4)
-      GM_CUDA(cudaFuncSetAttribute(tc::k_contract_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smax));
+    if constexpr (sizeof(T) == 4) GM_TRY(ensure_smem(tc::k_contract_tc, (size_t)smax));
     lowrank = true;
     return 0;
   }
@@ -769,17 +781,10 @@ struct PlanT final : gmmnlse_plan {
         GM_CUDA(cudaDeviceGetAttribute(&smax0, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev0));
         return init_lowrank(h_S2, smax0);
       }
-      // auto picks the single-CTA form: measured 1.76 ms against 1.86 ms for CTA pairs at config 5
-      int cg = contraction == 2 ? 2 : 1;
-      // the tensor-memory (TS) form measured the same as the shared-memory (SS) form (1.68 vs 1.67 ms at config 5):
-      // auto keeps SS, the form the committed ncu profiles describe; 4 selects TS
-      tc_ts = contraction == 4;
-      tc_mc = contraction == 5 && N % (2 * tc::TM) == 0;
-      if (contraction == 5 && !tc_mc) return GMMNLSE_EUNSUPPORTED;
-      if (N % (tc::TM * cg) != 0) {
-        if (N % tc::TM == 0) cg = 1;
-        else if (contraction >= 2) return GMMNLSE_EUNSUPPORTED;
-        else return 0;
+      // dense 3xTF32 form: single CTA per tile, both operands in shared memory
+      if (N % tc::TM != 0) {
+        if (contraction >= 2) return GMMNLSE_EUNSUPPORTED;
+        return 0;
       }
       int dev = 0;
       GM_CUDA(cudaGetDevice(&dev));
@@ -791,9 +796,8 @@ struct PlanT final : gmmnlse_plan {
       int smax = 0;
       GM_CUDA(cudaDeviceGetAttribute(&smax, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
       tc_stages = tc::MAX_STAGES;
-      auto need = [&](int st) { return tc_ts ? tc::ts_smem_bytes(tc_NT, st) : tc::smem_bytes(tc_NT, cg, st); };
-      while (tc_stages > 1 && need(tc_stages) > (size_t)smax) --tc_stages;
-      if (need(tc_stages) > (size_t)smax) return GMMNLSE_EUNSUPPORTED;
+      while (tc_stages > 1 && tc::smem_bytes(tc_NT, tc_stages) > (size_t)smax) --tc_stages;
+      if (tc::smem_bytes(tc_NT, tc_stages) > (size_t)smax) return GMMNLSE_EUNSUPPORTED;
       std::vector<float> hi((size_t)Rp * Qp, 0.f), lo((size_t)Rp * Qp, 0.f);
       for (int r = 0; r < Q; ++r)
         for (int q = 0; q < Q; ++q) {
@@ -806,21 +810,13 @@ struct PlanT final : gmmnlse_plan {
       GM_TRY(dalloc(&S2lo, lo.size())); GM_TRY(upload(S2lo, lo));
       const cuuint64_t dims[2] = {(cuuint64_t)Qp, (cuuint64_t)Rp};
       const cuuint64_t strides[1] = {(cuuint64_t)Qp * 4};
-      const cuuint32_t box[2] = {tc::BK, (cuuint32_t)(tc_NT / (tc_mc ? 2 : cg))};
+      const cuuint32_t box[2] = {tc::BK, (cuuint32_t)tc_NT};
       const CUtensorMapSwizzle bsw = tc::BK == 32 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B;
       GM_TRY(encode_tmap_f32(&tmShi, S2hi, 2, dims, strides, box, bsw));
       GM_TRY(encode_tmap_f32(&tmSlo, S2lo, 2, dims, strides, box, bsw));
       GM_TRY(make_v_tmap(&tmV, V, M + 1));
-      const int smem = (int)need(tc_stages);
-      if (tc_ts)
-        GM_CUDA(cudaFuncSetAttribute(tc::k_contract_ts, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-      else if (tc_mc)
-        GM_CUDA(cudaFuncSetAttribute(tc::k_contract_tc<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-      else if (cg == 2)
-        GM_CUDA(cudaFuncSetAttribute(tc::k_contract_tc<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-      else
-        GM_CUDA(cudaFuncSetAttribute(tc::k_contract_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-      tc_cg = cg;
+      GM_TRY(ensure_smem(tc::k_contract_tc, tc::smem_bytes(tc_NT, tc_stages)));
+      tc_on = true;
       return 0;
     }
   }
@@ -833,31 +829,16 @@ struct PlanT final : gmmnlse_plan {
       prm.U = Uout;
       prm.u_plane_stride = QN;
       prm.Q = Q; prm.N = N; prm.NT = tc_NT; prm.KB = tc_KB; prm.n_rt = tc_nrt;
-      const int cl = tc_mc ? 2 : tc_cg;                          // CTAs per cluster
-      prm.t_tiles = N / (tc::TM * cl);
+      prm.t_tiles = N / tc::TM;
       prm.total_tiles = planes * prm.t_tiles * tc_nrt;
       prm.plane0 = plane0; prm.stages = tc_stages; prm.kchunk = tc_kchunk;
-      prm.probe = tc_probe;
-      if (tc_stage_cap > 0 && tc_stage_cap < prm.stages) prm.stages = tc_stage_cap;
-      const int pairs = std::min(n_sm / cl, prm.total_tiles);
       cudaLaunchConfig_t cfg = {};
-      cfg.gridDim = dim3((unsigned)(pairs * cl));
+      cfg.gridDim = dim3((unsigned)std::min(n_sm, prm.total_tiles));
       cfg.blockDim = dim3(tc::NTHREADS);
-      cfg.dynamicSmemBytes = tc_ts ? tc::ts_smem_bytes(tc_NT, prm.stages) : tc::smem_bytes(tc_NT, tc_cg, tc_stages);
+      cfg.dynamicSmemBytes = tc::smem_bytes(tc_NT, tc_stages);
       cfg.stream = stream;
-      cudaLaunchAttribute attr[1];
-      attr[0].id = cudaLaunchAttributeClusterDimension;
-      attr[0].val.clusterDim.x = (unsigned)cl;
-      attr[0].val.clusterDim.y = 1;
-      attr[0].val.clusterDim.z = 1;
-      cfg.attrs = attr;
-      cfg.numAttrs = 1;
       prof_begin(GMMNLSE_KIND_CONTRACT);
-      cudaError_t e;
-      if (tc_ts) e = cudaLaunchKernelEx(&cfg, tc::k_contract_ts, vmap, tmShi, tmSlo, prm);
-      else if (tc_mc) e = cudaLaunchKernelEx(&cfg, tc::k_contract_tc<1, true>, vmap, tmShi, tmSlo, prm);
-      else if (tc_cg == 2) e = cudaLaunchKernelEx(&cfg, tc::k_contract_tc<2>, vmap, tmShi, tmSlo, prm);
-      else e = cudaLaunchKernelEx(&cfg, tc::k_contract_tc<1>, vmap, tmShi, tmSlo, prm);
+      cudaError_t e = cudaLaunchKernelEx(&cfg, tc::k_contract_tc, vmap, tmShi, tmSlo, prm);
       prof_end();
       GM_CUDA(e);
       return 0;
@@ -870,12 +851,7 @@ struct PlanT final : gmmnlse_plan {
                    const C* post_tab, long long tab_ps, T scale, int rows, int planes, const T* rscale) {
     constexpr int NT = (1 << LOG2N) / 16;
     const size_t smem = sizeof(C) * fft_smem_elems(1 << LOG2N);
-    static bool configured = false;
-    if (!configured) {
-      GM_CUDA(cudaFuncSetAttribute(k_fft_rows<T, LOG2N, DIR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)smem));
-      configured = true;
-    }
+    GM_TRY(ensure_smem(k_fft_rows<T, LOG2N, DIR>, smem));
     prof_begin(DIR > 0 ? GMMNLSE_KIND_FFT_TO_FREQ : GMMNLSE_KIND_FFT_TO_TIME);
     k_fft_rows<T, LOG2N, DIR><<<dim3(rows, planes), NT, smem, stream>>>(in, in_ps, out, out_ps, pre, post_vec,
                                                                          post_tab, tab_ps, scale, tw, rscale);
@@ -911,12 +887,7 @@ struct PlanT final : gmmnlse_plan {
   int launch_pairs_t(const C* A, long long a_ps, T* Vout, long long v_ps, int planes) {
     constexpr int NT = (1 << LOG2N) / 16;
     const size_t smem = RAMAN ? sizeof(C) * fft_smem_elems(1 << LOG2N) : 0;
-    static bool configured = false;
-    if (!configured) {
-      GM_CUDA(cudaFuncSetAttribute(k_pair_conv<T, LOG2N, RAMAN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)smem));
-      configured = true;
-    }
+    GM_TRY(ensure_smem(k_pair_conv<T, LOG2N, RAMAN>, smem));
     prof_begin(GMMNLSE_KIND_PAIR_CONV);
     k_pair_conv<T, LOG2N, RAMAN><<<dim3((Q + 1) / 2, planes), NT, smem, stream>>>(A, a_ps, Vout, v_ps, pair_m,
                                                                                   pair_n, Q, H, tw, spec(), cur_ho);
@@ -996,7 +967,7 @@ struct PlanT final : gmmnlse_plan {
       }
       return tc_run(lr2, tmZ, 0, Uout, QN, planes);
     }
-    if (tc_cg) {
+    if (tc_on) {
       if (Vin >= V && Vin < V + (size_t)(M + 1) * QN)              // the plan's own buffer
         return launch_contract_tc(tmV, (int)((Vin - V) / QN), Uout, planes);
       CUtensorMap tmp;
@@ -1021,11 +992,7 @@ struct PlanT final : gmmnlse_plan {
   int launch_mode_reduce(const T* Uin, const C* A, C* Nout, int planes) {
     if (general) {
       const size_t smem = sizeof(C) * P * 128;
-      static size_t configured_g = 0;
-      if (smem > configured_g) {
-        GM_CUDA(cudaFuncSetAttribute(k_mode_reduce_gen<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured_g = smem;
-      }
+      GM_TRY(ensure_smem(k_mode_reduce_gen<T>, smem));
       const int Gg = P >= 12 ? 4 : (P >= 4 ? 2 : 1);
       prof_begin(GMMNLSE_KIND_MODE_REDUCE);
       k_mode_reduce_gen<T><<<dim3((N + 127) / 128, planes), 128 * Gg, smem, stream>>>(Uin, QN, A, PN, Nout, PN, P, Bp,
@@ -1034,19 +1001,13 @@ struct PlanT final : gmmnlse_plan {
       GM_CUDA(cudaGetLastError());
       return 0;
     }
-    const int tw = mr_tile > 0 ? mr_tile : (P >= 32 && N >= 64 ? 32 : 128);
-    const int G = tw == 128 ? (P >= 12 ? 4 : (P >= 4 ? 2 : 1)) : (tw == 64 ? 8 : 8);   // mode groups per CTA
+    const int tw = P >= 32 && N >= 64 ? 32 : 128;                   // samples per CTA
+    const int G = tw == 128 ? (P >= 12 ? 4 : (P >= 4 ? 2 : 1)) : 8; // mode groups per CTA
     const size_t smem = sizeof(C) * P * tw;
-    static size_t configured = 0;
-    if (smem > configured) {
-      GM_CUDA(cudaFuncSetAttribute(k_mode_reduce<T, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)(sizeof(C) * P * 128)));
-      configured = sizeof(C) * P * 128;
-    }
+    GM_TRY(tw == 32 ? ensure_smem(k_mode_reduce<T, 32>, smem) : ensure_smem(k_mode_reduce<T, 128>, smem));
     const dim3 grid((N + tw - 1) / tw, planes);
     prof_begin(GMMNLSE_KIND_MODE_REDUCE);
     if (tw == 32) k_mode_reduce<T, 32><<<grid, 32 * G, smem, stream>>>(Uin, QN, A, PN, Nout, PN, P, N);
-    else if (tw == 64) k_mode_reduce<T, 64><<<grid, 64 * G, smem, stream>>>(Uin, QN, A, PN, Nout, PN, P, N);
     else k_mode_reduce<T, 128><<<grid, 128 * G, smem, stream>>>(Uin, QN, A, PN, Nout, PN, P, N);
     prof_end();
     GM_CUDA(cudaGetLastError());
@@ -1277,18 +1238,21 @@ struct PlanT final : gmmnlse_plan {
       n_launch += gsteps * (lg_c0 - lg_cb + lg_ca) + lg_cb * h_stats->iters;
       if (h_stats->noconv > 0) { n_noconv += h_stats->noconv; status = GMMNLSE_WARN_NOCONV; }
       if (last_on_device) last_err = h_stats->last_err;
-    } else if (fixed_iter > 0) {
-      GM_CUDA(cudaMemcpyAsync(h_err, d_err, sizeof(double), cudaMemcpyDeviceToHost, stream));
+    } else {                     // host loop: same completion semantics (A_out complete on return)
+      if (fixed_iter > 0) GM_CUDA(cudaMemcpyAsync(h_err, d_err, sizeof(double), cudaMemcpyDeviceToHost, stream));
       GM_CUDA(cudaStreamSynchronize(stream));
-      last_err = nsteps > 0 ? *h_err : 0.0;
+      if (fixed_iter > 0) last_err = nsteps > 0 ? *h_err : 0.0;
     }
     return status;
   }
 
-  static bool is_pinned(const void* p) {          // page-locked (cudaMallocHost / cudaHostRegister) host memory?
+  // 1 page-locked host memory (cudaMallocHost / cudaHostRegister), 0 pageable host memory, -1 device or managed
+  // memory (not a host buffer: the caller wants gmmnlse_propagate)
+  static int host_kind(const void* p) {
     cudaPointerAttributes a;
-    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
-    return a.type == cudaMemoryTypeHost;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return 0; }
+    if (a.type == cudaMemoryTypeHost) return 1;
+    return a.type == cudaMemoryTypeUnregistered ? 0 : -1;
   }
 
   // Host entry: H2D, propagate, D2H on the plan's stream, one synchronise.  Page-locked caller buffers are copied
@@ -1296,7 +1260,9 @@ struct PlanT final : gmmnlse_plan {
   int propagate_host(const void* A_in, double L, void* A_out) override {
     const size_t bytes = sizeof(C) * (size_t)PN;
     if (!d_io) GM_TRY(dalloc(&d_io, (size_t)PN));
-    const bool pin_in = is_pinned(A_in), pin_out = is_pinned(A_out);
+    const int k_in = host_kind(A_in), k_out = host_kind(A_out);
+    if (k_in < 0 || k_out < 0) return GMMNLSE_EINVAL;
+    const bool pin_in = k_in == 1, pin_out = k_out == 1;
     if ((!pin_in || !pin_out) && !h_in) {
       GM_CUDA(cudaMallocHost(&h_in, bytes));
       GM_CUDA(cudaMallocHost(&h_out, bytes));
@@ -1324,11 +1290,7 @@ struct PlanT final : gmmnlse_plan {
 
   int launch_couple(const C* src, long long src_ps, const C* Etab, const T* gf, const T* gi, C* Gout, int planes) {
     const size_t smem = sizeof(C) * P * 64;
-    static size_t configured = 0;
-    if (smem > configured) {
-      GM_CUDA(cudaFuncSetAttribute(k_couple<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      configured = smem;
-    }
+    GM_TRY(ensure_smem(k_couple<T>, smem));
     prof_begin(GMMNLSE_KIND_MISC);
     k_couple<T><<<dim3((N + 63) / 64, planes), 256, smem, stream>>>(src, src_ps, Etab, gf, gi, Qc, Gout, PN, P, N);
     prof_end();
@@ -1414,7 +1376,7 @@ struct PlanT final : gmmnlse_plan {
       rkg = nullptr;
       rkg_exec = nullptr;
       cudaGetLastError();
-      loop_state = -1;
+      rk_graph_failed = true;
     }
     return st;
   }
@@ -1445,7 +1407,7 @@ struct PlanT final : gmmnlse_plan {
       rk_warmed = true;
       s = 1;
     }
-    const bool replay = graph == 0 && !prof_on && loop_state >= 0 && s < nsteps && (rkg_exec || build_rk4_graph() == 0);
+    const bool replay = graph == 0 && !prof_on && !rk_graph_failed && s < nsteps && (rkg_exec || build_rk4_graph() == 0);
     for (; s < nsteps; ++s) {
       if (replay) {
         GM_CUDA(cudaGraphLaunch(rkg_exec, stream));
@@ -1484,7 +1446,7 @@ struct PlanT final : gmmnlse_plan {
   }
   int contraction_kind() const override {
     if (tc_h) return lowrank ? 8 : 7;
-    return lowrank ? 6 : (tc_cg ? (tc_ts ? 4 : (tc_mc ? 5 : 1 + tc_cg)) : 1);
+    return lowrank ? 6 : (tc_on ? 3 : 1);
   }
   int lowrank_rank() const override { return lowrank ? lr_R : 0; }
   int raman_kind() const override { return f_R == 0.0 ? 0 : (iir ? 2 : 1); }
@@ -1493,16 +1455,6 @@ struct PlanT final : gmmnlse_plan {
     cudaStreamSynchronize(stream);
     drop_loop_graph();
     tc_kchunk = k;
-    return 0;
-  }
-  int set_probe(int probe_bits, int stage_cap, int a7_tile) override {
-    if (probe_bits < 0 || stage_cap < 0 || (a7_tile != 0 && a7_tile != 32 && a7_tile != 64 && a7_tile != 128))
-      return GMMNLSE_EINVAL;
-    cudaStreamSynchronize(stream);
-    drop_loop_graph();
-    tc_probe = probe_bits;               // timing probes (gemm_tc.cuh Params::probe); results are wrong when set
-    tc_stage_cap = stage_cap;            // cap on smem stages (0 = as many as fit)
-    mr_tile = a7_tile;                   // a7 samples per CTA (0 = auto)
     return 0;
   }
   int debug_contract(const void* Vin, void* Uout, int n_planes) override {
@@ -1541,10 +1493,13 @@ static int create_plan(gmmnlse_plan** out, int P, int N, int M, double dt, doubl
   if (opt) o = *opt;
   if (P < 1 || N < 1 || M < 1 || n_beta < 1 || !beta || !S) return GMMNLSE_EINVAL;
   if (N & (N - 1)) return GMMNLSE_EINVAL;
-  if (!(dt > 0) || !(dz > 0) || !(omega0 > 0) || !std::isfinite(n2) || !std::isfinite(f_R)) return GMMNLSE_EINVAL;
+  if (!(dt > 0) || !(dz > 0) || !(omega0 > 0) || !std::isfinite(n2)) return GMMNLSE_EINVAL;
+  if (!(f_R >= 0.0 && f_R <= 1.0)) return GMMNLSE_EINVAL;      // a fraction; the fp16 range bound assumes it
   if ((f_R != 0.0) != (h_R != nullptr)) return GMMNLSE_EINVAL;
   if (o.precision != 0 && o.precision != 1) return GMMNLSE_EINVAL;
-  if (o.raman < 0 || o.raman > 2 || o.contraction < 0 || o.contraction > 8) return GMMNLSE_EINVAL;
+  if (o.raman < 0 || o.raman > 2) return GMMNLSE_EINVAL;
+  if (o.contraction != 0 && o.contraction != 1 && o.contraction != 3 && (o.contraction < 6 || o.contraction > 8))
+    return GMMNLSE_EINVAL;
   if (o.graph < 0 || o.graph > 1) return GMMNLSE_EINVAL;
   if (o.shock && M_PI / dt >= omega0) return GMMNLSE_EINVAL;
   if (!(o.tol > 0)) o.tol = 1e-6;
@@ -1582,6 +1537,7 @@ static int create_plan(gmmnlse_plan** out, int P, int N, int M, double dt, doubl
   pl->contraction = o.contraction;
   pl->raman = o.raman;
   pl->graph = o.graph;
+  if (cudaGetDevice(&pl->device) != cudaSuccess) { delete pl; g_cuda_err = "cudaGetDevice failed"; return GMMNLSE_ECUDA; }
   pl->general = general;
   pl->gen_complex = general && tensors_complex;
   pl->gen_SR = S_R;
@@ -1617,9 +1573,21 @@ int gmmnlse_plan_create_general(gmmnlse_plan** out, int P, int N, int M, double 
                      opt);
 }
 
+namespace {
+struct StreamForCall {          // a non-NULL `stream` argument applies to this call only
+  gmmnlse_plan* plan;
+  cudaStream_t saved;
+  StreamForCall(gmmnlse_plan* p, void* s) : plan(p), saved(p->stream) {
+    if (s) p->stream = (cudaStream_t)s;
+  }
+  ~StreamForCall() { plan->stream = saved; }
+};
+}  // namespace
+
 int gmmnlse_propagate(gmmnlse_plan* plan, const void* A_in, double L, void* A_out, void* stream) {
   if (!plan || !A_in || !A_out) return GMMNLSE_EINVAL;
-  if (stream) plan->stream = (cudaStream_t)stream;
+  DeviceGuard dg(plan->device);
+  StreamForCall sc(plan, stream);
   return plan->propagate(A_in, L, A_out);
 }
 
@@ -1627,23 +1595,32 @@ int gmmnlse_propagate_host(gmmnlse_plan* plan, const void* A_in_host, double L, 
   if (!plan || !A_in_host || !A_out_host) return GMMNLSE_EINVAL;
   const double ns = L / plan->dz;
   if (!(L >= 0) || std::fabs(ns - std::round(ns)) > 1e-9 * std::fmax(1.0, ns)) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
   return plan->propagate_host(A_in_host, L, A_out_host);
 }
 
 int gmmnlse_propagate_rk4ip(gmmnlse_plan* plan, const void* A_in, double L, void* A_out, void* stream) {
   if (!plan || !A_in || !A_out) return GMMNLSE_EINVAL;
-  if (stream) plan->stream = (cudaStream_t)stream;
+  DeviceGuard dg(plan->device);
+  StreamForCall sc(plan, stream);
   return plan->propagate_rk4ip(A_in, L, A_out);
 }
 
-int gmmnlse_set_gain(gmmnlse_plan* plan, const double* g) { return plan ? plan->set_gain(g) : GMMNLSE_EINVAL; }
+int gmmnlse_set_gain(gmmnlse_plan* plan, const double* g) {
+  if (!plan) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
+  return plan->set_gain(g);
+}
 
 int gmmnlse_set_coupling(gmmnlse_plan* plan, const double* Q) {
-  return plan ? plan->set_coupling(Q) : GMMNLSE_EINVAL;
+  if (!plan) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
+  return plan->set_coupling(Q);
 }
 
 int gmmnlse_nonlinear_op(gmmnlse_plan* plan, const void* A, void* dA) {
   if (!plan || !A || !dA || A == dA) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
   return plan->nonlinear_op(A, dA);
 }
 
@@ -1667,6 +1644,7 @@ long long gmmnlse_launch_count(const gmmnlse_plan* plan) { return plan ? plan->n
 
 int gmmnlse_profile_enable(gmmnlse_plan* plan, int on) {
   if (!plan) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
   if (plan->prof_collect() < 0) return GMMNLSE_ECUDA;
   plan->prof_on = on != 0;
   if (on)
@@ -1676,6 +1654,7 @@ int gmmnlse_profile_enable(gmmnlse_plan* plan, int on) {
 
 int gmmnlse_profile_get(gmmnlse_plan* plan, int kind, double* total_ms, long long* launches) {
   if (!plan || kind < 0 || kind >= GMMNLSE_KIND_COUNT) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
   if (plan->prof_collect() < 0) return GMMNLSE_ECUDA;
   if (total_ms) *total_ms = plan->prof_ms[kind];
   if (launches) *launches = plan->prof_n[kind];
@@ -1684,21 +1663,25 @@ int gmmnlse_profile_get(gmmnlse_plan* plan, int kind, double* total_ms, long lon
 
 int gmmnlse_debug_get_planes(gmmnlse_plan* plan, void* out_host) {
   if (!plan || !out_host) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
   return plan->get_planes(out_host);
 }
 
 int gmmnlse_debug_fft(gmmnlse_plan* plan, const void* in, void* out, int rows, int dir) {
   if (!plan || !in || !out) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
   return plan->debug_fft(in, out, rows, dir);
 }
 
 int gmmnlse_debug_pairs(gmmnlse_plan* plan, const void* A, void* V, int n_planes) {
   if (!plan || !A || !V) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
   return plan->debug_pairs(A, V, n_planes);
 }
 
 int gmmnlse_debug_contract(gmmnlse_plan* plan, const void* V, void* U, int n_planes) {
   if (!plan || !V || !U || V == U) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
   return plan->debug_contract(V, U, n_planes);
 }
 
@@ -1710,12 +1693,16 @@ int gmmnlse_lowrank_rank(const gmmnlse_plan* plan) { return plan ? plan->lowrank
 
 int gmmnlse_loop_kind(const gmmnlse_plan* plan) { return plan ? plan->loop_state : 0; }
 
-int gmmnlse_debug_set_tc_chunk(gmmnlse_plan* plan, int k) { return plan ? plan->set_tc_chunk(k) : GMMNLSE_EINVAL; }
-
-int gmmnlse_debug_set_probe(gmmnlse_plan* plan, int probe_bits, int stage_cap, int a7_tile) {
-  return plan ? plan->set_probe(probe_bits, stage_cap, a7_tile) : GMMNLSE_EINVAL;
+int gmmnlse_debug_set_tc_chunk(gmmnlse_plan* plan, int k) {
+  if (!plan) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
+  return plan->set_tc_chunk(k);
 }
 
-void gmmnlse_plan_destroy(gmmnlse_plan* plan) { delete plan; }
+void gmmnlse_plan_destroy(gmmnlse_plan* plan) {
+  if (!plan) return;
+  DeviceGuard dg(plan->device);
+  delete plan;
+}
 
 }  // extern "C"

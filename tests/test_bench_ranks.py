@@ -55,3 +55,20 @@ def test_reference_arm_only_rank0_prints():
     d = json.loads(r.stdout.strip().splitlines()[-1])
     assert d["impl"] == "reference" and d["value"] > 0 and d["unit"] == "z-steps/s"
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_bench_gpus_flag_starts_its_own_ranks():
+    """`python bench.py --gpus 2` outside torchrun re-launches itself as 2 ranks (one per GPU on the box; here on CPU
+    over gloo with the measurement stubbed to 10 ms x (1 + rank)): one JSON line, from rank 0, n_gpus = 2, the time the
+    slowest rank's, the value the whole job's."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_PORT")}
+    env["GMMNLSE_BENCH_STUB_MS"] = "10.0"
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "4", "--config", "5"],
+                       capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["scaling"] == "weak"
+    assert d["ms_per_step"] == pytest.approx(20.0 / 4)                 # max over ranks: rank 1 took 20 ms
+    assert d["value"] == pytest.approx(2 * 4 * 20 / 20e-3)             # 2 ranks x 4 steps x 20 z-steps in 20 ms

@@ -446,15 +446,14 @@ def _packed_S2(S):
 
 
 @pytest.mark.parametrize("cfg,N,kw,kind", [
-    (3, 1024, {}, 1), (3, 1024, {}, 3), (3, 1024, {}, 2), (3, 1024, {}, 4),   # Q = 120: one r-tile of 128
-    (4, 512, {}, 3), (4, 512, {}, 2), (4, 512, {}, 4),             # Q = 210: two r-tiles of 112
-    (5, 256, {}, 3), (5, 256, {}, 2), (5, 256, {}, 1), (5, 256, {}, 4), (5, 256, {}, 5),   # Q = 1035: 5 r-tiles of 208
-    (3, 1024, {}, 5), (4, 512, {}, 5),                              # multicast pairs
+    (3, 1024, {}, 1), (3, 1024, {}, 3),                            # Q = 120: one r-tile of 128
+    (4, 512, {}, 3),                                               # Q = 210: two r-tiles of 112
+    (5, 256, {}, 3), (5, 256, {}, 1),                              # Q = 1035: 5 r-tiles of 208
     (3, 1024, {}, 6), (4, 512, {}, 6), (5, 256, {}, 6),             # exact low-rank form (rank 45 / ~120 / 153)
     (3, 1024, {}, 7), (4, 512, {}, 7), (5, 256, {}, 7),             # kind::f16 on fp16 hi / lo splits (auto's choice)
     (3, 1024, {}, 8), (4, 512, {}, 8), (5, 256, {}, 8),             # low-rank form on the kind::f16 kernel
     (3, 128, dict(max_group=3), 7),
-    (3, 128, dict(max_group=3), 3), (3, 128, dict(max_group=3), 4),       # Q = 55 < 64: tensor path forced, N = 128
+    (3, 128, dict(max_group=3), 3),                                 # Q = 55 < 64: tensor path forced, N = 128
 ])
 def test_contraction_vs_fp64_matmul(B, cfg, N, kw, kind):
     w = W.make_config(cfg, N=N, **kw)
@@ -464,7 +463,7 @@ def test_contraction_vs_fp64_matmul(B, cfg, N, kw, kind):
     # pair streams with the dynamic range of |A|^2 products: peak to 1e-6 of peak along t
     V = (rng.standard_normal((planes, Q, N)) * np.exp(rng.uniform(-7, 7, (planes, 1, N)))).astype(np.float32)
     with B.plan_from_workload(w, contraction=kind) as plan:
-        assert plan.contraction_kind() == {1: 1, 2: 3, 3: 2, 4: 4, 5: 5, 6: 6, 7: 7, 8: 8}[kind]
+        assert plan.contraction_kind() == kind
         Vd = torch.from_numpy(V).cuda()
         U = torch.full((planes, Q, N), float("nan"), dtype=torch.float32, device="cuda")
         plan.debug_contract(Vd, U, planes)
@@ -519,7 +518,11 @@ def test_contraction_auto_selects_tensor_cores_for_large_P(B):
         assert plan.contraction_kind() == 7
     w = W.make_config(3, N=1024)                       # Q = 120: 3xTF32 (the f16 form's extra launches do not pay)
     with B.plan_from_workload(w) as plan:
-        assert plan.contraction_kind() == 2
+        assert plan.contraction_kind() == 3
+    for removed in (2, 4, 5):                          # cta_group::2, TMEM-operand and multicast forms: gone
+        with pytest.raises(B.GmmnlseError) as e:
+            B.plan_from_workload(w, contraction=removed)
+        assert e.value.status == B.EINVAL
     w = W.make_config(2, N=1024)
     with B.plan_from_workload(w) as plan:
         assert plan.contraction_kind() == 1
