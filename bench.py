@@ -91,7 +91,7 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------ algorithmic work per launch
-def algorithmic(kind, w, planes):
+def algorithmic(kind, w, planes, a7_fused=False):
     """(bytes, flops) one launch of `kind` must move / execute for `planes` planes."""
     P, N = w.P, w.N
     Q = P * (P + 1) // 2
@@ -102,6 +102,8 @@ def algorithmic(kind, w, planes):
     if kind == "pair_conv":
         return (c * P * N + r * Q * N) * planes, 0
     if kind == "contract":
+        if a7_fused:                    # V in; A in and N_p out instead of U out (a7 runs in the epilogue)
+            return (r * Q * N + 2 * c * P * N) * planes, (2.0 * Q * Q + 4.0 * P * P) * N * planes
         return 2 * r * Q * N * planes, 2.0 * Q * Q * N * planes
     if kind == "mode_reduce":
         return (r * Q * N + 2 * c * P * N) * planes, 4.0 * P * P * N * planes
@@ -261,11 +263,12 @@ def run_gpu(args):
         "pair_conv": iters * w.M + large, "contract": iters * w.M + large, "mode_reduce": iters * w.M + large,
         "scan": iters * w.M, "advance": large, "misc": 0}
     shares = {}
+    fused = "mode_reduce" not in prof
     for k, (ms_k, n_k) in prof.items():
-        by, fl = algorithmic(k, w, planes_total.get(k, 0))
+        by, fl = algorithmic(k, w, planes_total.get(k, 0), fused)
         shares[k] = dict(ms=round(ms_k, 4), launches=n_k, share=round(ms_k / tot_ms, 4),
                          GBps=round(by / (ms_k * 1e-3) / 1e9, 1), TFLOPs=round(fl / (ms_k * 1e-3) / 1e12, 3))
-    by, fl = algorithmic(dom, w, planes_total[dom])
+    by, fl = algorithmic(dom, w, planes_total[dom], fused)
     traffic, traffic_src = None, None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")     # written from an ncu --set full capture
     if os.path.exists(tpath):
@@ -284,7 +287,7 @@ def run_gpu(args):
         # the timed region is a fraction of a second at full clock, so the BURST figure is the denominator of
         # `frac`; the sustained one is printed beside it
         if ck in (7, 8):
-            kname, ratio, mult = "k_contract_h (a6 + a7, tcgen05 kind::f16 on fp16 hi/lo splits)", 1.0, 3
+            kname, ratio, mult = "k_contract_h (a6, tcgen05 kind::f16 on fp16 hi/lo splits)", 1.0, 3
             pnote = f"peak = {peaks['source']} bf16 burst (fp16 runs at the bf16 rate)"
         elif ck in (3, 6):
             kname, ratio, mult = "k_contract_tc (a6, tcgen05 3xTF32)", 0.5, 3
@@ -333,6 +336,7 @@ def run_gpu(args):
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = oracle_sample(cfg, 0, 0)
     out["config"]["contraction_kind"] = main["ckind"]
+    out["config"]["a7"] = "in the contraction's epilogue (U never reaches HBM)" if fused else "separate kernel"
     out["config"]["mpa_loop"] = ("device (one CUDA graph per large step, WHILE node)" if plain["loop"] == 1
                                  else "host (read-back per iteration)")
     if rank == 0 and world == 1 and args.contraction == 0 and cfg >= 3 and not args.no_variants:

@@ -48,9 +48,7 @@ typedef struct {                /* pass NULL for defaults                       
                                    7 = tcgen05 kind::f16 GEMM on fp16 hi/lo splits of both operands (22 mantissa
                                    bits, as 3xTF32, at twice its MMA rate): the pair kernels write V scaled by a
                                    power of two into fp16 range as two fp16 arrays, S is split per row at plan
-                                   time, the scales are undone exactly in the epilogue, and a7 (sum_l U_pl A_l,
-                                   PAPER.md:53) runs in the same epilogue, so U never reaches HBM (DESIGN.md
-                                   section 7);
+                                   time, the scales are undone exactly in the epilogue;
                                    6 = exact low-rank form on the 3xTF32 kernel,
                                    8 = the same on the kind::f16 kernel: S_(pl),(mn) = sum_k L_(pl),k L_(mn),k
                                    by pivoted Cholesky at plan time (Eq. 2 makes S a Gram matrix; rank 153 of

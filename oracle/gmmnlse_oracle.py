@@ -308,14 +308,15 @@ def rk4ip_propagate(A0, L, dz, beta, S, kappa, omega0, f_R, h_R, dt, shock=True,
 
 # --------------------------------------------------------------------- O4: MPA
 def mpa_large_step(psi0, M, dz, D, nl_time, K, tol=1e-6, max_iter=None, fixed_iter=0,
-                   history=None, coupling=None):
+                   history=None, coupling=None, first_iterate=None, planes_out=None):
     """One MPA large step z0 -> z0 + M dz  (Eqs. 11-12).
 
     psi0[p][w] = At(z0).  Planes j = 0..M (reading S10).  ``nl_time(A_t)`` returns
     N_p[A](t); ``K[w] = i kappa (1 + w/w0)``.  Returns (At(z0 + M dz), n_iter,
     last_err, converged).
 
-      first iterate      psi_j = psi_0
+      first iterate      psi_j = psi_0; ``first_iterate[j]`` (optional,
+                         [M+1][P][N], plane 0 ignored) replaces it: the predictor of reading S11, see mpa_propagate
       each iteration     A_j = psi_j exp(D j dz)            (Eq. 11)
                          G_j = K exp(-D j dz) F{N[A_j]}     (Eq. 12 integrand)
                          psi_j <- psi_0 + dz [G_0/2 + G_1 + .. + G_{j-1} + G_j/2]
@@ -326,6 +327,8 @@ def mpa_large_step(psi0, M, dz, D, nl_time, K, tol=1e-6, max_iter=None, fixed_it
     if max_iter is None:
         max_iter = 2 * M + 4
     psi = np.broadcast_to(psi0, (M + 1, P, N)).copy()
+    if first_iterate is not None:
+        psi[1:] = first_iterate[1:]
     G = np.zeros((M + 1, P, N), dtype=np.complex128)
     # extra right-hand-side term in the frequency domain (linear coupling), rotated like the nonlinear one
     extra = (lambda Af: 0.0) if coupling is None else (lambda Af: coupling_term(Af, coupling))
@@ -360,12 +363,22 @@ def mpa_large_step(psi0, M, dz, D, nl_time, K, tol=1e-6, max_iter=None, fixed_it
             break
         elif n_iter >= max_iter:
             break
+    if planes_out is not None:
+        planes_out.append(psi)
     return psi[M] * np.exp(D * (M * dz)), n_iter, err, converged
 
 
 def mpa_propagate(A0, L, dz, M, beta, S, kappa, omega0, f_R, h_R, dt, shock=True,
-                  tol=1e-6, max_iter=None, fixed_iter=0, stats=None, history=None, gain=None, coupling=None):
-    """Propagate with MPA; the last large step uses M' = (L/dz) mod M planes."""
+                  tol=1e-6, max_iter=None, fixed_iter=0, stats=None, history=None, gain=None, coupling=None,
+                  predictor=0):
+    """Propagate with MPA; the last large step uses M' = (L/dz) mod M planes.
+
+    ``predictor`` (reading S11: an optimisation of the first iterate, off by default = the paper's psi_j = psi_0):
+    1 starts the planes of a large step from the previous large step's converged increments carried into the new
+    interaction picture, psi_j^(1) = psi_0' + exp(D M dz) (psi_j^prev - psi_0^prev): the increment of plane j is
+    dz times the trapezoid sum of G, and under linear propagation over one large step every phase-matched term of
+    G_p picks up the phase of mode p (the factor exp(D M dz)); what is left for the iteration is the change of the
+    envelopes over one large step and the non-phase-matched terms.  Same fixed point, same stopping rule."""
     A0 = np.asarray(A0, dtype=np.complex128)
     N = A0.shape[-1]
     omega = omega_grid(N, dt)
@@ -376,11 +389,18 @@ def mpa_propagate(A0, L, dz, M, beta, S, kappa, omega0, f_R, h_R, dt, shock=True
     psi0 = to_freq(A0)
     done = 0
     tot_it, n_large, n_noconv, last_err = 0, 0, 0, 0.0
+    prev = None                                           # (planes, psi_0) of the previous large step
     while done < n_small:
         Mc = min(M, n_small - done)
         hist = [] if history is not None else None
+        first = None
+        if predictor == 1 and prev is not None and prev[0].shape[0] == Mc + 1:
+            first = psi0[None] + np.exp(D * (prev[0].shape[0] - 1) * dz)[None] * (prev[0] - prev[1][None])
+        keep = []
+        start = psi0
         psi0, it, last_err, conv = mpa_large_step(psi0, Mc, dz, D, nl_time, K, tol,
-                                                   max_iter, fixed_iter, hist, coupling)
+                                                   max_iter, fixed_iter, hist, coupling, first, keep)
+        prev = (keep[0], start)
         if history is not None:
             history.append(hist)
         tot_it += it

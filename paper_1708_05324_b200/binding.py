@@ -225,7 +225,7 @@ class Plan:
         _check(self._lib, self._lib.gmmnlse_debug_contract(self._h, _ptr(V), _ptr(U), n_planes))
 
     def contraction_kind(self) -> int:
-        """1 CUDA cores, 3 tcgen05 3xTF32, 7 tcgen05 kind::f16 (a7 fused), 6 / 8 the low-rank pairs of those."""
+        """1 CUDA cores, 3 tcgen05 3xTF32, 7 tcgen05 kind::f16, 6 / 8 the low-rank pairs of those."""
         return int(self._lib.gmmnlse_contraction_kind(self._h))
 
     def lowrank_rank(self) -> int:

@@ -67,8 +67,6 @@ struct Params {
   float bound_gain;            // the A operand was scaled by v_scale(bound_gain * *vbound)
   float zgain;                 // OUT_H: |Z| <= zgain * *vbound
   int Q, N, NT, KB, n_rt, t_tiles, total_tiles, plane0, stages, kchunk;
-  int probe;                   // timing probes only (results wrong): 2 skip TMA loads after the first fill, 4 skip
-                               // the stores, 32 skip the MMAs
 };
 
 __host__ __device__ inline int b_bytes(int NT) { return NT * BK * 2; }
@@ -139,19 +137,14 @@ k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ C
           mbar_wait(bar_empty + 8 * stage, phase ^ 1u, 1);
           const uint32_t fb = bar_full + 8 * stage;
           const uint32_t sa = tiles_addr + stage * sbytes;
-          const bool warm = tile != cta || kb >= stages;
-          if (warm && (p.probe & 2)) {
-            mbar_arrive(fb);
-          } else {
-            mbar_arrive_expect_tx(fb, (uint32_t)(2 * A_BYTES + 2 * nb));
+          mbar_arrive_expect_tx(fb, (uint32_t)(2 * A_BYTES + 2 * nb));
 #pragma unroll
-            for (int i = 0; i < TM / 64; ++i) {                   // 2 boxes of 64 t x BK q per operand half
-              tma_load_3d(sa + i * (BK * 128), &tmVh, fb, t0 + 64 * i, kb * BK, p.plane0 + pl);
-              tma_load_3d(sa + A_BYTES + i * (BK * 128), &tmVl, fb, t0 + 64 * i, kb * BK, p.plane0 + pl);
-            }
-            tma_load_2d(sa + 2 * A_BYTES, &tmSh, fb, kb * BK, r0);
-            tma_load_2d(sa + 2 * A_BYTES + nb, &tmSl, fb, kb * BK, r0);
+          for (int i = 0; i < TM / 64; ++i) {                     // 2 boxes of 64 t x BK q per operand half
+            tma_load_3d(sa + i * (BK * 128), &tmVh, fb, t0 + 64 * i, kb * BK, p.plane0 + pl);
+            tma_load_3d(sa + A_BYTES + i * (BK * 128), &tmVl, fb, t0 + 64 * i, kb * BK, p.plane0 + pl);
           }
+          tma_load_2d(sa + 2 * A_BYTES, &tmSh, fb, kb * BK, r0);
+          tma_load_2d(sa + 2 * A_BYTES + nb, &tmSl, fb, kb * BK, r0);
           if (++stage == stages) { stage = 0; phase ^= 1u; }
         }
       }
@@ -177,7 +170,6 @@ k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ C
           const uint64_t a_lo = make_smem_desc(sa + A_BYTES, BK * 128, 1024, 2);
           const uint64_t b_hi = make_smem_desc(sa + 2 * A_BYTES, 16, 512, 4);
           const uint64_t b_lo = make_smem_desc(sa + 2 * A_BYTES + nb, 16, 512, 4);
-          if (!(p.probe & 32))
 #pragma unroll
           for (int kk = 0; kk < BK / 16; ++kk) {
             const uint64_t da = (uint64_t)(kk * (2048 >> 4));      // next 16 q of A: two 8-q groups
@@ -249,7 +241,7 @@ k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ C
 #pragma unroll
         for (int c = 0; c < EPI_COLS; ++c) {
           const int r = rbase + c;
-          if (c < ncols && r < p.Q && !(p.probe & 4)) {
+          if (c < ncols && r < p.Q) {
             const float z = accr[c] * (rs[c] * inv_sv) * sz;
             const __half h = __float2half_rn(z);
             Zh[(long long)r * p.N] = h;
@@ -261,7 +253,7 @@ k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ C
 #pragma unroll
         for (int c = 0; c < EPI_COLS; ++c) {
           const int r = rbase + c;
-          if (c < ncols && r < p.Q && !(p.probe & 4)) Uout[(long long)r * p.N] = accr[c] * (rs[c] * inv_sv);
+          if (c < ncols && r < p.Q) Uout[(long long)r * p.N] = accr[c] * (rs[c] * inv_sv);
         }
       }
     }
