@@ -3,6 +3,7 @@
 #pragma once
 #include "fft.cuh"
 #include "gemm_h.cuh"
+#include "ptx_sm100.cuh"
 
 namespace gm {
 
@@ -314,6 +315,166 @@ k_pair_iir(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restric
     const cplx<T> v = sm[fft_pad(n)];
     v0[n] = v.x;
     if (has1) v0[N + n] = v.y;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// a4 + a5, recursive form, register-blocked over mode rows (complex64, scalar-mode path).  The kernel above moves
+// 1.75 field rows through L2 per pair stream and transposes every sample through shared memory twice; it is bound
+// by L1/L2 throughput and latency, not by the HBM write of V.  Here a thread owns 16 CONSECUTIVE samples (128 B)
+// of a row.  TMA brings each warp's 32 x 128 B slice of a field row into shared memory under the 128-byte swizzle
+// (16-byte chunk c of thread t at slot c ^ (t & 7): conflict-free 128-bit reads, no transpose, no load
+// instructions, no registers held across the latency); the rows m0, m0 + 1 of a CTA stay parked, the rows n of
+// its range stream through one buffer that is refilled for n + 1 as soon as x = Re(A_m A_n*) has been formed:
+// two streams (m0, n), (m0 + 1, n) per row load, 0.56-0.63 rows of L2 traffic per stream.  The recurrence
+// w[i] = x[i] + zeta w[i-1] runs from a zero state per thread, chunk totals are combined by a warp-shuffle scan,
+// and the carry into a warp's first chunk is the zero-history total of the warp before it (the last warp for
+// warp 0: the periodic wrap): what that leaves out is zeta^512 of older history, < 1e-12 by the plan-time check
+// that selects this kernel.  V leaves as 256-bit stores (32 contiguous bytes per lane, full sectors).
+//   grid = (n_work, planes), block = N / 16; work[i] = (m0, n_begin, n_end): streams (m0, n), (m0 + 1, n), n in
+//   [n_begin, n_end), m <= n only.  V row of (m, n): q = m P - m (m - 1) / 2 + (n - m).
+//   tmA: field [planes][P][N/16][32 floats], box 32 x 32 x 1 x 1, SWIZZLE_128B; plane0 = first plane of the launch.
+//   HALF_OUT: V as fp16 hi / lo rows scaled by v_scale(*vbound) (HalfOut), else fp32.
+__device__ __forceinline__ void stg256(void* p, const uint32_t (&v)[8]) {
+  asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(v[0]), "r"(v[1]), "r"(v[2]),
+               "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]) : "memory");
+}
+struct PairWork { int m0, n_begin, n_end; };
+
+template <int LOG2N, bool HALF_OUT>
+__global__ void __launch_bounds__((1 << LOG2N) / 16, 1)
+k_pair_iir_rows(const __grid_constant__ CUtensorMap tmA, int plane0, float* __restrict__ V, long long v_plane_stride,
+                int P, const PairWork* __restrict__ work, float2 zeta, float2 cs, float omf,
+                const float2* __restrict__ zp, HalfOut ho) {
+  using namespace ptx;
+  constexpr int N = 1 << LOG2N, NT = N / 16, NW = NT / 32;
+  constexpr uint32_t ROW_BYTES = NT * 128, WARP_BYTES = 32 * 128;
+  extern __shared__ unsigned char smem_raw[];
+  const uint32_t raw_addr = smem_u32(smem_raw);
+  const uint32_t base = (raw_addr + 1023u) & ~1023u;                  // swizzle atoms are 1 KiB
+  unsigned char* sm = smem_raw + (base - raw_addr);
+  const float4* rows = reinterpret_cast<const float4*>(sm);           // [0] m0, [1] m0 + 1, [2] streamed n
+  float2* wt = reinterpret_cast<float2*>(sm + 3 * ROW_BYTES);         // [2 parity][NW][2 streams] warp totals
+  const uint32_t bars = base + 3 * ROW_BYTES + 2 * NW * 2 * 8;        // [NW][2]: parked rows, streamed row
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, j = blockIdx.y;
+  const PairWork wk = work[blockIdx.x];
+  const int m0 = wk.m0, m1 = m0 + 1;
+  const bool has_m1 = m1 < P;
+  const uint32_t bar_park = bars + 16 * warp, bar_b = bar_park + 8;
+  const uint32_t dst0 = base + warp * WARP_BYTES;                     // this warp's slice of row buffer 0
+  if (lane == 0) {
+    mbar_init(bar_park, 1);
+    mbar_init(bar_b, 1);
+    fence_barrier_init();
+    prefetch_tensormap(&tmA);
+  }
+  __syncwarp();
+  if (lane == 0) {                                                    // each warp fetches only what it reads itself
+    mbar_arrive_expect_tx(bar_park, 2 * WARP_BYTES);
+    tma_load_4d(dst0, &tmA, bar_park, 0, 32 * warp, m0, plane0 + j);
+    tma_load_4d(dst0 + ROW_BYTES, &tmA, bar_park, 0, 32 * warp, has_m1 ? m1 : m0, plane0 + j);
+    mbar_arrive_expect_tx(bar_b, WARP_BYTES);
+    tma_load_4d(dst0 + 2 * ROW_BYTES, &tmA, bar_b, 0, 32 * warp, wk.n_begin, plane0 + j);
+  }
+  const float sv = HALF_OUT ? hc::v_scale(*ho.vbound, false) : 1.f;
+  const float2 pl = zp[lane];                                         // zeta^(16 lane)
+  mbar_wait(bar_park, 0, 11);
+  int parity = 0;
+  for (int n = wk.n_begin; n < wk.n_end; ++n, parity ^= 1) {
+    // x0 = Re(A_m0 A_n*), x1 = Re(A_m1 A_n*) on this thread's 16 samples
+    float x0[16], x1[16];
+    mbar_wait(bar_b, (uint32_t)parity, 12);
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {                                     // chunk c = samples 2c, 2c + 1
+      const int slot = tid * 8 + (c ^ (tid & 7));
+      const float4 a0 = rows[slot], a1 = rows[NT * 8 + slot], b = rows[2 * NT * 8 + slot];
+      x0[2 * c] = a0.x * b.x + a0.y * b.y;
+      x0[2 * c + 1] = a0.z * b.z + a0.w * b.w;
+      x1[2 * c] = a1.x * b.x + a1.y * b.y;
+      x1[2 * c + 1] = a1.z * b.z + a1.w * b.w;
+    }
+    __syncwarp();                                                     // the warp is done with the streamed slice
+    if (lane == 0 && n + 1 < wk.n_end) {                              // refill it for n + 1 behind the arithmetic
+      mbar_arrive_expect_tx(bar_b, WARP_BYTES);
+      tma_load_4d(dst0 + 2 * ROW_BYTES, &tmA, bar_b, 0, 32 * warp, n + 1, plane0 + j);
+    }
+    // zero-state recurrence over the chunk
+    float2 w0 = make_float2(0.f, 0.f), w1 = w0;
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+      w0 = make_float2(x0[e] + zeta.x * w0.x - zeta.y * w0.y, zeta.x * w0.y + zeta.y * w0.x);
+      w1 = make_float2(x1[e] + zeta.x * w1.x - zeta.y * w1.y, zeta.x * w1.y + zeta.y * w1.x);
+    }
+    // inclusive scan of the chunk totals inside the warp: T_k = sum_{i<=k} zeta^(16 (k-i)) E_i
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const float2 pw = zp[d];
+      const float r0x = __shfl_up_sync(0xffffffffu, w0.x, d), r0y = __shfl_up_sync(0xffffffffu, w0.y, d);
+      const float r1x = __shfl_up_sync(0xffffffffu, w1.x, d), r1y = __shfl_up_sync(0xffffffffu, w1.y, d);
+      if (lane >= d) {
+        w0 = make_float2(w0.x + pw.x * r0x - pw.y * r0y, w0.y + pw.x * r0y + pw.y * r0x);
+        w1 = make_float2(w1.x + pw.x * r1x - pw.y * r1y, w1.y + pw.x * r1y + pw.y * r1x);
+      }
+    }
+    if (lane == 31) { wt[(parity * NW + warp) * 2] = w0; wt[(parity * NW + warp) * 2 + 1] = w1; }
+    float2 e0 = make_float2(__shfl_up_sync(0xffffffffu, w0.x, 1), __shfl_up_sync(0xffffffffu, w0.y, 1));
+    float2 e1 = make_float2(__shfl_up_sync(0xffffffffu, w1.x, 1), __shfl_up_sync(0xffffffffu, w1.y, 1));
+    if (lane == 0) { e0 = make_float2(0.f, 0.f); e1 = e0; }
+    __syncthreads();
+    {
+      const int pw = warp == 0 ? NW - 1 : warp - 1;                   // the warp before this one (periodic)
+      const float2 g0 = wt[(parity * NW + pw) * 2], g1 = wt[(parity * NW + pw) * 2 + 1];
+      // state before this thread's first sample: exclusive in-warp part + zeta^(16 lane) x the previous warp's total
+      w0 = make_float2(e0.x + pl.x * g0.x - pl.y * g0.y, e0.y + pl.x * g0.y + pl.y * g0.x);
+      w1 = make_float2(e1.x + pl.x * g1.x - pl.y * g1.y, e1.y + pl.x * g1.y + pl.y * g1.x);
+    }
+    // second pass from the true state: V = (1 - f_R) x + Im(cs w)
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+      w0 = make_float2(x0[e] + zeta.x * w0.x - zeta.y * w0.y, zeta.x * w0.y + zeta.y * w0.x);
+      w1 = make_float2(x1[e] + zeta.x * w1.x - zeta.y * w1.y, zeta.x * w1.y + zeta.y * w1.x);
+      x0[e] = omf * x0[e] + cs.x * w0.y + cs.y * w0.x;
+      x1[e] = omf * x1[e] + cs.x * w1.y + cs.y * w1.x;
+    }
+    const long long q0 = (long long)m0 * P - (long long)m0 * (m0 - 1) / 2 + (n - m0);
+    const long long q1 = (long long)m1 * P - (long long)m1 * (m1 - 1) / 2 + (n - m1);
+    const bool st1 = has_m1 && n >= m1;                               // (m1, n) exists only for n >= m1
+    if constexpr (HALF_OUT) {
+      __half* obase = ho.Vh + j * ho.plane_stride + 16 * tid;
+#pragma unroll
+      for (int s = 0; s < 2; ++s) {
+        if (s == 1 && !st1) break;
+        const float* x = s == 0 ? x0 : x1;
+        uint32_t hi[8], lo[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const float2 v = make_float2(x[2 * k] * sv, x[2 * k + 1] * sv);
+          const __half2 h = __float22half2_rn(v);
+          const float2 f = __half22float2(h);
+          const __half2 l = __float22half2_rn(make_float2(v.x - f.x, v.y - f.y));
+          hi[k] = *reinterpret_cast<const uint32_t*>(&h);
+          lo[k] = *reinterpret_cast<const uint32_t*>(&l);
+        }
+        __half* row = obase + (s == 0 ? q0 : q1) * N;
+        stg256(row, hi);
+        stg256(row + ho.lo_offset, lo);
+      }
+    } else {
+      float* obase = V + j * v_plane_stride + 16 * tid;
+#pragma unroll
+      for (int s = 0; s < 2; ++s) {
+        if (s == 1 && !st1) break;
+        const float* x = s == 0 ? x0 : x1;
+        float* row = obase + (s == 0 ? q0 : q1) * N;
+        uint32_t u[8];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+#pragma unroll
+          for (int k = 0; k < 8; ++k) u[k] = __float_as_uint(x[8 * h + k]);
+          stg256(row + 8 * h, u);
+        }
+      }
+    }
   }
 }
 
