@@ -259,6 +259,7 @@ struct PlanT final : gmmnlse_plan {
   bool iir_rows = false;
   PairWork* pair_work = nullptr;
   int n_pair_work = 0;
+  ZetaPow iir_zk;
   std::map<const void*, CUtensorMap> field_tmaps;   // field buffer -> TMA map (the plan's At, or a caller's array)
   // serial RK4IP comparison integrator (allocated on first use)
   C *rk_X = nullptr, *rk_AI = nullptr, *rk_K1 = nullptr, *rk_K2 = nullptr, *rk_K3 = nullptr;
@@ -508,6 +509,11 @@ struct PlanT final : gmmnlse_plan {
       std::vector<PairWork> wl;
       for (int m0 = 0; m0 < P; m0 += 2)
         for (int nb = m0; nb < P; nb += 8) wl.push_back(PairWork{m0, nb, std::min(P, nb + 8)});
+      for (int k = 0; k < 16; ++k) {
+        const double mag = std::exp(lnm * k), ph = arg * k;
+        iir_zk.re[k] = (float)(mag * std::cos(ph));
+        iir_zk.im[k] = (float)(mag * std::sin(ph));
+      }
       n_pair_work = (int)wl.size();
       GM_TRY(dalloc(&pair_work, wl.size()));
       GM_TRY(upload(pair_work, wl));
@@ -569,10 +575,10 @@ struct PlanT final : gmmnlse_plan {
       const dim3 grid(n_pair_work, planes);
       if (half)
         k_pair_iir_rows<LOG2N, true><<<grid, NT, smem, stream>>>(*tm, plane0, Vout, v_ps, P, pair_work, iir_zeta, iir_cs,
-                                                                 iir_omf, iir_zp, cur_ho);
+                                                                 iir_omf, iir_zp, cur_ho, iir_zk);
       else
         k_pair_iir_rows<LOG2N, false><<<grid, NT, smem, stream>>>(*tm, plane0, Vout, v_ps, P, pair_work, iir_zeta, iir_cs,
-                                                                  iir_omf, iir_zp, cur_ho);
+                                                                  iir_omf, iir_zp, cur_ho, iir_zk);
       prof_end();
       GM_CUDA(cudaGetLastError());
       return 0;

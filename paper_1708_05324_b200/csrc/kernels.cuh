@@ -340,12 +340,13 @@ __device__ __forceinline__ void stg256(void* p, const uint32_t (&v)[8]) {
                "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]) : "memory");
 }
 struct PairWork { int m0, n_begin, n_end; };
+struct ZetaPow { float re[16], im[16]; };                              // zeta^k, k = 0..15 (kernel argument: constant bank)
 
 template <int LOG2N, bool HALF_OUT>
 __global__ void __launch_bounds__((1 << LOG2N) / 16, 1)
 k_pair_iir_rows(const __grid_constant__ CUtensorMap tmA, int plane0, float* __restrict__ V, long long v_plane_stride,
                 int P, const PairWork* __restrict__ work, float2 zeta, float2 cs, float omf,
-                const float2* __restrict__ zp, HalfOut ho) {
+                const float2* __restrict__ zp, HalfOut ho, const ZetaPow zk) {
   using namespace ptx;
   constexpr int N = 1 << LOG2N, NT = N / 16, NW = NT / 32;
   constexpr uint32_t ROW_BYTES = NT * 128, WARP_BYTES = 32 * 128;
@@ -376,7 +377,14 @@ k_pair_iir_rows(const __grid_constant__ CUtensorMap tmA, int plane0, float* __re
     mbar_arrive_expect_tx(bar_b, WARP_BYTES);
     tma_load_4d(dst0 + 2 * ROW_BYTES, &tmA, bar_b, 0, 32 * warp, wk.n_begin, plane0 + j);
   }
+  // Output recurrence in real arithmetic.  With y = Im(cs w), z = Im(cs zeta w) and zeta^2 = a1 zeta + a2:
+  //   V_e = (omf + Im cs) x_e + z_{e-1},  y_e = Im(cs) x_e + z_{e-1},  z_e = Im(cs zeta) x_e + a1 z_{e-1} + a2 y_{e-1}
+  // (5 operations per sample instead of 7).  The power-of-two output scale sv rides on the coefficients: exact.
   const float sv = HALF_OUT ? hc::v_scale(*ho.vbound, false) : 1.f;
+  const float2 csv = make_float2(cs.x * sv, cs.y * sv);
+  const float2 czv = make_float2(csv.x * zeta.x - csv.y * zeta.y, csv.x * zeta.y + csv.y * zeta.x);   // cs zeta sv
+  const float a1 = 2.f * zeta.x, a2 = -(zeta.x * zeta.x + zeta.y * zeta.y);
+  const float kx = omf * sv + csv.y;
   const float2 pl = zp[lane];                                         // zeta^(16 lane)
   mbar_wait(bar_park, 0, 11);
   int parity = 0;
@@ -398,12 +406,12 @@ k_pair_iir_rows(const __grid_constant__ CUtensorMap tmA, int plane0, float* __re
       mbar_arrive_expect_tx(bar_b, WARP_BYTES);
       tma_load_4d(dst0 + 2 * ROW_BYTES, &tmA, bar_b, 0, 32 * warp, n + 1, plane0 + j);
     }
-    // zero-state recurrence over the chunk
+    // chunk total from a zero state: sum_e zeta^(15 - e) x_e
     float2 w0 = make_float2(0.f, 0.f), w1 = w0;
 #pragma unroll
     for (int e = 0; e < 16; ++e) {
-      w0 = make_float2(x0[e] + zeta.x * w0.x - zeta.y * w0.y, zeta.x * w0.y + zeta.y * w0.x);
-      w1 = make_float2(x1[e] + zeta.x * w1.x - zeta.y * w1.y, zeta.x * w1.y + zeta.y * w1.x);
+      w0.x = fmaf(x0[e], zk.re[15 - e], w0.x); w0.y = fmaf(x0[e], zk.im[15 - e], w0.y);
+      w1.x = fmaf(x1[e], zk.re[15 - e], w1.x); w1.y = fmaf(x1[e], zk.im[15 - e], w1.y);
     }
     // inclusive scan of the chunk totals inside the warp: T_k = sum_{i<=k} zeta^(16 (k-i)) E_i
 #pragma unroll
@@ -428,13 +436,20 @@ k_pair_iir_rows(const __grid_constant__ CUtensorMap tmA, int plane0, float* __re
       w0 = make_float2(e0.x + pl.x * g0.x - pl.y * g0.y, e0.y + pl.x * g0.y + pl.y * g0.x);
       w1 = make_float2(e1.x + pl.x * g1.x - pl.y * g1.y, e1.y + pl.x * g1.y + pl.y * g1.x);
     }
-    // second pass from the true state: V = (1 - f_R) x + Im(cs w)
+    // second pass from the true state: sv V = sv [(1 - f_R) x + Im(cs w)]
+    {
+      float y0 = csv.x * w0.y + csv.y * w0.x, z0 = czv.x * w0.y + czv.y * w0.x;
+      float y1 = csv.x * w1.y + csv.y * w1.x, z1 = czv.x * w1.y + czv.y * w1.x;
 #pragma unroll
-    for (int e = 0; e < 16; ++e) {
-      w0 = make_float2(x0[e] + zeta.x * w0.x - zeta.y * w0.y, zeta.x * w0.y + zeta.y * w0.x);
-      w1 = make_float2(x1[e] + zeta.x * w1.x - zeta.y * w1.y, zeta.x * w1.y + zeta.y * w1.x);
-      x0[e] = omf * x0[e] + cs.x * w0.y + cs.y * w0.x;
-      x1[e] = omf * x1[e] + cs.x * w1.y + cs.y * w1.x;
+      for (int e = 0; e < 16; ++e) {
+        const float xa = x0[e], xb = x1[e];
+        x0[e] = fmaf(kx, xa, z0);
+        x1[e] = fmaf(kx, xb, z1);
+        const float ya = fmaf(csv.y, xa, z0), yb = fmaf(csv.y, xb, z1);
+        z0 = fmaf(czv.y, xa, fmaf(a1, z0, a2 * y0));
+        z1 = fmaf(czv.y, xb, fmaf(a1, z1, a2 * y1));
+        y0 = ya; y1 = yb;
+      }
     }
     const long long q0 = (long long)m0 * P - (long long)m0 * (m0 - 1) / 2 + (n - m0);
     const long long q1 = (long long)m1 * P - (long long)m1 * (m1 - 1) / 2 + (n - m1);
@@ -448,7 +463,7 @@ k_pair_iir_rows(const __grid_constant__ CUtensorMap tmA, int plane0, float* __re
         uint32_t hi[8], lo[8];
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
-          const float2 v = make_float2(x[2 * k] * sv, x[2 * k + 1] * sv);
+          const float2 v = make_float2(x[2 * k], x[2 * k + 1]);
           const __half2 h = __float22half2_rn(v);
           const float2 f = __half22float2(h);
           const __half2 l = __float22half2_rn(make_float2(v.x - f.x, v.y - f.y));
