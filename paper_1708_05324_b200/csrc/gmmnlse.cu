@@ -1092,8 +1092,40 @@ struct PlanT final : gmmnlse_plan {
     return 0;
   }
 
+  // small P (CUDA-core contraction, Q < 64, scalar-mode path): a6 + a7 -- and a4 when there is no Raman term -- in
+  // one pointwise kernel, k_small_contract_reduce
+  bool small_fused() const { return !general && !tc_h && !tc_on && !lowrank && P <= 10; }
+  template <int PMAX, int SPLIT>
+  int launch_small_t(const T* Vin, const C* A, C* Nout, int planes) {
+    constexpr int TW = 256 / SPLIT, QMAX = PMAX * (PMAX + 1) / 2, KQ = (QMAX + SPLIT - 1) / SPLIT, QP = (KQ * SPLIT + 3) & ~3;
+    const bool inline_pairs = f_R == 0.0;
+    const size_t smem = sizeof(T) * (size_t)QMAX * QP + sizeof(C) * (size_t)P * TW;
+    GM_TRY(inline_pairs ? ensure_smem(k_small_contract_reduce<T, PMAX, SPLIT, true>, smem)
+                        : ensure_smem(k_small_contract_reduce<T, PMAX, SPLIT, false>, smem));
+    const dim3 grid((N + TW - 1) / TW, planes);
+    prof_begin(GMMNLSE_KIND_CONTRACT);
+    if (inline_pairs)
+      k_small_contract_reduce<T, PMAX, SPLIT, true><<<grid, 256, smem, stream>>>(S2, Vin, QN, A, PN, Nout, PN, pair_m,
+                                                                                 pair_n, P, Q, N);
+    else
+      k_small_contract_reduce<T, PMAX, SPLIT, false><<<grid, 256, smem, stream>>>(S2, Vin, QN, A, PN, Nout, PN, pair_m,
+                                                                                  pair_n, P, Q, N);
+    prof_end();
+    GM_CUDA(cudaGetLastError());
+    return 0;
+  }
+  int launch_small(const T* Vin, const C* A, C* Nout, int planes) {
+    if (P <= 2) return launch_small_t<2, 1>(Vin, A, Nout, planes);
+    if (P <= 6) return launch_small_t<6, 1>(Vin, A, Nout, planes);
+    return launch_small_t<10, 4>(Vin, A, Nout, planes);
+  }
+
   // N_p[A_j](t) for `planes` planes starting at plane j0 of At -> G (time domain)   (a4-a7)
   int nonlinear_term(int j0, int planes) {
+    if (small_fused()) {
+      if (f_R != 0.0) GM_TRY(launch_pairs(At + j0 * PN, PN, V + j0 * QN, QN, planes));     // a4 + a5
+      return launch_small(V + j0 * QN, At + j0 * PN, G + j0 * PN, planes);                 // (a4 +) a6 + a7
+    }
     GM_TRY(launch_pairs(At + j0 * PN, PN, V + j0 * QN, QN, planes));
     GM_TRY(launch_contract(V + j0 * QN, U + j0 * QN, planes));
     GM_TRY(launch_mode_reduce(U + j0 * QN, At + j0 * PN, G + j0 * PN, planes));

@@ -637,6 +637,95 @@ k_mode_reduce_gen(const T* __restrict__ U, long long u_plane_stride, const cplx<
 }
 
 // ------------------------------------------------------------------------------------------
+// a6 + a7 (and a4 when there is no Raman term) for small P in ONE CUDA-core kernel: with Q = P(P+1)/2 < 64 the
+// contraction is a 21 x 21 ... 55 x 55 matrix per sample, far below an MMA tile and not GEMM-bound (SURVEY.md
+// 8(d) "a6-a7 at P <= 20: plain FP32 ALUs").  Everything here is pointwise in t:
+//   U_r(t) = sum_q S2[r][q] V_q(t),  r = (p <= l);   N_p += U_r A_l,  N_l += U_r A_p  (l != p)
+// so no U (and with INLINE_PAIRS no V either) ever exists in memory.  SPLIT lanes share a sample: lane s holds the
+// streams q = s, s + SPLIT, ... of its sample in registers and takes that share of every inner product, log2 SPLIT
+// warp shuffles complete U_r, and every lane keeps N_p (all p) in registers (the triangle is walked with
+// compile-time (p, l)).  SPLIT = 1 up to P = 6 (21 streams fit one thread's registers), 4 up to P = 10.  S2 (rows
+// padded to a compile-time stride: 128-bit broadcast reads) and the field tile sit in shared memory.
+//   grid = (N / TW, planes), block = 256, TW = 256 / SPLIT samples.  PMAX = compile-time bound on P.
+//   INLINE_PAIRS: V_q = Re(A_m A_n*) formed here (f_R == 0: a4 is pointwise too), else V is read (a5 ran).
+template <typename T, int PMAX, int SPLIT, bool INLINE_PAIRS>
+__global__ void __launch_bounds__(256)
+k_small_contract_reduce(const T* __restrict__ S2, const T* __restrict__ V, long long v_plane_stride,
+                        const cplx<T>* __restrict__ A, long long a_plane_stride, cplx<T>* __restrict__ Nt,
+                        long long n_plane_stride, const int* __restrict__ pair_m, const int* __restrict__ pair_n,
+                        int P, int Q, int N) {
+  constexpr int TW = 256 / SPLIT, QMAX = PMAX * (PMAX + 1) / 2, KQ = (QMAX + SPLIT - 1) / SPLIT, QP = (KQ * SPLIT + 3) & ~3;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* s2 = reinterpret_cast<T*>(smem_raw);                               // [QMAX][QP], zero-padded
+  cplx<T>* a_s = reinterpret_cast<cplx<T>*>(s2 + QMAX * QP);             // [P][TW]
+  T* v_s = reinterpret_cast<T*>(a_s + (size_t)P * TW);                   // [Q][TW] (INLINE_PAIRS: unused)
+  const int tid = threadIdx.x, j = blockIdx.y, t0 = blockIdx.x * TW;
+  for (int i = tid; i < QMAX * QP; i += 256) {
+    const int rr = i / QP, qq = i % QP;
+    s2[i] = rr < Q && qq < Q ? S2[rr * Q + qq] : (T)0;
+  }
+  for (int i = tid; i < P * TW; i += 256) {
+    const int xx = i % TW;
+    a_s[i] = t0 + xx < N ? A[j * a_plane_stride + (long long)(i / TW) * N + t0 + xx] : mk((T)0, (T)0);
+  }
+  const int x = tid / SPLIT, sub = tid % SPLIT;                           // sample, lane among the sample's SPLIT lanes
+  T vq[KQ];
+  if constexpr (!INLINE_PAIRS) {                                          // this lane's streams straight from V (coalesced over x)
+#pragma unroll
+    for (int k = 0; k < KQ; ++k) {
+      const int q = SPLIT * k + sub;
+      vq[k] = q < Q && t0 + x < N ? V[j * v_plane_stride + (long long)q * N + t0 + x] : (T)0;
+    }
+  }
+  __syncthreads();
+  if constexpr (INLINE_PAIRS) {
+#pragma unroll
+    for (int k = 0; k < KQ; ++k) {
+      const int q = SPLIT * k + sub;
+      vq[k] = (T)0;
+      if (q < Q) {
+        const cplx<T> am = a_s[pair_m[q] * TW + x], an = a_s[pair_n[q] * TW + x];
+        vq[k] = am.x * an.x + am.y * an.y;                                // Re(A_m A_n*)
+      }
+    }
+  }
+  T nx[PMAX], ny[PMAX];
+#pragma unroll
+  for (int p = 0; p < PMAX; ++p) nx[p] = ny[p] = (T)0;
+  int r = 0;
+#pragma unroll
+  for (int p = 0; p < PMAX; ++p) {
+    if (p < P) {
+      const cplx<T> ap = a_s[p * TW + x];
+#pragma unroll
+      for (int l = p; l < PMAX; ++l) {
+        if (l < P) {
+          const T* srow = s2 + r * QP + sub;                              // padded entries are zero: no bound checks
+          T u = (T)0;
+#pragma unroll
+          for (int k = 0; k < KQ; ++k) u += srow[SPLIT * k] * vq[k];
+#pragma unroll
+          for (int d = 1; d < SPLIT; d <<= 1) u += __shfl_xor_sync(0xffffffffu, u, d);
+          const cplx<T> al = a_s[l * TW + x];
+          nx[p] += u * al.x;
+          ny[p] += u * al.y;
+          if (l != p) {
+            nx[l] += u * ap.x;
+            ny[l] += u * ap.y;
+          }
+          ++r;
+        }
+      }
+    }
+  }
+  if (sub == 0 && t0 + x < N) {
+#pragma unroll
+    for (int p = 0; p < PMAX; ++p)
+      if (p < P) Nt[j * n_plane_stride + (long long)p * N + t0 + x] = mk(nx[p], ny[p]);
+  }
+}
+
+// ------------------------------------------------------------------------------------------
 // a9 + a10: cumulative trapezoid over planes and the per-plane error norms.
 //   psi_j^new = psi_0 + dz [G_0/2 + G_1 + .. + G_{j-1} + G_j/2], j = 1..Mc
 //   errbuf[2 j] += sum |psi_j^new - psi_j^old|^2,  errbuf[2 j + 1] += sum |psi_j^new|^2
