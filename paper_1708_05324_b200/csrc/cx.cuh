@@ -28,4 +28,15 @@ template <int S, typename C> __host__ __device__ __forceinline__ C cmul_i(C a) {
   return S > 0 ? mk(-a.y, a.x) : mk(a.y, -a.x);
 }
 
+// Programmatic dependent launch: every kernel is launched with programmatic stream serialisation, so it may start
+// while its predecessor on the stream drains.  pdl_launch_dependents() lets the successor be scheduled; pdl_wait()
+// returns once every predecessor grid has completed and its memory is visible -- it precedes the kernel's first
+// access (read or write) to global memory.  Both are no-ops for a kernel launched without the attribute.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_prologue() {
+  pdl_launch_dependents();
+  pdl_wait();
+}
+
 }  // namespace gm

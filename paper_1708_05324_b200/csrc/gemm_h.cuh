@@ -31,6 +31,7 @@
 #include <cuda.h>
 #include <cuda_fp16.h>
 
+#include "cx.cuh"
 #include "ptx_sm100.cuh"
 
 namespace gm {
@@ -80,6 +81,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
 k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ CUtensorMap tmVl,
              const __grid_constant__ CUtensorMap tmSh, const __grid_constant__ CUtensorMap tmSl, const Params p) {
   using namespace ptx;
+  pdl_launch_dependents();
   extern __shared__ unsigned char smem_raw[];
   const uint32_t raw_addr = smem_u32(smem_raw);
   const uint32_t base = (raw_addr + 1023u) & ~1023u;     // 1024-byte aligned: swizzle atoms
@@ -120,6 +122,7 @@ k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ C
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  pdl_wait();                     // everything above touches no global data: it overlaps the predecessor's tail
 
   const int cta = blockIdx.x, nctas = gridDim.x;
   const int tiles_per_plane = p.n_rt * p.t_tiles;

@@ -31,6 +31,7 @@
 #pragma once
 #include <cuda.h>
 
+#include "cx.cuh"
 #include "ptx_sm100.cuh"
 
 namespace gm {
@@ -64,6 +65,7 @@ __global__ void __launch_bounds__(NTHREADS, 1)
 k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmShi,
               const __grid_constant__ CUtensorMap tmSlo, const Params p) {
   using namespace ptx;
+  pdl_launch_dependents();
   extern __shared__ unsigned char smem_raw[];
   const uint32_t raw_addr = smem_u32(smem_raw);
   const uint32_t base = (raw_addr + 1023u) & ~1023u;     // 1024-byte aligned: swizzle atoms
@@ -105,6 +107,7 @@ k_contract_tc(const __grid_constant__ CUtensorMap tmV, const __grid_constant__ C
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  pdl_wait();                     // everything above touches no global data: it overlaps the predecessor's tail
 
   const int pair = blockIdx.x, npairs = gridDim.x;
   const int tiles_per_plane = p.n_rt * p.t_tiles;

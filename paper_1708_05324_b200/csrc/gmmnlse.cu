@@ -11,6 +11,7 @@
 #include <mutex>
 #include <new>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/gmmnlse.h"
@@ -295,6 +296,27 @@ struct PlanT final : gmmnlse_plan {
   bool tc_on = false;          // dense 3xTF32 form (gemm_tc.cuh)
   int tc_NT = 0, tc_nrt = 0, tc_KB = 0, tc_stages = 0, tc_kchunk = 4, n_sm = 0;
   template <typename F> int ensure_smem(F fn, size_t bytes) { return ensure_dyn_smem(device, (const void*)fn, bytes); }
+  // Every kernel goes out with programmatic stream serialisation (PDL): the next kernel on the stream may be
+  // scheduled while this one drains and blocks in pdl_wait() until it has completed.  Captured into the loop graphs
+  // this turns the kernel-to-kernel edges into programmatic ones (the launch-bound small configurations).
+  bool pdl = true;
+  cudaLaunchAttribute pdl_attr[1];
+  void pdl_config(cudaLaunchConfig_t& cfg) {
+    pdl_attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    pdl_attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = pdl_attr;
+    cfg.numAttrs = pdl ? 1 : 0;
+  }
+  template <typename... KArgs, typename... Args>
+  void launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    pdl_config(cfg);
+    cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(std::forward<Args>(args))...);   // errors: cudaGetLastError() at the call site
+  }
 
   ~PlanT() override {
     cudaFree(tw); cudaFree(Kw); cudaFree(H); cudaFree(E); cudaFree(EM_d); cudaFree(S2);
@@ -505,10 +527,17 @@ struct PlanT final : gmmnlse_plan {
     iir_omf = (T)(1.0 - f_R);
     iir = true;
     if (sizeof(T) == 4 && !general && log2N >= 9 && log2N <= 13 && lnm * 512.0 < std::log(1e-12)) {
-      // work list: CTA = rows (m0, m0 + 1) against up to 8 rows n >= m0
+      // work list: CTA = rows (m0, m0 + 1) against up to G rows n >= m0.  G = 8 amortises the two parked rows;
+      // with few modes that leaves most SMs without a CTA, so G shrinks until a launch of M planes has two per SM
+      int dev = 0, sms = 148;
+      GM_CUDA(cudaGetDevice(&dev));
+      GM_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+      int G = 8;
+      auto n_ctas = [&](int g) { long long c = 0; for (int m0 = 0; m0 < P; m0 += 2) c += (P - m0 + g - 1) / g; return c * M; };
+      while (G > 1 && n_ctas(G) < 2LL * sms) G /= 2;
       std::vector<PairWork> wl;
       for (int m0 = 0; m0 < P; m0 += 2)
-        for (int nb = m0; nb < P; nb += 8) wl.push_back(PairWork{m0, nb, std::min(P, nb + 8)});
+        for (int nb = m0; nb < P; nb += G) wl.push_back(PairWork{m0, nb, std::min(P, nb + G)});
       for (int k = 0; k < 16; ++k) {
         const double mag = std::exp(lnm * k), ph = arg * k;
         iir_zk.re[k] = (float)(mag * std::cos(ph));
@@ -530,10 +559,10 @@ struct PlanT final : gmmnlse_plan {
     prof_begin(GMMNLSE_KIND_PAIR_CONV);
     const dim3 grid((Q + 1) / 2, planes);
     if (general)
-      k_pair_iir<T, LOG2N, true><<<grid, NT, smem, stream>>>(A, a_ps, Vout, v_ps, pair_m, pair_n, Q, iir_zeta, iir_cs,
+      launch_k(k_pair_iir<T, LOG2N, true>, grid, NT, smem, A, a_ps, Vout, v_ps, pair_m, pair_n, Q, iir_zeta, iir_cs,
                                                              iir_omf, iir_zp, spec(), cur_ho);
     else
-      k_pair_iir<T, LOG2N, false><<<grid, NT, smem, stream>>>(A, a_ps, Vout, v_ps, pair_m, pair_n, Q, iir_zeta,
+      launch_k(k_pair_iir<T, LOG2N, false>, grid, NT, smem, A, a_ps, Vout, v_ps, pair_m, pair_n, Q, iir_zeta,
                                                               iir_cs, iir_omf, iir_zp, spec(), cur_ho);
     prof_end();
     GM_CUDA(cudaGetLastError());
@@ -574,10 +603,10 @@ struct PlanT final : gmmnlse_plan {
       prof_begin(GMMNLSE_KIND_PAIR_CONV);
       const dim3 grid(n_pair_work, planes);
       if (half)
-        k_pair_iir_rows<LOG2N, true><<<grid, NT, smem, stream>>>(*tm, plane0, Vout, v_ps, P, pair_work, iir_zeta, iir_cs,
+        launch_k(k_pair_iir_rows<LOG2N, true>, grid, NT, smem, *tm, plane0, Vout, v_ps, P, pair_work, iir_zeta, iir_cs,
                                                                  iir_omf, iir_zp, cur_ho, iir_zk);
       else
-        k_pair_iir_rows<LOG2N, false><<<grid, NT, smem, stream>>>(*tm, plane0, Vout, v_ps, P, pair_work, iir_zeta, iir_cs,
+        launch_k(k_pair_iir_rows<LOG2N, false>, grid, NT, smem, *tm, plane0, Vout, v_ps, P, pair_work, iir_zeta, iir_cs,
                                                                   iir_omf, iir_zp, cur_ho, iir_zk);
       prof_end();
       GM_CUDA(cudaGetLastError());
@@ -663,6 +692,7 @@ struct PlanT final : gmmnlse_plan {
       cfg.blockDim = dim3(tc::NTHREADS);
       cfg.dynamicSmemBytes = tc::smem_bytes(g.NT, g.stages);
       cfg.stream = stream;
+      pdl_config(cfg);
       prof_begin(GMMNLSE_KIND_CONTRACT);
       cudaError_t e = cudaLaunchKernelEx(&cfg, tc::k_contract_tc, amap, g.tmHi, g.tmLo, prm);
       prof_end();
@@ -742,6 +772,7 @@ struct PlanT final : gmmnlse_plan {
       cfg.blockDim = dim3(hc::NTHREADS);
       cfg.dynamicSmemBytes = hc::smem_bytes(g.NT, g.stages);
       cfg.stream = stream;
+      pdl_config(cfg);
       prof_begin(GMMNLSE_KIND_CONTRACT);
       cudaError_t e = outZ ? cudaLaunchKernelEx(&cfg, hc::k_contract_h<true>, mhi, mlo, g.tmHi, g.tmLo, prm)
                            : cudaLaunchKernelEx(&cfg, hc::k_contract_h<false>, mhi, mlo, g.tmHi, g.tmLo, prm);
@@ -915,6 +946,7 @@ struct PlanT final : gmmnlse_plan {
       cfg.blockDim = dim3(tc::NTHREADS);
       cfg.dynamicSmemBytes = tc::smem_bytes(tc_NT, tc_stages);
       cfg.stream = stream;
+      pdl_config(cfg);
       prof_begin(GMMNLSE_KIND_CONTRACT);
       cudaError_t e = cudaLaunchKernelEx(&cfg, tc::k_contract_tc, vmap, tmShi, tmSlo, prm);
       prof_end();
@@ -931,7 +963,7 @@ struct PlanT final : gmmnlse_plan {
     const size_t smem = sizeof(C) * fft_smem_elems(1 << LOG2N);
     GM_TRY(ensure_smem(k_fft_rows<T, LOG2N, DIR>, smem));
     prof_begin(DIR > 0 ? GMMNLSE_KIND_FFT_TO_FREQ : GMMNLSE_KIND_FFT_TO_TIME);
-    k_fft_rows<T, LOG2N, DIR><<<dim3(rows, planes), NT, smem, stream>>>(in, in_ps, out, out_ps, pre, post_vec,
+    launch_k(k_fft_rows<T, LOG2N, DIR>, dim3(rows, planes), NT, smem, in, in_ps, out, out_ps, pre, post_vec,
                                                                          post_tab, tab_ps, scale, tw, rscale);
     prof_end();
     GM_CUDA(cudaGetLastError());
@@ -967,7 +999,7 @@ struct PlanT final : gmmnlse_plan {
     const size_t smem = RAMAN ? sizeof(C) * fft_smem_elems(1 << LOG2N) : 0;
     GM_TRY(ensure_smem(k_pair_conv<T, LOG2N, RAMAN>, smem));
     prof_begin(GMMNLSE_KIND_PAIR_CONV);
-    k_pair_conv<T, LOG2N, RAMAN><<<dim3((Q + 1) / 2, planes), NT, smem, stream>>>(A, a_ps, Vout, v_ps, pair_m,
+    launch_k(k_pair_conv<T, LOG2N, RAMAN>, dim3((Q + 1) / 2, planes), NT, smem, A, a_ps, Vout, v_ps, pair_m,
                                                                                   pair_n, Q, H, tw, spec(), cur_ho);
     prof_end();
     GM_CUDA(cudaGetLastError());
@@ -980,7 +1012,7 @@ struct PlanT final : gmmnlse_plan {
       if (tc_h && own_v(Vout)) {                    // the f16 contraction follows: V as fp16 hi / lo planes
         GM_CUDA(cudaMemsetAsync(d_vbound, 0, sizeof(float), stream));
         prof_begin(GMMNLSE_KIND_PAIR_CONV);
-        k_bound_field<T><<<dim3(32, planes), 256, 0, stream>>>(A, a_ps, PN, v_gain, d_vbound);
+        launch_k(k_bound_field<T>, dim3(32, planes), 256, 0, A, a_ps, PN, v_gain, d_vbound);
         prof_end();
         GM_CUDA(cudaGetLastError());
         cur_ho = HalfOut{reinterpret_cast<__half*>(Vout), 2 * QN, QN, N, d_vbound};
@@ -1020,8 +1052,8 @@ struct PlanT final : gmmnlse_plan {
           const long long total = (long long)planes * QN;
           GM_CUDA(cudaMemsetAsync(d_vbound, 0, sizeof(float), stream));
           prof_begin(GMMNLSE_KIND_CONTRACT);
-          k_bound_real<T><<<592, 256, 0, stream>>>(Vin, total, d_vbound);
-          k_v_encode<<<1184, 256, 0, stream>>>(Vin, QN, total,
+          launch_k(k_bound_real<T>, 592, 256, 0, Vin, total, d_vbound);
+          launch_k(k_v_encode, 1184, 256, 0, Vin, QN, total,
                                                HalfOut{reinterpret_cast<__half*>(V), 2 * QN, QN, N, d_vbound});
           prof_end();
           GM_CUDA(cudaGetLastError());
@@ -1056,11 +1088,11 @@ struct PlanT final : gmmnlse_plan {
     if (Q <= 32) {
       constexpr int BM = 32, BN = 128, BK = 8, TM = 4, TN = 4;
       dim3 grid((N + BN - 1) / BN, (Q + BM - 1) / BM, planes);
-      k_contract<T, BM, BN, BK, TM, TN><<<grid, (BM / TM) * (BN / TN), 0, stream>>>(S2, Vin, QN, Uout, QN, Q, N);
+      launch_k(k_contract<T, BM, BN, BK, TM, TN>, grid, (BM / TM) * (BN / TN), 0, S2, Vin, QN, Uout, QN, Q, N);
     } else {
       constexpr int BM = 128, BN = 128, BK = 8, TM = 8, TN = 8;
       dim3 grid((N + BN - 1) / BN, (Q + BM - 1) / BM, planes);
-      k_contract<T, BM, BN, BK, TM, TN><<<grid, (BM / TM) * (BN / TN), 0, stream>>>(S2, Vin, QN, Uout, QN, Q, N);
+      launch_k(k_contract<T, BM, BN, BK, TM, TN>, grid, (BM / TM) * (BN / TN), 0, S2, Vin, QN, Uout, QN, Q, N);
     }
     prof_end();
     GM_CUDA(cudaGetLastError());
@@ -1073,7 +1105,7 @@ struct PlanT final : gmmnlse_plan {
       GM_TRY(ensure_smem(k_mode_reduce_gen<T>, smem));
       const int Gg = P >= 12 ? 4 : (P >= 4 ? 2 : 1);
       prof_begin(GMMNLSE_KIND_MODE_REDUCE);
-      k_mode_reduce_gen<T><<<dim3((N + 127) / 128, planes), 128 * Gg, smem, stream>>>(Uin, QN, A, PN, Nout, PN, P, Bp,
+      launch_k(k_mode_reduce_gen<T>, dim3((N + 127) / 128, planes), 128 * Gg, smem, Uin, QN, A, PN, Nout, PN, P, Bp,
                                                                                         N);
       prof_end();
       GM_CUDA(cudaGetLastError());
@@ -1085,8 +1117,8 @@ struct PlanT final : gmmnlse_plan {
     GM_TRY(tw == 32 ? ensure_smem(k_mode_reduce<T, 32>, smem) : ensure_smem(k_mode_reduce<T, 128>, smem));
     const dim3 grid((N + tw - 1) / tw, planes);
     prof_begin(GMMNLSE_KIND_MODE_REDUCE);
-    if (tw == 32) k_mode_reduce<T, 32><<<grid, 32 * G, smem, stream>>>(Uin, QN, A, PN, Nout, PN, P, N);
-    else k_mode_reduce<T, 128><<<grid, 128 * G, smem, stream>>>(Uin, QN, A, PN, Nout, PN, P, N);
+    if (tw == 32) launch_k(k_mode_reduce<T, 32>, grid, 32 * G, smem, Uin, QN, A, PN, Nout, PN, P, N);
+    else launch_k(k_mode_reduce<T, 128>, grid, 128 * G, smem, Uin, QN, A, PN, Nout, PN, P, N);
     prof_end();
     GM_CUDA(cudaGetLastError());
     return 0;
@@ -1097,7 +1129,8 @@ struct PlanT final : gmmnlse_plan {
   bool small_fused() const { return !general && !tc_h && !tc_on && !lowrank && P <= 10; }
   template <int PMAX, int SPLIT>
   int launch_small_t(const T* Vin, const C* A, C* Nout, int planes) {
-    constexpr int TW = 256 / SPLIT, QMAX = PMAX * (PMAX + 1) / 2, KQ = (QMAX + SPLIT - 1) / SPLIT, QP = (KQ * SPLIT + 3) & ~3;
+    constexpr int TW = kSmallThreads / SPLIT, QMAX = PMAX * (PMAX + 1) / 2, KQ = (QMAX + SPLIT - 1) / SPLIT,
+                  QP = (KQ * SPLIT + 3) & ~3;
     const bool inline_pairs = f_R == 0.0;
     const size_t smem = sizeof(T) * (size_t)QMAX * QP + sizeof(C) * (size_t)P * TW;
     GM_TRY(inline_pairs ? ensure_smem(k_small_contract_reduce<T, PMAX, SPLIT, true>, smem)
@@ -1105,10 +1138,10 @@ struct PlanT final : gmmnlse_plan {
     const dim3 grid((N + TW - 1) / TW, planes);
     prof_begin(GMMNLSE_KIND_CONTRACT);
     if (inline_pairs)
-      k_small_contract_reduce<T, PMAX, SPLIT, true><<<grid, 256, smem, stream>>>(S2, Vin, QN, A, PN, Nout, PN, pair_m,
+      launch_k(k_small_contract_reduce<T, PMAX, SPLIT, true>, grid, kSmallThreads, smem, S2, Vin, QN, A, PN, Nout, PN, pair_m,
                                                                                  pair_n, P, Q, N);
     else
-      k_small_contract_reduce<T, PMAX, SPLIT, false><<<grid, 256, smem, stream>>>(S2, Vin, QN, A, PN, Nout, PN, pair_m,
+      launch_k(k_small_contract_reduce<T, PMAX, SPLIT, false>, grid, kSmallThreads, smem, S2, Vin, QN, A, PN, Nout, PN, pair_m,
                                                                                   pair_n, P, Q, N);
     prof_end();
     GM_CUDA(cudaGetLastError());
@@ -1135,7 +1168,7 @@ struct PlanT final : gmmnlse_plan {
   int to_master(const C* src) {   // psi0_d <- src (promote)
     const long long n = 2 * PN;
     prof_begin(GMMNLSE_KIND_MISC);
-    k_convert<T, double><<<(unsigned)((n + 255) / 256), 256, 0, stream>>>((const T*)src, (double*)psi0_d, n);
+    launch_k(k_convert<T, double>, (unsigned)((n + 255) / 256), 256, 0, (const T*)src, (double*)psi0_d, n);
     prof_end();
     GM_CUDA(cudaGetLastError());
     return 0;
@@ -1157,7 +1190,7 @@ struct PlanT final : gmmnlse_plan {
                            gfwd ? gfwd + j0 * P : nullptr, ginv ? ginv + j0 * P : nullptr, G + j0 * PN, np));
     // a9 + a10
     prof_begin(GMMNLSE_KIND_SCAN);
-    k_trapz_scan<T><<<sblocks, 256, sizeof(double) * 2 * (Mc + 1), stream>>>(psi, G, psi, PN, Mc, (T)dz,
+    launch_k(k_trapz_scan<T>, sblocks, 256, sizeof(double) * 2 * (Mc + 1), psi, G, psi, PN, Mc, (T)dz,
                                                                              first ? 1 : 0, errbuf, PN);
     prof_end();
     GM_CUDA(cudaGetLastError());
@@ -1167,7 +1200,7 @@ struct PlanT final : gmmnlse_plan {
   int enqueue_advance(int Mc, const double2* EM) {                           // a11
     const unsigned sblocks = (unsigned)((PN + 255) / 256);
     prof_begin(GMMNLSE_KIND_ADVANCE);
-    k_advance<T><<<sblocks, 256, 0, stream>>>(psi0_d, psi, G, PN, Mc, dz, EM, PN);
+    launch_k(k_advance<T>, sblocks, 256, 0, psi0_d, psi, G, PN, Mc, dz, EM, PN);
     prof_end();
     GM_CUDA(cudaGetLastError());
     return 0;
@@ -1192,7 +1225,7 @@ struct PlanT final : gmmnlse_plan {
     while (true) {
       GM_TRY(enqueue_iteration(Mc, it == 0));
       prof_begin(GMMNLSE_KIND_MISC);
-      k_err_finalize<<<1, 32, 0, stream>>>(errbuf, Mc, d_err);
+      launch_k(k_err_finalize, 1, 32, 0, errbuf, Mc, d_err);
       prof_end();
       GM_CUDA(cudaGetLastError());
       ++it;
@@ -1236,7 +1269,7 @@ struct PlanT final : gmmnlse_plan {
     GM_CUDA(cudaGraphConditionalHandleCreate(&handle, lg, 0, 0));
     auto finalize = [&]() -> int {
       prof_begin(GMMNLSE_KIND_MISC);
-      k_err_finalize_loop<<<1, 32, 0, stream>>>(errbuf, M, d_err, tol, cap, fixed_iter > 0 ? 1 : 0, handle, d_stats);
+      launch_k(k_err_finalize_loop, 1, 32, 0, errbuf, M, d_err, tol, cap, fixed_iter > 0 ? 1 : 0, handle, d_stats);
       prof_end();
       GM_CUDA(cudaGetLastError());
       return 0;
@@ -1402,7 +1435,7 @@ struct PlanT final : gmmnlse_plan {
     const size_t smem = sizeof(C) * P * 64;
     GM_TRY(ensure_smem(k_couple<T>, smem));
     prof_begin(GMMNLSE_KIND_MISC);
-    k_couple<T><<<dim3((N + 63) / 64, planes), 256, smem, stream>>>(src, src_ps, Etab, gf, gi, Qc, Gout, PN, P, N);
+    launch_k(k_couple<T>, dim3((N + 63) / 64, planes), 256, smem, src, src_ps, Etab, gf, gi, Qc, Gout, PN, P, N);
     prof_end();
     GM_CUDA(cudaGetLastError());
     return 0;
@@ -1459,7 +1492,7 @@ struct PlanT final : gmmnlse_plan {
     for (int stage = 1; stage <= 4; ++stage) {
       GM_TRY(nonlinear_freq(stage == 1 ? psi : rk_X));
       prof_begin(GMMNLSE_KIND_ADVANCE);
-      k_rk4_stage<T><<<blocks, 256, 0, stream>>>(stage, psi0_d, psi, EH_d, G, rk_AI, rk_K1, rk_K2, rk_K3, rk_X, dz, PN);
+      launch_k(k_rk4_stage<T>, blocks, 256, 0, stage, psi0_d, psi, EH_d, G, rk_AI, rk_K1, rk_K2, rk_K3, rk_X, dz, PN);
       prof_end();
       GM_CUDA(cudaGetLastError());
     }

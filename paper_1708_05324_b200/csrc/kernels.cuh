@@ -21,6 +21,7 @@ k_fft_rows(const cplx<T>* __restrict__ in, long long in_plane_stride, cplx<T>* _
            long long out_plane_stride, const cplx<T>* __restrict__ pre, const cplx<T>* __restrict__ post_vec,
            const cplx<T>* __restrict__ post_tab, long long tab_plane_stride, T scale,
            const cplx<T>* __restrict__ tw, const T* __restrict__ row_scale) {
+  pdl_prologue();
   constexpr int N = 1 << LOG2N;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
@@ -70,6 +71,7 @@ struct HalfOut {
 template <typename T>
 __global__ void __launch_bounds__(256)
 k_bound_field(const cplx<T>* __restrict__ A, long long a_plane_stride, long long n, float gain, float* bound) {
+  pdl_prologue();
   const cplx<T>* a = A + blockIdx.y * a_plane_stride;
   float m = 0.f;
   for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256) {
@@ -84,6 +86,7 @@ k_bound_field(const cplx<T>* __restrict__ A, long long a_plane_stride, long long
 template <typename T>
 __global__ void __launch_bounds__(256)
 k_bound_real(const T* __restrict__ V, long long n, float* bound) {
+  pdl_prologue();
   float m = 0.f;
   for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256)
     m = fmaxf(m, fabsf((float)V[i]));
@@ -95,6 +98,7 @@ k_bound_real(const T* __restrict__ V, long long n, float* bound) {
 // fp32 V[planes][Q][N] -> fp16 split planes (for a caller-supplied V: gmmnlse_debug_contract)
 __global__ void __launch_bounds__(256)
 k_v_encode(const float* __restrict__ Vin, long long QN, long long total, HalfOut ho) {
+  pdl_prologue();
   for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < total; i += (long long)gridDim.x * 256) {
     const int j = (int)(i / QN);
     const long long r = i - j * QN;
@@ -127,6 +131,7 @@ __global__ void __launch_bounds__((1 << LOG2N) / 16)
 k_pair_conv(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restrict__ V, long long v_plane_stride,
             const int* __restrict__ pair_m, const int* __restrict__ pair_n, int Q,
             const cplx<T>* __restrict__ H, const cplx<T>* __restrict__ tw, StreamSpec<T> gs, HalfOut ho) {
+  pdl_prologue();
   constexpr int N = 1 << LOG2N, NT = N / 16;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
@@ -203,6 +208,7 @@ __global__ void __launch_bounds__((1 << LOG2N) / 16)
 k_pair_iir(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restrict__ V, long long v_plane_stride,
            const int* __restrict__ pair_m, const int* __restrict__ pair_n, int Q, cplx<T> zeta, cplx<T> cs, T omf,
            const cplx<T>* __restrict__ zp, StreamSpec<T> gs, HalfOut ho) {
+  pdl_prologue();
   constexpr int N = 1 << LOG2N, NT = N / 16, NW = (NT + 31) / 32;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);         // fft_smem_elems(N) + 2 * (NW + 1) complex
@@ -347,6 +353,7 @@ __global__ void __launch_bounds__((1 << LOG2N) / 16, 1)
 k_pair_iir_rows(const __grid_constant__ CUtensorMap tmA, int plane0, float* __restrict__ V, long long v_plane_stride,
                 int P, const PairWork* __restrict__ work, float2 zeta, float2 cs, float omf,
                 const float2* __restrict__ zp, HalfOut ho, const ZetaPow zk) {
+  pdl_prologue();
   using namespace ptx;
   constexpr int N = 1 << LOG2N, NT = N / 16, NW = NT / 32;
   constexpr uint32_t ROW_BYTES = NT * 128, WARP_BYTES = 32 * 128;
@@ -501,6 +508,7 @@ template <typename T, int BM, int BN, int BK, int TM, int TN>
 __global__ void __launch_bounds__((BM / TM) * (BN / TN))
 k_contract(const T* __restrict__ S2, const T* __restrict__ V, long long v_plane_stride, T* __restrict__ U,
            long long u_plane_stride, int Q, int N) {
+  pdl_prologue();
   constexpr int NTH = (BM / TM) * (BN / TN);
   __shared__ T As[BK][BM + 4];
   __shared__ T Bs[BK][BN];
@@ -562,6 +570,7 @@ template <typename T, int TW>
 __global__ void __launch_bounds__(512)
 k_mode_reduce(const T* __restrict__ U, long long u_plane_stride, const cplx<T>* __restrict__ A,
               long long a_plane_stride, cplx<T>* __restrict__ Nt, long long n_plane_stride, int P, int N) {
+  pdl_prologue();
   // TW = samples per CTA (32 / 64 / 128): a narrow tile keeps the CTA's slice of U (Q x TW x 4 B) small enough
   // that its second read (U_lp) still finds the first (U_pl) in L2
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -607,6 +616,7 @@ template <typename T>
 __global__ void __launch_bounds__(512)
 k_mode_reduce_gen(const T* __restrict__ U, long long u_plane_stride, const cplx<T>* __restrict__ A,
                   long long a_plane_stride, cplx<T>* __restrict__ Nt, long long n_plane_stride, int P, int Bp, int N) {
+  pdl_prologue();
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* a_s = reinterpret_cast<cplx<T>*>(smem_raw);        // [P][128]
   const int tx = threadIdx.x & 127, g = threadIdx.x >> 7, G = blockDim.x >> 7, j = blockIdx.y;
@@ -646,25 +656,28 @@ k_mode_reduce_gen(const T* __restrict__ U, long long u_plane_stride, const cplx<
 // warp shuffles complete U_r, and every lane keeps N_p (all p) in registers (the triangle is walked with
 // compile-time (p, l)).  SPLIT = 1 up to P = 6 (21 streams fit one thread's registers), 4 up to P = 10.  S2 (rows
 // padded to a compile-time stride: 128-bit broadcast reads) and the field tile sit in shared memory.
-//   grid = (N / TW, planes), block = 256, TW = 256 / SPLIT samples.  PMAX = compile-time bound on P.
+//   grid = (N / TW, planes), block = 128, TW = 128 / SPLIT samples.  PMAX = compile-time bound on P.
 //   INLINE_PAIRS: V_q = Re(A_m A_n*) formed here (f_R == 0: a4 is pointwise too), else V is read (a5 ran).
+constexpr int kSmallThreads = 128;
 template <typename T, int PMAX, int SPLIT, bool INLINE_PAIRS>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(kSmallThreads)
 k_small_contract_reduce(const T* __restrict__ S2, const T* __restrict__ V, long long v_plane_stride,
                         const cplx<T>* __restrict__ A, long long a_plane_stride, cplx<T>* __restrict__ Nt,
                         long long n_plane_stride, const int* __restrict__ pair_m, const int* __restrict__ pair_n,
                         int P, int Q, int N) {
-  constexpr int TW = 256 / SPLIT, QMAX = PMAX * (PMAX + 1) / 2, KQ = (QMAX + SPLIT - 1) / SPLIT, QP = (KQ * SPLIT + 3) & ~3;
+  pdl_prologue();
+  constexpr int NTH = kSmallThreads, TW = NTH / SPLIT, QMAX = PMAX * (PMAX + 1) / 2, KQ = (QMAX + SPLIT - 1) / SPLIT,
+                QP = (KQ * SPLIT + 3) & ~3;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* s2 = reinterpret_cast<T*>(smem_raw);                               // [QMAX][QP], zero-padded
   cplx<T>* a_s = reinterpret_cast<cplx<T>*>(s2 + QMAX * QP);             // [P][TW]
   T* v_s = reinterpret_cast<T*>(a_s + (size_t)P * TW);                   // [Q][TW] (INLINE_PAIRS: unused)
   const int tid = threadIdx.x, j = blockIdx.y, t0 = blockIdx.x * TW;
-  for (int i = tid; i < QMAX * QP; i += 256) {
+  for (int i = tid; i < QMAX * QP; i += NTH) {
     const int rr = i / QP, qq = i % QP;
     s2[i] = rr < Q && qq < Q ? S2[rr * Q + qq] : (T)0;
   }
-  for (int i = tid; i < P * TW; i += 256) {
+  for (int i = tid; i < P * TW; i += NTH) {
     const int xx = i % TW;
     a_s[i] = t0 + xx < N ? A[j * a_plane_stride + (long long)(i / TW) * N + t0 + xx] : mk((T)0, (T)0);
   }
@@ -701,9 +714,10 @@ k_small_contract_reduce(const T* __restrict__ S2, const T* __restrict__ V, long 
       for (int l = p; l < PMAX; ++l) {
         if (l < P) {
           const T* srow = s2 + r * QP + sub;                              // padded entries are zero: no bound checks
-          T u = (T)0;
+          T up[4] = {(T)0, (T)0, (T)0, (T)0};                            // four independent chains
 #pragma unroll
-          for (int k = 0; k < KQ; ++k) u += srow[SPLIT * k] * vq[k];
+          for (int k = 0; k < KQ; ++k) up[k & 3] += srow[SPLIT * k] * vq[k];
+          T u = (up[0] + up[1]) + (up[2] + up[3]);
 #pragma unroll
           for (int d = 1; d < SPLIT; d <<= 1) u += __shfl_xor_sync(0xffffffffu, u, d);
           const cplx<T> al = a_s[l * TW + x];
@@ -729,7 +743,7 @@ k_small_contract_reduce(const T* __restrict__ S2, const T* __restrict__ V, long 
 // a9 + a10: cumulative trapezoid over planes and the per-plane error norms.
 //   psi_j^new = psi_0 + dz [G_0/2 + G_1 + .. + G_{j-1} + G_j/2], j = 1..Mc
 //   errbuf[2 j] += sum |psi_j^new - psi_j^old|^2,  errbuf[2 j + 1] += sum |psi_j^new|^2
-// One thread per (p, w); 256-thread blocks.  Planes are walked four at a time so that the eight loads
+// One thread per (p, w); 256-thread blocks.  Planes are walked eight at a time so that the sixteen loads
 // of a batch are in flight together; norms are reduced warp -> shared memory (fp64) -> one global
 // atomic per plane per block (a global atomic per warp serialised on 2 Mc addresses: 0.36 ms at config 5).
 // Dynamic shared memory: 2 (Mc + 1) doubles.
@@ -737,6 +751,7 @@ template <typename T>
 __global__ void __launch_bounds__(256)
 k_trapz_scan(const cplx<T>* __restrict__ psi0, const cplx<T>* __restrict__ G, cplx<T>* __restrict__ psi,
              long long plane_stride, int Mc, T dz, int first_iter, double* __restrict__ errbuf, long long PN) {
+  pdl_prologue();
   extern __shared__ double s_err[];
   for (int i = threadIdx.x; i < 2 * (Mc + 1); i += blockDim.x) s_err[i] = 0.0;
   __syncthreads();
@@ -745,7 +760,7 @@ k_trapz_scan(const cplx<T>* __restrict__ psi0, const cplx<T>* __restrict__ G, cp
   const long long ii = live ? i : 0;                 // dead threads read a valid address, write nothing
   const cplx<T> p0 = psi0[ii];
   cplx<T> acc = cscale(G[ii], (T)0.5);
-  constexpr int B = 4;
+  constexpr int B = 8;
   for (int j0 = 1; j0 <= Mc; j0 += B) {
     cplx<T> g[B], old[B];
 #pragma unroll
@@ -780,18 +795,23 @@ k_trapz_scan(const cplx<T>* __restrict__ psi0, const cplx<T>* __restrict__ G, cp
 }
 
 // err = max_j sqrt(num_j / den_j); result -> out[0]; accumulators cleared for the next iteration
-__global__ void k_err_finalize(double* __restrict__ errbuf, int Mc, double* __restrict__ out) {
-  if (threadIdx.x == 0 && blockIdx.x == 0) {
-    double e = 0.0;
-    for (int j = 1; j <= Mc; ++j) {
-      const double num = errbuf[2 * j], den = errbuf[2 * j + 1];
-      const double r = den > 0.0 ? sqrt(num / den) : 0.0;
-      e = fmax(e, r);
-      errbuf[2 * j] = 0.0;
-      errbuf[2 * j + 1] = 0.0;
-    }
-    out[0] = e;
+// (one warp: lane i takes planes i + 1, i + 33, ...; fmax is exact, so the lane order does not matter)
+__device__ __forceinline__ double err_max_over_planes(double* __restrict__ errbuf, int Mc) {
+  double e = 0.0;
+  for (int j = 1 + (int)threadIdx.x; j <= Mc; j += 32) {
+    const double num = errbuf[2 * j], den = errbuf[2 * j + 1];
+    e = fmax(e, den > 0.0 ? sqrt(num / den) : 0.0);
+    errbuf[2 * j] = 0.0;
+    errbuf[2 * j + 1] = 0.0;
   }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) e = fmax(e, __shfl_xor_sync(0xffffffffu, e, d));
+  return e;
+}
+__global__ void k_err_finalize(double* __restrict__ errbuf, int Mc, double* __restrict__ out) {
+  pdl_prologue();
+  const double e = err_max_over_planes(errbuf, Mc);
+  if (threadIdx.x == 0) out[0] = e;
 }
 
 // a10 taken on the device (the loop of PAPER.md:218 as a CUDA-graph WHILE node): the same
@@ -805,15 +825,9 @@ struct LoopStats {
 };
 __global__ void k_err_finalize_loop(double* __restrict__ errbuf, int Mc, double* __restrict__ out, double tol, int cap,
                                     int fixed, cudaGraphConditionalHandle handle, LoopStats* __restrict__ st) {
-  if (threadIdx.x == 0 && blockIdx.x == 0) {
-    double e = 0.0;
-    for (int j = 1; j <= Mc; ++j) {
-      const double num = errbuf[2 * j], den = errbuf[2 * j + 1];
-      const double r = den > 0.0 ? sqrt(num / den) : 0.0;
-      e = fmax(e, r);
-      errbuf[2 * j] = 0.0;
-      errbuf[2 * j + 1] = 0.0;
-    }
+  pdl_prologue();
+  const double e = err_max_over_planes(errbuf, Mc);
+  if (threadIdx.x == 0) {
     out[0] = e;
     const int it = st->it + 1;
     st->it = it;
@@ -838,6 +852,7 @@ template <typename T>
 __global__ void __launch_bounds__(256)
 k_advance(double2* __restrict__ psi0_d, cplx<T>* __restrict__ psi0, const cplx<T>* __restrict__ G,
           long long plane_stride, int Mc, double dz, const double2* __restrict__ EM, long long PN) {
+  pdl_prologue();
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= PN) return;
   double ax = 0.5 * (double)G[i].x, ay = 0.5 * (double)G[i].y;
@@ -871,6 +886,7 @@ __global__ void __launch_bounds__(256)
 k_rk4_stage(int stage, double2* __restrict__ At_d, cplx<T>* __restrict__ At, const double2* __restrict__ EH,
             const cplx<T>* __restrict__ G, cplx<T>* __restrict__ AI, cplx<T>* __restrict__ K1,
             cplx<T>* __restrict__ K2, cplx<T>* __restrict__ K3, cplx<T>* __restrict__ X, double h, long long PN) {
+  pdl_prologue();
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= PN) return;
   const double2 e = EH[i];
@@ -911,6 +927,7 @@ __global__ void __launch_bounds__(256)
 k_couple(const cplx<T>* __restrict__ src, long long src_plane_stride, const cplx<T>* __restrict__ E,
          const T* __restrict__ gfwd, const T* __restrict__ ginv, const cplx<T>* __restrict__ Qc,
          cplx<T>* __restrict__ G, long long plane_stride, int P, int N) {
+  pdl_prologue();
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* a_s = reinterpret_cast<cplx<T>*>(smem_raw);        // [P][64]
   const int x = threadIdx.x & 63, g = threadIdx.x >> 6, j = blockIdx.y;
@@ -946,6 +963,7 @@ k_couple(const cplx<T>* __restrict__ src, long long src_plane_stride, const cplx
 
 template <typename TI, typename TO>
 __global__ void __launch_bounds__(256) k_convert(const TI* __restrict__ in, TO* __restrict__ out, long long n) {
+  pdl_prologue();
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) out[i] = (TO)in[i];
 }
