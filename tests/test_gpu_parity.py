@@ -238,10 +238,14 @@ def test_propagate_vs_rk4ip_and_mpa(B, cfg, kw):
     assert rel(out, ref_mpa) <= 1e-4           # same scheme: only fp32 rounding and +-1 iteration remain
     assert stats["large_steps"] == ost["large_steps"]
     assert abs(stats["iterations"] - ost["iterations"]) <= ost["large_steps"]
+    # reading S15: the GPU's own relative drift of the conserved quantity, |Q(L)/Q(0) - 1| ...
     q0 = O.conserved_quantity(A_in, w.dt, w.omega0, w.shock)
-    drift = abs(O.conserved_quantity(out, w.dt, w.omega0, w.shock)
-                - O.conserved_quantity(ref_mpa, w.dt, w.omega0, w.shock)) / q0
-    assert drift <= TOL_DRIFT, drift
+    d_gpu = O.conserved_quantity(out, w.dt, w.omega0, w.shock) / q0 - 1.0
+    d_ref = O.conserved_quantity(ref_mpa, w.dt, w.omega0, w.shock) / q0 - 1.0
+    # is the scheme's own O(dz^2) truncation (1.1e-6 for the two-group config-3 case at dz = 100 um, oracle and GPU
+    # alike) plus fp32 rounding: the bound is on the difference to the oracle MPA's drift, where the former cancels
+    assert abs(d_gpu - d_ref) <= TOL_DRIFT, (d_gpu, d_ref)
+    assert abs(d_gpu) <= abs(d_ref) + TOL_DRIFT
 
 
 def test_mpa_result_independent_of_M(B):
@@ -603,7 +607,7 @@ def test_full_shape_properties_invariant_M_independence_order(B, cfg):
     assert st == 0 and stats["not_converged"] == 0 and stats["large_steps"] == n_large
     q0 = O.conserved_quantity(A_in, w.dt, w.omega0, w.shock)
     q1 = O.conserved_quantity(out, w.dt, w.omega0, w.shock)
-    assert abs(q1 / q0 - 1.0) <= 2e-6, q1 / q0 - 1.0
+    drift = [q1 / q0 - 1.0]
     # M-independence: half as many planes per large step, same dz, same length
     M0 = w.M
     w.M = M0 // 2
@@ -620,6 +624,14 @@ def test_full_shape_properties_invariant_M_independence_order(B, cfg):
     e1, e2 = rel(outs[0], outs[2]), rel(outs[1], outs[2])
     assert e1 <= 1e-3
     assert 2.5 <= e1 / e2 <= 8.0 or e1 < 5e-6, (e1, e2)
+    # the drift of the conserved quantity is the implicit trapezoid rule's own truncation, O(dz^2): it falls towards the
+    # fp32 floor as dz is halved, and at dz / 4 it is inside the 1e-6 of north_star (no oracle run is affordable here;
+    # the bound against the oracle MPA's drift is asserted where one is: test_long_mpa_vs_stored_oracle_mpa)
+    drift += [O.conserved_quantity(o, w.dt, w.omega0, w.shock) / q0 - 1.0 for o in outs[1:]]
+    print(f"config {cfg}, {n_large} large steps: own drift Q(L)/Q(0) - 1 at dz, dz/2, dz/4 = "
+          + ", ".join(f"{d:.3e}" for d in drift))
+    assert abs(drift[0]) <= 2e-6 and abs(drift[2]) <= TOL_DRIFT
+    assert abs(drift[1]) <= max(0.6 * abs(drift[0]), 5e-7)
 
 
 # --------------------------------------------------- NEXT-1: serial RK4IP integrator on the same kernels
@@ -627,7 +639,8 @@ def test_full_shape_properties_invariant_M_independence_order(B, cfg):
     (2, dict(N=1024, L=40 * 50e-6), 2e-5, TOL_FIELD),
     # tcgen05 contraction, one plane per launch.  Config 3's dz = 100 um is 2.2 rad of inter-group beating per
     # step (4 x 5517 /m), so the second-order MPA and the fourth-order RK4IP differ by 1-2e-3 there whatever
-    # the length (oracle MPA vs oracle RK4IP do too): bound 5e-3 for the cross-check.
+    # the length: the ORACLE's two schemes differ by 2.36e-3 over 2 cm and both are measured against a converged
+    # reference in test_config3_scheme_distances_to_converged_reference; here only "same order as the oracle's".
     (3, dict(N=1024, L=20 * 100e-6), 2e-5, 5e-3),
     (1, dict(N=256, L=50 * 2.5e-3), 1e-10, TOL_FIELD),          # complex128
 ])
@@ -835,46 +848,44 @@ def test_gain_coupling_reject_bad_input(B):
 
 
 # ------------------------------------------ full-length propagation against stored oracle outputs (tests/golden)
-def _golden(fname):
+def _golden(name):
+    """(make_golden module, meta, whole [P][N] complex128 field) of a stored oracle run."""
     import importlib.util
     import os
     gdir = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
-    path = os.path.join(gdir, fname)
-    if not os.path.exists(path):
-        pytest.skip(f"{fname} not generated (python tests/golden/make_golden.py)")
     spec = importlib.util.spec_from_file_location("make_golden", os.path.join(gdir, "make_golden.py"))
     mg = importlib.util.module_from_spec(spec)
     spec.loader.exec_module(mg)
-    meta = {}
-    with open(path) as fh:
-        for line in fh:
-            if not line.startswith("#"):
-                break
-            for tok in line[1:].split():
-                if "=" in tok:
-                    k, v = tok.split("=", 1)
-                    meta[k] = v
-    data = np.loadtxt(path)
-    return mg, meta, data
+    got = mg.load_golden(name)
+    if got is None:
+        pytest.skip(f"{name} not generated (python tests/golden/make_golden.py)")
+    return mg, got[0], got[1]
 
 
-@pytest.mark.parametrize("fname,cfg,tol_rk,tol_mpa", [
-    # measured on B200 (GPU RK4IP / GPU MPA against the oracle's RK4IP): 1.2e-6 / 3.0e-5, 1.5e-6 / 2.4e-3,
-    # 3.0e-7 / 2.5e-5, 2.8e-7 / 1.5e-4
-    ("config2_rk4ip_3000steps.txt", 2, 2e-5, TOL_FIELD),     # BASELINE config 2 at its full length (15 cm)
-    ("config3_rk4ip_200steps.txt", 3, 2e-5, 5e-3),           # first 2 cm of config 3
-    ("config4_rk4ip_100steps.txt", 4, 2e-5, TOL_FIELD),      # first 5 mm of config 4 (5 large steps, full shape)
-    ("config5_rk4ip_40steps.txt", 5, 2e-5, TOL_FIELD),       # first 1 mm of config 5 (2 large steps, full shape)
-])
-def test_long_propagation_vs_stored_oracle_rk4ip(B, fname, cfg, tol_rk, tol_mpa):
-    mg, meta, data = _golden(fname)
-    w = W.make_config(cfg)
-    L, steps = float(meta["L_m"]), int(meta["steps"])
-    assert abs(steps * w.dz - L) < 1e-12 and int(meta["N"]) == w.N and int(meta["P"]) == w.P
+def _check_inputs(mg, meta, w):
     A_in = w.A0.astype(np.complex64).astype(np.complex128)
+    assert meta["N"] == w.N and meta["P"] == w.P
     assert mg.fingerprint_matches(meta, w, A_in), "golden is stale: inputs changed"
-    modes, samples = data[:, 0].astype(int), data[:, 1].astype(int)
-    ref = data[:, 2] + 1j * data[:, 3]
+    return A_in
+
+
+@pytest.mark.parametrize("name,cfg,tol_rk,tol_mpa", [
+    # measured on B200 (GPU RK4IP / GPU MPA against the oracle's RK4IP, every element of the field): 1.2e-6 / 3.0e-5,
+    # 1.5e-6 / 2.4e-3, 3.0e-7 / 2.5e-5, 2.8e-7 / 1.5e-4
+    ("config2_rk4ip_3000steps", 2, 2e-5, TOL_FIELD),       # BASELINE config 2 at its full length (15 cm)
+    # first 2 cm of config 3: the MPA's bound against RK4IP is the SCHEME distance the oracle itself has there
+    # (oracle MPA vs oracle RK4IP 2.36e-3, tests/test_workloads.py::test_config3_schemes_against_converged_reference);
+    # the 1e-3 bounds at config 3 are same-scheme, below
+    ("config3_rk4ip_200steps", 3, 2e-5, None),
+    ("config4_rk4ip_100steps", 4, 2e-5, TOL_FIELD),        # first 5 mm of config 4 (5 large steps, full shape)
+    ("config5_rk4ip_40steps", 5, 2e-5, TOL_FIELD),         # first 1 mm of config 5 (2 large steps, full shape)
+])
+def test_long_propagation_vs_stored_oracle_rk4ip(B, name, cfg, tol_rk, tol_mpa):
+    mg, meta, ref = _golden(name)
+    w = W.make_config(cfg)
+    L = meta["L_m"]
+    assert abs(meta["steps"] * w.dz - L) < 1e-12
+    A_in = _check_inputs(mg, meta, w)
     Ad = dev(w.A0, np.complex64)
     out_mpa, out_rk = torch.empty_like(Ad), torch.empty_like(Ad)
     with B.plan_from_workload(w) as plan:
@@ -885,36 +896,97 @@ def test_long_propagation_vs_stored_oracle_rk4ip(B, fname, cfg, tol_rk, tol_mpa)
     assert st == 0 and stats["not_converged"] == 0
     o_rk = out_rk.cpu().numpy().astype(np.complex128)
     o_mpa = out_mpa.cpu().numpy().astype(np.complex128)
-    assert rel(o_rk[modes, samples], ref) <= tol_rk
-    assert rel(o_mpa[modes, samples], ref) <= tol_mpa
-    # conserved quantity of the full field against the oracle's own drift (stored in the header), same scheme (S15)
-    pn_ref = float(meta["photon_number_ratio"])
+    assert rel(o_rk, ref) <= tol_rk
+    if tol_mpa is not None:
+        assert rel(o_mpa, ref) <= tol_mpa
+    # conserved quantity against the oracle's own drift, same scheme (S15)
     pn = O.photon_number(o_rk, w.dt, w.omega0) / O.photon_number(A_in, w.dt, w.omega0)
-    assert abs(pn - pn_ref) <= TOL_DRIFT
+    assert abs(pn - meta["photon_number_ratio"]) <= TOL_DRIFT
 
 
-@pytest.mark.parametrize("cfg,fname", [(3, "config3_mpa_200steps.txt"), (5, "config5_mpa_40steps.txt")])
-def test_long_mpa_vs_stored_oracle_mpa(B, cfg, fname):
+@pytest.mark.parametrize("cfg,name", [(3, "config3_mpa_200steps"), (5, "config5_mpa_40steps")])
+def test_long_mpa_vs_stored_oracle_mpa(B, cfg, name):
     """Configs 3 (20 large steps) and 5 (the shape bench.py times, 2 large steps) at full shape against the oracle's
     own MPA (O4, stored): same scheme, so the distance is fp32 rounding plus at most one iteration of difference
     per large step, not the O(dz^2) of the RK4IP comparison."""
-    mg, meta, data = _golden(fname)
+    mg, meta, ref = _golden(name)
     w = W.make_config(cfg)
-    L = float(meta["L_m"])
-    A_in = w.A0.astype(np.complex64).astype(np.complex128)
-    assert mg.fingerprint_matches(meta, w, A_in), "golden is stale: inputs changed"
-    assert int(meta["M"]) == w.M and float(meta["tol"]) == w.tol
-    modes, samples = data[:, 0].astype(int), data[:, 1].astype(int)
-    ref = data[:, 2] + 1j * data[:, 3]
+    L = meta["L_m"]
+    A_in = _check_inputs(mg, meta, w)
+    assert meta["M"] == w.M and meta["tol"] == w.tol
     Ad = dev(w.A0, np.complex64)
     out = torch.empty_like(Ad)
     with B.plan_from_workload(w) as plan:
         st = plan.propagate(Ad, L, out)
         torch.cuda.synchronize()
         stats = plan.stats()
-    assert st == 0 and stats["large_steps"] == int(meta["large_steps"])
-    assert abs(stats["iterations"] - int(meta["iterations"])) <= stats["large_steps"]
+    assert st == 0 and stats["large_steps"] == meta["large_steps"]
+    assert abs(stats["iterations"] - meta["iterations"]) <= stats["large_steps"]
     o = out.cpu().numpy().astype(np.complex128)
-    assert rel(o[modes, samples], ref) <= 1e-4
+    assert rel(o, ref) <= 1e-4
     pn = O.photon_number(o, w.dt, w.omega0) / O.photon_number(A_in, w.dt, w.omega0)
-    assert abs(pn - float(meta["photon_number_ratio"])) <= TOL_DRIFT
+    assert abs(pn - meta["photon_number_ratio"]) <= TOL_DRIFT
+
+
+def test_config3_full_length_both_integrators_vs_stored_oracle(B):
+    """BASELINE config 3 over its full 1 m (10^4 small steps, 1000 MPA large steps), every element of the output
+    field: the GPU MPA against the oracle's MPA and the GPU RK4IP against the oracle's RK4IP, each at the 1e-3
+    bound of north_star, with the conserved quantity of reading S15 against the oracle's own drift."""
+    w = W.make_config(3)
+    mg, m_mpa, ref_mpa = _golden("config3_mpa_10000steps")
+    _, m_rk, ref_rk = _golden("config3_rk4ip_10000steps")
+    A_in = _check_inputs(mg, m_mpa, w)
+    _check_inputs(mg, m_rk, w)
+    assert m_mpa["L_m"] == w.L == m_rk["L_m"] and m_mpa["steps"] == 10000
+    Ad = dev(w.A0, np.complex64)
+    out_mpa, out_rk = torch.empty_like(Ad), torch.empty_like(Ad)
+    with B.plan_from_workload(w) as plan:
+        st = plan.propagate(Ad, w.L, out_mpa)
+        torch.cuda.synchronize()
+        stats = plan.stats()
+        plan.propagate_rk4ip(Ad, w.L, out_rk)
+        torch.cuda.synchronize()
+    assert st == 0 and stats["not_converged"] == 0 and stats["large_steps"] == m_mpa["large_steps"] == 1000
+    assert abs(stats["iterations"] - m_mpa["iterations"]) <= 0.05 * m_mpa["iterations"]
+    o_mpa = out_mpa.cpu().numpy().astype(np.complex128)
+    o_rk = out_rk.cpu().numpy().astype(np.complex128)
+    e_mpa, e_rk = rel(o_mpa, ref_mpa), rel(o_rk, ref_rk)
+    print(f"config 3, 1 m: GPU MPA vs oracle MPA {e_mpa:.3e}, GPU RK4IP vs oracle RK4IP {e_rk:.3e}, "
+          f"iterations {stats['iterations']} (oracle {m_mpa['iterations']})")
+    assert e_mpa <= TOL_FIELD and e_rk <= TOL_FIELD
+    q0 = O.photon_number(A_in, w.dt, w.omega0)
+    assert abs(O.photon_number(o_mpa, w.dt, w.omega0) / q0 - m_mpa["photon_number_ratio"]) <= 2 * TOL_DRIFT
+    assert abs(O.photon_number(o_rk, w.dt, w.omega0) / q0 - m_rk["photon_number_ratio"]) <= 2 * TOL_DRIFT
+    # the GPU's own drift over 1 m (MPA: the implicit trapezoid rule): |Q(L)/Q(0) - 1|
+    assert abs(O.photon_number(o_mpa, w.dt, w.omega0) / q0 - 1.0) <= 5e-5
+
+
+def test_config3_scheme_distances_to_converged_reference(B):
+    """The 1e-3 field bound at config 3, measured instead of exempted: against the oracle's RK4IP at dz/4 over the
+    first 2 cm (converged to ~1e-6), GPU RK4IP(dz) sits at the oracle RK4IP(dz)'s distance (2.1e-4), GPU MPA(dz) at
+    the oracle MPA(dz)'s (2.2e-3: second order at a step that does not resolve the inter-group beating,
+    PAPER.md:214-218), GPU MPA(dz/2) at a quarter of that and inside the bound."""
+    w = W.make_config(3)
+    mg, meta, ref = _golden("config3_rk4ip_200steps_dzdiv4")
+    _check_inputs(mg, meta, w)
+    L = meta["L_m"]
+    o_rk = mg.load_golden("config3_rk4ip_200steps")[1]
+    o_mpa = mg.load_golden("config3_mpa_200steps")[1]
+    Ad = dev(w.A0, np.complex64)
+    def run(dz, rk):
+        w2 = W.make_config(3)
+        w2.dz = dz
+        out = torch.empty_like(Ad)
+        with B.plan_from_workload(w2) as plan:
+            (plan.propagate_rk4ip if rk else plan.propagate)(Ad, L, out)
+            torch.cuda.synchronize()
+        return out.cpu().numpy().astype(np.complex128)
+    d_rk = rel(run(w.dz, True), ref)
+    d_mpa = rel(run(w.dz, False), ref)
+    d_mpa2 = rel(run(w.dz / 2, False), ref)
+    print(f"config 3, 2 cm, distance to RK4IP(dz/4): GPU RK4IP(dz) {d_rk:.3e} (oracle {rel(o_rk, ref):.3e}), "
+          f"GPU MPA(dz) {d_mpa:.3e} (oracle {rel(o_mpa, ref):.3e}), GPU MPA(dz/2) {d_mpa2:.3e}")
+    assert abs(d_rk - rel(o_rk, ref)) <= 2e-5 and d_rk <= TOL_FIELD
+    assert abs(d_mpa - rel(o_mpa, ref)) <= 1e-4
+    assert 3.0 <= d_mpa / d_mpa2 <= 5.0                 # second order in dz
+    assert d_mpa2 <= TOL_FIELD

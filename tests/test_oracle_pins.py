@@ -228,14 +228,54 @@ def test_shock_term_against_analytic_derivative():
 
 # ------------------------------------------------------------------ integrators
 def test_fundamental_soliton_config1():
-    # BASELINE config 1: |A| invariant, phase z / (2 L_D)
+    # BASELINE config 1 over its full 5 dispersion lengths (1000 steps): |A| invariant, phase z / (2 L_D)
     wl = W.make_config(1)
     assert abs(wl.meta["P0"] - 712.737) < 1e-3 and abs(wl.meta["L_D"] - 0.5) < 1e-12
     assert abs(wl.kappa * wl.S[0, 0, 0, 0] - 2.80608e-3) < 1e-8
-    z = 0.5 * wl.meta["L_D"]
+    z = 5.0 * wl.meta["L_D"]
+    assert abs(z - wl.L) < 1e-12 and abs(z / wl.dz - 1000) < 1e-9
     A = O.rk4ip_propagate(wl.A0, z, wl.dz, wl.beta, wl.S, wl.kappa, wl.omega0, 0.0, None, wl.dt, shock=False)
     exact = wl.A0 * np.exp(1j * z / (2 * wl.meta["L_D"]))
     assert rel(A, exact) < 5e-9
+    assert abs(rel(np.abs(A), np.abs(wl.A0))) < 5e-9                 # shape-invariant
+    # the MPA reaches the same soliton at second order in dz (implicit trapezoid rule): error / 4 on halving dz
+    zs = 0.5 * wl.meta["L_D"]
+    ex = wl.A0 * np.exp(1j * zs / (2 * wl.meta["L_D"]))
+    errs = []
+    for k in (1, 2):
+        Am = O.mpa_propagate(wl.A0, zs, wl.dz / k, 10, wl.beta, wl.S, wl.kappa, wl.omega0, 0.0, None, wl.dt,
+                             shock=False, tol=1e-12)
+        errs.append(rel(Am, ex))
+    assert errs[0] < 1e-5 and 3.5 < errs[0] / errs[1] < 4.5
+
+
+def test_mpa_not_converged_branch_and_predictor():
+    """(i) max_iter reached: the last iterate is used, converged = False, the step is counted (reading R2) -- and that
+    iterate IS the fixed_iter = max_iter result.  (ii) the predictor of reading S11 changes the first iterate only:
+    same fixed point to the tolerance, never more iterations, first large step untouched."""
+    wl = _small_mm()
+    L = 3 * 10 * wl.dz
+    args = (wl.beta, wl.S, wl.kappa, wl.omega0, wl.f_R, wl.h_R, wl.dt)
+    st = {}
+    A2 = O.mpa_propagate(wl.A0, L, wl.dz, 10, *args, tol=1e-12, max_iter=2, stats=st)
+    assert st["not_converged"] == 3 and st["iterations"] == 6 and st["large_steps"] == 3 and st["last_err"] > 1e-12
+    Af = O.mpa_propagate(wl.A0, L, wl.dz, 10, *args, fixed_iter=2)
+    assert np.array_equal(A2, Af)
+    omega = O.omega_grid(wl.N, wl.dt)
+    D = O.dispersion_operator(wl.beta, omega)
+    K = 1j * wl.kappa * (1 + omega / wl.omega0)
+    nlt = lambda A: O.nonlinear_term(A, wl.S, wl.f_R, wl.h_R, wl.dt)
+    _, n_it, err, conv = O.mpa_large_step(O.to_freq(wl.A0), 10, wl.dz, D, nlt, K, tol=1e-12, max_iter=1)
+    assert n_it == 1 and not conv and err > 1e-6
+    # predictor
+    s0, s1 = {}, {}
+    Lp = 6 * 10 * wl.dz
+    ref = O.mpa_propagate(wl.A0, Lp, wl.dz, 10, *args, tol=1e-8, stats=s0)
+    got = O.mpa_propagate(wl.A0, Lp, wl.dz, 10, *args, tol=1e-8, stats=s1, predictor=1)
+    assert rel(got, ref) < 5e-8 and s1["iterations"] <= s0["iterations"] and s1["not_converged"] == 0
+    one0 = O.mpa_propagate(wl.A0, 10 * wl.dz, wl.dz, 10, *args, tol=1e-8)
+    one1 = O.mpa_propagate(wl.A0, 10 * wl.dz, wl.dz, 10, *args, tol=1e-8, predictor=1)
+    assert np.array_equal(one0, one1)                                # no history yet: the paper's psi_j = psi_0
 
 
 def _small_mm(P=3, N=256, seed=0, shock=True, fR=0.18):

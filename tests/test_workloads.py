@@ -5,6 +5,7 @@ import math
 import numpy as np
 import pytest
 
+from oracle import gmmnlse_oracle as O
 from paper_1708_05324_b200 import workloads as W
 
 
@@ -87,28 +88,58 @@ def test_configs_shapes_and_seeding(idx):
         assert abs((above[-1] - above[0]) / a.meta["fwhm"] - 1) < 0.05
 
 
-def test_stored_goldens_match_current_inputs():
-    """Every stored oracle output under tests/golden names the inputs it was computed from (fingerprint of the launch
-    field, S, beta, h_R); a change of the seeded generators must regenerate them."""
-    import glob
+def _make_golden_module():
     import importlib.util
     import os
     gdir = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
     spec = importlib.util.spec_from_file_location("make_golden", os.path.join(gdir, "make_golden.py"))
     mg = importlib.util.module_from_spec(spec)
     spec.loader.exec_module(mg)
-    for path in glob.glob(os.path.join(gdir, "config*_*steps.txt")):
-        meta = {}
+    return mg, gdir
+
+
+def test_stored_goldens_match_current_inputs():
+    """Every stored oracle output under tests/golden names the inputs it was computed from (fingerprint of the launch
+    field, S, beta, h_R); a change of the seeded generators must regenerate them.  The stored field is the whole
+    [P][N] complex128 array."""
+    import glob
+    import json
+    import os
+    mg, gdir = _make_golden_module()
+    paths = glob.glob(os.path.join(gdir, "config*_*steps*.json"))
+    assert len(paths) >= 9
+    for path in paths:
         with open(path) as fh:
-            for line in fh:
-                if not line.startswith("#"):
-                    break
-                for tok in line[1:].split():
-                    if "=" in tok:
-                        k, v = tok.split("=", 1)
-                        meta[k] = v
-        cfg = int(os.path.basename(path)[len("config")])
-        w = W.make_config(cfg)
+            meta = json.load(fh)
+        w = W.make_config(meta["config"])
         A_in = w.A0.astype(np.complex64).astype(np.complex128)
         assert mg.fingerprint_matches(meta, w, A_in), path
-        assert int(meta["steps"]) == int(round(float(meta["L_m"]) / w.dz))
+        assert meta["steps"] == int(round(meta["L_m"] / w.dz)) * meta["dz_div"]
+        field = np.load(path[:-5] + ".npy")
+        assert field.shape == (w.P, w.N) and field.dtype == np.complex128 and np.isfinite(field).all()
+        # the stored conserved-quantity ratio is the stored field's own (oracle function, independent of the integrator)
+        pn = O.photon_number(field, w.dt, w.omega0) / O.photon_number(A_in, w.dt, w.omega0)
+        assert abs(pn - meta["photon_number_ratio"]) < 1e-12
+
+
+def test_config3_schemes_against_converged_reference():
+    """What BASELINE's dz = 100 um means at config 3 (2.2 rad of inter-group beating per step, against PAPER.md:214-216
+    'dz << z_IM'), from stored oracle runs alone: over the first 2 cm the fourth-order RK4IP at dz is 2.1e-4 from the
+    converged reference (RK4IP at dz/4, itself ~1e-6 from the limit), the second-order MPA at dz 2.2e-3 -- so at this dz
+    the two SCHEMES differ by more than the 1e-3 field bound, whatever the implementation; over the full 1 m they
+    differ by 1.1e-2.  The GPU tests therefore hold each GPU integrator to the oracle's SAME scheme at 1e-3 and
+    measure the scheme distances beside the converged reference (test_gpu_parity.py)."""
+    mg, _ = _make_golden_module()
+    rel = lambda a, b: np.linalg.norm(a - b) / np.linalg.norm(b)
+    ref = mg.load_golden("config3_rk4ip_200steps_dzdiv4")[1]
+    rk = mg.load_golden("config3_rk4ip_200steps")[1]
+    mpa = mg.load_golden("config3_mpa_200steps")[1]
+    d_rk, d_mpa = rel(rk, ref), rel(mpa, ref)
+    assert 1e-4 < d_rk < 4e-4 and 1.5e-3 < d_mpa < 3e-3, (d_rk, d_mpa)
+    assert abs(rel(mpa, rk) - d_mpa) < 2 * d_rk                      # triangle: the MPA's distance is its own truncation
+    meta_f, mpa_full = mg.load_golden("config3_mpa_10000steps")
+    rk_meta, rk_full = mg.load_golden("config3_rk4ip_10000steps")
+    assert 5e-3 < rel(mpa_full, rk_full) < 2e-2
+    # the implicit trapezoid rule keeps the photon number 15x better than RK4IP at this step over 1 m
+    assert abs(meta_f["photon_number_ratio"] - 1) < 5e-5 < abs(rk_meta["photon_number_ratio"] - 1) < 1e-3
+    assert meta_f["large_steps"] == 1000 and meta_f["not_converged"] == 0
