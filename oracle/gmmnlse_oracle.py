@@ -34,7 +34,7 @@ import numpy as np
 
 __all__ = [
     "dft_direct", "fft_radix2", "to_freq", "to_time", "omega_grid",
-    "dispersion_operator", "coupling_term", "raman_transfer", "pair_products",
+    "dispersion_operator", "coupling_term", "coupling_at", "saturation_term", "raman_transfer", "pair_products",
     "raman_convolve_direct", "raman_convolve", "nonlinear_term",
     "nonlinear_term_literal", "nonlinear_term_general", "nonlinear_term_general_literal",
     "nonlinear_op", "nonlinear_op_freq",
@@ -125,6 +125,34 @@ def coupling_term(At: np.ndarray, Qc) -> np.ndarray:
     to the right-hand side.  ``Qc[n][p]`` = Q_np [1/m], constant over the call and over frequency, so the sum
     reads the same in the time and the frequency domain."""
     return 1j * (np.asarray(Qc, dtype=np.complex128).T @ At)
+
+
+def coupling_at(coupling, z):
+    """Q_np at position z (measured from the start of the call).  ``coupling`` is a constant matrix, a callable z -> matrix,
+    or a pair (Q0, f) meaning Q(z) = f(z) Q0: the separable perturbation eps(x, y) f(z) of PAPER.md:277 (gratings:
+    f periodic; disorder: f a stochastic function)."""
+    if callable(coupling):
+        return np.asarray(coupling(z), dtype=np.complex128)
+    if isinstance(coupling, tuple):
+        return float(coupling[1](z)) * np.asarray(coupling[0], dtype=np.complex128)
+    return np.asarray(coupling, dtype=np.complex128)
+
+
+def saturation_term(A: np.ndarray, S, g_sat: float, dt: float) -> np.ndarray:
+    """First-order gain saturation (section F.2): the Taylor expansion of
+    g(I) = g0 / [1 + int dt I / I_sat] projected on the modes adds, beside g_p A_p,
+
+        - g_sat sum_lmn S_plmn A_l(t) int dtau A_m(tau) A_n*(tau),      g_sat = g0 / I_sat  [m/J]
+
+    (reading S22: the paper prints the term without its gain prefactor; with S in 1/m^2 and the integral in J the sum is
+    J/m^2, so the coefficient that makes it a gain per length is g0 / I_sat).  The time integral is the rectangle sum
+    dt sum_t over the periodic window.  Linear in A_l with a matrix that depends on the field only through its
+    time-integrated pair products, so it reads the same in the time and the frequency domain."""
+    A = np.asarray(A, dtype=np.complex128)
+    S = np.asarray(S[1] if isinstance(S, tuple) else S)          # general form: the Raman tensor, as printed
+    E = dt * (A @ np.conj(A).T)                                   # E_mn = int A_m A_n* dtau
+    W = np.einsum("plmn,mn->pl", S, E)
+    return -g_sat * (W @ A)
 
 
 # ---------------------------------------------------------------- nonlinear part
@@ -273,25 +301,28 @@ def nonlinear_op(A, S, kappa, omega0, f_R, h_R, dt, shock=True):
 
 
 # ------------------------------------------------------------------- O3: RK4IP
-def rk4ip_step(At, h, D, nl):
+def rk4ip_step(At, h, D, nl, z=None):
     """One RK4IP step (textbook interaction-picture RK4; named by north_star).
 
-    ``nl(At)`` is the frequency-domain nonlinear operator; E = exp(D h / 2).
+    ``nl(At)`` is the frequency-domain nonlinear operator; E = exp(D h / 2).  With ``z`` given (a right-hand side
+    that depends on position: z-dependent coupling) it is called as ``nl(At, z_stage)`` at z, z + h/2, z + h/2, z + h.
     """
+    f = nl if z is None else None
     E = np.exp(D * (h / 2.0))
     AI = E * At
-    k1 = E * (h * nl(At))
-    k2 = h * nl(AI + k1 / 2.0)
-    k3 = h * nl(AI + k2 / 2.0)
-    k4 = h * nl(E * (AI + k3))
+    k1 = E * (h * (f(At) if f else nl(At, z)))
+    k2 = h * (f(AI + k1 / 2.0) if f else nl(AI + k1 / 2.0, z + h / 2.0))
+    k3 = h * (f(AI + k2 / 2.0) if f else nl(AI + k2 / 2.0, z + h / 2.0))
+    k4 = h * (f(E * (AI + k3)) if f else nl(E * (AI + k3), z + h))
     return E * (AI + k1 / 6.0 + k2 / 3.0 + k3 / 3.0) + k4 / 6.0
 
 
 def rk4ip_propagate(A0, L, dz, beta, S, kappa, omega0, f_R, h_R, dt, shock=True, n_steps=None,
-                    gain=None, coupling=None):
+                    gain=None, coupling=None, g_sat=0.0):
     """Propagate A0[p][t] over L with fixed step dz using RK4IP; returns A(L)[p][t].
 
-    ``gain`` joins D; ``coupling`` (Q_np) is integrated with the nonlinear term (it does not commute with D)."""
+    ``gain`` joins D; ``coupling`` (Q_np, see :func:`coupling_at`) and the saturation term (``g_sat``,
+    :func:`saturation_term`) are integrated with the nonlinear term (they do not commute with D)."""
     A0 = np.asarray(A0, dtype=np.complex128)
     N = A0.shape[-1]
     omega = omega_grid(N, dt)
@@ -299,16 +330,28 @@ def rk4ip_propagate(A0, L, dz, beta, S, kappa, omega0, f_R, h_R, dt, shock=True,
     if n_steps is None:
         n_steps = int(round(L / dz))
     nl0 = lambda X: nonlinear_op_freq(X, S, kappa, omega, omega0, f_R, h_R, dt, shock)
-    nl = nl0 if coupling is None else (lambda X: nl0(X) + coupling_term(X, coupling))
+    if coupling is None and g_sat == 0.0:
+        At = to_freq(A0)
+        for _ in range(n_steps):
+            At = rk4ip_step(At, dz, D, nl0)
+        return to_time(At)
+
+    def nl(X, z):
+        out = nl0(X)
+        if coupling is not None:
+            out = out + coupling_term(X, coupling_at(coupling, z))
+        if g_sat != 0.0:
+            out = out + to_freq(saturation_term(to_time(X), S, g_sat, dt))
+        return out
     At = to_freq(A0)
-    for _ in range(n_steps):
-        At = rk4ip_step(At, dz, D, nl)
+    for i in range(n_steps):
+        At = rk4ip_step(At, dz, D, nl, z=i * dz)
     return to_time(At)
 
 
 # --------------------------------------------------------------------- O4: MPA
 def mpa_large_step(psi0, M, dz, D, nl_time, K, tol=1e-6, max_iter=None, fixed_iter=0,
-                   history=None, coupling=None, first_iterate=None, planes_out=None):
+                   history=None, coupling=None, first_iterate=None, planes_out=None, z0=0.0, extra_time=None):
     """One MPA large step z0 -> z0 + M dz  (Eqs. 11-12).
 
     psi0[p][w] = At(z0).  Planes j = 0..M (reading S10).  ``nl_time(A_t)`` returns
@@ -330,14 +373,21 @@ def mpa_large_step(psi0, M, dz, D, nl_time, K, tol=1e-6, max_iter=None, fixed_it
     if first_iterate is not None:
         psi[1:] = first_iterate[1:]
     G = np.zeros((M + 1, P, N), dtype=np.complex128)
-    # extra right-hand-side term in the frequency domain (linear coupling), rotated like the nonlinear one
-    extra = (lambda Af: 0.0) if coupling is None else (lambda Af: coupling_term(Af, coupling))
-    G[0] = K * to_freq(nl_time(to_time(psi0))) + extra(psi0)   # depends on psi_0 only (S10)
+    # extra right-hand-side terms (linear coupling at the plane's position z0 + j dz; ``extra_time``: a term given in the
+    # time domain, e.g. the gain saturation), rotated like the nonlinear one
+    def extra(Af, j):
+        out = 0.0
+        if coupling is not None:
+            out = out + coupling_term(Af, coupling_at(coupling, z0 + j * dz))
+        if extra_time is not None:
+            out = out + to_freq(extra_time(to_time(Af)))
+        return out
+    G[0] = K * to_freq(nl_time(to_time(psi0))) + extra(psi0, 0)   # depends on psi_0 only (S10)
     n_iter, err, converged = 0, np.inf, False
     while True:
         for j in range(1, M + 1):
             Afj = psi[j] * np.exp(D * (j * dz))
-            G[j] = np.exp(-D * (j * dz)) * (K * to_freq(nl_time(to_time(Afj))) + extra(Afj))
+            G[j] = np.exp(-D * (j * dz)) * (K * to_freq(nl_time(to_time(Afj))) + extra(Afj, j))
         new = np.empty_like(psi)
         new[0] = psi0
         for j in range(1, M + 1):
@@ -370,7 +420,7 @@ def mpa_large_step(psi0, M, dz, D, nl_time, K, tol=1e-6, max_iter=None, fixed_it
 
 def mpa_propagate(A0, L, dz, M, beta, S, kappa, omega0, f_R, h_R, dt, shock=True,
                   tol=1e-6, max_iter=None, fixed_iter=0, stats=None, history=None, gain=None, coupling=None,
-                  predictor=0):
+                  predictor=0, g_sat=0.0):
     """Propagate with MPA; the last large step uses M' = (L/dz) mod M planes.
 
     ``predictor`` (reading S11: an optimisation of the first iterate, off by default = the paper's psi_j = psi_0):
@@ -398,8 +448,10 @@ def mpa_propagate(A0, L, dz, M, beta, S, kappa, omega0, f_R, h_R, dt, shock=True
             first = psi0[None] + np.exp(D * (prev[0].shape[0] - 1) * dz)[None] * (prev[0] - prev[1][None])
         keep = []
         start = psi0
+        sat = None if g_sat == 0.0 else (lambda A: saturation_term(A, S, g_sat, dt))
         psi0, it, last_err, conv = mpa_large_step(psi0, Mc, dz, D, nl_time, K, tol,
-                                                   max_iter, fixed_iter, hist, coupling, first, keep)
+                                                   max_iter, fixed_iter, hist, coupling, first, keep,
+                                                   z0=done * dz, extra_time=sat)
         prev = (keep[0], start)
         if history is not None:
             history.append(hist)

@@ -441,3 +441,69 @@ def test_linear_coupling_two_mode_coupler_closed_form():
     Q1 = np.zeros((2, 2), complex); Q1[0, 1] = kap
     out = O.rk4ip_propagate(A0, z, z / 100, np.zeros((2, 1)), S0, KAPPA, W.OMEGA0, 0.0, None, dt, shock=False, coupling=Q1)
     assert abs(out[0, 0] - 1.0) < 1e-12 and abs(out[1, 0] - 1j * kap * z) < 1e-9
+
+
+# ------------------------------------------ section F: gain saturation and z-dependent coupling
+def test_gain_saturation_logistic_energy_closed_form():
+    """P = 1, no dispersion, no Kerr: dA/dz = g A - g_sat S E(z) A with E = int |A|^2 dt, so the energy obeys the
+    logistic law E(z) = E0 e^{2gz} / [1 + (g_sat S E0 / g)(e^{2gz} - 1)] and the pulse keeps its shape
+    (PAPER.md:297-299 with reading S22)."""
+    N, dt = 256, 10e-15
+    t = (np.arange(N) - N // 2) * dt
+    A0 = (30.0 * np.exp(-t ** 2 / (2 * (80e-15) ** 2)))[None, :].astype(np.complex128)
+    S = np.full((1, 1, 1, 1), 2.0e10)
+    g, z = 4.0, 0.3
+    E0 = O.energy(A0, dt)
+    g_sat = 0.6 * g / (S[0, 0, 0, 0] * E0)                      # saturation is strong: g_sat S E0 = 0.6 g
+    beta = np.zeros((1, 3))
+    for integ in ("rk", "mpa"):
+        if integ == "rk":
+            A = O.rk4ip_propagate(A0, z, z / 60, beta, S, 0.0, W.OMEGA0, 0.0, None, dt, shock=False, gain=[g], g_sat=g_sat)
+        else:
+            A = O.mpa_propagate(A0, z, z / 600, 10, beta, S, 0.0, W.OMEGA0, 0.0, None, dt, shock=False, gain=[g],
+                                g_sat=g_sat, tol=1e-12)
+        Ez = E0 * np.exp(2 * g * z) / (1 + (g_sat * S[0, 0, 0, 0] * E0 / g) * (np.exp(2 * g * z) - 1))
+        assert abs(O.energy(A, dt) / Ez - 1) < (1e-7 if integ == "rk" else 1e-5)
+        assert rel(A, A0 * np.sqrt(Ez / E0)) < (1e-7 if integ == "rk" else 1e-5)
+    # the literal triple sum of the printed term on a small multimode field
+    rng = np.random.default_rng(5)
+    P = 3
+    Sm = rng.standard_normal((P, P, P, P))
+    Am = rng.standard_normal((P, 16)) + 1j * rng.standard_normal((P, 16))
+    lit = np.zeros_like(Am)
+    for p in range(P):
+        for l in range(P):
+            for m in range(P):
+                for n in range(P):
+                    lit[p] -= 0.7 * Sm[p, l, m, n] * Am[l] * (dt * np.sum(Am[m] * np.conj(Am[n])))
+    assert rel(O.saturation_term(Am, Sm, 0.7, dt), lit) < 1e-13
+
+
+def test_z_dependent_coupling_against_library_ode_solver():
+    """Two modes, no nonlinearity, Q(z) = f(z) Q0 with a grating profile f: per frequency the field
+    obeys a 2 x 2 linear ODE, integrated here by scipy's solve_ivp as an independent witness; a grating whose period
+    matches the modes' beat length transfers power that the unmodulated coupler (strongly mismatched) cannot."""
+    from scipy.integrate import solve_ivp
+    N, dt = 64, 5e-15
+    A0 = np.zeros((2, N), np.complex128)
+    A0[0] = 1.0
+    Dm, kap, z = 900.0, 25.0, 0.05
+    beta = np.array([[0.0], [Dm]])
+    Q0 = np.array([[0, kap], [kap, 0]], dtype=complex)
+    f = lambda zz: 2.0 * np.cos(Dm * zz)
+    S0 = np.zeros((2, 2, 2, 2))
+    rhs = lambda zz, a: 1j * np.array([0.0, Dm]) * a + 1j * f(zz) * (Q0.T @ a)
+    sol = solve_ivp(rhs, (0, z), np.array([1.0 + 0j, 0.0 + 0j]), rtol=1e-11, atol=1e-13)
+    want = sol.y[:, -1]
+    A = O.rk4ip_propagate(A0, z, z / 400, beta, S0, 0.0, W.OMEGA0, 0.0, None, dt, shock=False, coupling=(Q0, f))
+    assert np.abs(A[:, 3] - want).max() < 2e-7                       # O(h^4) of the 400-step RK4IP against the 1e-11 witness
+    Am = O.mpa_propagate(A0, z, z / 2000, 10, beta, S0, 0.0, W.OMEGA0, 0.0, None, dt, shock=False, coupling=(Q0, f),
+                         tol=1e-12)
+    assert np.abs(Am[:, 3] - want).max() < 2e-5
+    assert abs(want[1]) ** 2 > 0.7                                    # phase matched by the grating: sin^2(kap z) = 0.90
+    flat = O.rk4ip_propagate(A0, z, z / 400, beta, S0, 0.0, W.OMEGA0, 0.0, None, dt, shock=False, coupling=Q0)
+    assert abs(flat[1, 3]) ** 2 < 0.02                                # without it: 4 kap^2 / D^2 at most
+    # a constant profile is the constant coupler
+    same = O.rk4ip_propagate(A0, z, z / 400, beta, S0, 0.0, W.OMEGA0, 0.0, None, dt, shock=False,
+                             coupling=(Q0, lambda zz: 1.0))
+    assert np.array_equal(same, flat)
