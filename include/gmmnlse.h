@@ -137,16 +137,26 @@ int gmmnlse_propagate_rk4ip(gmmnlse_plan *plan, const void *A_in, double L, void
 /* Other effects within the GMMNLSE (section F), both integrators:
  *   set_gain:     small-signal FIELD gain g_p A_p; g: HOST [P] in 1/m (negative = loss), NULL or all
  *                 zero = none.  Linear and diagonal, so it joins D_w as its real part: the rotation tables
- *                 exp(+-D_w j dz) get the factors exp(+-g_p j dz).  Frequency-independent gain only; the
- *                 Taylor-expanded saturation term of section F.2 is not built.
+ *                 exp(+-D_w j dz) get the factors exp(+-g_p j dz).  Frequency-independent gain only.
+ *   set_gain_saturation: first-order saturation of that gain (the Taylor expansion of
+ *                 g(I) = g0 / [1 + int dt I / I_sat] projected on the modes), the additional term
+ *                   - g_sat sum_lmn S_plmn A_l(t) int dtau A_m(tau) A_n*(tau),    g_sat = g0 / I_sat in m/J
+ *                 (the paper prints the term without its gain prefactor: DESIGN.md reading S22); the time integral is
+ *                 dt sum_t over the window.  0 = off.  Scalar-mode plans only (EUNSUPPORTED on a general plan).
  *   set_coupling: linear mode coupling C_p = i sum_n Q_np A_n (Eq. 13 for Q_np); Q: HOST [P][P]
  *                 (re, im) interleaved, entry (n P + p) = Q_np in 1/m, NULL or all zero = none.  Constant over
- *                 a call and over frequency; a z-dependent Q(z) (disorder, gratings) is propagated in segments
- *                 with set_coupling between the calls.  Integrated with the nonlinear term (same trapezoid /
- *                 RK4 stages).  gmmnlse_nonlinear_op does not include it.
- * Both synchronise the plan's stream, copy their argument, and return EINVAL on non-finite input.               */
+ *                 frequency.  Integrated with the nonlinear term (same trapezoid / RK4 stages).
+ *   set_coupling_profile: z-dependence of the coupling, Q(z) = f(z) Q: the separable index perturbation
+ *                 eps(x, y) f(z) of PAPER.md:277 (a grating: f periodic; disorder: f a stochastic function).  f: HOST
+ *                 [n] samples f(k dz / 2), k = 0..n-1, measured from the START of each propagate call (the RK4IP
+ *                 stages sit on half steps; the MPA planes use the even samples); a call over L needs
+ *                 n >= 2 L / dz + 1, else EINVAL.  NULL = constant coupling (f = 1).
+ * gmmnlse_nonlinear_op includes none of these.  All four synchronise the plan's stream, copy their argument, and
+ * return EINVAL on non-finite input.                                                                              */
 int gmmnlse_set_gain(gmmnlse_plan *plan, const double *g);
 int gmmnlse_set_coupling(gmmnlse_plan *plan, const double *Q);
+int gmmnlse_set_coupling_profile(gmmnlse_plan *plan, const double *f, int n);
+int gmmnlse_set_gain_saturation(gmmnlse_plan *plan, double g_sat);
 
 /* One evaluation of the last term of Eq. 1:
  *   dA_p(t) = i n2 w0/c (1 + i/w0 d_t) sum_lmn S_plmn A_l [(1-fR) A_m A_n* + fR (h_R (*) A_m A_n*)]

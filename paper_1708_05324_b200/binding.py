@@ -48,6 +48,8 @@ SIGNATURES = {
     "gmmnlse_nonlinear_op": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "gmmnlse_set_gain": (C.c_int, [C.c_void_p, _DP]),
     "gmmnlse_set_coupling": (C.c_int, [C.c_void_p, _DP]),
+    "gmmnlse_set_coupling_profile": (C.c_int, [C.c_void_p, _DP, C.c_int]),
+    "gmmnlse_set_gain_saturation": (C.c_int, [C.c_void_p, C.c_double]),
     "gmmnlse_set_stream": (C.c_int, [C.c_void_p, C.c_void_p]),
     "gmmnlse_get_stats": (C.c_int, [C.c_void_p, _LLP, _LLP, _DP, _LLP]),
     "gmmnlse_launch_count": (C.c_longlong, [C.c_void_p]),
@@ -184,6 +186,18 @@ class Plan:
         if Q.size != self.P * self.P:
             raise GmmnlseError(EINVAL, "Q must hold P x P entries")
         _check(self._lib, self._lib.gmmnlse_set_coupling(self._h, C.cast(Q.ctypes.data, _DP)))
+
+    def set_coupling_profile(self, f) -> None:
+        """gmmnlse_set_coupling_profile: f(k dz / 2), k = 0..n-1, from the start of each call (None: constant)."""
+        if f is None:
+            _check(self._lib, self._lib.gmmnlse_set_coupling_profile(self._h, None, 0))
+            return
+        f = np.ascontiguousarray(f, dtype=np.float64)
+        _check(self._lib, self._lib.gmmnlse_set_coupling_profile(self._h, f.ctypes.data_as(_DP), int(f.size)))
+
+    def set_gain_saturation(self, g_sat: float) -> None:
+        """gmmnlse_set_gain_saturation: g0 / I_sat in m/J (0 = off)."""
+        _check(self._lib, self._lib.gmmnlse_set_gain_saturation(self._h, float(g_sat)))
 
     # -- helpers -----------------------------------------------------------------------------------
     def set_stream(self, stream) -> None:

@@ -195,6 +195,8 @@ struct gmmnlse_plan {
   virtual int propagate_rk4ip(const void* A_in, double L, void* A_out) = 0;
   virtual int set_gain(const double* g) = 0;
   virtual int set_coupling(const double* Qri) = 0;
+  virtual int set_coupling_profile(const double* f, int n) = 0;
+  virtual int set_gain_saturation(double g) = 0;
   virtual int nonlinear_op(const void* A, void* dA) = 0;
   virtual int get_planes(void* out) = 0;
   virtual int debug_fft(const void* in, void* out, int rows, int dir) = 0;
@@ -247,6 +249,13 @@ struct PlanT final : gmmnlse_plan {
   std::vector<double> gain;                // [P], 1/m; empty = none
   T *gfwd = nullptr, *ginv = nullptr;      // [(M+1)][P]: exp(+g_p j dz), exp(-g_p j dz)
   C* Qc = nullptr;                         // [P][P], Qc[n P + p] = Q_np
+  C* Xconst = nullptr;                     // [P][P] i Q: the extra-term matrix when it is the same for every plane
+  C* Xext = nullptr;                       // [(M+1)][P][P] per-plane matrix i f(z_j) Q - g_sat W_j (k_ext_matrix)
+  T* Epair = nullptr;                      // [(M+1)][Q] time-integrated pair products (gain saturation)
+  double g_sat = 0;                        // first-order gain saturation coefficient g0 / I_sat [m/J], 0 = off
+  double* fprof_d = nullptr;               // z-profile of the coupling, sampled every dz / 2 from the start of a call
+  int n_fprof = 0;
+  int* d_step2 = nullptr;                  // device: twice the small steps taken so far in the current call
   int Bp = 0;                              // general mode: rows per Re / Im block of U, streams per Kerr / Raman block
   int* st_kind = nullptr;
   T *st_wk = nullptr, *st_wr = nullptr;
@@ -330,7 +339,7 @@ struct PlanT final : gmmnlse_plan {
     if (cap_stream) cudaStreamDestroy(cap_stream);
     cudaFree(d_stats);
     if (h_stats) cudaFreeHost(h_stats);
-    cudaFree(gfwd); cudaFree(ginv); cudaFree(Qc); cudaFree(st_kind); cudaFree(st_wk); cudaFree(st_wr); cudaFree(iir_zp); cudaFree(pair_work); cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
+    cudaFree(gfwd); cudaFree(ginv); cudaFree(Qc); cudaFree(Xconst); cudaFree(Xext); cudaFree(Epair); cudaFree(fprof_d); cudaFree(d_step2); cudaFree(st_kind); cudaFree(st_wk); cudaFree(st_wr); cudaFree(iir_zp); cudaFree(pair_work); cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
     if (h_err) cudaFreeHost(h_err);
     if (h_in) cudaFreeHost(h_in);
     if (h_out) cudaFreeHost(h_out);
@@ -468,6 +477,8 @@ struct PlanT final : gmmnlse_plan {
     GM_TRY(dalloc(&G, (size_t)(M + 1) * PN));
     GM_TRY(dalloc(&V, (size_t)(M + 1) * QN));
     GM_TRY(dalloc(&U, (size_t)(M + 1) * QN));
+    GM_TRY(dalloc(&d_step2, 1));
+    GM_CUDA(cudaMemset(d_step2, 0, sizeof(int)));
     GM_TRY(dalloc(&errbuf, (size_t)2 * (M + 2)));
     GM_TRY(dalloc(&d_err, 1));
     GM_CUDA(cudaMemset(errbuf, 0, sizeof(double) * 2 * (M + 2)));
@@ -1185,9 +1196,9 @@ struct PlanT final : gmmnlse_plan {
     // a8: G_j = K(w) exp(-D j dz) F{N_p}
     GM_TRY(launch_fft(+1, G + j0 * PN, PN, G + j0 * PN, PN, nullptr, Kw, E + j0 * PN, PN, (T)1, P, np,
                       ginv ? ginv + j0 * P : nullptr));
-    if (Qc)                                                                 // + exp(-D j dz) i Q^T (psi_j exp(D j dz))
-      GM_TRY(launch_couple(first ? psi : psi + j0 * PN, first ? 0 : PN, E + j0 * PN,
-                           gfwd ? gfwd + j0 * P : nullptr, ginv ? ginv + j0 * P : nullptr, G + j0 * PN, np));
+    if (ext_any())                                                          // + exp(-D j dz) X_j^T (psi_j exp(D j dz))
+      GM_TRY(launch_ext(first ? psi : psi + j0 * PN, first ? 0 : PN, E + j0 * PN, gfwd ? gfwd + j0 * P : nullptr,
+                        ginv ? ginv + j0 * P : nullptr, G + j0 * PN, np, j0, 0));
     // a9 + a10
     prof_begin(GMMNLSE_KIND_SCAN);
     launch_k(k_trapz_scan<T>, sblocks, 256, sizeof(double) * 2 * (Mc + 1), psi, G, psi, PN, Mc, (T)dz,
@@ -1200,7 +1211,7 @@ struct PlanT final : gmmnlse_plan {
   int enqueue_advance(int Mc, const double2* EM) {                           // a11
     const unsigned sblocks = (unsigned)((PN + 255) / 256);
     prof_begin(GMMNLSE_KIND_ADVANCE);
-    launch_k(k_advance<T>, sblocks, 256, 0, psi0_d, psi, G, PN, Mc, dz, EM, PN);
+    launch_k(k_advance<T>, sblocks, 256, 0, psi0_d, psi, G, PN, Mc, dz, EM, PN, d_step2);
     prof_end();
     GM_CUDA(cudaGetLastError());
     return 0;
@@ -1345,6 +1356,8 @@ struct PlanT final : gmmnlse_plan {
     const double ns = L / dz;
     const long long nsteps = llround(ns);
     if (!(L >= 0) || std::fabs(ns - (double)nsteps) > 1e-9 * std::fmax(1.0, ns)) return GMMNLSE_EINVAL;
+    if (fprof_d && Qc && 2 * nsteps + 1 > n_fprof) return GMMNLSE_EINVAL;   // the z-profile must cover the call
+    GM_CUDA(cudaMemsetAsync(d_step2, 0, sizeof(int), stream));
     // a1: psi_0 = F{A(z0)}
     GM_TRY(launch_fft(+1, (const C*)A_in, 0, psi, 0, nullptr, nullptr, nullptr, 0, (T)1, P, 1));
     GM_TRY(to_master(psi));
@@ -1423,19 +1436,45 @@ struct PlanT final : gmmnlse_plan {
   }
 
   // Nh(X) = K F{N[F^-1 X]} for one [P][N] field in the frequency domain -> G plane 0      (a3-a8, one plane)
-  int nonlinear_freq(const C* Xf) {
+  // f_off: position of the evaluation inside the step in half small steps (RK4IP stages: 0, 1, 1, 2)
+  int nonlinear_freq(const C* Xf, int f_off) {
     GM_TRY(launch_fft(-1, Xf, 0, At, 0, nullptr, nullptr, nullptr, 0, (T)(1.0 / N), P, 1));
     GM_TRY(nonlinear_term(0, 1));
     GM_TRY(launch_fft(+1, G, 0, G, 0, nullptr, Kw, nullptr, 0, (T)1, P, 1));
-    if (Qc) GM_TRY(launch_couple(Xf, 0, nullptr, nullptr, nullptr, G, 1));
+    if (ext_any()) GM_TRY(launch_ext(Xf, 0, nullptr, nullptr, nullptr, G, 1, 0, f_off));
     return 0;
   }
 
-  int launch_couple(const C* src, long long src_ps, const C* Etab, const T* gf, const T* gi, C* Gout, int planes) {
+  // Linear extra terms of section F: coupling i Q (constant, or f(z) Q with a z-profile) and the
+  // first-order gain saturation.  The matrix is the same for every plane only for constant coupling alone.
+  bool ext_any() const { return Qc != nullptr || g_sat != 0.0; }
+  bool ext_dynamic() const { return g_sat != 0.0 || (Qc && fprof_d); }
+  // G_j += R-_j X_j^T (R+_j src_j) for `planes` planes starting at plane j0 (At planes j0.. hold the fields in time)
+  int launch_ext(const C* src, long long src_ps, const C* Etab, const T* gf, const T* gi, C* Gout, int planes, int j0,
+                 int f_off) {
+    const C* X = Xconst;
+    long long x_ps = 0;
+    if (ext_dynamic()) {
+      if (!Xext) GM_TRY(dalloc(&Xext, (size_t)(M + 1) * P * P));
+      if (g_sat != 0.0) {
+        if (!Epair) GM_TRY(dalloc(&Epair, (size_t)(M + 1) * Q));
+        prof_begin(GMMNLSE_KIND_MISC);
+        launch_k(k_pair_energy<T>, dim3(Q, planes), 256, 0, At + j0 * PN, PN, pair_m, pair_n, Epair + (size_t)j0 * Q, Q, N, dt);
+        prof_end();
+        GM_CUDA(cudaGetLastError());
+      }
+      prof_begin(GMMNLSE_KIND_MISC);
+      launch_k(k_ext_matrix<T>, planes, 256, 0, Qc, S2, g_sat != 0.0 ? Epair + (size_t)j0 * Q : nullptr, (T)g_sat, fprof_d,
+               n_fprof, d_step2, j0, f_off, Xext + (size_t)j0 * P * P, P, Q);
+      prof_end();
+      GM_CUDA(cudaGetLastError());
+      X = Xext + (size_t)j0 * P * P;
+      x_ps = (long long)P * P;
+    }
     const size_t smem = sizeof(C) * P * 64;
     GM_TRY(ensure_smem(k_couple<T>, smem));
     prof_begin(GMMNLSE_KIND_MISC);
-    launch_k(k_couple<T>, dim3((N + 63) / 64, planes), 256, smem, src, src_ps, Etab, gf, gi, Qc, Gout, PN, P, N);
+    launch_k(k_couple<T>, dim3((N + 63) / 64, planes), 256, smem, src, src_ps, Etab, gf, gi, X, x_ps, Gout, PN, P, N);
     prof_end();
     GM_CUDA(cudaGetLastError());
     return 0;
@@ -1473,7 +1512,9 @@ struct PlanT final : gmmnlse_plan {
     GM_CUDA(cudaStreamSynchronize(stream));
     drop_loop_graph();
     cudaFree(Qc);
+    cudaFree(Xconst);
     Qc = nullptr;
+    Xconst = nullptr;
     if (!Qri) return 0;
     std::vector<C> q((size_t)P * P);
     bool any = false;
@@ -1484,15 +1525,46 @@ struct PlanT final : gmmnlse_plan {
     }
     if (!any) return 0;
     GM_TRY(dalloc(&Qc, q.size()));
-    return upload(Qc, q);
+    GM_TRY(upload(Qc, q));
+    std::vector<C> x(q.size());
+    for (size_t i = 0; i < q.size(); ++i) x[i] = mk(-q[i].y, q[i].x);      // i Q
+    GM_TRY(dalloc(&Xconst, x.size()));
+    return upload(Xconst, x);
+  }
+
+  // z-profile of the coupling: Q(z) = f(z) Q (index perturbation eps(x, y) f(z)), f sampled every dz / 2
+  // from the start of each propagate call (the RK4IP stages sit on half steps)
+  int set_coupling_profile(const double* f, int n) override {
+    GM_CUDA(cudaStreamSynchronize(stream));
+    drop_loop_graph();
+    cudaFree(fprof_d);
+    fprof_d = nullptr;
+    n_fprof = 0;
+    if (!f) return 0;
+    if (n < 1) return GMMNLSE_EINVAL;
+    for (int i = 0; i < n; ++i)
+      if (!std::isfinite(f[i])) return GMMNLSE_EINVAL;
+    GM_TRY(dalloc(&fprof_d, (size_t)n));
+    GM_CUDA(cudaMemcpy(fprof_d, f, sizeof(double) * (size_t)n, cudaMemcpyHostToDevice));
+    n_fprof = n;
+    return 0;
+  }
+
+  int set_gain_saturation(double g) override {
+    if (!std::isfinite(g)) return GMMNLSE_EINVAL;
+    if (g != 0.0 && general) return GMMNLSE_EUNSUPPORTED;           // needs the packed symmetric S2
+    GM_CUDA(cudaStreamSynchronize(stream));
+    drop_loop_graph();
+    g_sat = g;
+    return 0;
   }
 
   int enqueue_rk4_step() {
     const unsigned blocks = (unsigned)((PN + 255) / 256);
     for (int stage = 1; stage <= 4; ++stage) {
-      GM_TRY(nonlinear_freq(stage == 1 ? psi : rk_X));
+      GM_TRY(nonlinear_freq(stage == 1 ? psi : rk_X, stage == 1 ? 0 : (stage == 4 ? 2 : 1)));
       prof_begin(GMMNLSE_KIND_ADVANCE);
-      launch_k(k_rk4_stage<T>, blocks, 256, 0, stage, psi0_d, psi, EH_d, G, rk_AI, rk_K1, rk_K2, rk_K3, rk_X, dz, PN);
+      launch_k(k_rk4_stage<T>, blocks, 256, 0, stage, psi0_d, psi, EH_d, G, rk_AI, rk_K1, rk_K2, rk_K3, rk_X, dz, PN, d_step2);
       prof_end();
       GM_CUDA(cudaGetLastError());
     }
@@ -1542,6 +1614,8 @@ struct PlanT final : gmmnlse_plan {
       GM_TRY(dalloc(&EH_d, (size_t)PN));
       GM_TRY(upload(EH_d, eh));
     }
+    if (fprof_d && Qc && 2 * nsteps + 1 > n_fprof) return GMMNLSE_EINVAL;
+    GM_CUDA(cudaMemsetAsync(d_step2, 0, sizeof(int), stream));
     GM_TRY(launch_fft(+1, (const C*)A_in, 0, psi, 0, nullptr, nullptr, nullptr, 0, (T)1, P, 1));
     GM_TRY(to_master(psi));
     long long s = 0;
@@ -1759,6 +1833,18 @@ int gmmnlse_set_coupling(gmmnlse_plan* plan, const double* Q) {
   if (!plan) return GMMNLSE_EINVAL;
   DeviceGuard dg(plan->device);
   return plan->set_coupling(Q);
+}
+
+int gmmnlse_set_coupling_profile(gmmnlse_plan* plan, const double* f, int n) {
+  if (!plan) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
+  return plan->set_coupling_profile(f, n);
+}
+
+int gmmnlse_set_gain_saturation(gmmnlse_plan* plan, double g_sat) {
+  if (!plan) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
+  return plan->set_gain_saturation(g_sat);
 }
 
 int gmmnlse_nonlinear_op(gmmnlse_plan* plan, const void* A, void* dA) {

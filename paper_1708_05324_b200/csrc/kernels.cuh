@@ -851,9 +851,11 @@ __global__ void k_err_finalize_loop(double* __restrict__ errbuf, int Mc, double*
 template <typename T>
 __global__ void __launch_bounds__(256)
 k_advance(double2* __restrict__ psi0_d, cplx<T>* __restrict__ psi0, const cplx<T>* __restrict__ G,
-          long long plane_stride, int Mc, double dz, const double2* __restrict__ EM, long long PN) {
+          long long plane_stride, int Mc, double dz, const double2* __restrict__ EM, long long PN,
+          int* __restrict__ step2) {
   pdl_prologue();
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0 && step2) *step2 += 2 * Mc;               // position along the call, in half small steps (z-profiles)
   if (i >= PN) return;
   double ax = 0.5 * (double)G[i].x, ay = 0.5 * (double)G[i].y;
   for (int j = 1; j < Mc; ++j) {
@@ -885,9 +887,11 @@ template <typename T>
 __global__ void __launch_bounds__(256)
 k_rk4_stage(int stage, double2* __restrict__ At_d, cplx<T>* __restrict__ At, const double2* __restrict__ EH,
             const cplx<T>* __restrict__ G, cplx<T>* __restrict__ AI, cplx<T>* __restrict__ K1,
-            cplx<T>* __restrict__ K2, cplx<T>* __restrict__ K3, cplx<T>* __restrict__ X, double h, long long PN) {
+            cplx<T>* __restrict__ K2, cplx<T>* __restrict__ K3, cplx<T>* __restrict__ X, double h, long long PN,
+            int* __restrict__ step2) {
   pdl_prologue();
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0 && stage == 4 && step2) *step2 += 2;
   if (i >= PN) return;
   const double2 e = EH[i];
   const double gx = (double)G[i].x * h, gy = (double)G[i].y * h;
@@ -918,15 +922,18 @@ k_rk4_stage(int stage, double2* __restrict__ At_d, cplx<T>* __restrict__ At, con
 }
 
 // ------------------------------------------------------------------------------------------
-// Linear mode coupling (section F.1): G_j[p] += R-_j[p] i sum_n Q_np (R+_j[n] src_j[n])
-// per frequency, where R+-_j = exp(+-D_w j dz) = E^(+-1) x gain factor rotates between the interaction picture of
-// plane j and the field (tables null: no rotation, the RK4IP stages).  Q[n][p] constant over the call.
+// Terms linear in the field with a frequency-independent P x P matrix (section F; SURVEY.md 8(f)
+// NEXT-3): G_j[p] += R-_j[p] sum_n X_j[n][p] (R+_j[n] src_j[n]) per frequency, where R+-_j = exp(+-D_w j dz) =
+// E^(+-1) x gain factor rotates between the interaction picture of plane j and the field (tables null: no rotation,
+// the RK4IP stages).  X_j = i f(z_j) Q - g_sat W_j: linear coupling C_p = i sum_n Q_np A_n (f: the z-profile of the
+// perturbation) and first-order gain saturation (W_j from the plane's time-integrated pair products, k_ext_matrix);
+// x_plane_stride = 0 when X is the same for every plane (constant coupling alone).
 //   grid = (N / 64, n_planes), block = 256: 64 frequencies x 4 mode groups; the rotated field tile sits in smem.
 template <typename T>
 __global__ void __launch_bounds__(256)
 k_couple(const cplx<T>* __restrict__ src, long long src_plane_stride, const cplx<T>* __restrict__ E,
-         const T* __restrict__ gfwd, const T* __restrict__ ginv, const cplx<T>* __restrict__ Qc,
-         cplx<T>* __restrict__ G, long long plane_stride, int P, int N) {
+         const T* __restrict__ gfwd, const T* __restrict__ ginv, const cplx<T>* __restrict__ X,
+         long long x_plane_stride, cplx<T>* __restrict__ G, long long plane_stride, int P, int N) {
   pdl_prologue();
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* a_s = reinterpret_cast<cplx<T>*>(smem_raw);        // [P][64]
@@ -934,6 +941,7 @@ k_couple(const cplx<T>* __restrict__ src, long long src_plane_stride, const cplx
   const int w0 = blockIdx.x * 64, w = w0 + x;
   const cplx<T>* sj = src + j * src_plane_stride;
   const cplx<T>* Ej = E ? E + j * plane_stride : nullptr;
+  const cplx<T>* Xj = X + j * x_plane_stride;
   for (int i = threadIdx.x; i < P * 64; i += blockDim.x) {
     const int n = i >> 6, xx = i & 63;
     cplx<T> a = mk((T)0, (T)0);
@@ -949,15 +957,77 @@ k_couple(const cplx<T>* __restrict__ src, long long src_plane_stride, const cplx
   for (int p = g; p < P; p += 4) {
     T sx = 0, sy = 0;
     for (int n = 0; n < P; ++n) {
-      const cplx<T> q = Qc[n * P + p], a = a_s[n * 64 + x];
+      const cplx<T> q = Xj[n * P + p], a = a_s[n * 64 + x];
       sx += q.x * a.x - q.y * a.y;
       sy += q.x * a.y + q.y * a.x;
     }
-    cplx<T> c = mk(-sy, sx);                                    // times i
+    cplx<T> c = mk(sx, sy);
     if (Ej) c = cmulc(c, Ej[(long long)p * N + w]);
     if (ginv) c = cscale(c, ginv[j * P + p]);
     cplx<T>* out = G + j * plane_stride + (long long)p * N + w;
     *out = cadd(*out, c);
+  }
+}
+
+// Time-integrated pair products of the planes' fields (gain saturation): Ep[j][q] = dt sum_t Re(A_m A_n*),
+// q = packed (m <= n).  grid = (Q, n_planes), block = 256; fp64 accumulation.
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_pair_energy(const cplx<T>* __restrict__ A, long long a_plane_stride, const int* __restrict__ pair_m,
+              const int* __restrict__ pair_n, T* __restrict__ Ep, int Q, int N, double dt) {
+  pdl_prologue();
+  __shared__ double red[8];
+  const int q = blockIdx.x, j = blockIdx.y;
+  const cplx<T>* am = A + j * a_plane_stride + (long long)pair_m[q] * N;
+  const cplx<T>* an = A + j * a_plane_stride + (long long)pair_n[q] * N;
+  double s = 0.0;
+  for (int t = threadIdx.x; t < N; t += 256) {
+    const cplx<T> a = am[t], b = an[t];
+    s += (double)(a.x * b.x + a.y * b.y);
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double tot = 0.0;
+    for (int k = 0; k < 8; ++k) tot += red[k];
+    Ep[(long long)j * Q + q] = (T)(tot * dt);
+  }
+}
+
+// Per-plane matrix of the linear extra terms: X_j[n][p] = i f(z_j) Q_np - g_sat W_j,np with
+// W_j,pl = sum_mn S_plmn E_j,mn = sum_q S2[r(p,l)][q] Ep[j][q] (real, symmetric; S2 carries the m < n doubling).
+// f(z_j) = fprof[*step2 + 2 (j0 + j) + f_off] (profile sampled every dz / 2 from the start of the call; *step2 = twice the
+// small steps already taken, kept on the device by k_advance / k_rk4_stage), 1 without a profile.
+//   grid = n_planes, block = 256.  Qc, Ep, fprof may be null (term absent).
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_ext_matrix(const cplx<T>* __restrict__ Qc, const T* __restrict__ S2, const T* __restrict__ Ep, T g_sat,
+             const double* __restrict__ fprof, int n_fprof, const int* __restrict__ step2, int j0, int f_off,
+             cplx<T>* __restrict__ X, int P, int Q) {
+  pdl_prologue();
+  const int j = blockIdx.x;
+  T f = (T)1;
+  if (fprof) {
+    int idx = (step2 ? *step2 : 0) + 2 * (j0 + j) + f_off;
+    idx = idx < 0 ? 0 : (idx >= n_fprof ? n_fprof - 1 : idx);
+    f = (T)fprof[idx];
+  }
+  for (int i = threadIdx.x; i < P * P; i += 256) {
+    const int n = i / P, p = i - n * P;
+    cplx<T> x = mk((T)0, (T)0);
+    if (Qc) x = mk(-f * Qc[i].y, f * Qc[i].x);                    // i f Q_np
+    if (Ep) {
+      const int a = n < p ? n : p, b = n < p ? p : n;
+      const long long r = (long long)a * P - (long long)a * (a - 1) / 2 + (b - a);
+      const T* srow = S2 + r * Q;
+      const T* e = Ep + (long long)j * Q;
+      T w = (T)0;
+      for (int q = 0; q < Q; ++q) w += srow[q] * e[q];
+      x.x -= g_sat * w;
+    }
+    X[(long long)j * P * P + i] = x;
   }
 }
 

@@ -835,6 +835,105 @@ def test_gain_and_coupling_with_nonlinearity_vs_oracle(B, general):
     assert rel(out.cpu().numpy(), ref_rk) <= TOL_FIELD
 
 
+def test_gain_saturation_and_coupling_profile_closed_forms_on_gpu(B):
+    """Section F.2 / F.1 on the GPU, no nonlinearity: the logistic energy law of the saturating amplifier
+    (reading S22) and the grating-assisted coupler Q(z) = f(z) Q0 against scipy's
+    ODE solver, both integrators, complex64 and complex128."""
+    from scipy.integrate import solve_ivp
+    N, dt = 256, 10e-15
+    t = (np.arange(N) - N // 2) * dt
+    A0 = (30.0 * np.exp(-t ** 2 / (2 * (80e-15) ** 2)))[None, :].astype(np.complex128)
+    S1 = np.full((1, 1, 1, 1), 2.0e10)
+    g, z, nst = 4.0, 0.3, 600
+    E0 = O.energy(A0, dt)
+    g_sat = 0.6 * g / (S1[0, 0, 0, 0] * E0)
+    Ez = E0 * np.exp(2 * g * z) / (1 + (g_sat * S1[0, 0, 0, 0] * E0 / g) * (np.exp(2 * g * z) - 1))
+    for precision, tol in ((0, 2e-5), (1, 1e-5)):
+        cdt = np.complex128 if precision else np.complex64
+        # n2 -> 0: the Kerr term vanishes, S still enters through the saturation
+        with B.Plan(1, N, 10, dt, z / nst, np.zeros((1, 3)), S1, 0.0, None, W.OMEGA0, 0.0, precision=precision,
+                    shock=False, tol=1e-10) as plan:
+            plan.set_gain(np.array([g]))
+            plan.set_gain_saturation(g_sat)
+            for fn in (plan.propagate, plan.propagate_rk4ip):
+                Ad = dev(A0, cdt); out = torch.empty_like(Ad)
+                fn(Ad, z, out); torch.cuda.synchronize()
+                o = out.cpu().numpy().astype(np.complex128)
+                assert abs(O.energy(o, dt) / Ez - 1) <= tol and rel(o, A0 * np.sqrt(Ez / E0)) <= tol
+            plan.set_gain_saturation(0.0)                  # cleared: plain exponential gain
+            Ad = dev(A0, cdt); out = torch.empty_like(Ad)
+            plan.propagate_rk4ip(Ad, z, out); torch.cuda.synchronize()
+            assert rel(out.cpu().numpy(), A0 * np.exp(g * z)) <= tol
+        # grating-assisted coupler
+        Dm, kap, zc, nc = 900.0, 25.0, 0.05, 2000
+        Q0 = np.array([[0, kap], [kap, 0]], dtype=complex)
+        f = lambda zz: 2.0 * np.cos(Dm * zz)
+        rhs = lambda zz, a: 1j * np.array([0.0, Dm]) * a + 1j * f(zz) * (Q0.T @ a)
+        want = solve_ivp(rhs, (0, zc), np.array([1.0 + 0j, 0.0 + 0j]), rtol=1e-11, atol=1e-13).y[:, -1]
+        Ac = np.zeros((2, N), np.complex128); Ac[0] = 1.0
+        dzc = zc / nc
+        with B.Plan(2, N, 10, dt, dzc, np.array([[0.0], [Dm]]), np.zeros((2, 2, 2, 2)), 0.0, None, W.OMEGA0, W.N2,
+                    precision=precision, shock=False, tol=1e-10) as plan:
+            plan.set_coupling(Q0)
+            plan.set_coupling_profile(f(0.5 * dzc * np.arange(2 * nc + 1)))
+            for fn, tl in ((plan.propagate_rk4ip, 2e-5 if precision == 0 else 1e-7), (plan.propagate, 3e-5)):
+                Ad = dev(Ac, cdt); out = torch.empty_like(Ad)
+                fn(Ad, zc, out); torch.cuda.synchronize()
+                assert np.abs(out.cpu().numpy()[:, 5] - want).max() <= tl
+                # the profile restarts with every call: two half-length calls see f(0 .. zc/2) twice, not f(0 .. zc)
+            Ad = dev(Ac, cdt); out = torch.empty_like(Ad)
+            plan.propagate_rk4ip(Ad, zc, out); torch.cuda.synchronize()
+            with pytest.raises(B.GmmnlseError) as e:       # a profile shorter than the call
+                plan.set_coupling_profile(np.ones(100))
+                plan.propagate(Ad, zc, out)
+            assert e.value.status == B.EINVAL
+            plan.set_coupling_profile(None)                # back to the constant coupler (strongly mismatched)
+            plan.propagate_rk4ip(Ad, zc, out); torch.cuda.synchronize()
+            assert np.abs(out.cpu().numpy()[1, 5]) ** 2 < 0.02 < abs(want[1]) ** 2
+
+
+@pytest.mark.parametrize("graph", [0, 1])
+def test_saturation_and_z_coupling_with_nonlinearity_vs_oracle(B, graph):
+    """All of section F at once on a 6-mode fibre with Kerr + Raman + shock: gain, first-order saturation and a
+    z-dependent (disorder-like, seeded) coupling profile, both integrators against the oracle; device loop and host loop."""
+    w = W.make_config(2, N=512, L=40 * 50e-6)
+    rng = np.random.default_rng(21)
+    g = rng.uniform(5.0, 25.0, w.P)
+    Q0 = rng.standard_normal((w.P, w.P)) + 1j * rng.standard_normal((w.P, w.P))
+    Qc = 40.0 * (Q0 + Q0.conj().T)
+    nst = int(round(w.L / w.dz))
+    # a seeded disorder profile with a correlation length of many steps (a few random Fourier components), every dz / 2
+    zz = 0.5 * w.dz * np.arange(2 * nst + 1)
+    prof = 1.0 + sum(a * np.cos(2 * np.pi * k * zz / w.L + ph) for k, a, ph in
+                     zip((1, 2, 3, 5), rng.uniform(0.2, 0.5, 4), rng.uniform(0, 2 * np.pi, 4)))
+    f = lambda zz: prof[int(round(zz / (0.5 * w.dz)))]
+    E0 = O.energy(w.A0, w.dt)
+    g_sat = 0.3 * g.mean() / (w.S[0, 0, 0, 0] * E0)
+    Ad = dev(w.A0, np.complex64)
+    out, out_rk = torch.empty_like(Ad), torch.empty_like(Ad)
+    with B.Plan(w.P, w.N, w.M, w.dt, w.dz, w.beta, w.S, w.f_R, w.h_R, w.omega0, w.n2, tol=w.tol, graph=graph) as plan:
+        plan.set_gain(g)
+        plan.set_gain_saturation(g_sat)
+        plan.set_coupling(Qc)
+        plan.set_coupling_profile(prof)
+        plan.propagate(Ad, w.L, out)
+        plan.propagate_rk4ip(Ad, w.L, out_rk)
+        torch.cuda.synchronize()
+        assert plan.loop_kind() == (1 if graph == 0 else 0)
+    A_in = Ad.cpu().numpy().astype(np.complex128)
+    args = (w.beta, w.S, w.kappa, w.omega0, w.f_R, w.h_R, w.dt)
+    kw = dict(shock=w.shock, gain=g, coupling=(Qc, f), g_sat=g_sat)
+    ref_rk = O.rk4ip_propagate(A_in, w.L, w.dz, *args, **kw)
+    ref_mpa = O.mpa_propagate(A_in, w.L, w.dz, w.M, *args, tol=w.tol, **kw)
+    # the terms matter: without them the field is somewhere else entirely
+    plain = O.rk4ip_propagate(A_in, w.L, w.dz, *args, shock=w.shock, gain=g, coupling=Qc)
+    assert rel(plain, ref_rk) > 1e-2
+    assert rel(out_rk.cpu().numpy(), ref_rk) <= 2e-5
+    assert rel(out.cpu().numpy(), ref_mpa) <= 1e-4
+    # across schemes: the oracle's own MPA-RK4IP distance (O(dz^2), coupling of a few 1e2 /m), no more
+    assert rel(out.cpu().numpy(), ref_rk) <= rel(ref_mpa, ref_rk) + 1e-4 <= 5 * TOL_FIELD
+
+
 def test_gain_coupling_reject_bad_input(B):
     w = W.make_config(2, N=256, max_group=1)
     with B.plan_from_workload(w) as plan:
@@ -845,6 +944,10 @@ def test_gain_coupling_reject_bad_input(B):
         bad = np.zeros((w.P, w.P), complex); bad[0, 1] = np.inf
         with pytest.raises(B.GmmnlseError):
             plan.set_coupling(bad)
+        with pytest.raises(B.GmmnlseError):
+            plan.set_coupling_profile(np.array([1.0, np.nan]))
+        with pytest.raises(B.GmmnlseError):
+            plan.set_gain_saturation(float("inf"))
 
 
 # ------------------------------------------ full-length propagation against stored oracle outputs (tests/golden)
