@@ -1110,7 +1110,59 @@ struct PlanT final : gmmnlse_plan {
     return 0;
   }
 
+  // TMA maps for the streaming a7: U (the plan's own buffer) and the field buffer seen as rows of float pairs
+  CUtensorMap tmU7, tmA7;
+  bool a7_maps = false;
+  int a7_nbox() const { return (Q + 255) / 256; }
+  int a7_rows_box() const { return (((Q + a7_nbox() - 1) / a7_nbox()) + 1) & ~1; }   // even: 128-byte aligned TMA boxes
+  size_t a7_smem() const { return (size_t)2 * ((size_t)a7_nbox() * a7_rows_box() * 64 + (size_t)P * 128) + 16 + 128; }
+  int a7_stream_setup() {
+    if (a7_maps) return 0;
+    {
+      const cuuint64_t dims[3] = {(cuuint64_t)N, (cuuint64_t)Q, (cuuint64_t)(M + 1)};
+      const cuuint64_t strides[2] = {(cuuint64_t)N * 4, (cuuint64_t)QN * 4};
+      const cuuint32_t box[3] = {16, (cuuint32_t)a7_rows_box(), 1};
+      GM_TRY(encode_tmap_f32(&tmU7, (void*)U, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_NONE));
+    }
+    {
+      const cuuint64_t dims[3] = {(cuuint64_t)2 * N, (cuuint64_t)P, (cuuint64_t)(M + 1)};
+      const cuuint64_t strides[2] = {(cuuint64_t)N * 8, (cuuint64_t)PN * 8};
+      const cuuint32_t box[3] = {32, (cuuint32_t)P, 1};
+      GM_TRY(encode_tmap_f32(&tmA7, (void*)At, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_NONE));
+    }
+    a7_maps = true;
+    return 0;
+  }
+  // streaming a7 applies to the plan's own U and At planes of a complex64 scalar-mode plan with enough slices to
+  // occupy the device and a slice pair that fits shared memory
+  bool a7_streams(const T* Uin, const C* A, int planes) const {
+    if (sizeof(T) != 4 || general || N % 16 != 0 || P > 256 || n_sm <= 0) return false;
+    if (!(Uin >= U && Uin < U + (size_t)(M + 1) * QN) || !(A >= At && A < At + (size_t)(M + 1) * PN)) return false;
+    return a7_smem() <= 200 * 1024 && (long long)planes * (N / 16) >= 4LL * n_sm;
+  }
+
   int launch_mode_reduce(const T* Uin, const C* A, C* Nout, int planes) {
+    if constexpr (sizeof(T) == 4) {
+      if (a7_streams(Uin, A, planes)) {
+        GM_TRY(a7_stream_setup());
+        const size_t smem = a7_smem();
+        GM_TRY(ensure_smem(k_mode_reduce_stream, smem));
+        const int n_slices = planes * (N / 16);
+        prof_begin(GMMNLSE_KIND_MODE_REDUCE);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)std::min(n_sm, n_slices));
+        cfg.blockDim = dim3(16u * (unsigned)std::min(64, (P + 1) & ~1));     // one mode per thread up to P = 64
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = stream;
+        pdl_config(cfg);
+        cudaError_t e = cudaLaunchKernelEx(&cfg, k_mode_reduce_stream, tmU7, tmA7, (int)((Uin - U) / QN),
+                                           (int)((A - At) / PN), (float2*)Nout, PN, P, Q, N, n_slices, a7_nbox(),
+                                           a7_rows_box());
+        prof_end();
+        GM_CUDA(e);
+        return 0;
+      }
+    }
     if (general) {
       const size_t smem = sizeof(C) * P * 128;
       GM_TRY(ensure_smem(k_mode_reduce_gen<T>, smem));
