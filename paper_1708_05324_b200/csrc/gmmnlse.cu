@@ -1136,7 +1136,9 @@ struct PlanT final : gmmnlse_plan {
   // streaming a7 applies to the plan's own U and At planes of a complex64 scalar-mode plan with enough slices to
   // occupy the device and a slice pair that fits shared memory
   bool a7_streams(const T* Uin, const C* A, int planes) const {
-    if (sizeof(T) != 4 || general || N % 16 != 0 || P > 256 || n_sm <= 0) return false;
+    // a slice is Q x 64 B: below ~16 KB (configs 3-4: 120 / 210 packed pairs) the per-slice barrier and TMA issue cost
+    // more than the second read they save (measured: config 3 16.0k -> 12.3k z-steps/s, config 4 8.4k -> 6.6k)
+    if (sizeof(T) != 4 || general || N % 16 != 0 || P > 256 || n_sm <= 0 || Q < 256) return false;
     if (!(Uin >= U && Uin < U + (size_t)(M + 1) * QN) || !(A >= At && A < At + (size_t)(M + 1) * PN)) return false;
     return a7_smem() <= 200 * 1024 && (long long)planes * (N / 16) >= 4LL * n_sm;
   }
