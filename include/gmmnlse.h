@@ -223,6 +223,18 @@ int gmmnlse_raman_kind(const gmmnlse_plan *plan);
  *          accumulate.  1 <= k <= 255.                        */
 int gmmnlse_debug_set_tc_chunk(gmmnlse_plan *plan, int k);
 
+/* The nonlinear coupling tensor of Eq. 2 by quadrature, on the GPU:
+ *   S_plmn = sum_g F_p F_l F_m F_n dA / sqrt(sum_g F_p^2 dA ... sum_g F_n^2 dA)       [1/m^2]
+ * for P real scalar mode fields sampled on G grid points of area dA.  S is the Gram matrix of the P(P+1)/2 pair
+ * functions F_p F_l, so the work is one (Q x G)(G x Q) product: it runs on the tcgen05 kind::f16 kernel of a6 with
+ * K = G (fp16 hi / lo splits of both operands, two-level accumulation: relative accuracy ~1e-6 of the largest entry);
+ * normalisation and expansion to [P]^4 are done in fp64 on the host.
+ *   F      HOST [P][G] fp64, any units (the normalisation cancels them);  dA [m^2];
+ *   S_out  HOST [P][P][P][P], index ((p*P + l)*P + m)*P + n -- the array gmmnlse_plan_create takes.
+ * Runs on the current device and synchronises it.  EINVAL: sizes < 1, NULL pointers, non-finite F, a mode of zero
+ * norm; EUNSUPPORTED: G not a multiple of 32.                                                                  */
+int gmmnlse_overlap_tensor(int P, long long G, const double *F, double dA, double *S_out);
+
 void gmmnlse_plan_destroy(gmmnlse_plan *plan);
 const char *gmmnlse_status_string(int status);
 const char *gmmnlse_last_cuda_error(void);

@@ -34,6 +34,7 @@ import numpy as np
 
 __all__ = [
     "dft_direct", "fft_radix2", "to_freq", "to_time", "omega_grid",
+    "overlap_tensor", "overlap_tensor_literal",
     "dispersion_operator", "coupling_term", "coupling_at", "saturation_term", "raman_transfer", "pair_products",
     "raman_convolve_direct", "raman_convolve", "nonlinear_term",
     "nonlinear_term_literal", "nonlinear_term_general", "nonlinear_term_general_literal",
@@ -97,6 +98,39 @@ def omega_grid(N: int, dt: float) -> np.ndarray:
     k = np.arange(N)
     kp = np.where(k < N // 2, k, k - N)
     return 2.0 * np.pi * kp / (N * dt)
+
+
+# ------------------------------------------------------------------ Eq. 2
+def overlap_tensor(F: np.ndarray, dA: float) -> np.ndarray:
+    """S_plmn = int F_p F_l F_m F_n dA / [int F_p^2 dA int F_l^2 dA int F_m^2 dA int F_n^2 dA]^(1/2)  (PAPER.md:60,
+    Eq. 2) for real scalar mode fields F[p][grid] by the rectangle (midpoint) rule on the grid: all P^2 ORDERED pair
+    functions F_p F_l, one matmul over the grid, no symmetry used."""
+    F = np.asarray(F, dtype=np.float64)
+    P = F.shape[0]
+    f = F.reshape(P, -1)
+    nrm = np.sqrt(np.sum(f * f, axis=1) * dA)
+    pair = (f[:, None, :] * f[None, :, :]).reshape(P * P, -1)         # [(p l)][g]
+    S = (pair @ pair.T) * dA
+    S = S.reshape(P, P, P, P) / (nrm[:, None, None, None] * nrm[None, :, None, None] *
+                                 nrm[None, None, :, None] * nrm[None, None, None, :])
+    return S
+
+
+def overlap_tensor_literal(F: np.ndarray, dA: float) -> np.ndarray:
+    """The same as four nested loops over the modes (tiny P only)."""
+    F = np.asarray(F, dtype=np.float64)
+    P = F.shape[0]
+    f = F.reshape(P, -1)
+    S = np.zeros((P, P, P, P))
+    for p in range(P):
+        for l in range(P):
+            for m in range(P):
+                for n in range(P):
+                    num = np.sum(f[p] * f[l] * f[m] * f[n]) * dA
+                    den = math.sqrt(np.sum(f[p] ** 2) * dA * np.sum(f[l] ** 2) * dA * np.sum(f[m] ** 2) * dA *
+                                    np.sum(f[n] ** 2) * dA)
+                    S[p, l, m, n] = num / den
+    return S
 
 
 # ------------------------------------------------------------------ linear part

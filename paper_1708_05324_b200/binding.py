@@ -64,6 +64,7 @@ SIGNATURES = {
     "gmmnlse_lowrank_rank": (C.c_int, [C.c_void_p]),
     "gmmnlse_loop_kind": (C.c_int, [C.c_void_p]),
     "gmmnlse_debug_set_tc_chunk": (C.c_int, [C.c_void_p, C.c_int]),
+    "gmmnlse_overlap_tensor": (C.c_int, [C.c_int, C.c_longlong, _DP, C.c_double, _DP]),
     "gmmnlse_plan_destroy": (None, [C.c_void_p]),
     "gmmnlse_status_string": (C.c_char_p, [C.c_int]),
     "gmmnlse_last_cuda_error": (C.c_char_p, []),
@@ -271,6 +272,17 @@ class Plan:
 
     def __exit__(self, *exc):
         self.destroy()
+
+
+def overlap_tensor(F, dA: float) -> np.ndarray:
+    """gmmnlse_overlap_tensor: S_plmn of Eq. 2 from P mode fields F[P][...grid] (any grid shape), on the GPU."""
+    lib = load_library()
+    F = np.ascontiguousarray(F, dtype=np.float64)
+    P = F.shape[0]
+    F = F.reshape(P, -1)
+    S = np.empty((P, P, P, P), dtype=np.float64)
+    _check(lib, lib.gmmnlse_overlap_tensor(P, F.shape[1], F.ctypes.data_as(_DP), float(dA), S.ctypes.data_as(_DP)))
+    return S
 
 
 def _stream_ptr(stream) -> int:

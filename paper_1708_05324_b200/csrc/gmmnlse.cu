@@ -1734,12 +1734,137 @@ struct PlanT final : gmmnlse_plan {
   }
 };
 
+// ------------------------------------------------------------------ Eq. 2 by quadrature on the GPU (NEXT-4)
+struct DevBufs {                      // frees what it owns when the routine leaves, on every path
+  std::vector<void*> p;
+  ~DevBufs() { for (void* q : p) cudaFree(q); }
+  template <typename X> int alloc(X** out, size_t n) {
+    cudaError_t e = cudaMalloc((void**)out, n * sizeof(X));
+    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return GMMNLSE_ENOMEM; }
+    GM_CUDA(e);
+    p.push_back(*out);
+    return 0;
+  }
+};
+
+// S_plmn = int F_p F_l F_m F_n dA / sqrt(int F_p^2 dA ... int F_n^2 dA): the Gram matrix of the pair
+// functions F_p F_l (p <= l) over the G grid points is one (Q x G) (G x Q) product -- K = G on the kind::f16 tcgen05
+// kernel of gemm_h.cuh, both operands split into fp16 hi / lo with exact power-of-two scales -- then the
+// normalisation and the expansion to [P]^4 on the host in fp64.
+int overlap_tensor_gpu(int P, long long G, const double* F, double dA, double* S_out) {
+  const int Q = P * (P + 1) / 2;
+  const int Npad = (Q + hc::TM - 1) / hc::TM * hc::TM;           // pair index as the GEMM's M (t) dimension
+  const int nrt = (Q + 207) / 208;
+  const int NT = (((Q + nrt - 1) / nrt) + 15) / 16 * 16;
+  const int Rp = nrt * NT;
+  const int KB = (int)(G / hc::BK);
+  int dev = 0, n_sm = 0, smax = 0;
+  GM_CUDA(cudaGetDevice(&dev));
+  GM_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+  GM_CUDA(cudaDeviceGetAttribute(&smax, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+  int stages = 3;
+  while (stages > 1 && hc::smem_bytes(NT, stages) > (size_t)smax) --stages;
+  if (hc::smem_bytes(NT, stages) > (size_t)smax) return GMMNLSE_EUNSUPPORTED;
+  std::vector<int> pp(Q), pl(Q);
+  for (int p = 0, q = 0; p < P; ++p)
+    for (int l = p; l < P; ++l, ++q) { pp[q] = p; pl[q] = l; }
+  DevBufs bufs;
+  double* dF = nullptr;
+  int *dpp = nullptr, *dpl = nullptr;
+  float *PhiT = nullptr, *Ug = nullptr, *rscale = nullptr, *vbound = nullptr;
+  __half *Ah = nullptr, *Bh = nullptr, *Bl = nullptr;
+  GM_TRY(bufs.alloc(&dF, (size_t)P * G));
+  GM_TRY(bufs.alloc(&dpp, (size_t)Q));
+  GM_TRY(bufs.alloc(&dpl, (size_t)Q));
+  GM_TRY(bufs.alloc(&PhiT, (size_t)G * Npad));
+  GM_TRY(bufs.alloc(&Ah, (size_t)2 * G * Npad));                  // hi rows [G][Npad], then lo rows
+  GM_TRY(bufs.alloc(&Bh, (size_t)Rp * G));
+  GM_TRY(bufs.alloc(&Bl, (size_t)Rp * G));
+  GM_TRY(bufs.alloc(&rscale, (size_t)Rp));
+  GM_TRY(bufs.alloc(&vbound, (size_t)1));
+  GM_TRY(bufs.alloc(&Ug, (size_t)Q * Npad));
+  // normalise the modes first (fp64, host): unnormalised Hermite-Gauss fields of high order are orders of magnitude
+  // larger than the fundamental, and the fp16 operands share one power-of-two range
+  std::vector<double> Fn((size_t)P * G);
+  for (int p = 0; p < P; ++p) {
+    long double acc = 0;
+    for (long long g = 0; g < G; ++g) acc += (long double)F[p * G + g] * F[p * G + g];
+    const double nrm = std::sqrt((double)acc * dA);
+    if (!(nrm > 0) || !std::isfinite(nrm)) return GMMNLSE_EINVAL;
+    for (long long g = 0; g < G; ++g) Fn[(size_t)p * G + g] = F[p * G + g] / nrm;
+  }
+  GM_CUDA(cudaMemcpy(dF, Fn.data(), sizeof(double) * (size_t)P * G, cudaMemcpyHostToDevice));
+  GM_CUDA(cudaMemcpy(dpp, pp.data(), sizeof(int) * Q, cudaMemcpyHostToDevice));
+  GM_CUDA(cudaMemcpy(dpl, pl.data(), sizeof(int) * Q, cudaMemcpyHostToDevice));
+  GM_CUDA(cudaMemset(vbound, 0, sizeof(float)));
+  const long long total = G * Npad;
+  k_pair_fields_t<<<2368, 256>>>(dF, G, dpp, dpl, Q, Npad, PhiT);
+  k_bound_real<float><<<592, 256>>>(PhiT, total, vbound);
+  k_v_encode<<<2368, 256>>>(PhiT, total, total, HalfOut{Ah, 2 * total, total, Npad, vbound});
+  k_pair_fields_b<<<Rp, 256>>>(dF, G, dpp, dpl, Q, Bh, Bl, rscale);
+  GM_CUDA(cudaGetLastError());
+  CUtensorMap tmAh, tmAl, tmBh, tmBl;
+  {
+    const cuuint64_t dims[3] = {(cuuint64_t)Npad, (cuuint64_t)G, 1};
+    const cuuint64_t strides[2] = {(cuuint64_t)Npad * 2, (cuuint64_t)G * Npad * 4};
+    const cuuint32_t box[3] = {64, hc::BK, 1};
+    GM_TRY(encode_tmap(&tmAh, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, Ah, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B));
+    GM_TRY(encode_tmap(&tmAl, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, Ah + total, 3, dims, strides, box,
+                       CU_TENSOR_MAP_SWIZZLE_128B));
+  }
+  {
+    const cuuint64_t dims[2] = {(cuuint64_t)G, (cuuint64_t)Rp};
+    const cuuint64_t strides[1] = {(cuuint64_t)G * 2};
+    const cuuint32_t box[2] = {hc::BK, (cuuint32_t)NT};
+    GM_TRY(encode_tmap(&tmBh, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, Bh, 2, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_64B));
+    GM_TRY(encode_tmap(&tmBl, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, Bl, 2, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_64B));
+  }
+  hc::Params prm = {};
+  prm.U = Ug; prm.Zh = nullptr; prm.u_plane_stride = (long long)Q * Npad;
+  prm.rscale = rscale; prm.vbound = vbound; prm.bound_gain = 1.f; prm.zgain = 0.f;
+  prm.Q = Q; prm.N = Npad; prm.NT = NT; prm.KB = KB; prm.n_rt = nrt;
+  prm.t_tiles = Npad / hc::TM;
+  prm.total_tiles = prm.t_tiles * nrt;
+  prm.plane0 = 0; prm.stages = stages; prm.kchunk = 4;
+  GM_TRY(ensure_dyn_smem(dev, (const void*)hc::k_contract_h<false>, hc::smem_bytes(NT, stages)));
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)std::min(n_sm, prm.total_tiles));
+  cfg.blockDim = dim3(hc::NTHREADS);
+  cfg.dynamicSmemBytes = hc::smem_bytes(NT, stages);
+  GM_CUDA(cudaLaunchKernelEx(&cfg, hc::k_contract_h<false>, tmAh, tmAl, tmBh, tmBl, prm));
+  std::vector<float> Uh((size_t)Q * Npad);
+  GM_CUDA(cudaMemcpy(Uh.data(), Ug, sizeof(float) * Uh.size(), cudaMemcpyDeviceToHost));   // synchronises
+  // expansion to [P]^4 in fp64 on the host (the modes were normalised before the product)
+  std::vector<int> idx((size_t)P * P);
+  for (int q = 0; q < Q; ++q) { idx[(size_t)pp[q] * P + pl[q]] = q; idx[(size_t)pl[q] * P + pp[q]] = q; }
+  for (int p = 0; p < P; ++p)
+    for (int l = 0; l < P; ++l) {
+      const int r = idx[(size_t)p * P + l];
+      for (int m = 0; m < P; ++m)
+        for (int n = 0; n < P; ++n) {
+          const int q = idx[(size_t)m * P + n];
+          // the Gram matrix is symmetric: average the two computed halves
+          const double gsum = 0.5 * ((double)Uh[(size_t)r * Npad + q] + (double)Uh[(size_t)q * Npad + r]);
+          S_out[(((size_t)p * P + l) * P + m) * P + n] = gsum * dA;
+        }
+    }
+  return 0;
+}
+
 }  // namespace
 
 // ============================================================================================
 extern "C" {
 
-int gmmnlse_abi_version(void) { return 1; }
+int gmmnlse_abi_version(void) { return 2; }
+
+int gmmnlse_overlap_tensor(int P, long long G, const double* F, double dA, double* S_out) {
+  if (P < 1 || G < 1 || !F || !S_out || !(dA > 0)) return GMMNLSE_EINVAL;
+  if (G % hc::BK != 0) return GMMNLSE_EUNSUPPORTED;
+  for (long long i = 0; i < (long long)P * G; ++i)
+    if (!std::isfinite(F[i])) return GMMNLSE_EINVAL;
+  return overlap_tensor_gpu(P, G, F, dA, S_out);
+}
 
 const char* gmmnlse_last_cuda_error(void) { return g_cuda_err.c_str(); }
 

@@ -1106,6 +1106,67 @@ k_ext_matrix(const cplx<T>* __restrict__ Qc, const T* __restrict__ S2, const T* 
   }
 }
 
+// ------------------------------------------------------------------------------------------
+// Eq. 2 on the GPU: S_plmn is the Gram matrix of the pair functions
+// Phi_r = F_p F_l, r = (p <= l), on the quadrature grid: Gram[r][q] = sum_g Phi_r(g) Phi_q(g).  The product runs on
+// the same kind::f16 tcgen05 kernel as a6 (K = grid points); these two kernels prepare its operands from the fp64
+// mode fields F[P][G].
+//   k_pair_fields_t: A operand, PhiT[g][Npad] fp32 (pair index contiguous, zero beyond Q) -> k_v_encode splits it.
+//   k_pair_fields_b: B operand, rows r of Phi as fp16 hi / lo [Rp][G] scaled per row by 2^(14 - e_r) (exact), with
+//                    rscale[r] = 2^-(14 - e_r); one CTA per row (row maximum first, then the split).
+__global__ void __launch_bounds__(256)
+k_pair_fields_t(const double* __restrict__ F, long long G, const int* __restrict__ pair_p, const int* __restrict__ pair_l,
+                int Q, int Npad, float* __restrict__ PhiT) {
+  pdl_prologue();
+  const long long total = G * Npad;
+  for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < total; i += (long long)gridDim.x * 256) {
+    const long long g = i / Npad;
+    const int r = (int)(i - g * Npad);
+    PhiT[i] = r < Q ? (float)(F[pair_p[r] * G + g] * F[pair_l[r] * G + g]) : 0.f;
+  }
+}
+__global__ void __launch_bounds__(256)
+k_pair_fields_b(const double* __restrict__ F, long long G, const int* __restrict__ pair_p, const int* __restrict__ pair_l,
+                int Q, __half* __restrict__ hi, __half* __restrict__ lo, float* __restrict__ rscale) {
+  pdl_prologue();
+  __shared__ double red[8];
+  __shared__ int s_sh;
+  const int r = blockIdx.x;
+  __half* hrow = hi + (long long)r * G;
+  __half* lrow = lo + (long long)r * G;
+  if (r >= Q) {                                                        // padded rows of the r-tiles: zero
+    for (long long g = threadIdx.x; g < G; g += 256) { hrow[g] = __float2half_rn(0.f); lrow[g] = __float2half_rn(0.f); }
+    if (threadIdx.x == 0) rscale[r] = 1.f;
+    return;
+  }
+  const double* fp = F + pair_p[r] * G;
+  const double* fl = F + pair_l[r] * G;
+  double m = 0.0;
+  for (long long g = threadIdx.x; g < G; g += 256) m = fmax(m, fabs(fp[g] * fl[g]));
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, d));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double amax = 0.0;
+    for (int k = 0; k < 8; ++k) amax = fmax(amax, red[k]);
+    int e = 0;
+    if (amax > 0.0) frexp(amax, &e);
+    int sh = amax > 0.0 ? hc::V_RANGE_LOG2 - e : 0;
+    sh = sh > 120 ? 120 : (sh < -120 ? -120 : sh);
+    s_sh = sh;
+    rscale[r] = (float)ldexp(1.0, -sh);
+  }
+  __syncthreads();
+  const int sh = s_sh;
+  for (long long g = threadIdx.x; g < G; g += 256) {
+    const double v = ldexp(fp[g] * fl[g], sh);
+    const __half h = __float2half_rn((float)v);
+    hrow[g] = h;
+    lrow[g] = __float2half_rn((float)(v - (double)__half2float(h)));
+  }
+}
+
 template <typename TI, typename TO>
 __global__ void __launch_bounds__(256) k_convert(const TI* __restrict__ in, TO* __restrict__ out, long long n) {
   pdl_prologue();

@@ -2,6 +2,8 @@
 same seeded inputs.  Bounds are BASELINE.json's: relative L2 <= 1e-5 for one nonlinear-operator
 evaluation (and for per-iteration MPA planes in fixed_iter mode), <= 1e-3 on the propagated field,
 <= 1e-6 on the drift of the conserved quantity (reading S15)."""
+import math
+
 import numpy as np
 import pytest
 
@@ -948,6 +950,56 @@ def test_gain_coupling_reject_bad_input(B):
             plan.set_coupling_profile(np.array([1.0, np.nan]))
         with pytest.raises(B.GmmnlseError):
             plan.set_gain_saturation(float("inf"))
+
+
+# ------------------------------------------------ NEXT-4: Eq. 2 by quadrature on the GPU (tcgen05 Gram product)
+@pytest.mark.parametrize("kind,arg,n_grid", [
+    ("grin", 2, 256),        # P = 6  (Q = 21: one 128-wide tile), the 256 x 256 grid of the configurations
+    ("grin", 4, 256),        # P = 15 (Q = 120)
+    ("step", 20, 128),       # P = 20 step-index LP modes (Q = 210: two r-tiles)
+    ("grin", 8, 64),         # P = 45 (Q = 1035: 5 r-tiles x 9 t-tiles), coarser grid so that the oracle stays cheap
+])
+def test_overlap_tensor_gpu_vs_oracle(B, kind, arg, n_grid):
+    """gmmnlse_overlap_tensor against the oracle's Eq. 2 (plain fp64 matmul over all ordered pairs): every entry to
+    2e-6 of the largest, the closed form S_1111 = 1/(pi w^2) for the GRIN sets, and one nonlinear-operator evaluation
+    with the GPU-made tensor against the oracle with the oracle-made one."""
+    if kind == "grin":
+        F, dA, _ = W.grin_modes(arg, n_grid=n_grid)
+    else:
+        F, dA, _, _ = W.step_index_modes(arg, n_grid=n_grid)
+    S_ref = O.overlap_tensor(F, dA)
+    S_gpu = B.overlap_tensor(F, dA)
+    assert S_gpu.shape == S_ref.shape and np.isfinite(S_gpu).all()
+    assert np.abs(S_gpu - S_ref).max() <= 2e-6 * np.abs(S_ref).max()
+    assert rel(S_gpu, S_ref) <= 1e-6
+    if kind == "grin" and n_grid == 256:
+        assert abs(S_gpu[0, 0, 0, 0] * math.pi * W.grin_spot_size() ** 2 - 1) <= 2e-6
+    if F.shape[0] <= 20:
+        cfg = 2 if kind == "grin" else 4
+        w = W.make_config(cfg, N=256) if kind == "step" else W.make_config(3 if arg == 4 else 2, N=256)
+        assert w.P == F.shape[0]
+        Ad = dev(w.A0, np.complex64)
+        dA_out = torch.empty_like(Ad)
+        with B.Plan(w.P, w.N, w.M, w.dt, w.dz, w.beta, S_gpu, w.f_R, w.h_R, w.omega0, w.n2) as plan:
+            plan.nonlinear_op(Ad, dA_out)
+            torch.cuda.synchronize()
+        ref = O.nonlinear_op(Ad.cpu().numpy().astype(np.complex128), S_ref, w.kappa, w.omega0, w.f_R, w.h_R, w.dt, w.shock)
+        assert rel(dA_out.cpu().numpy(), ref) <= TOL_OP
+
+
+def test_overlap_tensor_rejects_bad_arguments(B):
+    F = np.ones((2, 48))
+    with pytest.raises(B.GmmnlseError) as e:                         # grid size not a multiple of 32
+        B.overlap_tensor(F, 1.0)
+    assert e.value.status == B.EUNSUPPORTED
+    F = np.ones((2, 64)); F[1, 3] = np.nan
+    with pytest.raises(B.GmmnlseError) as e:
+        B.overlap_tensor(F, 1.0)
+    assert e.value.status == B.EINVAL
+    F = np.ones((2, 64)); F[1] = 0.0                                 # a mode of zero norm
+    with pytest.raises(B.GmmnlseError) as e:
+        B.overlap_tensor(F, 1.0)
+    assert e.value.status == B.EINVAL
 
 
 # ------------------------------------------ full-length propagation against stored oracle outputs (tests/golden)

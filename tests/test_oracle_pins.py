@@ -507,3 +507,25 @@ def test_z_dependent_coupling_against_library_ode_solver():
     same = O.rk4ip_propagate(A0, z, z / 400, beta, S0, 0.0, W.OMEGA0, 0.0, None, dt, shock=False,
                              coupling=(Q0, lambda zz: 1.0))
     assert np.array_equal(same, flat)
+
+
+# ------------------------------------------------------------------ Eq. 2
+def test_overlap_tensor_closed_forms_and_symmetries():
+    """Eq. 2 on the GRIN Hermite-Gauss modes of the configurations: S_1111 = 1 / (pi w^2) (the Gaussian
+    mode's effective area), S_2222 = 3/4 S_1111 (HG10), S_1122 = 1/2 S_1111; all 24 index permutations equal
+    (PAPER.md:60-63); staged matmul form = the literal four loops."""
+    F, dA, _ = W.grin_modes(2)                                   # 6 modes on the 256 x 256 grid
+    S = O.overlap_tensor(F, dA)
+    w0 = W.grin_spot_size()
+    s1111 = 1.0 / (math.pi * w0 ** 2)
+    assert abs(S[0, 0, 0, 0] / s1111 - 1) < 1e-12
+    assert abs(S[1, 1, 1, 1] / (0.75 * s1111) - 1) < 1e-12
+    assert abs(S[0, 0, 1, 1] / (0.5 * s1111) - 1) < 1e-12
+    import itertools
+    for perm in itertools.permutations(range(4)):
+        assert np.allclose(S, S.transpose(perm), rtol=0, atol=1e-12 * s1111)
+    rng = np.random.default_rng(3)
+    Fr = rng.standard_normal((3, 40))
+    assert np.allclose(O.overlap_tensor(Fr, 0.3), O.overlap_tensor_literal(Fr, 0.3), rtol=1e-13, atol=0)
+    # scale invariance: the normalisation removes the units of F
+    assert np.allclose(O.overlap_tensor(7.0 * Fr, 0.3), O.overlap_tensor(Fr, 0.3), rtol=1e-13, atol=0)
