@@ -158,6 +158,33 @@ int gmmnlse_set_coupling(gmmnlse_plan *plan, const double *Q);
 int gmmnlse_set_coupling_profile(gmmnlse_plan *plan, const double *f, int n);
 int gmmnlse_set_gain_saturation(gmmnlse_plan *plan, double g_sat);
 
+/* Plane-axis sharding of one MPA large step over several GPUs (the M planes are
+ * the parallel axis).  Every shard holds a plan of the SAME arguments on its own device and owns the planes
+ * j_lo+1 .. j_hi of the current large step's Mc planes (shard 0 also plane 0); the collectives between the calls are
+ * the caller's (paper_1708_05324_b200/sharded.py drives them over NCCL), all pointers are DEVICE pointers:
+ *   shard_begin(A_in)                  psi_0 = F{A_in}, on every shard                                        (a1)
+ *   repeat
+ *     shard_iterate(j_lo, j_hi, Mc, first, block_sum)
+ *                                      a3-a8 on the shard's planes; block_sum [P][N] <- sum_j w_j G_j over them,
+ *                                      w = 1/2 on planes 0 and Mc, else 1 (trapezoid rule).
+ *                                      first != 0: the first iterate psi_j = psi_0 (and shard 0 forms G_0)
+ *     -- all-gather of the block sums -> all_sums [n_shards][P][N], shard order --
+ *     shard_update(..., all_sums, shard, n_shards, &err_local)
+ *                                      a9 on the shard's planes from the exclusive prefix of the block sums;
+ *                                      err_local = max over ITS planes of |psi_new - psi_old| / |psi_new| (a10);
+ *                                      synchronises the stream (8-byte read-back)
+ *     -- max all-reduce of err_local; stop when < tol or at max_iter --
+ *   shard_advance(Mc, all_sums, n_shards)   psi_0 <- (psi_0 + dz sum_g block_g) exp(D Mc dz) on every shard   (a11)
+ *   shard_end(A_out)                   A_out = F^-1{psi_0}
+ * With n_shards = 1 (j_lo = 0, j_hi = Mc) the sequence is the host loop of gmmnlse_propagate.  EINVAL on plane
+ * ranges outside 0 <= j_lo < j_hi <= Mc <= M.  The counters of gmmnlse_get_stats count this shard's calls.      */
+int gmmnlse_shard_begin(gmmnlse_plan *plan, const void *A_in);
+int gmmnlse_shard_iterate(gmmnlse_plan *plan, int j_lo, int j_hi, int Mc, int first, void *block_sum);
+int gmmnlse_shard_update(gmmnlse_plan *plan, int j_lo, int j_hi, int Mc, int first, const void *all_sums, int shard,
+                         int n_shards, double *err_local);
+int gmmnlse_shard_advance(gmmnlse_plan *plan, int Mc, const void *all_sums, int n_shards);
+int gmmnlse_shard_end(gmmnlse_plan *plan, void *A_out);
+
 /* One evaluation of the last term of Eq. 1:
  *   dA_p(t) = i n2 w0/c (1 + i/w0 d_t) sum_lmn S_plmn A_l [(1-fR) A_m A_n* + fR (h_R (*) A_m A_n*)]
  * A, dA: DEVICE [P][N] as above (dA must not alias A); enqueued on the plan's stream.      */

@@ -46,6 +46,12 @@ SIGNATURES = {
     "gmmnlse_propagate_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]),
     "gmmnlse_propagate_rk4ip": (C.c_int, [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]),
     "gmmnlse_nonlinear_op": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "gmmnlse_shard_begin": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "gmmnlse_shard_iterate": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]),
+    "gmmnlse_shard_update": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_int, C.c_int,
+                                       _DP]),
+    "gmmnlse_shard_advance": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_int]),
+    "gmmnlse_shard_end": (C.c_int, [C.c_void_p, C.c_void_p]),
     "gmmnlse_set_gain": (C.c_int, [C.c_void_p, _DP]),
     "gmmnlse_set_coupling": (C.c_int, [C.c_void_p, _DP]),
     "gmmnlse_set_coupling_profile": (C.c_int, [C.c_void_p, _DP, C.c_int]),
@@ -167,6 +173,26 @@ class Plan:
 
     def nonlinear_op(self, A, dA) -> int:
         return _check(self._lib, self._lib.gmmnlse_nonlinear_op(self._h, _ptr(A), _ptr(dA)))
+
+    # -- plane-axis sharding (one large step in pieces; the collectives are the caller's: sharded.py) -----
+    def shard_begin(self, A_in) -> None:
+        _check(self._lib, self._lib.gmmnlse_shard_begin(self._h, _ptr(A_in)))
+
+    def shard_iterate(self, j_lo, j_hi, Mc, first, block_sum) -> None:
+        _check(self._lib, self._lib.gmmnlse_shard_iterate(self._h, int(j_lo), int(j_hi), int(Mc), int(bool(first)),
+                                                          _ptr(block_sum)))
+
+    def shard_update(self, j_lo, j_hi, Mc, first, all_sums, shard, n_shards) -> float:
+        err = C.c_double()
+        _check(self._lib, self._lib.gmmnlse_shard_update(self._h, int(j_lo), int(j_hi), int(Mc), int(bool(first)),
+                                                         _ptr(all_sums), int(shard), int(n_shards), C.byref(err)))
+        return err.value
+
+    def shard_advance(self, Mc, all_sums, n_shards) -> None:
+        _check(self._lib, self._lib.gmmnlse_shard_advance(self._h, int(Mc), _ptr(all_sums), int(n_shards)))
+
+    def shard_end(self, A_out) -> None:
+        _check(self._lib, self._lib.gmmnlse_shard_end(self._h, _ptr(A_out)))
 
     def set_gain(self, g) -> None:
         """gmmnlse_set_gain: g[P] field gain in 1/m (None clears it)."""

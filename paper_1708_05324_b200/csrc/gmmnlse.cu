@@ -197,6 +197,12 @@ struct gmmnlse_plan {
   virtual int set_coupling(const double* Qri) = 0;
   virtual int set_coupling_profile(const double* f, int n) = 0;
   virtual int set_gain_saturation(double g) = 0;
+  virtual int shard_begin(const void* A_in) = 0;
+  virtual int shard_iterate(int j_lo, int j_hi, int Mc, int first, void* block_sum) = 0;
+  virtual int shard_update(int j_lo, int j_hi, int Mc, int first, const void* all_sums, int shard, int n_shards,
+                           double* err_local) = 0;
+  virtual int shard_advance(int Mc, const void* all_sums, int n_shards) = 0;
+  virtual int shard_end(void* A_out) = 0;
   virtual int nonlinear_op(const void* A, void* dA) = 0;
   virtual int get_planes(void* out) = 0;
   virtual int debug_fft(const void* in, void* out, int rows, int dir) = 0;
@@ -339,7 +345,7 @@ struct PlanT final : gmmnlse_plan {
     if (cap_stream) cudaStreamDestroy(cap_stream);
     cudaFree(d_stats);
     if (h_stats) cudaFreeHost(h_stats);
-    cudaFree(gfwd); cudaFree(ginv); cudaFree(Qc); cudaFree(Xconst); cudaFree(Xext); cudaFree(Epair); cudaFree(fprof_d); cudaFree(d_step2); cudaFree(st_kind); cudaFree(st_wk); cudaFree(st_wr); cudaFree(iir_zp); cudaFree(pair_work); cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
+    cudaFree(gfwd); cudaFree(ginv); cudaFree(Qc); cudaFree(Xconst); cudaFree(Xext); cudaFree(Epair); cudaFree(fprof_d); cudaFree(d_step2); cudaFree(shard_pre); cudaFree(st_kind); cudaFree(st_wk); cudaFree(st_wr); cudaFree(iir_zp); cudaFree(pair_work); cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
     if (h_err) cudaFreeHost(h_err);
     if (h_in) cudaFreeHost(h_in);
     if (h_out) cudaFreeHost(h_out);
@@ -1271,19 +1277,87 @@ struct PlanT final : gmmnlse_plan {
     return 0;
   }
 
-  int large_step(int Mc, bool* converged) {
-    double2* EM = EM_d;
+  int get_EM(int Mc, double2** out) {        // exp(D Mc dz) in fp64: the plan's table, or one made for a ragged last step
+    *out = EM_d;
     if (Mc != M) {
       auto it = EM_ragged.find(Mc);
       if (it == EM_ragged.end()) {
         double2* p = nullptr;
         GM_TRY(make_EM(Mc, &p));
         EM_ragged[Mc] = p;
-        EM = p;
+        *out = p;
       } else {
-        EM = it->second;
+        *out = it->second;
       }
     }
+    return 0;
+  }
+
+  // ---- plane-axis sharding over several GPUs: the pieces of one large step that a shard runs on its
+  // own planes j_lo+1 .. j_hi of the Mc planes; the collectives between them belong to the caller (sharded.py)
+  C* shard_pre = nullptr;
+  int shard_begin(const void* A_in) override {
+    GM_CUDA(cudaMemsetAsync(d_step2, 0, sizeof(int), stream));
+    GM_TRY(launch_fft(+1, (const C*)A_in, 0, psi, 0, nullptr, nullptr, nullptr, 0, (T)1, P, 1));   // a1, on every shard
+    return to_master(psi);
+  }
+  int shard_iterate(int j_lo, int j_hi, int Mc, int first, void* block_sum) override {
+    if (Mc < 1 || Mc > M || j_lo < 0 || j_hi <= j_lo || j_hi > Mc) return GMMNLSE_EINVAL;
+    const int ja = (first && j_lo == 0) ? 0 : j_lo + 1, np = j_hi - ja + 1;      // G_0 is formed once, by the first shard
+    GM_TRY(launch_fft(-1, first ? psi : psi + ja * PN, first ? 0 : PN, At + ja * PN, PN, E + ja * PN, nullptr, nullptr, PN,
+                      (T)(1.0 / N), P, np, gfwd ? gfwd + ja * P : nullptr));                        // a3
+    GM_TRY(nonlinear_term(ja, np));                                                                 // a4-a7
+    GM_TRY(launch_fft(+1, G + ja * PN, PN, G + ja * PN, PN, nullptr, Kw, E + ja * PN, PN, (T)1, P, np,
+                      ginv ? ginv + ja * P : nullptr));                                             // a8
+    if (ext_any())
+      GM_TRY(launch_ext(first ? psi : psi + ja * PN, first ? 0 : PN, E + ja * PN, gfwd ? gfwd + ja * P : nullptr,
+                        ginv ? ginv + ja * P : nullptr, G + ja * PN, np, ja, 0));
+    prof_begin(GMMNLSE_KIND_SCAN);
+    launch_k(k_shard_block_sum<T>, (unsigned)((PN + 255) / 256), 256, 0, G, PN, j_lo, j_hi, Mc, (C*)block_sum, PN);
+    prof_end();
+    GM_CUDA(cudaGetLastError());
+    return 0;
+  }
+  int shard_update(int j_lo, int j_hi, int Mc, int first, const void* all_sums, int shard, int n_shards,
+                   double* err_local) override {
+    if (Mc < 1 || Mc > M || j_lo < 0 || j_hi <= j_lo || j_hi > Mc || shard < 0 || shard >= n_shards || !err_local)
+      return GMMNLSE_EINVAL;
+    if (!shard_pre) GM_TRY(dalloc(&shard_pre, (size_t)PN));
+    const unsigned blocks = (unsigned)((PN + 255) / 256);
+    prof_begin(GMMNLSE_KIND_SCAN);
+    launch_k(k_shard_prefix<T>, blocks, 256, 0, (const C*)all_sums, shard, G, shard_pre, PN);
+    launch_k(k_shard_scan<T>, blocks, 256, 0, psi, G, psi, PN, j_lo, j_hi, (T)dz, first, shard_pre, errbuf, PN);
+    prof_end();
+    prof_begin(GMMNLSE_KIND_MISC);
+    launch_k(k_err_finalize, 1, 32, 0, errbuf, Mc, d_err);
+    prof_end();
+    GM_CUDA(cudaGetLastError());
+    GM_CUDA(cudaMemcpyAsync(h_err, d_err, sizeof(double), cudaMemcpyDeviceToHost, stream));
+    GM_CUDA(cudaStreamSynchronize(stream));
+    *err_local = *h_err;
+    last_err = *h_err;
+    ++n_iter;
+    return 0;
+  }
+  int shard_advance(int Mc, const void* all_sums, int n_shards) override {
+    if (Mc < 1 || Mc > M || n_shards < 1) return GMMNLSE_EINVAL;
+    double2* EM = nullptr;
+    GM_TRY(get_EM(Mc, &EM));
+    prof_begin(GMMNLSE_KIND_ADVANCE);
+    launch_k(k_shard_advance<T>, (unsigned)((PN + 255) / 256), 256, 0, psi0_d, psi, (const C*)all_sums, n_shards, dz, EM, PN,
+             d_step2, Mc);
+    prof_end();
+    GM_CUDA(cudaGetLastError());
+    ++n_large;
+    return 0;
+  }
+  int shard_end(void* A_out) override {
+    return launch_fft(-1, psi, 0, (C*)A_out, 0, nullptr, nullptr, nullptr, 0, (T)(1.0 / N), P, 1);
+  }
+
+  int large_step(int Mc, bool* converged) {
+    double2* EM = nullptr;
+    GM_TRY(get_EM(Mc, &EM));
     const int cap = fixed_iter > 0 ? fixed_iter : max_iter;
     int it = 0;
     *converged = false;
@@ -2024,6 +2098,37 @@ int gmmnlse_set_gain_saturation(gmmnlse_plan* plan, double g_sat) {
   if (!plan) return GMMNLSE_EINVAL;
   DeviceGuard dg(plan->device);
   return plan->set_gain_saturation(g_sat);
+}
+
+int gmmnlse_shard_begin(gmmnlse_plan* plan, const void* A_in) {
+  if (!plan || !A_in) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
+  return plan->shard_begin(A_in);
+}
+
+int gmmnlse_shard_iterate(gmmnlse_plan* plan, int j_lo, int j_hi, int Mc, int first, void* block_sum) {
+  if (!plan || !block_sum) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
+  return plan->shard_iterate(j_lo, j_hi, Mc, first, block_sum);
+}
+
+int gmmnlse_shard_update(gmmnlse_plan* plan, int j_lo, int j_hi, int Mc, int first, const void* all_sums, int shard,
+                         int n_shards, double* err_local) {
+  if (!plan || !all_sums) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
+  return plan->shard_update(j_lo, j_hi, Mc, first, all_sums, shard, n_shards, err_local);
+}
+
+int gmmnlse_shard_advance(gmmnlse_plan* plan, int Mc, const void* all_sums, int n_shards) {
+  if (!plan || !all_sums) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
+  return plan->shard_advance(Mc, all_sums, n_shards);
+}
+
+int gmmnlse_shard_end(gmmnlse_plan* plan, void* A_out) {
+  if (!plan || !A_out) return GMMNLSE_EINVAL;
+  DeviceGuard dg(plan->device);
+  return plan->shard_end(A_out);
 }
 
 int gmmnlse_nonlinear_op(gmmnlse_plan* plan, const void* A, void* dA) {

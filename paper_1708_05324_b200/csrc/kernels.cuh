@@ -921,6 +921,96 @@ __global__ void k_err_finalize_loop(double* __restrict__ errbuf, int Mc, double*
 }
 
 // ------------------------------------------------------------------------------------------
+// Plane-axis sharding over several GPUs (the M planes are the parallel axis).
+// Shard g owns planes j_lo+1 .. j_hi (shard 0 also plane 0), runs a3-a8 on them and forms its block sum
+//   B_g = sum_{j in shard} w_j G_j,  w_0 = 1/2, w_M = 1/2, else 1          (the trapezoid weights of PAPER.md:218)
+// One all-gather of the block sums (P N complex each) gives every shard its exclusive prefix sum_{g' < g} B_g',
+// from which its planes follow exactly as in k_trapz_scan; sum_g B_g is the whole integral, so every shard can
+// advance psi_0 by itself (no broadcast).  The convergence test adds one scalar max all-reduce.
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_shard_block_sum(const cplx<T>* __restrict__ G, long long plane_stride, int j_lo, int j_hi, int Mc,
+                  cplx<T>* __restrict__ out, long long PN) {
+  pdl_prologue();
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= PN) return;
+  cplx<T> acc = j_lo == 0 ? cscale(G[i], (T)0.5) : mk((T)0, (T)0);
+  for (int j = j_lo + 1; j <= j_hi; ++j) {
+    const cplx<T> g = G[j * plane_stride + i];
+    acc = cadd(acc, j == Mc ? cscale(g, (T)0.5) : g);
+  }
+  out[i] = acc;
+}
+// start value of shard `shard`'s running sum: G_0 / 2 on the first shard, else the sum of the earlier shards' blocks
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_shard_prefix(const cplx<T>* __restrict__ all_sums, int shard, const cplx<T>* __restrict__ G0,
+               cplx<T>* __restrict__ out, long long PN) {
+  pdl_prologue();
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= PN) return;
+  cplx<T> acc = mk((T)0, (T)0);
+  if (shard == 0) acc = cscale(G0[i], (T)0.5);
+  for (int g = 0; g < shard; ++g) acc = cadd(acc, all_sums[g * PN + i]);
+  out[i] = acc;
+}
+// a9 + a10 on the shard's planes: psi_j^new = psi_0 + dz [prefix + G_{j_lo+1} + .. + G_{j-1} + G_j / 2]
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_shard_scan(const cplx<T>* __restrict__ psi0, const cplx<T>* __restrict__ G, cplx<T>* __restrict__ psi,
+             long long plane_stride, int j_lo, int j_hi, T dz, int first_iter, const cplx<T>* __restrict__ prefix,
+             double* __restrict__ errbuf, long long PN) {
+  pdl_prologue();
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool live = i < PN;
+  const long long ii = live ? i : 0;
+  const cplx<T> p0 = psi0[ii];
+  cplx<T> acc = prefix[ii];
+  for (int j = j_lo + 1; j <= j_hi; ++j) {
+    const cplx<T> g = G[j * plane_stride + ii];
+    const cplx<T> old = first_iter ? p0 : psi[j * plane_stride + ii];
+    const cplx<T> pn = mk(p0.x + dz * (acc.x + (T)0.5 * g.x), p0.y + dz * (acc.y + (T)0.5 * g.y));
+    acc = cadd(acc, g);
+    const cplx<T> d = csub(pn, old);
+    double num = live ? (double)(d.x * d.x + d.y * d.y) : 0.0;
+    double den = live ? (double)(pn.x * pn.x + pn.y * pn.y) : 0.0;
+    if (live) psi[j * plane_stride + i] = pn;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      num += __shfl_xor_sync(0xffffffffu, num, o);
+      den += __shfl_xor_sync(0xffffffffu, den, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+      atomicAdd(&errbuf[2 * j], num);
+      atomicAdd(&errbuf[2 * j + 1], den);
+    }
+  }
+}
+// a11 from the gathered block sums: psi0_d <- (psi0_d + dz sum_g B_g) exp(D Mc dz), on every shard alike
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_shard_advance(double2* __restrict__ psi0_d, cplx<T>* __restrict__ psi0, const cplx<T>* __restrict__ all_sums,
+                int n_shards, double dz, const double2* __restrict__ EM, long long PN, int* __restrict__ step2, int Mc) {
+  pdl_prologue();
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0 && step2) *step2 += 2 * Mc;
+  if (i >= PN) return;
+  double ax = 0.0, ay = 0.0;
+  for (int g = 0; g < n_shards; ++g) {
+    const cplx<T> b = all_sums[g * PN + i];
+    ax += (double)b.x;
+    ay += (double)b.y;
+  }
+  double2 p = psi0_d[i];
+  p.x += dz * ax;
+  p.y += dz * ay;
+  const double2 e = EM[i];
+  const double2 q = make_double2(p.x * e.x - p.y * e.y, p.x * e.y + p.y * e.x);
+  psi0_d[i] = q;
+  psi0[i] = mk((T)q.x, (T)q.y);
+}
+
+// ------------------------------------------------------------------------------------------
 // a11: advance the fp64 master state by one large step and refresh its working-precision copy.
 //   psi0_d <- (psi0_d + dz [G_0/2 + G_1 + .. + G_{Mc-1} + G_Mc/2]) * exp(D Mc dz)
 template <typename T>
