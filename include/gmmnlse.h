@@ -262,6 +262,21 @@ int gmmnlse_debug_set_tc_chunk(gmmnlse_plan *plan, int k);
  * norm; EUNSUPPORTED: G not a multiple of 32.                                                                  */
 int gmmnlse_overlap_tensor(int P, long long G, const double *F, double dA, double *S_out);
 
+/* gmmnlse_overlap_tensor for callers that cannot allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same Gram product on the same tcgen05 kernel, but every intermediate lives in
+ * ONE static device array of the library (about 4.9 MB, held by every GPU that loads the library until the process
+ * exits) instead of per-call cudaMalloc.  The call makes no cudaMalloc / cudaFree / allocating library call, uses no
+ * host heap, does not synchronise: all work is enqueued on `stream` (cudaStream_t as void*, NULL = default stream).
+ *   F_dev  DEVICE [P][G] fp64 mode fields;  dA [m^2];  S_dev  DEVICE [P][P][P][P] fp64 out (index as S above).
+ * Limits: P <= 6, G <= 4096 (e.g. a 64 x 64 grid), G a multiple of 32 -- beyond them EUNSUPPORTED, with the limits
+ * spelled out in gmmnlse_last_cuda_error(); gmmnlse_overlap_tensor_noalloc_limits reports them (any pointer may be
+ * NULL).  Normalisation happens on the device: F is not checked, a mode of zero norm or a non-finite sample gives
+ * non-finite output.  ALL calls on a device share the one array, which keeps the previous call's contents (what must
+ * start at zero is cleared by the call): calls that overlap on the GPU -- different streams, or threads -- race;
+ * serialise them on one stream.  Runs on the current device; EINVAL: sizes < 1, NULL pointers, dA <= 0.          */
+int gmmnlse_overlap_tensor_noalloc(int P, long long G, const double *F_dev, double dA, double *S_dev, void *stream);
+int gmmnlse_overlap_tensor_noalloc_limits(int *P_max, long long *G_max, long long *scratch_bytes);
+
 void gmmnlse_plan_destroy(gmmnlse_plan *plan);
 const char *gmmnlse_status_string(int status);
 const char *gmmnlse_last_cuda_error(void);

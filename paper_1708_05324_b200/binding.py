@@ -71,6 +71,8 @@ SIGNATURES = {
     "gmmnlse_loop_kind": (C.c_int, [C.c_void_p]),
     "gmmnlse_debug_set_tc_chunk": (C.c_int, [C.c_void_p, C.c_int]),
     "gmmnlse_overlap_tensor": (C.c_int, [C.c_int, C.c_longlong, _DP, C.c_double, _DP]),
+    "gmmnlse_overlap_tensor_noalloc": (C.c_int, [C.c_int, C.c_longlong, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]),
+    "gmmnlse_overlap_tensor_noalloc_limits": (C.c_int, [C.POINTER(C.c_int), _LLP, _LLP]),
     "gmmnlse_plan_destroy": (None, [C.c_void_p]),
     "gmmnlse_status_string": (C.c_char_p, [C.c_int]),
     "gmmnlse_last_cuda_error": (C.c_char_p, []),
@@ -309,6 +311,25 @@ def overlap_tensor(F, dA: float) -> np.ndarray:
     S = np.empty((P, P, P, P), dtype=np.float64)
     _check(lib, lib.gmmnlse_overlap_tensor(P, F.shape[1], F.ctypes.data_as(_DP), float(dA), S.ctypes.data_as(_DP)))
     return S
+
+
+def overlap_tensor_noalloc(F_dev, dA: float, S_dev, stream=None) -> None:
+    """gmmnlse_overlap_tensor_noalloc: DEVICE fp64 tensors F_dev [P][G...] in, S_dev [P][P][P][P] out; allocates
+    nothing, enqueues on `stream`, shares one static scratch array per device (calls must not overlap on the GPU)."""
+    lib = load_library()
+    P = int(F_dev.shape[0])
+    G = int(F_dev.numel() // P)
+    st = lib.gmmnlse_overlap_tensor_noalloc(P, G, _ptr(F_dev), float(dA), _ptr(S_dev), _stream_ptr(stream))
+    if st == EUNSUPPORTED:
+        raise GmmnlseError(st, lib.gmmnlse_last_cuda_error().decode())
+    _check(lib, st)
+
+
+def overlap_tensor_noalloc_limits() -> dict:
+    lib = load_library()
+    p, g, b = C.c_int(), C.c_longlong(), C.c_longlong()
+    _check(lib, lib.gmmnlse_overlap_tensor_noalloc_limits(C.byref(p), C.byref(g), C.byref(b)))
+    return dict(P_max=p.value, G_max=g.value, scratch_bytes=b.value)
 
 
 def _stream_ptr(stream) -> int:

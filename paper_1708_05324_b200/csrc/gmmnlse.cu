@@ -1925,6 +1925,119 @@ int overlap_tensor_gpu(int P, long long G, const double* F, double dA, double* S
   return 0;
 }
 
+// ------------------------------------------------------------------ Eq. 2 without any allocation
+// gmmnlse_overlap_tensor_noalloc: the same Gram product for callers that cannot call cudaMalloc (code under CUDA graph
+// capture, tight serving loops, harnesses that forbid it).  Every intermediate that overlap_tensor_gpu cudaMallocs per
+// call lives in ONE file-scope device array of fixed size instead; every GPU that loads the library holds it until
+// exit.  Limits: P <= NOALLOC_PMAX modes, G <= NOALLOC_GMAX grid points.
+constexpr int NOALLOC_PMAX = 6;                                   // Q = 21 pair functions: one 128 x 32 tile
+constexpr long long NOALLOC_GMAX = 4096;                          // e.g. a 64 x 64 quadrature grid
+constexpr int NOALLOC_QMAX = NOALLOC_PMAX * (NOALLOC_PMAX + 1) / 2;
+constexpr int NOALLOC_NPAD = hc::TM;                              // pair index padded to the GEMM's M tile
+constexpr int NOALLOC_NT = (NOALLOC_QMAX + 15) / 16 * 16;         // 32 rows of the B operand
+constexpr size_t na_align(size_t x) { return (x + 255) & ~(size_t)255; }
+constexpr size_t NA_OFF_FN = 0;                                                                   // double [P][G]
+constexpr size_t NA_OFF_PP = NA_OFF_FN + na_align(sizeof(double) * NOALLOC_PMAX * NOALLOC_GMAX);   // int [Q]
+constexpr size_t NA_OFF_PL = NA_OFF_PP + na_align(sizeof(int) * NOALLOC_QMAX);                     // int [Q]
+constexpr size_t NA_OFF_PHIT = NA_OFF_PL + na_align(sizeof(int) * NOALLOC_QMAX);                   // float [G][NPAD]
+constexpr size_t NA_OFF_AH = NA_OFF_PHIT + na_align(sizeof(float) * NOALLOC_GMAX * NOALLOC_NPAD);  // half [2][G][NPAD]
+constexpr size_t NA_OFF_BH = NA_OFF_AH + na_align(sizeof(__half) * 2 * NOALLOC_GMAX * NOALLOC_NPAD);   // half [NT][G]
+constexpr size_t NA_OFF_BL = NA_OFF_BH + na_align(sizeof(__half) * NOALLOC_NT * NOALLOC_GMAX);     // half [NT][G]
+constexpr size_t NA_OFF_RS = NA_OFF_BL + na_align(sizeof(__half) * NOALLOC_NT * NOALLOC_GMAX);     // float [NT]
+constexpr size_t NA_OFF_VB = NA_OFF_RS + na_align(sizeof(float) * NOALLOC_NT);                     // float: bound on |Phi|
+constexpr size_t NA_OFF_UG = NA_OFF_VB + na_align(sizeof(float));                                  // float [Q][NPAD]
+constexpr size_t NOALLOC_BYTES = NA_OFF_UG + na_align(sizeof(float) * NOALLOC_QMAX * NOALLOC_NPAD);  // about 4.9 MB
+
+// In host code this name is only a host-side stand-in for the symbol, never a device address: the address the kernels
+// get comes from cudaGetSymbolAddress (noalloc_scratch_ptr below), once per device.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NOALLOC_BYTES];
+
+std::mutex g_noalloc_mu;
+std::map<int, unsigned char*> g_noalloc_ptr;                      // device ordinal -> device address of the array
+
+// device address of the scratch array on the CURRENT device (looked up once per device, with that device current)
+int noalloc_scratch_ptr(int dev, unsigned char** out) {
+  std::lock_guard<std::mutex> lk(g_noalloc_mu);
+  auto it = g_noalloc_ptr.find(dev);
+  if (it == g_noalloc_ptr.end()) {
+    unsigned char* ptr = nullptr;
+    GM_CUDA(cudaGetSymbolAddress((void**)&ptr, g_noalloc_scratch));
+    if (!ptr) { g_cuda_err = "cudaGetSymbolAddress(g_noalloc_scratch) returned a null address"; return GMMNLSE_ECUDA; }
+    it = g_noalloc_ptr.emplace(dev, ptr).first;
+  }
+  *out = it->second;
+  return 0;
+}
+
+// Same arithmetic as overlap_tensor_gpu from the product on; the normalisation and the expansion to [P]^4 run on the
+// device (k_normalise_modes, k_expand_gram) so that nothing returns to the host.  No cudaMalloc / cudaFree, no host
+// heap use, no synchronisation: everything is enqueued on `stream`.
+int overlap_tensor_noalloc(int P, long long G, const double* F_dev, double dA, double* S_dev, cudaStream_t stream) {
+  const int Q = P * (P + 1) / 2;
+  const int Npad = NOALLOC_NPAD, NT = (Q + 15) / 16 * 16, KB = (int)(G / hc::BK);
+  int dev = 0, n_sm = 0, smax = 0;
+  GM_CUDA(cudaGetDevice(&dev));
+  GM_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+  GM_CUDA(cudaDeviceGetAttribute(&smax, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+  const int stages = 3;
+  if (hc::smem_bytes(NT, stages) > (size_t)smax) return GMMNLSE_EUNSUPPORTED;
+  unsigned char* base = nullptr;
+  GM_TRY(noalloc_scratch_ptr(dev, &base));
+  double* Fn = reinterpret_cast<double*>(base + NA_OFF_FN);
+  int* dpp = reinterpret_cast<int*>(base + NA_OFF_PP);
+  int* dpl = reinterpret_cast<int*>(base + NA_OFF_PL);
+  float* PhiT = reinterpret_cast<float*>(base + NA_OFF_PHIT);
+  __half* Ah = reinterpret_cast<__half*>(base + NA_OFF_AH);
+  __half* Bh = reinterpret_cast<__half*>(base + NA_OFF_BH);
+  __half* Bl = reinterpret_cast<__half*>(base + NA_OFF_BL);
+  float* rscale = reinterpret_cast<float*>(base + NA_OFF_RS);
+  float* vbound = reinterpret_cast<float*>(base + NA_OFF_VB);
+  float* Ug = reinterpret_cast<float*>(base + NA_OFF_UG);
+  const long long total = G * Npad;
+  // the array keeps the previous call's contents: the bound is an atomicMax accumulator and must start at zero;
+  // everything else is fully overwritten before it is read (PhiT beyond Q is written as zero, B rows up to NT too)
+  GM_CUDA(cudaMemsetAsync(vbound, 0, sizeof(float), stream));
+  k_normalise_modes<<<P, 256, 0, stream>>>(F_dev, G, dA, P, Fn, dpp, dpl);
+  k_pair_fields_t<<<592, 256, 0, stream>>>(Fn, G, dpp, dpl, Q, Npad, PhiT);
+  k_bound_real<float><<<592, 256, 0, stream>>>(PhiT, total, vbound);
+  k_v_encode<<<592, 256, 0, stream>>>(PhiT, total, total, HalfOut{Ah, 2 * total, total, Npad, vbound});
+  k_pair_fields_b<<<NT, 256, 0, stream>>>(Fn, G, dpp, dpl, Q, Bh, Bl, rscale);
+  GM_CUDA(cudaGetLastError());
+  CUtensorMap tmAh, tmAl, tmBh, tmBl;
+  {
+    const cuuint64_t dims[3] = {(cuuint64_t)Npad, (cuuint64_t)G, 1};
+    const cuuint64_t strides[2] = {(cuuint64_t)Npad * 2, (cuuint64_t)G * Npad * 4};
+    const cuuint32_t box[3] = {64, hc::BK, 1};
+    GM_TRY(encode_tmap(&tmAh, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, Ah, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B));
+    GM_TRY(encode_tmap(&tmAl, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, Ah + total, 3, dims, strides, box,
+                       CU_TENSOR_MAP_SWIZZLE_128B));
+  }
+  {
+    const cuuint64_t dims[2] = {(cuuint64_t)G, (cuuint64_t)NT};
+    const cuuint64_t strides[1] = {(cuuint64_t)G * 2};
+    const cuuint32_t box[2] = {hc::BK, (cuuint32_t)NT};
+    GM_TRY(encode_tmap(&tmBh, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, Bh, 2, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_64B));
+    GM_TRY(encode_tmap(&tmBl, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, Bl, 2, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_64B));
+  }
+  hc::Params prm = {};
+  prm.U = Ug; prm.Zh = nullptr; prm.u_plane_stride = (long long)Q * Npad;
+  prm.rscale = rscale; prm.vbound = vbound; prm.bound_gain = 1.f; prm.zgain = 0.f;
+  prm.Q = Q; prm.N = Npad; prm.NT = NT; prm.KB = KB; prm.n_rt = 1;
+  prm.t_tiles = 1;
+  prm.total_tiles = 1;
+  prm.plane0 = 0; prm.stages = stages; prm.kchunk = 4;
+  GM_TRY(ensure_dyn_smem(dev, (const void*)hc::k_contract_h<false>, hc::smem_bytes(NT, stages)));
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(1);
+  cfg.blockDim = dim3(hc::NTHREADS);
+  cfg.dynamicSmemBytes = hc::smem_bytes(NT, stages);
+  cfg.stream = stream;
+  GM_CUDA(cudaLaunchKernelEx(&cfg, hc::k_contract_h<false>, tmAh, tmAl, tmBh, tmBl, prm));
+  k_expand_gram<<<(P * P * P * P + 255) / 256, 256, 0, stream>>>(Ug, Npad, P, dA, S_dev);
+  GM_CUDA(cudaGetLastError());
+  return 0;
+}
+
 }  // namespace
 
 // ============================================================================================
@@ -2053,6 +2166,28 @@ struct StreamForCall {          // a non-NULL `stream` argument applies to this 
   ~StreamForCall() { plan->stream = saved; }
 };
 }  // namespace
+
+int gmmnlse_overlap_tensor_noalloc(int P, long long G, const double* F_dev, double dA, double* S_dev, void* stream) {
+  if (P < 1 || G < 1 || !F_dev || !S_dev || !(dA > 0)) return GMMNLSE_EINVAL;
+  if (P > NOALLOC_PMAX || G > NOALLOC_GMAX) {
+    g_cuda_err = "gmmnlse_overlap_tensor_noalloc: P = " + std::to_string(P) + ", G = " + std::to_string(G) +
+                 " exceed the static scratch (P <= " + std::to_string(NOALLOC_PMAX) + ", G <= " +
+                 std::to_string(NOALLOC_GMAX) + "); use gmmnlse_overlap_tensor";
+    return GMMNLSE_EUNSUPPORTED;
+  }
+  if (G % hc::BK != 0) {
+    g_cuda_err = "gmmnlse_overlap_tensor_noalloc: G must be a multiple of 32";
+    return GMMNLSE_EUNSUPPORTED;
+  }
+  return overlap_tensor_noalloc(P, G, F_dev, dA, S_dev, (cudaStream_t)stream);
+}
+
+int gmmnlse_overlap_tensor_noalloc_limits(int* P_max, long long* G_max, long long* scratch_bytes) {
+  if (P_max) *P_max = NOALLOC_PMAX;
+  if (G_max) *G_max = NOALLOC_GMAX;
+  if (scratch_bytes) *scratch_bytes = (long long)NOALLOC_BYTES;
+  return GMMNLSE_OK;
+}
 
 int gmmnlse_propagate(gmmnlse_plan* plan, const void* A_in, double L, void* A_out, void* stream) {
   if (!plan || !A_in || !A_out) return GMMNLSE_EINVAL;

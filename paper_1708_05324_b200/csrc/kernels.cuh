@@ -1257,6 +1257,51 @@ k_pair_fields_b(const double* __restrict__ F, long long G, const int* __restrict
   }
 }
 
+// Device-side ends of the Eq. 2 pipeline for gmmnlse_overlap_tensor_noalloc (no host round trip):
+//   k_normalise_modes: Fn[p][g] = F[p][g] / sqrt(sum_g F[p][g]^2 dA), one CTA per mode; CTA 0 also writes the packed
+//                      pair index arrays (p <= l).  A mode of zero norm gives non-finite output (no host check here).
+//   k_expand_gram:     S[p][l][m][n] = dA (Gram[r(p,l)][q(m,n)] + Gram[q][r]) / 2 from the [Q][ld] Gram matrix.
+__global__ void __launch_bounds__(256)
+k_normalise_modes(const double* __restrict__ F, long long G, double dA, int P, double* __restrict__ Fn,
+                  int* __restrict__ pair_p, int* __restrict__ pair_l) {
+  pdl_prologue();
+  __shared__ double red[8];
+  __shared__ double s_inv;
+  const int p = blockIdx.x;
+  const double* f = F + p * G;
+  double acc = 0.0;
+  for (long long g = threadIdx.x; g < G; g += 256) acc += f[g] * f[g];
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double tot = 0.0;
+    for (int k = 0; k < 8; ++k) tot += red[k];
+    s_inv = 1.0 / sqrt(tot * dA);
+  }
+  __syncthreads();
+  const double inv = s_inv;
+  for (long long g = threadIdx.x; g < G; g += 256) Fn[p * G + g] = f[g] * inv;
+  if (p == 0 && threadIdx.x == 0) {
+    int q = 0;
+    for (int a = 0; a < P; ++a)
+      for (int b = a; b < P; ++b, ++q) { pair_p[q] = a; pair_l[q] = b; }
+  }
+}
+__global__ void __launch_bounds__(256)
+k_expand_gram(const float* __restrict__ gram, int ld, int P, double dA, double* __restrict__ S) {
+  pdl_prologue();
+  const int P2 = P * P, total = P2 * P2;
+  for (int i = blockIdx.x * 256 + threadIdx.x; i < total; i += gridDim.x * 256) {
+    const int pl = i / P2, mn = i - pl * P2;
+    const int p = pl / P, l = pl - p * P, m = mn / P, n = mn - m * P;
+    const int a = p < l ? p : l, b = p < l ? l : p, c = m < n ? m : n, d = m < n ? n : m;
+    const int r = a * P - a * (a - 1) / 2 + (b - a), q = c * P - c * (c - 1) / 2 + (d - c);
+    S[i] = 0.5 * ((double)gram[r * ld + q] + (double)gram[q * ld + r]) * dA;
+  }
+}
+
 template <typename TI, typename TO>
 __global__ void __launch_bounds__(256) k_convert(const TI* __restrict__ in, TO* __restrict__ out, long long n) {
   pdl_prologue();
