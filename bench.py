@@ -182,7 +182,7 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def measure(cfg, K, Wm, with_events, host_path=False, seed_offset=0, contraction=None):
+    def measure(cfg, K, Wm, with_events, host_path=False, seed_offset=0, contraction=None, stop_rule=0):
         w = workloads.make_config(cfg)
         n_large = LARGE_PER_STEP[cfg]
         L_step = n_large * w.M * w.dz
@@ -191,7 +191,7 @@ def run_gpu(args):
         A0 = w.A0.astype(cdt)
         A0 = replica_launch_field(A0, seed_offset, workloads.SEED_BASE)
         plan = binding.plan_from_workload(w, contraction=args.contraction if contraction is None else contraction,
-                                          graph=1 if args.host_loop else 0)
+                                          graph=1 if args.host_loop else 0, stop_rule=stop_rule)
         ckind, crank = plan.contraction_kind(), plan.lowrank_rank()
         stream = torch.cuda.current_stream()
         A = torch.from_numpy(A0).cuda()
@@ -351,6 +351,12 @@ def run_gpu(args):
                 "iterations_per_large_step": round(lr["iters"] / max(lr["large"], 1), 3)}
         except binding.GmmnlseError as exc:
             out["variants"]["lowrank_contraction"] = {"unavailable": str(exc)}
+        # reading S25: the a-posteriori stopping rule, same dense contraction; reported beside the headline
+        # with its own iteration count (SURVEY.md reading S11/S12: variants of the iteration are allowed if both are)
+        ap = measure(cfg, K, Wm, with_events=False, stop_rule=1)
+        out["variants"]["aposteriori_stop_rule"] = {
+            "value": round(ap["z_steps"] / (ap["ms"] * 1e-3), 2), "unit": UNIT, "ms_per_step": round(ap["ms"] / K, 4),
+            "iterations_per_large_step": round(ap["iters"] / max(ap["large"], 1), 3), "not_converged": ap["not_conv"]}
         try:                                         # the dense contraction on the 3xTF32 kernel (r01c-r01i's default)
             tf = measure(cfg, K, Wm, with_events=False, contraction=3)
             out["variants"]["tf32_contraction"] = {

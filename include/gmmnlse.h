@@ -70,6 +70,13 @@ typedef struct {                /* pass NULL for defaults                       
                                    same iteration counts.  The first large step of a plan, a ragged last step
                                    ((L/dz) mod M planes) and calls under gmmnlse_profile_enable use the host
                                    loop in either case                                               */
+  int    stop_rule;             /* when an MPA large step counts as converged ("once the accuracy reaches a
+                                   given threshold"): 0 (default, reading S12) = err_n < tol, err_n the
+                                   relative change of the planes in iteration n; 1 (reading S25) = also when the
+                                   a-posteriori bound on the iterate's distance to the fixed point,
+                                   err_n rho / (1 - rho) with rho the larger of the last two ratios err_n / err_{n-1}
+                                   (n >= 3), is below tol.  The result differs by less than tol; one iteration less
+                                   wherever the last one only confirmed convergence.  Other values: EINVAL          */
 } gmmnlse_options;
 
 /* Build a plan: precompute D_w^(p), the rotation tables exp(+-D_w j dz) (j = 0..M) in

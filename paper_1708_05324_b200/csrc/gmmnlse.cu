@@ -140,7 +140,7 @@ int ilog2(int n) {
 // ============================================================================================
 struct gmmnlse_plan {
   int P = 0, N = 0, M = 0, log2N = 0, Q = 0, precision = 0, shock = 1, max_iter = 0, fixed_iter = 0;
-  int contraction = 0, raman = 0, graph = 0;
+  int contraction = 0, raman = 0, graph = 0, stop_rule = 0;
   int loop_state = 0;                      // 0 host loop so far, 1 device loop (CUDA graph) in use, -1 graph build failed
   int device = 0;                          // the CUDA device the plan was created on (every call runs there)
   // general form of Eq. 1 (gmmnlse_plan_create_general): separate, possibly complex tensors, no symmetry
@@ -1360,6 +1360,7 @@ struct PlanT final : gmmnlse_plan {
     GM_TRY(get_EM(Mc, &EM));
     const int cap = fixed_iter > 0 ? fixed_iter : max_iter;
     int it = 0;
+    double err_prev = 1e300, rho_prev = 1e300;
     *converged = false;
     while (true) {
       GM_TRY(enqueue_iteration(Mc, it == 0));
@@ -1376,7 +1377,11 @@ struct PlanT final : gmmnlse_plan {
       GM_CUDA(cudaMemcpyAsync(h_err, d_err, sizeof(double), cudaMemcpyDeviceToHost, stream));
       GM_CUDA(cudaStreamSynchronize(stream));
       last_err = *h_err;
-      if (last_err < tol) { *converged = true; break; }
+      double rho = 0.0;
+      const bool conv = mpa_converged(last_err, tol, stop_rule, it, err_prev, rho_prev, &rho);
+      err_prev = last_err;
+      rho_prev = it == 1 ? 1e300 : rho;
+      if (conv) { *converged = true; break; }
       if (it >= cap) break;
     }
     GM_TRY(enqueue_advance(Mc, EM));
@@ -1408,7 +1413,7 @@ struct PlanT final : gmmnlse_plan {
     GM_CUDA(cudaGraphConditionalHandleCreate(&handle, lg, 0, 0));
     auto finalize = [&]() -> int {
       prof_begin(GMMNLSE_KIND_MISC);
-      launch_k(k_err_finalize_loop, 1, 32, 0, errbuf, M, d_err, tol, cap, fixed_iter > 0 ? 1 : 0, handle, d_stats);
+      launch_k(k_err_finalize_loop, 1, 32, 0, errbuf, M, d_err, tol, cap, fixed_iter > 0 ? 1 : 0, handle, d_stats, stop_rule);
       prof_end();
       GM_CUDA(cudaGetLastError());
       return 0;
@@ -2043,7 +2048,7 @@ int overlap_tensor_noalloc(int P, long long G, const double* F_dev, double dA, d
 // ============================================================================================
 extern "C" {
 
-int gmmnlse_abi_version(void) { return 2; }
+int gmmnlse_abi_version(void) { return 3; }
 
 int gmmnlse_overlap_tensor(int P, long long G, const double* F, double dA, double* S_out) {
   if (P < 1 || G < 1 || !F || !S_out || !(dA > 0)) return GMMNLSE_EINVAL;
@@ -2072,7 +2077,7 @@ static int create_plan(gmmnlse_plan** out, int P, int N, int M, double dt, doubl
                        double f_R, const double* h_R, double omega0, double n2, const gmmnlse_options* opt) {
   if (!out) return GMMNLSE_EINVAL;
   *out = nullptr;
-  gmmnlse_options o = {0, 1, 1e-6, 0, 0, 0, 0, 0};
+  gmmnlse_options o = {0, 1, 1e-6, 0, 0, 0, 0, 0, 0};
   if (opt) o = *opt;
   if (P < 1 || N < 1 || M < 1 || n_beta < 1 || !beta || !S) return GMMNLSE_EINVAL;
   if (N & (N - 1)) return GMMNLSE_EINVAL;
@@ -2084,6 +2089,7 @@ static int create_plan(gmmnlse_plan** out, int P, int N, int M, double dt, doubl
   if (o.contraction != 0 && o.contraction != 1 && o.contraction != 3 && (o.contraction < 6 || o.contraction > 8))
     return GMMNLSE_EINVAL;
   if (o.graph < 0 || o.graph > 1) return GMMNLSE_EINVAL;
+  if (o.stop_rule < 0 || o.stop_rule > 1) return GMMNLSE_EINVAL;
   if (o.shock && M_PI / dt >= omega0) return GMMNLSE_EINVAL;
   if (!(o.tol > 0)) o.tol = 1e-6;
   for (long long i = 0; i < (long long)P * n_beta; ++i)
@@ -2120,6 +2126,7 @@ static int create_plan(gmmnlse_plan** out, int P, int N, int M, double dt, doubl
   pl->contraction = o.contraction;
   pl->raman = o.raman;
   pl->graph = o.graph;
+  pl->stop_rule = o.stop_rule;
   if (cudaGetDevice(&pl->device) != cudaSuccess) { delete pl; g_cuda_err = "cudaGetDevice failed"; return GMMNLSE_ECUDA; }
   pl->general = general;
   pl->gen_complex = general && tensors_complex;

@@ -897,9 +897,24 @@ struct LoopStats {
   int it, noconv;
   long long iters;
   double last_err;
+  double err_prev, rho_prev;     // stop_rule 1: previous error and previous ratio of this large step
 };
+// convergence decision shared by the host loop and the device loop: err < tol, or (stop_rule 1, it >= 3) the
+// a-posteriori bound err rho / (1 - rho) < tol with rho the larger of the last two error ratios (reading S25)
+__host__ __device__ inline bool mpa_converged(double err, double tol, int stop_rule, int it, double err_prev,
+                                              double rho_prev, double* rho_out) {
+  const double rho_now = err_prev > 0.0 ? err / err_prev : 0.0;
+  *rho_out = rho_now;
+  if (err < tol) return true;
+  if (stop_rule == 1 && it >= 3) {
+    const double rho = rho_now > rho_prev ? rho_now : rho_prev;
+    if (rho < 1.0 && err * rho / (1.0 - rho) < tol) return true;
+  }
+  return false;
+}
 __global__ void k_err_finalize_loop(double* __restrict__ errbuf, int Mc, double* __restrict__ out, double tol, int cap,
-                                    int fixed, cudaGraphConditionalHandle handle, LoopStats* __restrict__ st) {
+                                    int fixed, cudaGraphConditionalHandle handle, LoopStats* __restrict__ st,
+                                    int stop_rule) {
   pdl_prologue();
   const double e = err_max_over_planes(errbuf, Mc);
   if (threadIdx.x == 0) {
@@ -912,7 +927,12 @@ __global__ void k_err_finalize_loop(double* __restrict__ errbuf, int Mc, double*
     if (fixed) {
       cont = it < cap;
     } else {
-      const bool conv = e < tol;
+      const bool first = it == 1;                        // st->it was zeroed at the head of the large step
+      double rho = 0.0;
+      const bool conv = mpa_converged(e, tol, stop_rule, it, first ? 1e300 : st->err_prev, first ? 1e300 : st->rho_prev,
+                                      &rho);
+      st->err_prev = e;
+      st->rho_prev = first ? 1e300 : rho;
       cont = !conv && it < cap;
       if (!conv && !cont) st->noconv += 1;
     }

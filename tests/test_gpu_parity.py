@@ -383,6 +383,36 @@ def test_device_loop_on_a_user_stream_and_under_profiling(B):
 
 
 # ----------------------------------------------------------------------------------- edge cases
+@pytest.mark.parametrize("cfg,kw", [(2, dict(N=1024, L=60 * 50e-6)), (4, dict(N=1024, L=60 * 50e-6))])
+def test_aposteriori_stop_rule_vs_oracle_and_default(B, cfg, kw):
+    """options.stop_rule = 1 (reading S25): the same decision on the device (CUDA-graph loop) and on the host, bit for
+    bit; iteration counts follow the oracle's with the same rule (within one per large step) and are fewer than the
+    default's; the field stays within tol-level distance of the default result and on the oracle's."""
+    w = W.make_config(cfg, **kw)
+    f_dev, _, st_dev, loop_dev, _ = _run_loop(B, w, 0, stop_rule=1)
+    f_host, _, st_host, loop_host, _ = _run_loop(B, w, 1, stop_rule=1)
+    assert loop_dev == 1 and loop_host == 0
+    assert np.array_equal(f_dev, f_host)
+    assert st_dev["iterations"] == st_host["iterations"] and st_dev["not_converged"] == 0
+    f_def, _, st_def, _, _ = _run_loop(B, w, 0)
+    assert st_dev["iterations"] <= st_def["iterations"] and st_dev["large_steps"] == st_def["large_steps"]
+    assert rel(f_dev, f_def) <= 5e-6
+    A_in = w.A0.astype(np.complex64).astype(np.complex128)
+    ost, ost0 = {}, {}
+    ref = O.mpa_propagate(A_in, w.L, w.dz, w.M, w.beta, w.S, w.kappa, w.omega0, w.f_R, w.h_R, w.dt, shock=w.shock,
+                          tol=w.tol, stats=ost, stop_rule=1)
+    O.mpa_propagate(A_in, w.L, w.dz, w.M, w.beta, w.S, w.kappa, w.omega0, w.f_R, w.h_R, w.dt, shock=w.shock,
+                    tol=w.tol, stats=ost0)
+    assert abs(st_dev["iterations"] - ost["iterations"]) <= ost["large_steps"]
+    # where the rule saves iterations for the oracle (config 2: one per large step) it does on the GPU
+    if ost0["iterations"] - ost["iterations"] >= ost["large_steps"]:
+        assert st_dev["iterations"] < st_def["iterations"]
+    assert rel(f_dev, ref) <= 1e-4
+    with pytest.raises(B.GmmnlseError) as e:
+        B.plan_from_workload(w, stop_rule=2)
+    assert e.value.status == B.EINVAL
+
+
 def test_zero_length_is_identity(B):
     w = W.make_config(2, N=256)
     w.L = 0.0

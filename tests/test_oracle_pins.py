@@ -529,3 +529,39 @@ def test_overlap_tensor_closed_forms_and_symmetries():
     assert np.allclose(O.overlap_tensor(Fr, 0.3), O.overlap_tensor_literal(Fr, 0.3), rtol=1e-13, atol=0)
     # scale invariance: the normalisation removes the units of F
     assert np.allclose(O.overlap_tensor(7.0 * Fr, 0.3), O.overlap_tensor(Fr, 0.3), rtol=1e-13, atol=0)
+
+
+def test_aposteriori_stop_rule_keeps_the_result_within_tol_and_saves_iterations():
+    """Reading S25: stopping on the a-posteriori bound err rho / (1 - rho) instead of the raw difference of the last
+    two iterates.  (i) the bound holds: at every iteration the distance of the iterate to the fixed point (taken from a
+    run converged to 1e-13) is below it; (ii) the propagated field differs from the S12 result by less than tol;
+    (iii) it never takes more iterations, and fewer where the last S12 iteration only confirmed convergence."""
+    wl = W.make_config(2, N=256, max_group=1)
+    args = (wl.beta, wl.S, wl.kappa, wl.omega0, wl.f_R, wl.h_R, wl.dt)
+    omega = O.omega_grid(wl.N, wl.dt)
+    D = O.dispersion_operator(wl.beta, omega)
+    K = 1j * wl.kappa * (1 + omega / wl.omega0)
+    nlt = lambda A: O.nonlinear_term(A, wl.S, wl.f_R, wl.h_R, wl.dt)
+    psi0 = O.to_freq(3.0 * wl.A0)                                   # stronger nonlinearity: more iterations to look at
+    hist, keep = [], []
+    O.mpa_large_step(psi0, 10, wl.dz, D, nlt, K, tol=1e-13, history=hist, planes_out=keep)
+    star = keep[0]
+    dist = [max(np.linalg.norm(h[j] - star[j]) / np.linalg.norm(star[j]) for j in range(1, 11)) for h in hist]
+    errs = [max(np.linalg.norm(hist[i][j] - (hist[i - 1][j] if i else psi0)) / np.linalg.norm(hist[i][j])
+                for j in range(1, 11)) for i in range(len(hist))]
+    for i in range(2, len(hist) - 2):
+        rho = max(errs[i] / errs[i - 1], errs[i - 1] / errs[i - 2])      # the ratios alternate: take the larger
+        assert rho < 1 and dist[i] <= errs[i] * rho / (1 - rho), i
+        assert dist[i] < errs[i]                                     # the raw difference over-estimates the error
+    L = 6 * 10 * wl.dz
+    s0, s1 = {}, {}
+    ref = O.mpa_propagate(wl.A0, L, wl.dz, 10, *args, tol=1e-6, stats=s0)
+    got = O.mpa_propagate(wl.A0, L, wl.dz, 10, *args, tol=1e-6, stats=s1, stop_rule=1)
+    assert rel(got, ref) < 1e-6 and s1["not_converged"] == 0
+    assert s1["iterations"] < s0["iterations"] and s1["large_steps"] == s0["large_steps"]
+    # never more iterations, whatever the strength of the nonlinearity
+    for amp in (0.3, 3.0):
+        a0, a1 = {}, {}
+        r0 = O.mpa_propagate(amp * wl.A0, L, wl.dz, 10, *args, tol=1e-6, stats=a0)
+        r1 = O.mpa_propagate(amp * wl.A0, L, wl.dz, 10, *args, tol=1e-6, stats=a1, stop_rule=1)
+        assert a1["iterations"] <= a0["iterations"] and rel(r1, r0) < 1e-6
