@@ -351,6 +351,14 @@ def run_gpu(args):
                 "iterations_per_large_step": round(lr["iters"] / max(lr["large"], 1), 3)}
         except binding.GmmnlseError as exc:
             out["variants"]["lowrank_contraction"] = {"unavailable": str(exc)}
+        try:                                         # NEXT-4: the same dense product with S2's zero blocks skipped
+            sp = measure(cfg, K, Wm, with_events=False, contraction=9)
+            out["variants"]["block_sparse_contraction"] = {
+                "value": round(sp["z_steps"] / (sp["ms"] * 1e-3), 2), "unit": UNIT, "ms_per_step": round(sp["ms"] / K, 4),
+                "contraction_kind": sp["ckind"],
+                "iterations_per_large_step": round(sp["iters"] / max(sp["large"], 1), 3)}
+        except binding.GmmnlseError as exc:
+            out["variants"]["block_sparse_contraction"] = {"unavailable": str(exc)}
         # reading S25: the a-posteriori stopping rule, same dense contraction; reported beside the headline
         # with its own iteration count (SURVEY.md reading S11/S12: variants of the iteration are allowed if both are)
         ap = measure(cfg, K, Wm, with_events=False, stop_rule=1)

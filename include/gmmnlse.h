@@ -53,9 +53,16 @@ typedef struct {                /* pass NULL for defaults                       
                                    8 = the same on the kind::f16 kernel: S_(pl),(mn) = sum_k L_(pl),k L_(mn),k
                                    by pivoted Cholesky at plan time (Eq. 2 makes S a Gram matrix; rank 153 of
                                    1035 for 45 Hermite-Gauss modes), two GEMMs Q x R and R x Q instead of Q x Q;
-                                   EUNSUPPORTED if S is not positive semi-definite.  Never chosen by auto:
-                                   BASELINE.json names the dense contraction.  3-8 need complex64 and
-                                   N % 128 == 0, else EUNSUPPORTED.  Other values: EINVAL                */
+                                   EUNSUPPORTED if S is not positive semi-definite;
+                                   9 = block-sparse form of the dense product on the kind::f16 kernel: the packed
+                                   pairs fall into classes that S never couples (the parities of F_p F_l in x and
+                                   y for Hermite-Gauss modes: Eq. 2's integrand is odd otherwise), found at plan
+                                   time as the connected components of |S2| > 1e-13 max|S2|; operands are stored
+                                   in class order and every output tile multiplies only its own class's blocks
+                                   (about 1/4 of the multiply-adds for a GRIN fibre).  Same result as 7 up to the
+                                   dropped entries; EUNSUPPORTED if there is one class only or on a general plan.
+                                   6, 8, 9 are never chosen by auto: BASELINE.json names the dense contraction.
+                                   3-9 need complex64 and N % 128 == 0, else EUNSUPPORTED.  Other values: EINVAL */
   int    raman;                 /* a5 kernel: 0 = auto, 1 = FFT . h~_R . IFFT on the pair streams (any h_R),
                                    2 = one-pole recurrence along t, exact when the samples are a damped
                                    oscillation h_R[j] = Im(c zeta^j) (the tau1/tau2 form); auto picks 2 when
@@ -239,12 +246,15 @@ int gmmnlse_debug_pairs(gmmnlse_plan *plan, const void *A, void *V, int n_planes
  *          [n_planes][Q][N] real of the plan's precision, U must not alias V.
  *   contraction_kind: which a6 kernel the plan selected (the values of options.contraction): 1 CUDA cores,
  *          3 tcgen05 3xTF32, 6 low-rank pair of 3xTF32 GEMMs, 7 tcgen05 kind::f16 on fp16 hi/lo splits,
- *          8 low-rank pair of kind::f16 GEMMs.  With 7 and 8 debug_pairs still writes fp32 V, and
+ *          8 low-rank pair of kind::f16 GEMMs, 9 block-sparse kind::f16.  With 7 and 8 debug_pairs still writes fp32 V, and
  *          debug_contract splits the caller's fp32 V into fp16 pairs first (scaled by its own max |V|).                                                            */
 int gmmnlse_debug_contract(gmmnlse_plan *plan, const void *V, void *U, int n_planes);
 int gmmnlse_contraction_kind(const gmmnlse_plan *plan);
 /*   lowrank_rank: rank R of the factorisation when contraction_kind is 6 or 8, else 0.            */
 int gmmnlse_lowrank_rank(const gmmnlse_plan *plan);
+/*   sparse_info: contraction_kind 9: number of uncoupled classes of packed pairs and the fraction of the dense
+ *          multiply-adds the block-sparse form executes (padding included); otherwise 0 and 1.  Pointers may be NULL. */
+int gmmnlse_sparse_info(const gmmnlse_plan *plan, int *classes, double *work_fraction);
 /*   loop_kind: how the MPA iteration loop of the last gmmnlse_propagate ran: 1 = on the device (CUDA-graph
  *          WHILE node, options.graph = 0), 0 = host loop only so far, -1 = the graph could not be built on this
  *          driver and the plan fell back to the host loop (gmmnlse_last_cuda_error() says why).          */

@@ -69,6 +69,7 @@ SIGNATURES = {
     "gmmnlse_contraction_kind": (C.c_int, [C.c_void_p]),
     "gmmnlse_raman_kind": (C.c_int, [C.c_void_p]),
     "gmmnlse_lowrank_rank": (C.c_int, [C.c_void_p]),
+    "gmmnlse_sparse_info": (C.c_int, [C.c_void_p, C.POINTER(C.c_int), _DP]),
     "gmmnlse_loop_kind": (C.c_int, [C.c_void_p]),
     "gmmnlse_debug_set_tc_chunk": (C.c_int, [C.c_void_p, C.c_int]),
     "gmmnlse_overlap_tensor": (C.c_int, [C.c_int, C.c_longlong, _DP, C.c_double, _DP]),
@@ -274,6 +275,12 @@ class Plan:
 
     def lowrank_rank(self) -> int:
         return int(self._lib.gmmnlse_lowrank_rank(self._h))
+
+    def sparse_info(self) -> dict:
+        """contraction 9: {classes, work_fraction} of the block-sparse form (0 and 1.0 otherwise)."""
+        c, f = C.c_int(), C.c_double()
+        _check(self._lib, self._lib.gmmnlse_sparse_info(self._h, C.byref(c), C.byref(f)))
+        return dict(classes=c.value, work_fraction=f.value)
 
     def loop_kind(self) -> int:
         return int(self._lib.gmmnlse_loop_kind(self._h))

@@ -68,6 +68,12 @@ struct Params {
   float bound_gain;            // the A operand was scaled by v_scale(bound_gain * *vbound)
   float zgain;                 // OUT_H: |Z| <= zgain * *vbound
   int Q, N, NT, KB, n_rt, t_tiles, total_tiles, plane0, stages, kchunk;
+  // block-sparse form (options.contraction = 9; all three null otherwise): r-tile rt only multiplies the k-blocks
+  // kb_begin[rt] .. + kb_count[rt] (>= 1) -- the rows and columns of the operands are permuted so that the non-zero
+  // blocks of S2 are contiguous -- and output row r of the permuted, padded row space goes to U row rowmap[r] (< 0: padding)
+  const int* kb_begin;
+  const int* kb_count;
+  const int* rowmap;
 };
 
 __host__ __device__ inline int b_bytes(int NT) { return NT * BK * 2; }
@@ -76,7 +82,10 @@ inline size_t smem_bytes(int NT, int stages) {
   return 1024 /*alignment slack*/ + 1024 /*barriers*/ + (size_t)stages * stage_bytes(NT);
 }
 
-template <bool OUT_H>
+// SPARSE = false compiles the three tables away: the dense instantiations are the code they were before r02's
+// block-sparse form (the row map inside the unrolled store loop cost the dense kernel 0.80 -> 0.99 ms when it was a
+// run-time branch).
+template <bool OUT_H, bool SPARSE = false>
 __global__ void __launch_bounds__(NTHREADS, 1)
 k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ CUtensorMap tmVl,
              const __grid_constant__ CUtensorMap tmSh, const __grid_constant__ CUtensorMap tmSl, const Params p) {
@@ -136,7 +145,8 @@ k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ C
         const int pl = tile / tiles_per_plane, rem = tile - pl * tiles_per_plane;
         const int tt = rem / p.n_rt, rt = rem - tt * p.n_rt;
         const int t0 = tt * TM, r0 = rt * p.NT;
-        for (int kb = 0; kb < p.KB; ++kb) {
+        const int k0 = SPARSE ? p.kb_begin[rt] : 0, kn = SPARSE ? p.kb_count[rt] : p.KB;
+        for (int kb = k0; kb < k0 + kn; ++kb) {
           mbar_wait(bar_empty + 8 * stage, phase ^ 1u, 1);
           const uint32_t fb = bar_full + 8 * stage;
           const uint32_t sa = tiles_addr + stage * sbytes;
@@ -160,7 +170,8 @@ k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ C
       int stage = 0, acc = 0;
       uint32_t phase = 0, acc_phase = 0;
       for (int tile = cta; tile < p.total_tiles; tile += nctas) {
-        for (int kb = 0, inchunk = 0; kb < p.KB; ++kb) {
+        const int kn = SPARSE ? p.kb_count[tile % p.n_rt] : p.KB;   // r-tile index is the fastest tile coordinate
+        for (int kb = 0, inchunk = 0; kb < kn; ++kb) {
           if (inchunk == 0) {                                      // new chunk: claim a TMEM accumulator
             mbar_wait(bar_tempty + 8 * acc, acc_phase ^ 1u, 2);
             tc_fence_after();
@@ -183,7 +194,7 @@ k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ C
           }
           mma_commit<1>(bar_empty + 8 * stage);
           if (++stage == stages) { stage = 0; phase ^= 1u; }
-          if (++inchunk == p.kchunk || kb == p.KB - 1) {           // chunk complete: hand it to the epilogue
+          if (++inchunk == p.kchunk || kb == kn - 1) {             // chunk complete: hand it to the epilogue
             mma_commit<1>(bar_tfull + 8 * acc);
             inchunk = 0;
             if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
@@ -198,7 +209,6 @@ k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ C
     const int cper = ((p.NT + 2) / 3 + 7) / 8 * 8;
     const int cbeg = third * cper;
     const int ncols = max(0, min(p.NT, cbeg + cper) - cbeg);       // multiple of 8, <= EPI_COLS
-    const int nchunks = (p.KB + p.kchunk - 1) / p.kchunk;
     const float vb = *p.vbound;
     const float inv_sv = v_scale(p.bound_gain * vb, true);
     const float sz = OUT_H ? v_scale(p.zgain * vb, false) : 1.f;
@@ -211,6 +221,7 @@ k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ C
       const int t = tt * TM + lg * 32 + lane;
 #pragma unroll
       for (int i = 0; i < EPI_COLS; ++i) accr[i] = 0.f;
+      const int nchunks = ((SPARSE ? p.kb_count[rt] : p.KB) + p.kchunk - 1) / p.kchunk;
       for (int ch = 0; ch < nchunks; ++ch) {
         mbar_wait(bar_tfull + 8 * acc, acc_phase, 5);
         tc_fence_after();
@@ -256,7 +267,14 @@ k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ C
 #pragma unroll
         for (int c = 0; c < EPI_COLS; ++c) {
           const int r = rbase + c;
-          if (c < ncols && r < p.Q) Uout[(long long)r * p.N] = accr[c] * (rs[c] * inv_sv);
+          if constexpr (SPARSE) {
+            if (c < ncols) {
+              const int rn = p.rowmap[r];
+              if (rn >= 0) Uout[(long long)rn * p.N] = accr[c] * (rs[c] * inv_sv);
+            }
+          } else {
+            if (c < ncols && r < p.Q) Uout[(long long)r * p.N] = accr[c] * (rs[c] * inv_sv);
+          }
         }
       }
     }

@@ -212,6 +212,7 @@ struct gmmnlse_plan {
   virtual int set_tc_chunk(int k) = 0;
   virtual int raman_kind() const = 0;
   virtual int lowrank_rank() const = 0;
+  virtual int sparse_info(int* classes, double* work_fraction) const = 0;
   virtual void drop_loop_graph() = 0;
 };
 
@@ -304,6 +305,12 @@ struct PlanT final : gmmnlse_plan {
   };
   bool tc_h = false;
   HGemm hg, hl1, hl2;
+  // block-sparse form (options.contraction = 9): classes of packed pairs that S2 does not couple
+  bool sparse = false;
+  int sp_classes = 0, sp_Qv = 0;             // number of classes; rows of the class-ordered, padded V planes
+  int *sp_kb_begin = nullptr, *sp_kb_count = nullptr, *sp_rowmap = nullptr, *sp_vrow = nullptr;
+  T* Vsp = nullptr;                          // [(M+1)][sp_Qv][N] (as fp16 hi rows then lo rows per plane)
+  double sp_work_fraction = 1.0;             // executed / dense multiply-adds
   float* d_vbound = nullptr;   // device scalar: bound on |V| of the current launch
   float v_gain = 1.f;          // |V| <= v_gain max |A|^2
   HalfOut cur_ho = {nullptr, 0, 0, 0, nullptr};
@@ -345,7 +352,8 @@ struct PlanT final : gmmnlse_plan {
     if (cap_stream) cudaStreamDestroy(cap_stream);
     cudaFree(d_stats);
     if (h_stats) cudaFreeHost(h_stats);
-    cudaFree(gfwd); cudaFree(ginv); cudaFree(Qc); cudaFree(Xconst); cudaFree(Xext); cudaFree(Epair); cudaFree(fprof_d); cudaFree(d_step2); cudaFree(shard_pre); cudaFree(st_kind); cudaFree(st_wk); cudaFree(st_wr); cudaFree(iir_zp); cudaFree(pair_work); cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
+    cudaFree(gfwd); cudaFree(ginv); cudaFree(Qc); cudaFree(Xconst); cudaFree(Xext); cudaFree(Epair); cudaFree(fprof_d); cudaFree(d_step2); cudaFree(shard_pre);
+    cudaFree(sp_kb_begin); cudaFree(sp_kb_count); cudaFree(sp_rowmap); cudaFree(sp_vrow); cudaFree(Vsp); cudaFree(st_kind); cudaFree(st_wk); cudaFree(st_wr); cudaFree(iir_zp); cudaFree(pair_work); cudaFree(rk_X); cudaFree(rk_AI); cudaFree(rk_K1); cudaFree(rk_K2); cudaFree(rk_K3); cudaFree(EH_d);
     if (h_err) cudaFreeHost(h_err);
     if (h_in) cudaFreeHost(h_in);
     if (h_out) cudaFreeHost(h_out);
@@ -718,10 +726,11 @@ struct PlanT final : gmmnlse_plan {
     }
   }
   // ------------------------------------------------------------------ kind::f16 form (gemm_h.cuh)
-  int h_build(HGemm& g, const std::vector<double>& mat, int rows, int K, int smax) {
+  int h_build(HGemm& g, const std::vector<double>& mat, int rows, int K, int smax, int force_NT = 0) {
     g.rows = rows; g.K = K;
     g.nrt = (rows + 207) / 208;
     g.NT = (((rows + g.nrt - 1) / g.nrt) + 15) / 16 * 16;
+    if (force_NT > 0) { g.NT = force_NT; g.nrt = (rows + force_NT - 1) / force_NT; }
     g.KB = (K + hc::BK - 1) / hc::BK;
     g.stages = hc::MAX_STAGES;
     while (g.stages > 1 && hc::smem_bytes(g.NT, g.stages) > (size_t)smax) --g.stages;
@@ -783,6 +792,8 @@ struct PlanT final : gmmnlse_plan {
       prm.t_tiles = N / hc::TM;
       prm.total_tiles = planes * prm.t_tiles * g.nrt;
       prm.plane0 = plane0; prm.stages = g.stages;
+      const bool sp = sparse && &g == &hg;
+      if (sp) { prm.kb_begin = sp_kb_begin; prm.kb_count = sp_kb_count; prm.rowmap = sp_rowmap; }
       prm.kchunk = tc_kchunk;                                    // k-blocks of 32 q here (16 q in the TF32 forms)
       cudaLaunchConfig_t cfg = {};
       cfg.gridDim = dim3((unsigned)std::min(n_sm, prm.total_tiles));
@@ -792,6 +803,7 @@ struct PlanT final : gmmnlse_plan {
       pdl_config(cfg);
       prof_begin(GMMNLSE_KIND_CONTRACT);
       cudaError_t e = outZ ? cudaLaunchKernelEx(&cfg, hc::k_contract_h<true>, mhi, mlo, g.tmHi, g.tmLo, prm)
+                      : sp ? cudaLaunchKernelEx(&cfg, hc::k_contract_h<false, true>, mhi, mlo, g.tmHi, g.tmLo, prm)
                            : cudaLaunchKernelEx(&cfg, hc::k_contract_h<false>, mhi, mlo, g.tmHi, g.tmLo, prm);
       prof_end();
       GM_CUDA(e);
@@ -879,6 +891,80 @@ struct PlanT final : gmmnlse_plan {
     return 0;
   }
 
+  // Block-sparse form of the dense contraction: the packed pairs fall into classes that S2 never couples (for the
+  // Hermite-Gauss modes of a GRIN fibre: the four parities of the pair function F_p F_l in x and y; Eq. 2's integrand
+  // is odd otherwise).  Classes = connected components of the graph r ~ q <=> |S2[r][q]| > 1e-13 max|S2| (union-find).
+  // The operand is rebuilt with rows and columns in class order, each class's rows padded to whole r-tiles and its
+  // columns to whole k-blocks, so an r-tile multiplies only its own class's k-blocks; the result is the dense
+  // product up to the dropped entries (< 1e-13 of the largest).  One class only: EUNSUPPORTED (nothing to skip).
+  int init_sparse(const std::vector<double>& h_S2, int smax) {
+    double amax = 0;
+    for (double v : h_S2) amax = std::fmax(amax, std::fabs(v));
+    const double thr = 1e-13 * amax;
+    std::vector<int> parent(Q);
+    for (int i = 0; i < Q; ++i) parent[i] = i;
+    auto find = [&](int x) { while (parent[x] != x) { parent[x] = parent[parent[x]]; x = parent[x]; } return x; };
+    for (int r = 0; r < Q; ++r)
+      for (int q = 0; q < Q; ++q)
+        if (std::fabs(h_S2[(size_t)r * Q + q]) > thr) { const int a = find(r), b = find(q); if (a != b) parent[a] = b; }
+    std::map<int, std::vector<int>> comp;
+    for (int i = 0; i < Q; ++i) comp[find(i)].push_back(i);
+    if (comp.size() < 2) return GMMNLSE_EUNSUPPORTED;
+    std::vector<std::vector<int>> cls;
+    for (auto& kv : comp) cls.push_back(kv.second);
+    sp_classes = (int)cls.size();
+    // tile height: the multiple of 16 in [16, 208] with the least cost.  Every r-tile re-reads its class's V k-blocks
+    // (16 KB each: the shared-memory traffic of 128 rows of S2) and pays a drain per chunk, so a tile costs about
+    // (NT + 128) per k-block, not NT: small tiles lose (NT = 16 measured 1.5x SLOWER than the dense form).
+    int best_NT = 208;
+    double best = 1e300, best_work = 0;
+    for (int nt = 16; nt <= 208; nt += 16) {
+      double cost = 0, work = 0;
+      for (auto& c : cls) {
+        const double tiles = (double)((c.size() + nt - 1) / nt), kq = (double)((c.size() + hc::BK - 1) / hc::BK * hc::BK);
+        cost += tiles * (nt + 128) * kq;
+        work += tiles * nt * kq;
+      }
+      if (cost <= best) { best = cost; best_NT = nt; best_work = work; }
+    }
+    sp_work_fraction = best_work / ((double)Q * Q);
+    int Rp = 0, Kp = 0;
+    std::vector<int> kb0, kbn, rowmap, vrow(Q, 0);
+    for (auto& c : cls) {
+      const int tiles = ((int)c.size() + best_NT - 1) / best_NT, kblocks = ((int)c.size() + hc::BK - 1) / hc::BK;
+      for (int t = 0; t < tiles; ++t) { kb0.push_back(Kp / hc::BK); kbn.push_back(kblocks); }
+      for (int i = 0; i < tiles * best_NT; ++i) rowmap.push_back(i < (int)c.size() ? c[i] : -1);
+      for (int i = 0; i < (int)c.size(); ++i) vrow[c[i]] = Kp + i;
+      Rp += tiles * best_NT;
+      Kp += kblocks * hc::BK;
+    }
+    sp_Qv = Kp;
+    std::vector<double> mat((size_t)Rp * Kp, 0.0);
+    for (int rr = 0; rr < Rp; ++rr) {
+      if (rowmap[rr] < 0) continue;
+      const double* src = &h_S2[(size_t)rowmap[rr] * Q];
+      for (int q = 0; q < Q; ++q)
+        if (std::fabs(src[q]) > thr) mat[(size_t)rr * Kp + vrow[q]] = src[q];
+    }
+    GM_TRY(h_build(hg, mat, Rp, Kp, smax, best_NT));
+    GM_TRY(dalloc(&sp_kb_begin, kb0.size())); GM_TRY(upload(sp_kb_begin, kb0));
+    GM_TRY(dalloc(&sp_kb_count, kbn.size())); GM_TRY(upload(sp_kb_count, kbn));
+    GM_TRY(dalloc(&sp_rowmap, rowmap.size())); GM_TRY(upload(sp_rowmap, rowmap));
+    GM_TRY(dalloc(&sp_vrow, vrow.size())); GM_TRY(upload(sp_vrow, vrow));
+    GM_TRY(dalloc(&Vsp, (size_t)(M + 1) * sp_Qv * N));
+    GM_CUDA(cudaMemset(Vsp, 0, sizeof(T) * (size_t)(M + 1) * sp_Qv * N));     // the padding rows stay zero for good
+    GM_TRY(dalloc(&d_vbound, 1));
+    GM_CUDA(cudaMemset(d_vbound, 0, sizeof(float)));
+    GM_TRY(h_a_tmaps(&tmVh, &tmVl, Vsp, sp_Qv, M + 1));
+    if constexpr (sizeof(T) == 4) {
+      GM_TRY(ensure_smem(hc::k_contract_h<false, true>, (size_t)smax));
+      GM_TRY(ensure_smem(hc::k_contract_h<false>, (size_t)smax));
+    }
+    tc_h = true;
+    sparse = true;
+    return 0;
+  }
+
   int init_tc(const std::vector<double>& h_S2) {
     if constexpr (sizeof(T) != 4) {
       if (contraction >= 2) return GMMNLSE_EUNSUPPORTED;
@@ -898,6 +984,14 @@ struct PlanT final : gmmnlse_plan {
         GM_CUDA(cudaDeviceGetAttribute(&smax0, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev0));
         GM_TRY(h_build(hg, h_S2, Q, Q, smax0));
         return init_h_common(smax0);
+      }
+      if (contraction == 9) {                          // block-sparse form (NEXT-4), scalar-mode path only
+        if (general || N % hc::TM != 0) return GMMNLSE_EUNSUPPORTED;
+        int dev0 = 0, smax0 = 0;
+        GM_CUDA(cudaGetDevice(&dev0));
+        GM_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev0));
+        GM_CUDA(cudaDeviceGetAttribute(&smax0, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev0));
+        return init_sparse(h_S2, smax0);
       }
       if (contraction == 6 || contraction == 8) {      // exact low-rank form (NEXT-4), scalar-mode path only
         if (general || N % tc::TM != 0) return GMMNLSE_EUNSUPPORTED;
@@ -1032,7 +1126,12 @@ struct PlanT final : gmmnlse_plan {
         launch_k(k_bound_field<T>, dim3(32, planes), 256, 0, A, a_ps, PN, v_gain, d_vbound);
         prof_end();
         GM_CUDA(cudaGetLastError());
-        cur_ho = HalfOut{reinterpret_cast<__half*>(Vout), 2 * QN, QN, N, d_vbound};
+        if (sparse) {                               // class-ordered, padded rows in the plan's Vsp planes
+          const long long vq = (long long)sp_Qv * N;
+          cur_ho = HalfOut{reinterpret_cast<__half*>(Vsp + ((Vout - V) / QN) * vq), 2 * vq, vq, N, d_vbound, sp_vrow};
+        } else {
+          cur_ho = HalfOut{reinterpret_cast<__half*>(Vout), 2 * QN, QN, N, d_vbound};
+        }
       }
     }
     return launch_pairs_impl(A, a_ps, Vout, v_ps, planes);
@@ -1070,8 +1169,10 @@ struct PlanT final : gmmnlse_plan {
           GM_CUDA(cudaMemsetAsync(d_vbound, 0, sizeof(float), stream));
           prof_begin(GMMNLSE_KIND_CONTRACT);
           launch_k(k_bound_real<T>, 592, 256, 0, Vin, total, d_vbound);
+          const long long vq = (long long)sp_Qv * N;
           launch_k(k_v_encode, 1184, 256, 0, Vin, QN, total,
-                                               HalfOut{reinterpret_cast<__half*>(V), 2 * QN, QN, N, d_vbound});
+                   sparse ? HalfOut{reinterpret_cast<__half*>(Vsp), 2 * vq, vq, N, d_vbound, sp_vrow}
+                          : HalfOut{reinterpret_cast<__half*>(V), 2 * QN, QN, N, d_vbound});
           prof_end();
           GM_CUDA(cudaGetLastError());
         }
@@ -1795,10 +1896,15 @@ struct PlanT final : gmmnlse_plan {
     return launch_pairs((const C*)A, PN, (T*)Vout, QN, n_planes);
   }
   int contraction_kind() const override {
-    if (tc_h) return lowrank ? 8 : 7;
+    if (tc_h) return sparse ? 9 : (lowrank ? 8 : 7);
     return lowrank ? 6 : (tc_on ? 3 : 1);
   }
   int lowrank_rank() const override { return lowrank ? lr_R : 0; }
+  int sparse_info(int* classes, double* work_fraction) const override {
+    if (classes) *classes = sparse ? sp_classes : 0;
+    if (work_fraction) *work_fraction = sparse ? sp_work_fraction : 1.0;
+    return 0;
+  }
   int raman_kind() const override { return f_R == 0.0 ? 0 : (iir ? 2 : 1); }
   int set_tc_chunk(int k) override {
     if (k < 1 || k > 255) return GMMNLSE_EINVAL;
@@ -2086,7 +2192,7 @@ static int create_plan(gmmnlse_plan** out, int P, int N, int M, double dt, doubl
   if ((f_R != 0.0) != (h_R != nullptr)) return GMMNLSE_EINVAL;
   if (o.precision != 0 && o.precision != 1) return GMMNLSE_EINVAL;
   if (o.raman < 0 || o.raman > 2) return GMMNLSE_EINVAL;
-  if (o.contraction != 0 && o.contraction != 1 && o.contraction != 3 && (o.contraction < 6 || o.contraction > 8))
+  if (o.contraction != 0 && o.contraction != 1 && o.contraction != 3 && (o.contraction < 6 || o.contraction > 9))
     return GMMNLSE_EINVAL;
   if (o.graph < 0 || o.graph > 1) return GMMNLSE_EINVAL;
   if (o.stop_rule < 0 || o.stop_rule > 1) return GMMNLSE_EINVAL;
@@ -2345,6 +2451,10 @@ int gmmnlse_contraction_kind(const gmmnlse_plan* plan) { return plan ? plan->con
 int gmmnlse_raman_kind(const gmmnlse_plan* plan) { return plan ? plan->raman_kind() : 0; }
 
 int gmmnlse_lowrank_rank(const gmmnlse_plan* plan) { return plan ? plan->lowrank_rank() : 0; }
+
+int gmmnlse_sparse_info(const gmmnlse_plan* plan, int* classes, double* work_fraction) {
+  return plan ? plan->sparse_info(classes, work_fraction) : GMMNLSE_EINVAL;
+}
 
 int gmmnlse_loop_kind(const gmmnlse_plan* plan) { return plan ? plan->loop_state : 0; }
 

@@ -56,10 +56,12 @@ struct HalfOut {
   long long lo_offset;         // halves from a hi row to its lo row (Q N)
   int N;
   const float* vbound;
+  const int* vrow;             // block-sparse form: stream q is stored at row vrow[q] (class order); null = row q
+  __device__ __forceinline__ long long row(long long q) const { return vrow ? (long long)vrow[q] : q; }
   __device__ __forceinline__ void store(int j, int q, int n, float v) const {
     const float x = v * hc::v_scale(*vbound, false);
     const __half h = __float2half_rn(x);
-    __half* d = Vh + j * plane_stride + (long long)q * N + n;
+    __half* d = Vh + j * plane_stride + row(q) * N + n;
     d[0] = h;
     d[lo_offset] = __float2half_rn(x - __half2float(h));
   }
@@ -296,8 +298,9 @@ k_pair_iir(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restric
   __syncthreads();
   if (ho.Vh) {                                                // fp16 hi / lo pairs, two samples per thread and store
     const float sv = hc::v_scale(*ho.vbound, false);
-    __half2* h0 = reinterpret_cast<__half2*>(ho.Vh + j * ho.plane_stride + (long long)q0 * N);
-    __half2* l0 = reinterpret_cast<__half2*>(ho.Vh + j * ho.plane_stride + ho.lo_offset + (long long)q0 * N);
+    __half2* h0 = reinterpret_cast<__half2*>(ho.Vh + j * ho.plane_stride + ho.row(q0) * N);
+    __half2* l0 = reinterpret_cast<__half2*>(ho.Vh + j * ho.plane_stride + ho.lo_offset + ho.row(q0) * N);
+    const long long d1 = has1 ? (ho.row(q1) - ho.row(q0)) * (N / 2) : 0;        // half2 units from row q0 to row q1
 #pragma unroll 4
     for (int e = 0; e < 8; ++e) {
       const int n2 = tid + e * NT;                            // samples 2 n2, 2 n2 + 1
@@ -308,8 +311,8 @@ k_pair_iir(const cplx<T>* __restrict__ A, long long a_plane_stride, T* __restric
       h0[n2] = hh0;
       l0[n2] = __float22half2_rn(make_float2(s0.x - f0.x, s0.y - f0.y));
       if (has1) {
-        h0[N / 2 + n2] = hh1;
-        l0[N / 2 + n2] = __float22half2_rn(make_float2(s1.x - f1.x, s1.y - f1.y));
+        h0[d1 + n2] = hh1;
+        l0[d1 + n2] = __float22half2_rn(make_float2(s1.x - f1.x, s1.y - f1.y));
       }
     }
     return;
@@ -477,7 +480,7 @@ k_pair_iir_rows(const __grid_constant__ CUtensorMap tmA, int plane0, float* __re
           hi[k] = *reinterpret_cast<const uint32_t*>(&h);
           lo[k] = *reinterpret_cast<const uint32_t*>(&l);
         }
-        __half* row = obase + (s == 0 ? q0 : q1) * N;
+        __half* row = obase + ho.row(s == 0 ? q0 : q1) * N;
         stg256(row, hi);
         stg256(row + ho.lo_offset, lo);
       }

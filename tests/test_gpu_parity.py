@@ -488,6 +488,7 @@ def _packed_S2(S):
     (3, 1024, {}, 6), (4, 512, {}, 6), (5, 256, {}, 6),             # exact low-rank form (rank 45 / ~120 / 153)
     (3, 1024, {}, 7), (4, 512, {}, 7), (5, 256, {}, 7),             # kind::f16 on fp16 hi / lo splits (auto's choice)
     (3, 1024, {}, 8), (4, 512, {}, 8), (5, 256, {}, 8),             # low-rank form on the kind::f16 kernel
+    (3, 1024, {}, 9), (4, 512, {}, 9), (5, 256, {}, 9),             # block-sparse form (classes of uncoupled pairs)
     (3, 128, dict(max_group=3), 7),
     (3, 128, dict(max_group=3), 3),                                 # Q = 55 < 64: tensor path forced, N = 128
 ])
@@ -520,7 +521,7 @@ def test_contraction_vs_fp64_matmul(B, cfg, N, kw, kind):
     # operands go subnormal: an absolute floor of 2^-38 of that largest value per operand (
     # 2^-33 when the low-rank form's intermediate Z is scaled by its bound), i.e. 1e-9 of the largest column here.
     cerr, cref = np.linalg.norm(Uh - ref, axis=1), np.linalg.norm(ref, axis=1)
-    floor = 1e-9 * cref.max() if kind in (7, 8) else 0.0
+    floor = 1e-9 * cref.max() if kind in (7, 8, 9) else 0.0
     assert (cerr <= 3e-6 * cref + floor).all(), (cerr / cref).max()
 
 
@@ -545,6 +546,33 @@ def test_lowrank_form_rank_operator_and_propagation(B, kind):
     S_bad[0, 0, 0, 0] = -abs(S_bad[0, 0, 0, 0])
     with pytest.raises(B.GmmnlseError) as e:
         B.Plan(w.P, w.N, w.M, w.dt, w.dz, w.beta, S_bad, w.f_R, w.h_R, w.omega0, w.n2, contraction=6)
+    assert e.value.status == B.EUNSUPPORTED
+
+
+def test_block_sparse_form_classes_operator_and_propagation(B):
+    """NEXT-4: the dense contraction with the structurally zero blocks of S2 skipped.  Hermite-Gauss pair functions
+    F_p F_l have a parity in x and in y, and Eq. 2's integrand is odd unless the two pairs' parities agree: four classes,
+    about a quarter of the multiply-adds.  Same operator and the same propagated field as the dense form, and U comes
+    back in natural row order (the a7 kernels are untouched)."""
+    w = W.make_config(3, N=1024, L=2 * 10 * 100e-6)
+    with B.plan_from_workload(w, contraction=9) as plan:
+        info = plan.sparse_info()
+        # Q = 120: classes of 18-42 pairs padded to whole 32-wide k-blocks and 16-row tiles leave about half the work
+        assert plan.contraction_kind() == 9 and info["classes"] == 4 and 0.2 < info["work_fraction"] < 0.75
+    assert _nonlinear_op_case(B, w, contraction=9) <= TOL_OP
+    _, out9, _, st9 = _propagate(B, w, contraction=9)
+    _, out7, _, st7 = _propagate(B, w, contraction=7)
+    assert rel(out9, out7) <= 2e-6 and st9["iterations"] == st7["iterations"]
+    w5 = W.make_config(5, N=256)
+    with B.plan_from_workload(w5, contraction=9) as plan:
+        info = plan.sparse_info()
+        assert info["classes"] == 4 and 0.2 < info["work_fraction"] < 0.35
+    assert _nonlinear_op_case(B, w5, contraction=9) <= TOL_OP
+    # a tensor that couples every pair with every other has one class: nothing to skip
+    rng = np.random.default_rng(2)
+    Sd = w.S + 1e-3 * np.abs(w.S).max() * np.ones_like(w.S)
+    with pytest.raises(B.GmmnlseError) as e:
+        B.Plan(w.P, w.N, w.M, w.dt, w.dz, w.beta, Sd, w.f_R, w.h_R, w.omega0, w.n2, contraction=9)
     assert e.value.status == B.EUNSUPPORTED
 
 
