@@ -1220,21 +1220,26 @@ struct PlanT final : gmmnlse_plan {
   // TMA maps for the streaming a7: U (the plan's own buffer) and the field buffer seen as rows of float pairs
   CUtensorMap tmU7, tmA7;
   bool a7_maps = false;
+  // slice width: 16 samples when the slice is large anyway (Q >= 256: 64 B x Q >= 16 KB), else 64 (measured at
+  // Q = 120 / 210 with 16: the per-slice barrier and TMA issue cost more than the second read of U they save)
+  int a7_tw() const { return Q >= 256 ? 16 : 64; }
   int a7_nbox() const { return (Q + 255) / 256; }
   int a7_rows_box() const { return (((Q + a7_nbox() - 1) / a7_nbox()) + 1) & ~1; }   // even: 128-byte aligned TMA boxes
-  size_t a7_smem() const { return (size_t)2 * ((size_t)a7_nbox() * a7_rows_box() * 64 + (size_t)P * 128) + 16 + 128; }
+  size_t a7_smem() const {
+    return (size_t)2 * ((size_t)a7_nbox() * a7_rows_box() * 4 * a7_tw() + (size_t)P * 8 * a7_tw()) + 16 + 128;
+  }
   int a7_stream_setup() {
     if (a7_maps) return 0;
     {
       const cuuint64_t dims[3] = {(cuuint64_t)N, (cuuint64_t)Q, (cuuint64_t)(M + 1)};
       const cuuint64_t strides[2] = {(cuuint64_t)N * 4, (cuuint64_t)QN * 4};
-      const cuuint32_t box[3] = {16, (cuuint32_t)a7_rows_box(), 1};
+      const cuuint32_t box[3] = {(cuuint32_t)a7_tw(), (cuuint32_t)a7_rows_box(), 1};
       GM_TRY(encode_tmap_f32(&tmU7, (void*)U, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_NONE));
     }
     {
       const cuuint64_t dims[3] = {(cuuint64_t)2 * N, (cuuint64_t)P, (cuuint64_t)(M + 1)};
       const cuuint64_t strides[2] = {(cuuint64_t)N * 8, (cuuint64_t)PN * 8};
-      const cuuint32_t box[3] = {32, (cuuint32_t)P, 1};
+      const cuuint32_t box[3] = {(cuuint32_t)(2 * a7_tw()), (cuuint32_t)P, 1};
       GM_TRY(encode_tmap_f32(&tmA7, (void*)At, 3, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_NONE));
     }
     a7_maps = true;
@@ -1243,11 +1248,9 @@ struct PlanT final : gmmnlse_plan {
   // streaming a7 applies to the plan's own U and At planes of a complex64 scalar-mode plan with enough slices to
   // occupy the device and a slice pair that fits shared memory
   bool a7_streams(const T* Uin, const C* A, int planes) const {
-    // a slice is Q x 64 B: below ~16 KB (configs 3-4: 120 / 210 packed pairs) the per-slice barrier and TMA issue cost
-    // more than the second read they save (measured: config 3 16.0k -> 12.3k z-steps/s, config 4 8.4k -> 6.6k)
-    if (sizeof(T) != 4 || general || N % 16 != 0 || P > 256 || n_sm <= 0 || Q < 256) return false;
+    if (sizeof(T) != 4 || general || N % 64 != 0 || P > 256 || n_sm <= 0 || Q < 64) return false;
     if (!(Uin >= U && Uin < U + (size_t)(M + 1) * QN) || !(A >= At && A < At + (size_t)(M + 1) * PN)) return false;
-    return a7_smem() <= 200 * 1024 && (long long)planes * (N / 16) >= 4LL * n_sm;
+    return a7_smem() <= 200 * 1024 && (long long)planes * (N / a7_tw()) >= 4LL * n_sm;
   }
 
   int launch_mode_reduce(const T* Uin, const C* A, C* Nout, int planes) {
@@ -1255,18 +1258,22 @@ struct PlanT final : gmmnlse_plan {
       if (a7_streams(Uin, A, planes)) {
         GM_TRY(a7_stream_setup());
         const size_t smem = a7_smem();
-        GM_TRY(ensure_smem(k_mode_reduce_stream, smem));
-        const int n_slices = planes * (N / 16);
+        const int tw7 = a7_tw();
+        GM_TRY(tw7 == 16 ? ensure_smem(k_mode_reduce_stream<16>, smem) : ensure_smem(k_mode_reduce_stream<64>, smem));
+        const int n_slices = planes * (N / tw7);
         prof_begin(GMMNLSE_KIND_MODE_REDUCE);
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3((unsigned)std::min(n_sm, n_slices));
-        cfg.blockDim = dim3(16u * (unsigned)std::min(64, (P + 1) & ~1));     // one mode per thread up to P = 64
+        // one mode per thread where the block size allows (16-sample slices: up to P = 64; 64-sample: up to 16)
+        cfg.blockDim = dim3((unsigned)tw7 * (unsigned)std::min(1024 / tw7, (P + 1) & ~1));
         cfg.dynamicSmemBytes = smem;
         cfg.stream = stream;
         pdl_config(cfg);
-        cudaError_t e = cudaLaunchKernelEx(&cfg, k_mode_reduce_stream, tmU7, tmA7, (int)((Uin - U) / QN),
-                                           (int)((A - At) / PN), (float2*)Nout, PN, P, Q, N, n_slices, a7_nbox(),
-                                           a7_rows_box());
+        cudaError_t e = tw7 == 16
+            ? cudaLaunchKernelEx(&cfg, k_mode_reduce_stream<16>, tmU7, tmA7, (int)((Uin - U) / QN), (int)((A - At) / PN),
+                                 (float2*)Nout, PN, P, Q, N, n_slices, a7_nbox(), a7_rows_box())
+            : cudaLaunchKernelEx(&cfg, k_mode_reduce_stream<64>, tmU7, tmA7, (int)((Uin - U) / QN), (int)((A - At) / PN),
+                                 (float2*)Nout, PN, P, Q, N, n_slices, a7_nbox(), a7_rows_box());
         prof_end();
         GM_CUDA(e);
         return 0;

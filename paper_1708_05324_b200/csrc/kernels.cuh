@@ -622,6 +622,7 @@ k_mode_reduce(const T* __restrict__ U, long long u_plane_stride, const cplx<T>* 
 //   P = 64); accumulators in registers as above.
 //   tmU: U [planes][Q][N] fp32, box 16 x rows_box x 1;  tmA: field [planes][P][2 N floats], box 32 floats x P x 1.
 //   grid = min(#SM, slices), block = 16 G, dynamic smem = 2 (n_box rows_box 64 + P 128) + 16 (+ alignment).
+template <int TW>                                                     // samples per slice: 16 (large Q) or 64
 __global__ void __launch_bounds__(1024, 1)
 k_mode_reduce_stream(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmA, int plane0_u,
                      int plane0_a, float2* __restrict__ Nt, long long n_plane_stride, int P, int Q, int N,
@@ -633,10 +634,11 @@ k_mode_reduce_stream(const __grid_constant__ CUtensorMap tmU, const __grid_const
   const uint32_t base = (raw_addr + 127u) & ~127u;
   unsigned char* sm = smem_raw + (base - raw_addr);
   // U arrives as n_box boxes of rows_box rows (n_box rows_box >= Q; rows past Q are zero-filled by TMA)
-  const uint32_t u_bytes = (uint32_t)(n_box * rows_box) * 64u, a_bytes = (uint32_t)P * 128u, buf_bytes = u_bytes + a_bytes;
+  const uint32_t u_bytes = (uint32_t)(n_box * rows_box) * (4u * TW), a_bytes = (uint32_t)P * (8u * TW),
+                 buf_bytes = u_bytes + a_bytes;
   const uint32_t bars = base + 2 * buf_bytes;
-  const int tid = threadIdx.x, t = tid & 15, g = tid >> 4;
-  const int per_plane = N / 16;
+  const int tid = threadIdx.x, t = tid % TW, g = tid / TW;
+  const int per_plane = N / TW;
   if (tid == 0) {
     mbar_init(bars, 1);
     mbar_init(bars + 8, 1);
@@ -647,10 +649,10 @@ k_mode_reduce_stream(const __grid_constant__ CUtensorMap tmU, const __grid_const
   __syncthreads();
   pdl_wait();
   auto issue = [&](int slice, int b) {                               // one thread: fill buffer b with `slice`
-    const int pl = slice / per_plane, t0 = (slice - pl * per_plane) * 16;
+    const int pl = slice / per_plane, t0 = (slice - pl * per_plane) * TW;
     const uint32_t dst = base + b * buf_bytes, bar = bars + 8 * b;
     mbar_arrive_expect_tx(bar, buf_bytes);
-    for (int k = 0; k < n_box; ++k) tma_load_3d(dst + k * rows_box * 64, &tmU, bar, t0, rows_box * k, plane0_u + pl);
+    for (int k = 0; k < n_box; ++k) tma_load_3d(dst + k * rows_box * (4 * TW), &tmU, bar, t0, rows_box * k, plane0_u + pl);
     tma_load_3d(dst + u_bytes, &tmA, bar, 2 * t0, 0, plane0_a + pl);
   };
   int it = 0;
@@ -662,22 +664,22 @@ k_mode_reduce_stream(const __grid_constant__ CUtensorMap tmU, const __grid_const
     mbar_wait(bars + 8 * b, (uint32_t)((it >> 1) & 1), 21);
     const float* us = reinterpret_cast<const float*>(sm + b * buf_bytes) + t;
     const float2* as = reinterpret_cast<const float2*>(sm + b * buf_bytes + u_bytes) + t;
-    const int pl = slice / per_plane, t0 = (slice - pl * per_plane) * 16;
-    for (int p = g; p < P; p += (int)(blockDim.x >> 4)) {
+    const int pl = slice / per_plane, t0 = (slice - pl * per_plane) * TW;
+    for (int p = g; p < P; p += (int)blockDim.x / TW) {
       float sx = 0.f, sy = 0.f;
       int r = p;                                                     // r(0, p)
 #pragma unroll 4
       for (int l = 0; l < p; ++l) {                                  // column part: U_lp, l < p
-        const float u = us[r * 16];
-        const float2 a = as[l * 16];
+        const float u = us[r * TW];
+        const float2 a = as[l * TW];
         sx = fmaf(u, a.x, sx);
         sy = fmaf(u, a.y, sy);
         r += P - l - 1;
       }
 #pragma unroll 4
       for (int l = p; l < P; ++l, ++r) {                             // row part: U_pl, l >= p; r == r(p, p) here
-        const float u = us[r * 16];
-        const float2 a = as[l * 16];
+        const float u = us[r * TW];
+        const float2 a = as[l * TW];
         sx = fmaf(u, a.x, sx);
         sy = fmaf(u, a.y, sy);
       }
