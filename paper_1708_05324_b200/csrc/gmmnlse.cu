@@ -551,7 +551,7 @@ struct PlanT final : gmmnlse_plan {
     iir_cs = mk((T)csd.real(), (T)csd.imag());
     iir_omf = (T)(1.0 - f_R);
     iir = true;
-    if (sizeof(T) == 4 && !general && log2N >= 9 && log2N <= 13 && lnm * 512.0 < std::log(1e-12)) {
+    if (sizeof(T) == 4 && !general && log2N >= 9 && log2N <= 14 && lnm * 512.0 < std::log(1e-12)) {
       // work list: CTA = rows (m0, m0 + 1) against up to G rows n >= m0.  G = 8 amortises the two parked rows;
       // with few modes that leaves most SMs without a CTA, so G shrinks until a launch of M planes has two per SM
       int dev = 0, sms = 148;
@@ -609,12 +609,12 @@ struct PlanT final : gmmnlse_plan {
     *out = &it->second;
     return 0;
   }
-  template <int LOG2N>
+  template <int LOG2N, int SEGS = 1>
   int launch_pairs_rows_t(const C* A, T* Vout, long long v_ps, int planes) {
     if constexpr (sizeof(T) != 4) {
       return GMMNLSE_EUNSUPPORTED;
     } else {
-      constexpr int NT = (1 << LOG2N) / 16, NW = NT / 32;
+      constexpr int NW = (1 << LOG2N) / 512 / SEGS + (SEGS > 1 ? 1 : 0), NT = 32 * NW;   // + the halo warp
       const size_t smem = 1024 + (size_t)3 * NT * 128 + (size_t)2 * NW * 2 * sizeof(float2) + (size_t)NW * 16;
       const bool half = cur_ho.Vh != nullptr;
       // the map addresses whole planes from a base: the plan's own At (any plane offset) or a caller's array
@@ -624,14 +624,15 @@ struct PlanT final : gmmnlse_plan {
       if (plane0 + planes > M + 1) return GMMNLSE_EINVAL;
       const CUtensorMap* tm = nullptr;
       GM_TRY(field_tmap(tbase, &tm));
-      GM_TRY(half ? ensure_smem(k_pair_iir_rows<LOG2N, true>, smem) : ensure_smem(k_pair_iir_rows<LOG2N, false>, smem));
+      GM_TRY(half ? ensure_smem(k_pair_iir_rows<LOG2N, true, SEGS>, smem)
+                  : ensure_smem(k_pair_iir_rows<LOG2N, false, SEGS>, smem));
       prof_begin(GMMNLSE_KIND_PAIR_CONV);
-      const dim3 grid(n_pair_work, planes);
+      const dim3 grid(n_pair_work * SEGS, planes);
       if (half)
-        launch_k(k_pair_iir_rows<LOG2N, true>, grid, NT, smem, *tm, plane0, Vout, v_ps, P, pair_work, iir_zeta, iir_cs,
+        launch_k(k_pair_iir_rows<LOG2N, true, SEGS>, grid, NT, smem, *tm, plane0, Vout, v_ps, P, pair_work, iir_zeta, iir_cs,
                                                                  iir_omf, iir_zp, cur_ho, iir_zk);
       else
-        launch_k(k_pair_iir_rows<LOG2N, false>, grid, NT, smem, *tm, plane0, Vout, v_ps, P, pair_work, iir_zeta, iir_cs,
+        launch_k(k_pair_iir_rows<LOG2N, false, SEGS>, grid, NT, smem, *tm, plane0, Vout, v_ps, P, pair_work, iir_zeta, iir_cs,
                                                                   iir_omf, iir_zp, cur_ho, iir_zk);
       prof_end();
       GM_CUDA(cudaGetLastError());
@@ -646,6 +647,7 @@ struct PlanT final : gmmnlse_plan {
         case 11: return launch_pairs_rows_t<11>(A, Vout, v_ps, planes);
         case 12: return launch_pairs_rows_t<12>(A, Vout, v_ps, planes);
         case 13: return launch_pairs_rows_t<13>(A, Vout, v_ps, planes);
+        case 14: return launch_pairs_rows_t<14, 2>(A, Vout, v_ps, planes);     // two half-row segments + a halo warp
       }
     }
 #define GM_IIR_CASE(L) case L: return launch_pairs_iir_t<L>(A, a_ps, Vout, v_ps, planes);

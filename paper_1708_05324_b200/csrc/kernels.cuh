@@ -351,14 +351,20 @@ __device__ __forceinline__ void stg256(void* p, const uint32_t (&v)[8]) {
 struct PairWork { int m0, n_begin, n_end; };
 struct ZetaPow { float re[16], im[16]; };                              // zeta^k, k = 0..15 (kernel argument: constant bank)
 
-template <int LOG2N, bool HALF_OUT>
-__global__ void __launch_bounds__((1 << LOG2N) / 16, 1)
+//   SEGS > 1 (N = 16384: three whole rows do not fit shared memory): a CTA handles one of SEGS segments of the row
+//   plus a HALO warp in front of it (local warp 0 = the global warp before the segment, circularly).  The carry into a
+//   warp's first chunk is the zero-history total of the warp before it, which depends on that warp's own 512 samples
+//   only, so the halo warp recomputes it (first pass + scan) and writes nothing.  grid.x = n_work * SEGS.
+template <int LOG2N, bool HALF_OUT, int SEGS = 1>
+__global__ void __launch_bounds__((1 << LOG2N) / 16 / SEGS + (SEGS > 1 ? 32 : 0), 1)
 k_pair_iir_rows(const __grid_constant__ CUtensorMap tmA, int plane0, float* __restrict__ V, long long v_plane_stride,
                 int P, const PairWork* __restrict__ work, float2 zeta, float2 cs, float omf,
                 const float2* __restrict__ zp, HalfOut ho, const ZetaPow zk) {
   pdl_prologue();
   using namespace ptx;
-  constexpr int N = 1 << LOG2N, NT = N / 16, NW = NT / 32;
+  constexpr bool HALO = SEGS > 1;
+  constexpr int N = 1 << LOG2N, NWG = N / 512, NWM = NWG / SEGS;       // warps per row; main warps per CTA
+  constexpr int NW = NWM + (HALO ? 1 : 0), NT = 32 * NW;               // local warps and threads (slices in shared memory)
   constexpr uint32_t ROW_BYTES = NT * 128, WARP_BYTES = 32 * 128;
   extern __shared__ unsigned char smem_raw[];
   const uint32_t raw_addr = smem_u32(smem_raw);
@@ -368,7 +374,12 @@ k_pair_iir_rows(const __grid_constant__ CUtensorMap tmA, int plane0, float* __re
   float2* wt = reinterpret_cast<float2*>(sm + 3 * ROW_BYTES);         // [2 parity][NW][2 streams] warp totals
   const uint32_t bars = base + 3 * ROW_BYTES + 2 * NW * 2 * 8;        // [NW][2]: parked rows, streamed row
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, j = blockIdx.y;
-  const PairWork wk = work[blockIdx.x];
+  const int seg = HALO ? (int)blockIdx.x % SEGS : 0;
+  const PairWork wk = work[HALO ? blockIdx.x / SEGS : blockIdx.x];
+  const bool halo_warp = HALO && warp == 0;
+  // this warp's place in the row: global warp index and the first sample of this thread
+  const int gw = HALO ? (seg * NWM + warp - 1 + NWG) % NWG : warp;
+  const int gsamp = gw * 512 + lane * 16;
   const int m0 = wk.m0, m1 = m0 + 1;
   const bool has_m1 = m1 < P;
   const uint32_t bar_park = bars + 16 * warp, bar_b = bar_park + 8;
@@ -382,10 +393,10 @@ k_pair_iir_rows(const __grid_constant__ CUtensorMap tmA, int plane0, float* __re
   __syncwarp();
   if (lane == 0) {                                                    // each warp fetches only what it reads itself
     mbar_arrive_expect_tx(bar_park, 2 * WARP_BYTES);
-    tma_load_4d(dst0, &tmA, bar_park, 0, 32 * warp, m0, plane0 + j);
-    tma_load_4d(dst0 + ROW_BYTES, &tmA, bar_park, 0, 32 * warp, has_m1 ? m1 : m0, plane0 + j);
+    tma_load_4d(dst0, &tmA, bar_park, 0, 32 * gw, m0, plane0 + j);
+    tma_load_4d(dst0 + ROW_BYTES, &tmA, bar_park, 0, 32 * gw, has_m1 ? m1 : m0, plane0 + j);
     mbar_arrive_expect_tx(bar_b, WARP_BYTES);
-    tma_load_4d(dst0 + 2 * ROW_BYTES, &tmA, bar_b, 0, 32 * warp, wk.n_begin, plane0 + j);
+    tma_load_4d(dst0 + 2 * ROW_BYTES, &tmA, bar_b, 0, 32 * gw, wk.n_begin, plane0 + j);
   }
   // Output recurrence in real arithmetic.  With y = Im(cs w), z = Im(cs zeta w) and zeta^2 = a1 zeta + a2:
   //   V_e = (omf + Im cs) x_e + z_{e-1},  y_e = Im(cs) x_e + z_{e-1},  z_e = Im(cs zeta) x_e + a1 z_{e-1} + a2 y_{e-1}
@@ -414,7 +425,7 @@ k_pair_iir_rows(const __grid_constant__ CUtensorMap tmA, int plane0, float* __re
     __syncwarp();                                                     // the warp is done with the streamed slice
     if (lane == 0 && n + 1 < wk.n_end) {                              // refill it for n + 1 behind the arithmetic
       mbar_arrive_expect_tx(bar_b, WARP_BYTES);
-      tma_load_4d(dst0 + 2 * ROW_BYTES, &tmA, bar_b, 0, 32 * warp, n + 1, plane0 + j);
+      tma_load_4d(dst0 + 2 * ROW_BYTES, &tmA, bar_b, 0, 32 * gw, n + 1, plane0 + j);
     }
     // chunk total from a zero state: sum_e zeta^(15 - e) x_e
     float2 w0 = make_float2(0.f, 0.f), w1 = w0;
@@ -439,8 +450,9 @@ k_pair_iir_rows(const __grid_constant__ CUtensorMap tmA, int plane0, float* __re
     float2 e1 = make_float2(__shfl_up_sync(0xffffffffu, w1.x, 1), __shfl_up_sync(0xffffffffu, w1.y, 1));
     if (lane == 0) { e0 = make_float2(0.f, 0.f); e1 = e0; }
     __syncthreads();
+    if (halo_warp) continue;                                          // its total is published; it writes no output
     {
-      const int pw = warp == 0 ? NW - 1 : warp - 1;                   // the warp before this one (periodic)
+      const int pw = HALO ? warp - 1 : (warp == 0 ? NW - 1 : warp - 1);   // the warp before this one (periodic)
       const float2 g0 = wt[(parity * NW + pw) * 2], g1 = wt[(parity * NW + pw) * 2 + 1];
       // state before this thread's first sample: exclusive in-warp part + zeta^(16 lane) x the previous warp's total
       w0 = make_float2(e0.x + pl.x * g0.x - pl.y * g0.y, e0.y + pl.x * g0.y + pl.y * g0.x);
@@ -465,7 +477,7 @@ k_pair_iir_rows(const __grid_constant__ CUtensorMap tmA, int plane0, float* __re
     const long long q1 = (long long)m1 * P - (long long)m1 * (m1 - 1) / 2 + (n - m1);
     const bool st1 = has_m1 && n >= m1;                               // (m1, n) exists only for n >= m1
     if constexpr (HALF_OUT) {
-      __half* obase = ho.Vh + j * ho.plane_stride + 16 * tid;
+      __half* obase = ho.Vh + j * ho.plane_stride + gsamp;
 #pragma unroll
       for (int s = 0; s < 2; ++s) {
         if (s == 1 && !st1) break;
@@ -485,7 +497,7 @@ k_pair_iir_rows(const __grid_constant__ CUtensorMap tmA, int plane0, float* __re
         stg256(row + ho.lo_offset, lo);
       }
     } else {
-      float* obase = V + j * v_plane_stride + 16 * tid;
+      float* obase = V + j * v_plane_stride + gsamp;
 #pragma unroll
       for (int s = 0; s < 2; ++s) {
         if (s == 1 && !st1) break;
