@@ -41,7 +41,8 @@ constexpr int BK = 32;                                  // q per k-block
 constexpr int TM = 128;                                 // t per CTA
 constexpr int NUM_EPI_WARPS = 12;
 constexpr int NTHREADS = 32 * (2 + NUM_EPI_WARPS);      // 448
-constexpr int EPI_COLS = 72;
+constexpr int EPI_COLS = 72;                            // columns per epilogue warp (default): NT <= 208
+constexpr int EPI_COLS_WIDE = 80;                       // wide instantiation: NT <= 240, one r-tile for Q <= 240
 constexpr int EPI_ROUND = 2;                            // tcgen05.ld groups (8 columns each) in flight per wait
 constexpr int A_BYTES = TM * BK * 2;                    // 8 KiB: one A tile (hi or lo)
 constexpr int MAX_STAGES = 8;
@@ -85,7 +86,7 @@ inline size_t smem_bytes(int NT, int stages) {
 // SPARSE = false compiles the three tables away: the dense instantiations are the code they were before r02's
 // block-sparse form (the row map inside the unrolled store loop cost the dense kernel 0.80 -> 0.99 ms when it was a
 // run-time branch).
-template <bool OUT_H, bool SPARSE = false>
+template <bool OUT_H, bool SPARSE = false, int EC = EPI_COLS>
 __global__ void __launch_bounds__(NTHREADS, 1)
 k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ CUtensorMap tmVl,
              const __grid_constant__ CUtensorMap tmSh, const __grid_constant__ CUtensorMap tmSl, const Params p) {
@@ -208,19 +209,19 @@ k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ C
     const int third = (warp - 2) >> 2;            // which slice of the NT columns
     const int cper = ((p.NT + 2) / 3 + 7) / 8 * 8;
     const int cbeg = third * cper;
-    const int ncols = max(0, min(p.NT, cbeg + cper) - cbeg);       // multiple of 8, <= EPI_COLS
+    const int ncols = max(0, min(p.NT, cbeg + cper) - cbeg);       // multiple of 8, <= EC
     const float vb = *p.vbound;
     const float inv_sv = v_scale(p.bound_gain * vb, true);
     const float sz = OUT_H ? v_scale(p.zgain * vb, false) : 1.f;
     int acc = 0;
     uint32_t acc_phase = 0;
-    float accr[EPI_COLS];
+    float accr[EC];
     for (int tile = cta; tile < p.total_tiles; tile += nctas) {
       const int pl = tile / tiles_per_plane, rem = tile - pl * tiles_per_plane;
       const int tt = rem / p.n_rt, rt = rem - tt * p.n_rt;
       const int t = tt * TM + lg * 32 + lane;
 #pragma unroll
-      for (int i = 0; i < EPI_COLS; ++i) accr[i] = 0.f;
+      for (int i = 0; i < EC; ++i) accr[i] = 0.f;
       const int nchunks = ((SPARSE ? p.kb_count[rt] : p.KB) + p.kchunk - 1) / p.kchunk;
       for (int ch = 0; ch < nchunks; ++ch) {
         mbar_wait(bar_tfull + 8 * acc, acc_phase, 5);
@@ -229,14 +230,14 @@ k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ C
         // EPI_ROUND groups of 8 columns in flight per wait (3 and 5 measured no faster: the drain is bound by the
         // tensor-memory read rate, not by the round trips)
 #pragma unroll
-        for (int g0 = 0; g0 < EPI_COLS / 8; g0 += EPI_ROUND) {
+        for (int g0 = 0; g0 < EC / 8; g0 += EPI_ROUND) {
           uint32_t v[EPI_ROUND][8];
 #pragma unroll
-          for (int g = g0; g < g0 + EPI_ROUND && g < EPI_COLS / 8; ++g)
+          for (int g = g0; g < g0 + EPI_ROUND && g < EC / 8; ++g)
             if (g * 8 < ncols) tmem_ld_x8(taddr + g * 8, v[g - g0]);
           tmem_ld_wait();
 #pragma unroll
-          for (int g = g0; g < g0 + EPI_ROUND && g < EPI_COLS / 8; ++g)
+          for (int g = g0; g < g0 + EPI_ROUND && g < EC / 8; ++g)
             if (g * 8 < ncols) {
 #pragma unroll
               for (int c = 0; c < 8; ++c) accr[g * 8 + c] += __uint_as_float(v[g - g0][c]);
@@ -253,7 +254,7 @@ k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ C
         __half* Zh = p.Zh + (long long)pl * p.u_plane_stride + t;
         __half* Zl = Zh + (long long)p.Q * p.N;
 #pragma unroll
-        for (int c = 0; c < EPI_COLS; ++c) {
+        for (int c = 0; c < EC; ++c) {
           const int r = rbase + c;
           if (c < ncols && r < p.Q) {
             const float z = accr[c] * (rs[c] * inv_sv) * sz;
@@ -265,7 +266,7 @@ k_contract_h(const __grid_constant__ CUtensorMap tmVh, const __grid_constant__ C
       } else {
         float* Uout = p.U + (long long)pl * p.u_plane_stride + t;
 #pragma unroll
-        for (int c = 0; c < EPI_COLS; ++c) {
+        for (int c = 0; c < EC; ++c) {
           const int r = rbase + c;
           if constexpr (SPARSE) {
             if (c < ncols) {

@@ -728,9 +728,12 @@ struct PlanT final : gmmnlse_plan {
     }
   }
   // ------------------------------------------------------------------ kind::f16 form (gemm_h.cuh)
-  int h_build(HGemm& g, const std::vector<double>& mat, int rows, int K, int smax, int force_NT = 0) {
+  int h_build(HGemm& g, const std::vector<double>& mat, int rows, int K, int smax, int force_NT = 0, bool allow_wide = false) {
     g.rows = rows; g.K = K;
-    g.nrt = (rows + 207) / 208;
+    // NT <= 208 (three epilogue slices of <= 72 columns); the dense U-output form may use ONE tile of <= 240 (slices
+    // of 80) when that covers all rows: the V tile is then loaded once instead of twice
+    const int cap = allow_wide && rows > 208 && rows <= 240 ? 240 : 208;
+    g.nrt = (rows + cap - 1) / cap;
     g.NT = (((rows + g.nrt - 1) / g.nrt) + 15) / 16 * 16;
     if (force_NT > 0) { g.NT = force_NT; g.nrt = (rows + force_NT - 1) / force_NT; }
     g.KB = (K + hc::BK - 1) / hc::BK;
@@ -804,8 +807,14 @@ struct PlanT final : gmmnlse_plan {
       cfg.stream = stream;
       pdl_config(cfg);
       prof_begin(GMMNLSE_KIND_CONTRACT);
+      // tiles wider than 208 columns (one r-tile for 208 < Q <= 240: config 4's Q = 210) need 80 columns per epilogue
+      // warp; the default instantiation keeps 72 (80 costs the config-5 kernel a spill and 1 %)
+      const bool wide = g.NT > 208;
+      if (wide && (outZ || sp)) return GMMNLSE_EUNSUPPORTED;
       cudaError_t e = outZ ? cudaLaunchKernelEx(&cfg, hc::k_contract_h<true>, mhi, mlo, g.tmHi, g.tmLo, prm)
                       : sp ? cudaLaunchKernelEx(&cfg, hc::k_contract_h<false, true>, mhi, mlo, g.tmHi, g.tmLo, prm)
+                    : wide ? cudaLaunchKernelEx(&cfg, hc::k_contract_h<false, false, hc::EPI_COLS_WIDE>, mhi, mlo, g.tmHi,
+                                                g.tmLo, prm)
                            : cudaLaunchKernelEx(&cfg, hc::k_contract_h<false>, mhi, mlo, g.tmHi, g.tmLo, prm);
       prof_end();
       GM_CUDA(e);
@@ -818,6 +827,7 @@ struct PlanT final : gmmnlse_plan {
     GM_TRY(h_a_tmaps(&tmVh, &tmVl, V, Q, M + 1));
     if constexpr (sizeof(T) == 4) {
       GM_TRY(ensure_smem(hc::k_contract_h<false>, (size_t)smax));
+      GM_TRY(ensure_smem(hc::k_contract_h<false, false, hc::EPI_COLS_WIDE>, (size_t)smax));
       GM_TRY(ensure_smem(hc::k_contract_h<true>, (size_t)smax));
     }
     tc_h = true;
@@ -984,7 +994,7 @@ struct PlanT final : gmmnlse_plan {
         GM_CUDA(cudaGetDevice(&dev0));
         GM_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev0));
         GM_CUDA(cudaDeviceGetAttribute(&smax0, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev0));
-        GM_TRY(h_build(hg, h_S2, Q, Q, smax0));
+        GM_TRY(h_build(hg, h_S2, Q, Q, smax0, 0, true));
         return init_h_common(smax0);
       }
       if (contraction == 9) {                          // block-sparse form (NEXT-4), scalar-mode path only
