@@ -41,8 +41,7 @@ typedef struct {                /* pass NULL for defaults                       
   double tol;                   /* MPA convergence threshold, default 1e-6         */
   int    max_iter;              /* cap on iterations per large step; <=0 -> 2*M + 4               */
   int    fixed_iter;            /* >0: run exactly this many iterations per large step (parity)   */
-  int    contraction;           /* a6 kernel: 0 = auto (complex64 and N % 128 == 0: 7 when Q = P(P+1)/2 >= 160,
-                                   3 when 64 <= Q < 160; else 1),
+  int    contraction;           /* a6 kernel: 0 = auto (complex64, N % 128 == 0 and Q = P(P+1)/2 >= 64: 7; else 1),
                                    1 = CUDA-core fp32/fp64 GEMM;
                                    3 = tcgen05 3xTF32 GEMM (kind::tf32 on hi/lo splits, both operands in shared memory);
                                    7 = tcgen05 kind::f16 GEMM on fp16 hi/lo splits of both operands (22 mantissa

@@ -984,11 +984,10 @@ struct PlanT final : gmmnlse_plan {
     } else {
       const bool want = contraction >= 2 || (contraction == 0 && Q >= 64);
       if (!want) return 0;
-      // auto: the kind::f16 form (0.82 ms per 20-plane launch at config 5 against 1.66 ms for the 3xTF32 form) once
-      // the GEMM is large enough to pay for the bound kernel and memset in front of the pair kernel: measured
-      // +18 % at config 4 (Q = 210) and +55 % at config 5, -3 % at the launch-bound config 3 (Q = 120), which
-      // therefore stays on the 3xTF32 form
-      if (contraction == 7 || (contraction == 0 && Q >= 160 && N % hc::TM == 0)) {   // dense, fp16 hi / lo operands
+      // auto: the kind::f16 form wherever the tensor path applies (Q >= 64).  Measured against the 3xTF32 form:
+      // +55 % at config 5, +18 % at config 4, +2 % at config 3 (r02: 19.7k vs 19.3k z-steps/s; in r01 the bound kernel
+      // and memset in front of the pair kernel still cost more than they saved there)
+      if (contraction == 7 || (contraction == 0 && N % hc::TM == 0)) {   // dense, fp16 hi / lo operands
         if (N % hc::TM != 0) return GMMNLSE_EUNSUPPORTED;
         int dev0 = 0, smax0 = 0;
         GM_CUDA(cudaGetDevice(&dev0));
