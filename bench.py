@@ -378,9 +378,9 @@ def run_gpu(args):
         for c in (1, 2, 3, 4):
             if c == cfg:
                 continue
-            m = measure(c, 3, 3, with_events=False)
+            m = measure(c, 10, 3, with_events=False)
             others.append({"workload": m["w"].name, "z_steps_per_s": round(m["z_steps"] / (m["ms"] * 1e-3), 1),
-                           "ms_per_step": round(m["ms"] / 3, 4), "z_steps_per_step": LARGE_PER_STEP[c] * m["w"].M,
+                           "ms_per_step": round(m["ms"] / 10, 4), "z_steps_per_step": LARGE_PER_STEP[c] * m["w"].M,
                            "iterations_per_large_step": round(m["iters"] / max(m["large"], 1), 3),
                            "mpa_loop": "device" if m["loop"] == 1 else "host"})
         out["other_workloads"] = others
