@@ -46,7 +46,12 @@ class TorchComm:
         self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
 
     def all_gather(self, out, block):
-        self._dist.all_gather_into_tensor(out, block, group=self._group) if out.is_cuda else \
+        import torch
+        if out.is_complex():                       # NCCL has no complex types: gather the (re, im) views
+            out, block = torch.view_as_real(out), torch.view_as_real(block)
+        if out.is_cuda:
+            self._dist.all_gather_into_tensor(out, block.contiguous(), group=self._group)
+        else:
             self._dist.all_gather(list(out.unbind(0)), block, group=self._group)
 
     def all_reduce_max(self, x: float) -> float:

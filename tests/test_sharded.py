@@ -197,3 +197,34 @@ def test_sharded_gpu_two_threads_equal_unsharded(cfg, kw, n_shards):
     omp = O.mpa_propagate(A_in, w.L, w.dz, w.M, w.beta, w.S, w.kappa, w.omega0, w.f_R, w.h_R, w.dt, shock=w.shock,
                           tol=w.tol)
     assert rel(outs[0], omp) <= 1e-4
+
+
+@pytest.mark.gpu
+def test_sharded_driver_over_a_real_nccl_group_of_one():
+    """The NCCL path of TorchComm (all_gather_into_tensor on the real view of complex blocks, max all-reduce on a
+    device scalar) on the one GPU this pool gives: a process group of world size 1, against the unsharded call."""
+    torch = pytest.importorskip("torch")
+    import torch.distributed as dist
+    from paper_1708_05324_b200 import binding as B
+    B.load_library()
+    if dist.is_initialized():
+        pytest.skip("a process group already exists in this process")
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(29900 + os.getpid() % 90), RANK="0", WORLD_SIZE="1")
+    torch.cuda.set_device(0)
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        w = W.make_config(2, N=1024, L=25 * 50e-6)
+        A = torch.from_numpy(w.A0.astype(np.complex64)).cuda()
+        ref_out, out = torch.empty_like(A), torch.empty_like(A)
+        st = {}
+        with B.plan_from_workload(w, graph=1) as plan:
+            plan.propagate(A, w.L, ref_out)
+            torch.cuda.synchronize()
+            ref_stats = plan.stats()
+        with B.plan_from_workload(w, graph=1) as plan:
+            sharded.propagate_sharded(plan, sharded.TorchComm(), A, w.L, out, M=w.M, dz=w.dz, tol=w.tol, stats=st)
+            torch.cuda.synchronize()
+        assert st["large_steps"] == ref_stats["large_steps"] and st["iterations"] == ref_stats["iterations"]
+        assert rel(out.cpu().numpy(), ref_out.cpu().numpy()) <= 5e-6
+    finally:
+        dist.destroy_process_group()
