@@ -62,8 +62,22 @@ class TorchComm:
         return float(t.item())
 
 
-def propagate_sharded(plan, comm, A_in, L, A_out, *, M, dz, tol=1e-6, max_iter=0, fixed_iter=0, empty_like=None,
-                      stats=None):
+def converged(err, tol, stop_rule, it, err_prev, rho_prev):
+    """The convergence decision of the library's loops (csrc/kernels.cuh mpa_converged): err < tol, or with
+    stop_rule 1 (reading S25) and it >= 3 the a-posteriori bound err rho / (1 - rho) < tol, rho the larger
+    of the last two error ratios.  Returns (decision, this iteration's ratio)."""
+    rho_now = err / err_prev if err_prev > 0 else 0.0
+    if err < tol:
+        return True, rho_now
+    if stop_rule == 1 and it >= 3:
+        rho = max(rho_now, rho_prev)
+        if rho < 1.0 and err * rho / (1.0 - rho) < tol:
+            return True, rho_now
+    return False, rho_now
+
+
+def propagate_sharded(plan, comm, A_in, L, A_out, *, M, dz, tol=1e-6, max_iter=0, fixed_iter=0, stop_rule=0,
+                      empty_like=None, stats=None):
     """Integrate over L with the MPA, this rank running its share of the planes of every large step.
 
     ``plan``: an object with the ``shard_*`` methods of :class:`binding.Plan` (same plan arguments on every rank);
@@ -85,7 +99,7 @@ def propagate_sharded(plan, comm, A_in, L, A_out, *, M, dz, tol=1e-6, max_iter=0
     while done < n_small:
         Mc = min(M, n_small - done)
         j_lo, j_hi = plane_ranges(Mc, world)[rank]
-        it = 0
+        it, err_prev, rho_prev = 0, 1e300, 1e300
         while True:
             first = it == 0
             if j_hi > j_lo:
@@ -96,10 +110,12 @@ def propagate_sharded(plan, comm, A_in, L, A_out, *, M, dz, tol=1e-6, max_iter=0
             e_loc = plan.shard_update(j_lo, j_hi, Mc, first, all_sums, rank, world) if j_hi > j_lo else 0.0
             err = comm.all_reduce_max(e_loc)
             it += 1
+            conv, rho = converged(err, tol, stop_rule, it, err_prev, rho_prev)   # every rank takes the same decision
+            err_prev, rho_prev = err, (1e300 if it == 1 else rho)
             if fixed_iter > 0:
                 if it >= cap:
                     break
-            elif err < tol:
+            elif conv:
                 break
             elif it >= cap:
                 n_noconv += 1

@@ -84,7 +84,7 @@ class NumpyShardPlan:
         self._c(A_out)[...] = O.to_time(self.psi0)
 
 
-def _gloo_worker(rank, world, port, M, n_small, out):
+def _gloo_worker(rank, world, port, M, n_small, out, stop_rule=0):
     import torch
     import torch.distributed as dist
     sys.path.insert(0, ROOT)
@@ -96,20 +96,23 @@ def _gloo_worker(rank, world, port, M, n_small, out):
     A_out = torch.empty_like(A_in)
     st = {}
     status = sharded.propagate_sharded(NumpyShardPlan(w), sharded.TorchComm(), A_in, n_small * w.dz, A_out, M=M,
-                                       dz=w.dz, tol=w.tol, stats=st)
+                                       dz=w.dz, tol=w.tol, stats=st, stop_rule=stop_rule)
     out.put((rank, status, st, A_out.numpy().view(np.complex128)[..., 0].copy()))
     dist.barrier()
     dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("M,n_small", [(10, 25), (3, 6), (1, 2)])      # ragged tail; uneven split; more ranks than planes
-def test_sharded_loop_world2_gloo_equals_oracle_mpa(M, n_small):
+@pytest.mark.parametrize("M,n_small,stop_rule", [
+    (10, 25, 0), (3, 6, 0), (1, 2, 0),          # ragged tail; uneven split; more ranks than planes
+    (10, 30, 1),                                # the a-posteriori stopping rule (reading S25)
+])
+def test_sharded_loop_world2_gloo_equals_oracle_mpa(M, n_small, stop_rule):
     pytest.importorskip("torch")
     import torch.multiprocessing as mp
     ctx = mp.get_context("spawn")
     out = ctx.Queue()
-    port = 29700 + (os.getpid() + 7 * M) % 2000
-    procs = [ctx.Process(target=_gloo_worker, args=(r, 2, port, M, n_small, out)) for r in range(2)]
+    port = 29700 + (os.getpid() + 7 * M + 3 * stop_rule) % 2000
+    procs = [ctx.Process(target=_gloo_worker, args=(r, 2, port, M, n_small, out, stop_rule)) for r in range(2)]
     for p in procs:
         p.start()
     res = sorted((out.get(timeout=240) for _ in procs), key=lambda t: t[0])
@@ -119,7 +122,7 @@ def test_sharded_loop_world2_gloo_equals_oracle_mpa(M, n_small):
     w = W.make_config(2, N=256, max_group=1)
     ost = {}
     ref = O.mpa_propagate(w.A0, n_small * w.dz, w.dz, M, w.beta, w.S, w.kappa, w.omega0, w.f_R, w.h_R, w.dt,
-                          shock=w.shock, tol=w.tol, stats=ost)
+                          shock=w.shock, tol=w.tol, stats=ost, stop_rule=stop_rule)
     for rank, status, st, field in res:
         assert status == 0
         assert st["large_steps"] == ost["large_steps"] and st["iterations"] == ost["iterations"]
