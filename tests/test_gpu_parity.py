@@ -142,10 +142,12 @@ def test_nonlinear_op_vs_oracle(B, cfg, kw):
 
 
 @pytest.mark.slow
-@pytest.mark.parametrize("cfg", [4, 5])
-def test_nonlinear_op_full_shape_large_P(B, cfg):
+@pytest.mark.parametrize("cfg,contraction", [(4, 0), (5, 0), (5, 9), (5, 8), (4, 9)])
+def test_nonlinear_op_full_shape_large_P(B, cfg, contraction):
+    """BASELINE's full shapes (N = 16384 / 8192) with the default contraction and with the block-sparse and low-rank
+    forms bench.py reports as variants."""
     w = W.make_config(cfg)
-    assert _nonlinear_op_case(B, w) <= TOL_OP
+    assert _nonlinear_op_case(B, w, contraction=contraction) <= TOL_OP
 
 
 def test_raman_path_selection_and_general_response(B):
