@@ -86,6 +86,15 @@ typedef struct {                /* pass NULL for defaults                       
                                    steps then end at an error near tol instead of ~10x below it, and these residuals
                                    add up over the large steps (measured: photon number +1.7e-7 per large step at
                                    tol = 1e-6) -- lower tol for long runs with tight invariants.  Other values: EINVAL */
+  int    async_call;            /* 0 (default): gmmnlse_propagate returns after one synchronise that follows its last
+                                   kernel (A_out complete, counters current, WARN_NOCONV reported by the return code).
+                                   1: with the loop on the device (options.graph = 0) the call returns as soon as its
+                                   work is enqueued -- A_out is complete once the stream is synchronised, the return
+                                   code is OK, and the loop counters (iterations, not_converged, last_err) are taken
+                                   in lazily by the next gmmnlse_get_stats / gmmnlse_launch_count / propagate call,
+                                   which waits for the stream if it has to.  Large steps that run on the host loop
+                                   (a plan's first one, a ragged last one, profiling) still synchronise per
+                                   iteration; gmmnlse_propagate_host always synchronises.  Other values: EINVAL   */
 } gmmnlse_options;
 
 /* Build a plan: precompute D_w^(p), the rotation tables exp(+-D_w j dz) (j = 0..M) in

@@ -28,7 +28,7 @@ class GmmnlseError(RuntimeError):
 class Options(C.Structure):
     _fields_ = [("precision", C.c_int), ("shock", C.c_int), ("tol", C.c_double), ("max_iter", C.c_int),
                 ("fixed_iter", C.c_int), ("contraction", C.c_int), ("raman", C.c_int), ("graph", C.c_int),
-                ("stop_rule", C.c_int)]
+                ("stop_rule", C.c_int), ("async_call", C.c_int)]
 
 
 _LIB = None
@@ -124,7 +124,7 @@ class Plan:
     """Owner of one ``gmmnlse_plan``; methods mirror the C calls one to one."""
 
     def __init__(self, P, N, M, dt, dz, beta, S, f_R, h_R, omega0, n2, *, precision=0, shock=True,
-                 tol=1e-6, max_iter=0, fixed_iter=0, contraction=0, raman=0, graph=0, stop_rule=0):
+                 tol=1e-6, max_iter=0, fixed_iter=0, contraction=0, raman=0, graph=0, stop_rule=0, async_call=0):
         self._lib = load_library()
         self._h = C.c_void_p()
         beta = np.ascontiguousarray(beta, dtype=np.float64).reshape(P, -1)
@@ -142,7 +142,7 @@ class Plan:
         if hR is not None and hR.size != N:
             raise GmmnlseError(EINVAL, "h_R must hold N samples")
         opt = Options(int(precision), int(bool(shock)), float(tol), int(max_iter), int(fixed_iter), int(contraction),
-                      int(raman), int(graph), int(stop_rule))
+                      int(raman), int(graph), int(stop_rule), int(async_call))
         hp = None if hR is None else hR.ctypes.data_as(_DP)
         if general:
             st = self._lib.gmmnlse_plan_create_general(

@@ -140,7 +140,7 @@ int ilog2(int n) {
 // ============================================================================================
 struct gmmnlse_plan {
   int P = 0, N = 0, M = 0, log2N = 0, Q = 0, precision = 0, shock = 1, max_iter = 0, fixed_iter = 0;
-  int contraction = 0, raman = 0, graph = 0, stop_rule = 0;
+  int contraction = 0, raman = 0, graph = 0, stop_rule = 0, async_call = 0;
   int loop_state = 0;                      // 0 host loop so far, 1 device loop (CUDA graph) in use, -1 graph build failed
   int device = 0;                          // the CUDA device the plan was created on (every call runs there)
   // general form of Eq. 1 (gmmnlse_plan_create_general): separate, possibly complex tensors, no symmetry
@@ -214,6 +214,7 @@ struct gmmnlse_plan {
   virtual int lowrank_rank() const = 0;
   virtual int sparse_info(int* classes, double* work_fraction) const = 0;
   virtual void drop_loop_graph() = 0;
+  virtual int fold_pending() = 0;          // async calls: wait for the last call and take its loop counters in
 };
 
 namespace {
@@ -246,6 +247,23 @@ struct PlanT final : gmmnlse_plan {
   LoopStats *d_stats = nullptr, *h_stats = nullptr;
   long long lg_c0 = 0, lg_cb = 0, lg_ca = 0;       // kernel launches in iteration 0, the loop body, a11
   bool warmed = false;                             // one host-loop large step has run (function attributes set)
+  // options.async_call: counters of the last call still on the device (copy to h_stats enqueued on pending_stream)
+  long long pending_gsteps = 0;
+  bool pending_last_on_device = false;
+  cudaStream_t pending_stream = nullptr;
+  void take_loop_stats(long long gsteps, bool last_on_device, int* status) {
+    n_iter += h_stats->iters;
+    n_launch += gsteps * (lg_c0 - lg_cb + lg_ca) + lg_cb * h_stats->iters;
+    if (h_stats->noconv > 0) { n_noconv += h_stats->noconv; if (status) *status = GMMNLSE_WARN_NOCONV; }
+    if (last_on_device) last_err = h_stats->last_err;
+  }
+  int fold_pending() override {
+    if (pending_gsteps == 0) return 0;
+    GM_CUDA(cudaStreamSynchronize(pending_stream));
+    take_loop_stats(pending_gsteps, pending_last_on_device, nullptr);
+    pending_gsteps = 0;
+    return 0;
+  }
   // serial RK4IP: one step (4 stages) as a graph, replayed; no decision inside, so no conditional node
   cudaGraph_t rkg = nullptr;
   cudaGraphExec_t rkg_exec = nullptr;
@@ -1416,6 +1434,7 @@ struct PlanT final : gmmnlse_plan {
   // own planes j_lo+1 .. j_hi of the Mc planes; the collectives between them belong to the caller (sharded.py)
   C* shard_pre = nullptr;
   int shard_begin(const void* A_in) override {
+    GM_TRY(fold_pending());
     GM_CUDA(cudaMemsetAsync(d_step2, 0, sizeof(int), stream));
     GM_TRY(launch_fft(+1, (const C*)A_in, 0, psi, 0, nullptr, nullptr, nullptr, 0, (T)1, P, 1));   // a1, on every shard
     return to_master(psi);
@@ -1511,6 +1530,7 @@ struct PlanT final : gmmnlse_plan {
 
   // ---- device-side loop (options.graph = 0): the large step above as one CUDA graph, no host decision inside
   void drop_loop_graph() override {
+    fold_pending();                                  // every caller has synchronised or is about to change the plan
     if (lg_exec) cudaGraphExecDestroy(lg_exec);
     if (lg) cudaGraphDestroy(lg);
     lg_exec = nullptr;
@@ -1609,6 +1629,7 @@ struct PlanT final : gmmnlse_plan {
     const long long nsteps = llround(ns);
     if (!(L >= 0) || std::fabs(ns - (double)nsteps) > 1e-9 * std::fmax(1.0, ns)) return GMMNLSE_EINVAL;
     if (fprof_d && Qc && 2 * nsteps + 1 > n_fprof) return GMMNLSE_EINVAL;   // the z-profile must cover the call
+    GM_TRY(fold_pending());
     GM_CUDA(cudaMemsetAsync(d_step2, 0, sizeof(int), stream));
     // a1: psi_0 = F{A(z0)}
     GM_TRY(launch_fft(+1, (const C*)A_in, 0, psi, 0, nullptr, nullptr, nullptr, 0, (T)1, P, 1));
@@ -1641,11 +1662,14 @@ struct PlanT final : gmmnlse_plan {
     if (d2h_dst) GM_CUDA(cudaMemcpyAsync(d2h_dst, A_out, d2h_bytes, cudaMemcpyDeviceToHost, stream));   // host entry
     if (gsteps > 0) {            // one read-back per call: iteration count, unconverged steps, last error
       GM_CUDA(cudaMemcpyAsync(h_stats, d_stats, sizeof(LoopStats), cudaMemcpyDeviceToHost, stream));
+      if (async_call && !d2h_dst) {                // return now; the counters are folded in when somebody needs them
+        pending_gsteps = gsteps;
+        pending_last_on_device = last_on_device;
+        pending_stream = stream;
+        return status;
+      }
       GM_CUDA(cudaStreamSynchronize(stream));
-      n_iter += h_stats->iters;
-      n_launch += gsteps * (lg_c0 - lg_cb + lg_ca) + lg_cb * h_stats->iters;
-      if (h_stats->noconv > 0) { n_noconv += h_stats->noconv; status = GMMNLSE_WARN_NOCONV; }
-      if (last_on_device) last_err = h_stats->last_err;
+      take_loop_stats(gsteps, last_on_device, &status);
     } else {                     // host loop: same completion semantics (A_out complete on return)
       if (fixed_iter > 0) GM_CUDA(cudaMemcpyAsync(h_err, d_err, sizeof(double), cudaMemcpyDeviceToHost, stream));
       GM_CUDA(cudaStreamSynchronize(stream));
@@ -1867,6 +1891,7 @@ struct PlanT final : gmmnlse_plan {
       GM_TRY(upload(EH_d, eh));
     }
     if (fprof_d && Qc && 2 * nsteps + 1 > n_fprof) return GMMNLSE_EINVAL;
+    GM_TRY(fold_pending());
     GM_CUDA(cudaMemsetAsync(d_step2, 0, sizeof(int), stream));
     GM_TRY(launch_fft(+1, (const C*)A_in, 0, psi, 0, nullptr, nullptr, nullptr, 0, (T)1, P, 1));
     GM_TRY(to_master(psi));
@@ -2172,7 +2197,7 @@ int overlap_tensor_noalloc(int P, long long G, const double* F_dev, double dA, d
 // ============================================================================================
 extern "C" {
 
-int gmmnlse_abi_version(void) { return 3; }
+int gmmnlse_abi_version(void) { return 4; }
 
 int gmmnlse_overlap_tensor(int P, long long G, const double* F, double dA, double* S_out) {
   if (P < 1 || G < 1 || !F || !S_out || !(dA > 0)) return GMMNLSE_EINVAL;
@@ -2201,7 +2226,7 @@ static int create_plan(gmmnlse_plan** out, int P, int N, int M, double dt, doubl
                        double f_R, const double* h_R, double omega0, double n2, const gmmnlse_options* opt) {
   if (!out) return GMMNLSE_EINVAL;
   *out = nullptr;
-  gmmnlse_options o = {0, 1, 1e-6, 0, 0, 0, 0, 0, 0};
+  gmmnlse_options o = {0, 1, 1e-6, 0, 0, 0, 0, 0, 0, 0};
   if (opt) o = *opt;
   if (P < 1 || N < 1 || M < 1 || n_beta < 1 || !beta || !S) return GMMNLSE_EINVAL;
   if (N & (N - 1)) return GMMNLSE_EINVAL;
@@ -2214,6 +2239,7 @@ static int create_plan(gmmnlse_plan** out, int P, int N, int M, double dt, doubl
     return GMMNLSE_EINVAL;
   if (o.graph < 0 || o.graph > 1) return GMMNLSE_EINVAL;
   if (o.stop_rule < 0 || o.stop_rule > 1) return GMMNLSE_EINVAL;
+  if (o.async_call < 0 || o.async_call > 1) return GMMNLSE_EINVAL;
   if (o.shock && M_PI / dt >= omega0) return GMMNLSE_EINVAL;
   if (!(o.tol > 0)) o.tol = 1e-6;
   for (long long i = 0; i < (long long)P * n_beta; ++i)
@@ -2251,6 +2277,7 @@ static int create_plan(gmmnlse_plan** out, int P, int N, int M, double dt, doubl
   pl->raman = o.raman;
   pl->graph = o.graph;
   pl->stop_rule = o.stop_rule;
+  pl->async_call = o.async_call;
   if (cudaGetDevice(&pl->device) != cudaSuccess) { delete pl; g_cuda_err = "cudaGetDevice failed"; return GMMNLSE_ECUDA; }
   pl->general = general;
   pl->gen_complex = general && tensors_complex;
@@ -2412,6 +2439,10 @@ int gmmnlse_set_stream(gmmnlse_plan* plan, void* stream) {
 int gmmnlse_get_stats(const gmmnlse_plan* plan, long long* large_steps, long long* iterations, double* last_err,
                       long long* not_converged) {
   if (!plan) return GMMNLSE_EINVAL;
+  {                                                  // options.async_call: the last call's counters may still be in flight
+    DeviceGuard dg(plan->device);
+    GM_TRY(const_cast<gmmnlse_plan*>(plan)->fold_pending());
+  }
   if (large_steps) *large_steps = plan->n_large;
   if (iterations) *iterations = plan->n_iter;
   if (last_err) *last_err = plan->last_err;
@@ -2419,7 +2450,12 @@ int gmmnlse_get_stats(const gmmnlse_plan* plan, long long* large_steps, long lon
   return GMMNLSE_OK;
 }
 
-long long gmmnlse_launch_count(const gmmnlse_plan* plan) { return plan ? plan->n_launch : 0; }
+long long gmmnlse_launch_count(const gmmnlse_plan* plan) {
+  if (!plan) return 0;
+  DeviceGuard dg(plan->device);
+  const_cast<gmmnlse_plan*>(plan)->fold_pending();
+  return plan->n_launch;
+}
 
 int gmmnlse_profile_enable(gmmnlse_plan* plan, int on) {
   if (!plan) return GMMNLSE_EINVAL;

@@ -415,6 +415,45 @@ def test_aposteriori_stop_rule_vs_oracle_and_default(B, cfg, kw):
     assert e.value.status == B.EINVAL
 
 
+def test_async_call_returns_before_the_gpu_finishes(B):
+    """options.async_call = 1: with the loop on the device gmmnlse_propagate only enqueues ("propagate
+    is asynchronous" once the convergence decision is device-side); same bits as the synchronous call, and the loop
+    counters arrive with the next get_stats."""
+    import time
+    w = W.make_config(3, N=8192, L=40 * 10 * 100e-6)               # 40 large steps of ~0.6 ms each
+    Ad = dev(w.A0, np.complex64)
+    ref = torch.empty_like(Ad)
+    with B.plan_from_workload(w) as plan:
+        plan.propagate(Ad, w.L, ref)
+        ref_stats = plan.stats()
+    out = torch.empty_like(Ad)
+    with B.plan_from_workload(w, async_call=1) as plan:
+        plan.propagate(Ad, 10 * w.dz, out)                          # the plan's first large step runs on the host loop
+        torch.cuda.synchronize()
+        s0 = plan.stats()
+        t0 = time.perf_counter()
+        st = plan.propagate(Ad, w.L, out)
+        t_call = time.perf_counter() - t0
+        torch.cuda.synchronize()
+        t_done = time.perf_counter() - t0
+        assert st == 0 and plan.loop_kind() == 1
+        assert t_call < 0.5 * t_done, (t_call, t_done)              # returned while the GPU was still working
+        s1 = plan.stats()
+        assert torch.equal(out, ref)
+        assert s1["large_steps"] - s0["large_steps"] == ref_stats["large_steps"]
+        assert s1["iterations"] - s0["iterations"] == ref_stats["iterations"] and s1["not_converged"] == 0
+        assert s1["last_err"] == pytest.approx(ref_stats["last_err"], rel=1e-9)     # fp64 atomic sums: order not fixed
+        # back-to-back asynchronous calls fold the previous call's counters in themselves
+        plan.propagate(Ad, w.L, out)
+        plan.propagate(Ad, w.L, out)
+        torch.cuda.synchronize()
+        assert plan.stats()["iterations"] - s0["iterations"] == 3 * ref_stats["iterations"]
+        assert torch.equal(out, ref)
+    with pytest.raises(B.GmmnlseError) as e:
+        B.plan_from_workload(w, async_call=2)
+    assert e.value.status == B.EINVAL
+
+
 def test_zero_length_is_identity(B):
     w = W.make_config(2, N=256)
     w.L = 0.0
