@@ -241,6 +241,42 @@ def run_gpu(args):
                     launches=l1 - l0, not_conv=s1["not_converged"] - s0["not_converged"], finite=finite,
                     bytes_io=int(A0.nbytes), ckind=ckind, crank=crank)
 
+    def measure_sharded_world1(cfg, K, Wm, local):
+        """paper_1708_05324_b200/sharded.py (host-driven loop, one all-gather + one max all-reduce per iteration over
+        NCCL) with a process group of world size 1: what the exchange step and the host loop cost on one GPU against
+        the device-side graph loop of `value`.  No scaling claim: this pool gives one GPU."""
+        import socket
+        from paper_1708_05324_b200 import sharded
+        w = workloads.make_config(cfg)
+        L_step = LARGE_PER_STEP[cfg] * w.M * w.dz
+        A = torch.from_numpy(w.A0.astype(np.complex128 if w.precision else np.complex64)).cuda()
+        own_group = not dist.is_initialized()
+        if own_group:
+            with socket.socket() as sk:
+                sk.bind(("127.0.0.1", 0))
+                port = sk.getsockname()[1]
+            os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+            dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", local))
+        try:
+            comm = sharded.TorchComm()
+            plan = binding.plan_from_workload(w, graph=1)
+            st = {}
+            for _ in range(Wm):
+                sharded.propagate_sharded(plan, comm, A, L_step, A, M=w.M, dz=w.dz, tol=w.tol)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            for _ in range(K):
+                sharded.propagate_sharded(plan, comm, A, L_step, A, M=w.M, dz=w.dz, tol=w.tol, stats=st)
+            torch.cuda.synchronize()
+            ms = (time.perf_counter() - t0) * 1e3
+            plan.destroy()
+        finally:
+            if own_group:
+                dist.destroy_process_group()
+        return {"value": round(K * LARGE_PER_STEP[cfg] * w.M / (ms * 1e-3), 2), "unit": UNIT, "ms_per_step": round(ms / K, 4),
+                "iterations_per_large_step": round(st["iterations"] / max(st["large_steps"], 1), 3), "world_size": 1,
+                "collectives_per_iteration": "all_gather of one [P][N] block + scalar max all_reduce (NCCL)"}
+
     cfg, K, Wm = args.config, args.steps, max(args.warmup, 3)
     peaks = _peaks()
     # `value`: the call a user makes (no per-kernel events; the MPA loop runs on the device as a CUDA graph).
@@ -365,6 +401,10 @@ def run_gpu(args):
         out["variants"]["aposteriori_stop_rule"] = {
             "value": round(ap["z_steps"] / (ap["ms"] * 1e-3), 2), "unit": UNIT, "ms_per_step": round(ap["ms"] / K, 4),
             "iterations_per_large_step": round(ap["iters"] / max(ap["large"], 1), 3), "not_converged": ap["not_conv"]}
+        try:                                         # the plane-sharded driver, here on a world of ONE rank
+            out["variants"]["plane_sharded_driver_world1"] = measure_sharded_world1(cfg, K, Wm, local)
+        except Exception as exc:                     # (torch.distributed unavailable, port in use, ...)
+            out["variants"]["plane_sharded_driver_world1"] = {"unavailable": str(exc)[:200]}
         try:                                         # the dense contraction on the 3xTF32 kernel (r01c-r01i's default)
             tf = measure(cfg, K, Wm, with_events=False, contraction=3)
             out["variants"]["tf32_contraction"] = {
