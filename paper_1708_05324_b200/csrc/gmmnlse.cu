@@ -1098,34 +1098,36 @@ struct PlanT final : gmmnlse_plan {
   // ------------------------------------------------------------------ kernel launchers
   template <int LOG2N, int DIR>
   int launch_fft_t(const C* in, long long in_ps, C* out, long long out_ps, const C* pre, const C* post_vec,
-                   const C* post_tab, long long tab_ps, T scale, int rows, int planes, const T* rscale) {
+                   const C* post_tab, long long tab_ps, T scale, int rows, int planes, const T* rscale, float* bound) {
     constexpr int NT = (1 << LOG2N) / 16;
     const size_t smem = sizeof(C) * fft_smem_elems(1 << LOG2N);
     GM_TRY(ensure_smem(k_fft_rows<T, LOG2N, DIR>, smem));
     prof_begin(DIR > 0 ? GMMNLSE_KIND_FFT_TO_FREQ : GMMNLSE_KIND_FFT_TO_TIME);
     launch_k(k_fft_rows<T, LOG2N, DIR>, dim3(rows, planes), NT, smem, in, in_ps, out, out_ps, pre, post_vec,
-                                                                         post_tab, tab_ps, scale, tw, rscale);
+             post_tab, tab_ps, scale, tw, rscale, bound, v_gain);
     prof_end();
     GM_CUDA(cudaGetLastError());
     return 0;
   }
+  // bound != nullptr: also accumulate v_gain max |out|^2 into it (zeroed by the caller): see launch_pairs
   int launch_fft(int dir, const C* in, long long in_ps, C* out, long long out_ps, const C* pre, const C* post_vec,
-                 const C* post_tab, long long tab_ps, T scale, int rows, int planes, const T* rscale = nullptr) {
+                 const C* post_tab, long long tab_ps, T scale, int rows, int planes, const T* rscale = nullptr,
+                 float* bound = nullptr) {
 #define GM_FFT_CASE(L)                                                                                       \
   case L:                                                                                                    \
     return dir > 0 ? launch_fft_t<L, +1>(in, in_ps, out, out_ps, pre, post_vec, post_tab, tab_ps, scale, rows, \
-                                         planes, rscale)                                                     \
+                                         planes, rscale, bound)                                              \
                    : launch_fft_t<L, -1>(in, in_ps, out, out_ps, pre, post_vec, post_tab, tab_ps, scale, rows, \
-                                         planes, rscale);
+                                         planes, rscale, bound);
     switch (log2N) {
       GM_FFT_CASE(4) GM_FFT_CASE(5) GM_FFT_CASE(6) GM_FFT_CASE(7) GM_FFT_CASE(8) GM_FFT_CASE(9)
       GM_FFT_CASE(10) GM_FFT_CASE(11) GM_FFT_CASE(12) GM_FFT_CASE(13)
       case 14:
         if constexpr (sizeof(T) == 4) {
           return dir > 0 ? launch_fft_t<14, +1>(in, in_ps, out, out_ps, pre, post_vec, post_tab, tab_ps, scale,
-                                                rows, planes, rscale)
+                                                rows, planes, rscale, bound)
                          : launch_fft_t<14, -1>(in, in_ps, out, out_ps, pre, post_vec, post_tab, tab_ps, scale,
-                                                rows, planes, rscale);
+                                                rows, planes, rscale, bound);
         }
         return GMMNLSE_EUNSUPPORTED;
     }
@@ -1146,15 +1148,19 @@ struct PlanT final : gmmnlse_plan {
     return 0;
   }
   bool own_v(const T* p) const { return p >= V && p < V + (size_t)(M + 1) * QN; }
+  bool bound_from_fft = false;   // d_vbound already holds the bound of the planes the next launch_pairs works on
   int launch_pairs(const C* A, long long a_ps, T* Vout, long long v_ps, int planes) {
     cur_ho.Vh = nullptr;
     if constexpr (sizeof(T) == 4) {
       if (tc_h && own_v(Vout)) {                    // the f16 contraction follows: V as fp16 hi / lo planes
-        GM_CUDA(cudaMemsetAsync(d_vbound, 0, sizeof(float), stream));
-        prof_begin(GMMNLSE_KIND_PAIR_CONV);
-        launch_k(k_bound_field<T>, dim3(32, planes), 256, 0, A, a_ps, PN, v_gain, d_vbound);
-        prof_end();
-        GM_CUDA(cudaGetLastError());
+        if (!bound_from_fft) {                      // (the MPA iteration gets the bound from its a3 FFT's stores)
+          GM_CUDA(cudaMemsetAsync(d_vbound, 0, sizeof(float), stream));
+          prof_begin(GMMNLSE_KIND_PAIR_CONV);
+          launch_k(k_bound_field<T>, dim3(32, planes), 256, 0, A, a_ps, PN, v_gain, d_vbound);
+          prof_end();
+          GM_CUDA(cudaGetLastError());
+        }
+        bound_from_fft = false;
         if (sparse) {                               // class-ordered, padded rows in the plan's Vsp planes
           const long long vq = (long long)sp_Qv * N;
           cur_ho = HalfOut{reinterpret_cast<__half*>(Vsp + ((Vout - V) / QN) * vq), 2 * vq, vq, N, d_vbound, sp_vrow};
@@ -1387,8 +1393,16 @@ struct PlanT final : gmmnlse_plan {
     const int j0 = first ? 0 : 1, np = Mc + 1 - j0;
     const unsigned sblocks = (unsigned)((PN + 255) / 256);
     // a3: A_j(t) = F^-1{psi_j exp(+D j dz)}; first iterate psi_j = psi_0
+    float* fb = nullptr;
+    if constexpr (sizeof(T) == 4) {
+      if (tc_h && !small_fused()) {                  // the fp16 pair streams' range bound rides on a3's stores
+        GM_CUDA(cudaMemsetAsync(d_vbound, 0, sizeof(float), stream));
+        fb = d_vbound;
+      }
+    }
     GM_TRY(launch_fft(-1, first ? psi : psi + j0 * PN, first ? 0 : PN, At + j0 * PN, PN, E + j0 * PN, nullptr,
-                      nullptr, PN, (T)(1.0 / N), P, np, gfwd ? gfwd + j0 * P : nullptr));
+                      nullptr, PN, (T)(1.0 / N), P, np, gfwd ? gfwd + j0 * P : nullptr, fb));
+    bound_from_fft = fb != nullptr;
     GM_TRY(nonlinear_term(j0, np));                                        // a4-a7
     // a8: G_j = K(w) exp(-D j dz) F{N_p}
     GM_TRY(launch_fft(+1, G + j0 * PN, PN, G + j0 * PN, PN, nullptr, Kw, E + j0 * PN, PN, (T)1, P, np,

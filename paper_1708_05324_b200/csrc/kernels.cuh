@@ -15,12 +15,14 @@ namespace gm {
 //   X_k   = FFT_DIR(x)
 //   out_k = X_k * scale * (post_vec ? post_vec[k] : 1) * (post_tab ? conj(post_tab[j][p][k]) : 1)
 //                                                        Eq. 12: K(w) exp(-D j dz) F{N_p}
+//   bound (optional; zeroed before the launch): bound[0] = max(bound[0], bound_gain max |out|^2) -- the range bound of
+//   the fp16 pair streams that k_bound_field would otherwise recompute from the stored planes (a3 of the MPA iteration).
 template <typename T, int LOG2N, int DIR>
 __global__ void __launch_bounds__((1 << LOG2N) / 16, ((1 << LOG2N) / 16 == 512 && sizeof(T) == 4) ? 2 : 1)
 k_fft_rows(const cplx<T>* __restrict__ in, long long in_plane_stride, cplx<T>* __restrict__ out,
            long long out_plane_stride, const cplx<T>* __restrict__ pre, const cplx<T>* __restrict__ post_vec,
            const cplx<T>* __restrict__ post_tab, long long tab_plane_stride, T scale,
-           const cplx<T>* __restrict__ tw, const T* __restrict__ row_scale) {
+           const cplx<T>* __restrict__ tw, const T* __restrict__ row_scale, float* __restrict__ bound, float bound_gain) {
   pdl_prologue();
   constexpr int N = 1 << LOG2N;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -32,6 +34,7 @@ k_fft_rows(const cplx<T>* __restrict__ in, long long in_plane_stride, cplx<T>* _
   const cplx<T>* pre_r = pre ? pre + toff : nullptr;
   const cplx<T>* post_r = post_tab ? post_tab + toff : nullptr;
   if (row_scale) scale *= row_scale[j * gridDim.x + p];     // gain: exp(+-g_p j dz), one factor per (plane, mode)
+  float amax = 0.f;
   block_fft<T, LOG2N, DIR>(
       sm, tw,
       [&](int n) {
@@ -44,7 +47,13 @@ k_fft_rows(const cplx<T>* __restrict__ in, long long in_plane_stride, cplx<T>* _
         if (post_vec) X = cmul(X, post_vec[k]);
         if (post_r) X = cmulc(X, post_r[k]);
         dst[k] = X;
+        if (bound) amax = fmaxf(amax, (float)(X.x * X.x + X.y * X.y));
       });
+  if (bound) {                                              // uniform branch: one atomic per warp
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, d));
+    if ((threadIdx.x & 31) == 0 && amax > 0.f) atomicMax(reinterpret_cast<unsigned int*>(bound), __float_as_uint(amax * bound_gain));
+  }
 }
 
 // fp16 split output of the pair kernels for the kind::f16 contraction (gemm_h.cuh): V' = sV V as Vh + Vl, two
